@@ -1,0 +1,12 @@
+"""B200-native batched fixed-lag SE(2) SLAM backbone (arxiv/paper_2603_25834, §III-D).
+
+The product is the C-ABI library declared in ``include/slam.h`` (built from ``csrc/``) and the thin
+ctypes binding in :mod:`paper_2603_25834_b200.binding`.  Importing this package does NOT load the
+CUDA library; ``binding`` does, and fails loudly if it is missing (there is no CPU fallback).
+
+:mod:`paper_2603_25834_b200.synth` is the seeded synthetic-trajectory generator that serves both the
+product tests/bench and the independent fp64 oracle under ``oracle/``; it contains none of the
+method's arithmetic.
+"""
+
+__all__ = ["binding", "synth"]

@@ -1,0 +1,44 @@
+"""Shared test helpers: drive one oracle environment from generator arrays (float64 path)."""
+import numpy as np
+
+
+def step_inputs(data, t, env):
+    """Inputs of step t (1-based) for one environment, as float64 numpy."""
+    L = data["cfg"].L
+    odom = data["odom"][t - 1, :, env].astype(np.float64)
+    back = int(data["lc_back"][t - 1, env])
+    zlc = data["lc_meas"][t - 1, :, env].astype(np.float64)
+    valid, zrb = rb_inputs(data, t, env)
+    return odom, back, zlc, valid, zrb
+
+
+def rb_inputs(data, t, env):
+    L = data["cfg"].L
+    if L == 0:
+        return None, None
+    valid = np.array([(int(data["rb_mask"][t, l // 32, env]) >> (l % 32)) & 1 for l in range(L)], np.int32)
+    zrb = data["rb_meas"][t, :, :, env].astype(np.float64).T.copy()  # [L][2]
+    return valid, zrb
+
+
+def drive(orc, data, env, iters, on_step=None, steps=None):
+    """reset -> (observe_first) -> for t: push, solve, cov, [marginalize iff full] (R19)."""
+    W = data["cfg"].W
+    T = data["T"] if steps is None else steps
+    orc.reset()
+    if data["cfg"].L:
+        orc.observe_first(*rb_inputs(data, 0, env))
+    out = []
+    for t in range(1, T + 1):
+        odom, back, zlc, valid, zrb = step_inputs(data, t, env)
+        orc.push(odom, back, zlc, valid, zrb)
+        sn = orc.solve(iters)
+        S, ld = orc.cov()
+        P = orc.poses()
+        rec = dict(t=t, step=sn, cov=S, logdet=ld, poses=P, count=orc.count)
+        if on_step is not None:
+            on_step(rec, orc)
+        out.append(rec)
+        if orc.count == W:
+            orc.marginalize()
+    return out
