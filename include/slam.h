@@ -1,0 +1,135 @@
+/*
+ * slam.h -- C ABI of the B200-native batched fixed-lag SE(2) SLAM backbone.
+ *
+ * What it computes (arxiv/paper_2603_25834, section III-D): for `batch` simulated
+ * robots at once, a sliding window of the last `window` SE(2) poses connected by
+ * odometry, loop-closure and range-bearing landmark factors is optimised by a few Gauss-Newton
+ * iterations (eq. (5)); the newest pose's 3x3 marginal covariance is the last
+ * block of the inverse Gauss-Newton Hessian (eq. (6)) and is compressed to the
+ * uncertainty scalar the reward consumes (D-optimality); the window then slides
+ * with bounded memory and constant cost per step by Schur-marginalising the oldest
+ * pose into a Gaussian prior.  Where the paper is silent the readings R1-R25 of DESIGN.md apply.
+ *
+ * Conventions
+ *  - Every array argument is a DEVICE pointer owned by the caller unless the name ends in `_host`.
+ *  - Layout is "environment fastest": an array documented [3][N] holds element (k, env) at k*N+env.
+ *  - All calls enqueue work on the stream given to slam_create and return without synchronising.
+ *    Nothing is allocated after slam_create; the caller owns the workspace.
+ *  - Return value: SLAM_OK or an error code; slam_last_error() gives a host string.  Numerical
+ *    trouble is per environment and asynchronous: a sticky status word (slam_get_status).
+ *  - All environments move in lock-step: one host-side window count (slam_count).
+ *  - Not re-entrant: one context per stream, one host thread per context.
+ *  - Arithmetic: fp32, except the final 6x6 -> 3x3 covariance/log-det tail (fp64, O(1) per env).
+ */
+#ifndef SLAM_H
+#define SLAM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct slam_ctx slam_ctx; /* opaque host object */
+
+enum { SLAM_OK = 0, SLAM_EINVAL = 1, SLAM_ESTATE = 2, SLAM_ENOMEM = 3, SLAM_ECUDA = 4 };
+/* bits of the per-environment status word */
+enum { SLAM_ENV_OK = 0, SLAM_ENV_NOT_PD = 1, SLAM_ENV_NONFINITE = 2 };
+
+#define SLAM_MAX_WINDOW 64    /* compiled maxima: window <= 64, landmarks <= 64 */
+#define SLAM_MAX_LANDMARKS 64
+
+/* Noise model: standard deviations, all > 0.  Defaults are BASELINE.json's values. */
+typedef struct {
+  float prior_sigma[3]; /* 0.01, 0.01, 0.005  (x, y, theta) of the first pose            */
+  float odo_sigma[3];   /* 0.05, 0.05, 0.02   odometry between-factor                     */
+  float lc_sigma[3];    /* 0.10, 0.10, 0.03   loop-closure between-factor                 */
+  float rb_sigma[2];    /* 0.05 (range, m), 0.01 (bearing, rad)                           */
+} slam_config;
+
+/* Fills *cfg with the defaults above. */
+void slam_default_config(slam_config* cfg);
+
+/* Bytes of device workspace slam_create needs for these sizes (0 if the sizes are invalid). */
+size_t slam_workspace_bytes(int batch, int window, int landmarks);
+
+/* Creates a context.  window in [2, SLAM_MAX_WINDOW], landmarks in [0, SLAM_MAX_LANDMARKS],
+ * batch >= 1.  `workspace` is device memory, >= slam_workspace_bytes(), 256-byte aligned, owned by
+ * the caller and must outlive the context.  `cuda_stream` is a cudaStream_t (NULL = default
+ * stream).  The context starts reset (count = 1, prior on pose 0 at the origin).
+ * Errors: SLAM_EINVAL (sizes, NULLs, alignment, sigma <= 0, workspace too small), SLAM_ECUDA. */
+int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam_config* cfg /* NULL: defaults */,
+                void* workspace, size_t workspace_bytes, void* cuda_stream);
+void slam_destroy(slam_ctx* ctx); /* frees the host object only */
+
+/* count = 1; anchor pose = init_pose ([3][N], NULL -> origin); prior N(init_pose, diag(prior_sigma^2))
+ * on it (reading R9); clears landmarks, factors and status. */
+int slam_reset(slam_ctx* ctx, const float* init_pose);
+
+/* S0 push (BASELINE.json "initial guess is dead-reckoned"): appends one pose with the
+ * dead-reckoned guess e_c = e_{c-1} (+) odom and records this step's factors.
+ *   odom    [3][N]  dx, dy, dtheta in the previous pose's frame
+ *   lc_back [N]     0 = none; k >= 1 = loop closure to the pose k steps older; k > count-1 (target
+ *                   already left the window) is ignored for that env.  NULL = none.
+ *   lc_meas [3][N]  newest pose expressed in the target pose's frame (required iff lc_back != NULL)
+ *   rb_mask [ceil(L/32)][N]  visibility bits from the NEW pose (NULL iff landmarks == 0)
+ *   rb_meas [2][L][N]        range (m), bearing (rad); newly seen landmarks are initialised by
+ *                            inverse projection from the new pose's guess (reading R6)
+ * Errors: SLAM_ESTATE if count == window (marginalise first), SLAM_EINVAL on NULL odom etc. */
+int slam_push_step(slam_ctx* ctx, const float* odom, const int32_t* lc_back, const float* lc_meas,
+                   const uint32_t* rb_mask, const float* rb_meas);
+
+/* Landmark observations from pose 0; only valid right after reset (count == 1). */
+int slam_observe_first(slam_ctx* ctx, const uint32_t* rb_mask, const float* rb_meas);
+
+/* S1-S3: exactly `iters` >= 0 plain Gauss-Newton iterations (eq. (5); no damping, reading R12):
+ * linearise every live factor, assemble H = Lambda + sum J'Omega J and b in shared memory, envelope
+ * Cholesky, triangular solves, additive update with wrapped angles. */
+int slam_solve(slam_ctx* ctx, int iters);
+
+/* S4 (eq. (6), readings R13-R15): relinearise at the current estimate, factorise, and return the
+ * newest pose's marginal covariance in GLOBAL (x, y, theta) coordinates, without forming the full
+ * inverse.  cov is [9][N] (row-major 3x3 per env).  The result is cached until the next push /
+ * solve / marginalise / reset, so slam_dopt after slam_marginal_cov costs one copy kernel. */
+int slam_marginal_cov(slam_ctx* ctx, float* cov);
+/* logdet[N] = ln det Sigma_t;  dopt[N] = det(Sigma_t)^(1/3) = exp(logdet/3) (NULL to skip). */
+int slam_dopt(slam_ctx* ctx, float* logdet, float* dopt);
+
+/* S5: Schur-complement marginalisation of the oldest pose into the Gaussian prior, re-anchoring of
+ * the window to the next pose, ring-buffer advance.  Requires count >= 2 (else SLAM_ESTATE). */
+int slam_marginalize_oldest(slam_ctx* ctx);
+
+/* Fused step: push -> solve(iters) -> covariance/log-det -> marginalise iff count == window after
+ * the push.  One kernel launch.  Bit-for-bit equal to the composition of the separate calls.
+ * cov [9][N], logdet [N] and last_pose [3][N] (newest pose, global) may each be NULL. */
+int slam_step(slam_ctx* ctx, const float* odom, const int32_t* lc_back, const float* lc_meas,
+              const uint32_t* rb_mask, const float* rb_meas, int iters, float* cov, float* logdet,
+              float* last_pose);
+
+/* The same step with HOST buffers (pinned memory recommended): copies the inputs to device staging
+ * inside the workspace, runs slam_step, copies cov/logdet/last_pose back, all asynchronously on the
+ * context's stream (the caller synchronises the stream before reading the outputs). */
+int slam_step_host(slam_ctx* ctx, const float* odom_host, const int32_t* lc_back_host, const float* lc_meas_host,
+                   const uint32_t* rb_mask_host, const float* rb_meas_host, int iters, float* cov_host,
+                   float* logdet_host, float* last_pose_host);
+
+/* Read-outs.  poses: [3][W][N] global poses of the window, slots >= count zero-filled (R21).
+ * lm: [2][L][N] global landmark positions (0 where inactive); active: [ceil(L/32)][N].
+ * status: [N] sticky OR of SLAM_ENV_* bits. */
+int slam_get_poses(slam_ctx* ctx, float* poses);
+int slam_get_landmarks(slam_ctx* ctx, float* lm, uint32_t* active);
+int slam_get_status(slam_ctx* ctx, int32_t* status);
+
+int slam_count(const slam_ctx* ctx);                /* host-side window count c in [1, window] */
+long long slam_launch_count(const slam_ctx* ctx);   /* kernels launched by this context so far */
+const char* slam_last_error(const slam_ctx* ctx);   /* message of the last non-zero return */
+
+/* Introspection for the benchmark's roofline accounting: smem bytes per CTA, warps per CTA and
+ * resident CTAs per SM of the step kernel for this context's sizes. */
+int slam_kernel_info(const slam_ctx* ctx, int* smem_bytes_per_cta, int* warps_per_cta, int* ctas_per_sm);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SLAM_H */

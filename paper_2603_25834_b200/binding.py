@@ -1,0 +1,230 @@
+"""Thin Python binding of the C-ABI library (``include/slam.h``): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of ``csrc/``; PyTorch is used for device memory
+and streams.  There is NO CPU fallback: if ``libslam_b200.so`` is missing and cannot be built with
+nvcc, importing this module raises.  Method names follow the C entry points.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import shutil
+
+import torch
+
+from . import build as _build
+
+SLAM_OK, SLAM_EINVAL, SLAM_ESTATE, SLAM_ENOMEM, SLAM_ECUDA = 0, 1, 2, 3, 4
+SLAM_ENV_NOT_PD, SLAM_ENV_NONFINITE = 1, 2
+_ERR = {1: "SLAM_EINVAL", 2: "SLAM_ESTATE", 3: "SLAM_ENOMEM", 4: "SLAM_ECUDA"}
+
+# every symbol include/slam.h declares (checked by tests/test_abi.py)
+SYMBOLS = (
+    "slam_default_config", "slam_workspace_bytes", "slam_create", "slam_destroy", "slam_reset",
+    "slam_push_step", "slam_observe_first", "slam_solve", "slam_marginal_cov", "slam_dopt",
+    "slam_marginalize_oldest", "slam_step", "slam_step_host", "slam_get_poses", "slam_get_landmarks",
+    "slam_get_status", "slam_count", "slam_launch_count", "slam_last_error", "slam_kernel_info",
+)
+
+
+class SlamConfig(C.Structure):
+    _fields_ = [("prior_sigma", C.c_float * 3), ("odo_sigma", C.c_float * 3), ("lc_sigma", C.c_float * 3),
+                ("rb_sigma", C.c_float * 2)]
+
+
+class SlamError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"{_ERR.get(code, code)}: {msg}")
+        self.code = code
+
+
+def _load() -> C.CDLL:
+    path = _build.LIB
+    if _build.needs_build():
+        if shutil.which("nvcc") or os.path.exists("/usr/local/cuda/bin/nvcc"):
+            _build.build()
+        elif not os.path.exists(path):
+            raise ImportError(f"{path} is missing and nvcc is not available: build it with __graft_entry__.build()")
+    lib = C.CDLL(path)
+    vp, fp, ip = C.c_void_p, C.c_void_p, C.c_void_p
+    lib.slam_default_config.argtypes = [C.POINTER(SlamConfig)]
+    lib.slam_default_config.restype = None
+    lib.slam_workspace_bytes.argtypes = [C.c_int, C.c_int, C.c_int]
+    lib.slam_workspace_bytes.restype = C.c_size_t
+    lib.slam_create.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_int, C.POINTER(SlamConfig), vp, C.c_size_t, vp]
+    lib.slam_destroy.argtypes = [vp]
+    lib.slam_destroy.restype = None
+    lib.slam_reset.argtypes = [vp, fp]
+    lib.slam_push_step.argtypes = [vp, fp, ip, fp, ip, fp]
+    lib.slam_observe_first.argtypes = [vp, ip, fp]
+    lib.slam_solve.argtypes = [vp, C.c_int]
+    lib.slam_marginal_cov.argtypes = [vp, fp]
+    lib.slam_dopt.argtypes = [vp, fp, fp]
+    lib.slam_marginalize_oldest.argtypes = [vp]
+    lib.slam_step.argtypes = [vp, fp, ip, fp, ip, fp, C.c_int, fp, fp, fp]
+    lib.slam_step_host.argtypes = [vp, fp, ip, fp, ip, fp, C.c_int, fp, fp, fp]
+    lib.slam_get_poses.argtypes = [vp, fp]
+    lib.slam_get_landmarks.argtypes = [vp, fp, ip]
+    lib.slam_get_status.argtypes = [vp, ip]
+    lib.slam_count.argtypes = [vp]
+    lib.slam_launch_count.argtypes = [vp]
+    lib.slam_launch_count.restype = C.c_longlong
+    lib.slam_last_error.argtypes = [vp]
+    lib.slam_last_error.restype = C.c_char_p
+    lib.slam_kernel_info.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int)]
+    return lib
+
+
+LIB = _load()
+
+
+def default_config() -> SlamConfig:
+    cfg = SlamConfig()
+    LIB.slam_default_config(C.byref(cfg))
+    return cfg
+
+
+def workspace_bytes(batch: int, window: int, landmarks: int) -> int:
+    return int(LIB.slam_workspace_bytes(batch, window, landmarks))
+
+
+class FixedLagSlam:
+    """One context = `batch` environments in lock-step on one CUDA stream."""
+
+    def __init__(self, batch: int, window: int, landmarks: int = 0, config: SlamConfig | None = None,
+                 device: str | torch.device = "cuda:0", stream: torch.cuda.Stream | None = None):
+        if not torch.cuda.is_available():
+            raise RuntimeError("FixedLagSlam needs a CUDA device (there is no CPU fallback)")
+        self.N, self.W, self.L = int(batch), int(window), int(landmarks)
+        self.nw = (self.L + 31) // 32
+        self.device = torch.device(device)
+        nbytes = workspace_bytes(self.N, self.W, self.L)
+        if nbytes == 0:
+            raise SlamError(SLAM_EINVAL, f"invalid sizes batch={batch} window={window} landmarks={landmarks}")
+        with torch.cuda.device(self.device):
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = self.workspace.data_ptr()
+            self._ws_ptr = (base + 255) & ~255
+            h = C.c_void_p()
+            rc = LIB.slam_create(C.byref(h), self.N, self.W, self.L, C.byref(config) if config is not None else None,
+                                 C.c_void_p(self._ws_ptr), nbytes, C.c_void_p(self.stream.cuda_stream))
+        if rc != SLAM_OK:
+            raise SlamError(rc, "slam_create failed")
+        self._h = h
+
+    def __del__(self):
+        h = getattr(self, "_h", None)
+        if h:
+            LIB.slam_destroy(h)
+            self._h = None
+
+    # ---- marshalling helpers
+    def _chk(self, rc: int):
+        if rc != SLAM_OK:
+            raise SlamError(rc, (LIB.slam_last_error(self._h) or b"").decode())
+
+    def _dev(self, t, shape, dtypes, name):
+        if t is None:
+            return None
+        if not isinstance(t, torch.Tensor) or t.device != self.device or t.dtype not in dtypes or not t.is_contiguous() \
+                or tuple(t.shape) != tuple(shape):
+            raise SlamError(SLAM_EINVAL, f"{name}: expected contiguous {dtypes[0]} tensor of shape {tuple(shape)} on {self.device}")
+        return C.c_void_p(t.data_ptr())
+
+    def _host(self, t, shape, dtypes, name):
+        if t is None:
+            return None
+        if not isinstance(t, torch.Tensor) or t.device.type != "cpu" or t.dtype not in dtypes or not t.is_contiguous() \
+                or tuple(t.shape) != tuple(shape):
+            raise SlamError(SLAM_EINVAL, f"{name}: expected contiguous host {dtypes[0]} tensor of shape {tuple(shape)}")
+        return C.c_void_p(t.data_ptr())
+
+    def _new(self, *shape, dtype=torch.float32):
+        return torch.empty(shape, dtype=dtype, device=self.device)
+
+    _F = (torch.float32,)
+    _I = (torch.int32,)
+    _U = (torch.int32, torch.uint32)
+
+    def _push_ptrs(self, conv, odom, lc_back, lc_meas, rb_mask, rb_meas):
+        N, L = self.N, self.L
+        return (conv(odom, (3, N), self._F, "odom"), conv(lc_back, (N,), self._I, "lc_back"),
+                conv(lc_meas, (3, N), self._F, "lc_meas"),
+                conv(rb_mask, (self.nw, N), self._U, "rb_mask") if L else None,
+                conv(rb_meas, (2, L, N), self._F, "rb_meas") if L else None)
+
+    # ---- the C entry points
+    def reset(self, init_pose=None):
+        self._chk(LIB.slam_reset(self._h, self._dev(init_pose, (3, self.N), self._F, "init_pose")))
+
+    def push_step(self, odom, lc_back=None, lc_meas=None, rb_mask=None, rb_meas=None):
+        self._chk(LIB.slam_push_step(self._h, *self._push_ptrs(self._dev, odom, lc_back, lc_meas, rb_mask, rb_meas)))
+
+    def observe_first(self, rb_mask, rb_meas):
+        if self.L == 0:
+            return
+        self._chk(LIB.slam_observe_first(self._h, self._dev(rb_mask, (self.nw, self.N), self._U, "rb_mask"),
+                                         self._dev(rb_meas, (2, self.L, self.N), self._F, "rb_meas")))
+
+    def solve(self, iters: int):
+        self._chk(LIB.slam_solve(self._h, int(iters)))
+
+    def marginal_cov(self, out=None):
+        out = self._new(9, self.N) if out is None else out
+        self._chk(LIB.slam_marginal_cov(self._h, self._dev(out, (9, self.N), self._F, "cov")))
+        return out
+
+    def dopt(self, logdet=None, dopt=None):
+        logdet = self._new(self.N) if logdet is None else logdet
+        dopt = self._new(self.N) if dopt is None else dopt
+        self._chk(LIB.slam_dopt(self._h, self._dev(logdet, (self.N,), self._F, "logdet"),
+                                self._dev(dopt, (self.N,), self._F, "dopt")))
+        return logdet, dopt
+
+    def marginalize_oldest(self):
+        self._chk(LIB.slam_marginalize_oldest(self._h))
+
+    def step(self, odom, lc_back=None, lc_meas=None, rb_mask=None, rb_meas=None, *, iters: int, cov=None, logdet=None,
+             last_pose=None):
+        ptrs = self._push_ptrs(self._dev, odom, lc_back, lc_meas, rb_mask, rb_meas)
+        self._chk(LIB.slam_step(self._h, *ptrs, int(iters), self._dev(cov, (9, self.N), self._F, "cov"),
+                                self._dev(logdet, (self.N,), self._F, "logdet"),
+                                self._dev(last_pose, (3, self.N), self._F, "last_pose")))
+
+    def step_host(self, odom, lc_back=None, lc_meas=None, rb_mask=None, rb_meas=None, *, iters: int, cov=None,
+                  logdet=None, last_pose=None):
+        ptrs = self._push_ptrs(self._host, odom, lc_back, lc_meas, rb_mask, rb_meas)
+        self._chk(LIB.slam_step_host(self._h, *ptrs, int(iters), self._host(cov, (9, self.N), self._F, "cov"),
+                                     self._host(logdet, (self.N,), self._F, "logdet"),
+                                     self._host(last_pose, (3, self.N), self._F, "last_pose")))
+
+    def get_poses(self, out=None):
+        out = self._new(3, self.W, self.N) if out is None else out
+        self._chk(LIB.slam_get_poses(self._h, self._dev(out, (3, self.W, self.N), self._F, "poses")))
+        return out
+
+    def get_landmarks(self):
+        lm = self._new(2, max(self.L, 1), self.N)[:, : self.L].contiguous()
+        act = self._new(max(self.nw, 1), self.N, dtype=torch.int32)[: self.nw].contiguous()
+        if self.L:
+            self._chk(LIB.slam_get_landmarks(self._h, C.c_void_p(lm.data_ptr()), C.c_void_p(act.data_ptr())))
+        return lm, act
+
+    def get_status(self):
+        out = self._new(self.N, dtype=torch.int32)
+        self._chk(LIB.slam_get_status(self._h, C.c_void_p(out.data_ptr())))
+        return out
+
+    @property
+    def count(self) -> int:
+        return int(LIB.slam_count(self._h))
+
+    @property
+    def launch_count(self) -> int:
+        return int(LIB.slam_launch_count(self._h))
+
+    def kernel_info(self) -> dict:
+        a, b, c = C.c_int(), C.c_int(), C.c_int()
+        self._chk(LIB.slam_kernel_info(self._h, C.byref(a), C.byref(b), C.byref(c)))
+        return dict(smem_bytes_per_cta=a.value, warps_per_cta=b.value, ctas_per_sm=c.value)

@@ -1,0 +1,447 @@
+// C ABI of the batched fixed-lag SLAM backbone (include/slam.h): host dispatcher + kernels.
+// Every step of the hot path runs in the kernels of slam_kernels.cuh; this file only checks
+// arguments, keeps the lock-step window bookkeeping (count, ring head) and launches.
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "../../include/slam.h"
+#include "slam_kernels.cuh"
+
+using namespace slamk;
+
+// ------------------------------------------------------------------ kernels
+// One warp per environment, `wpc` warps per CTA, persistent grid-stride loop over environments.
+// flags select the phases, so that the separate ABI calls and the fused slam_step share the same
+// device code and are bit-for-bit identical.
+__global__ void __launch_bounds__(256) slam_step_kernel(Layout ly, Params pr, float* state, int head, int c, int flags,
+                                                        int iters, StepIO io) {
+  extern __shared__ float4 smem4[];
+  float* smem = reinterpret_cast<float*>(smem4);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const WS w = make_ws(ly, smem + (size_t)warp * ly.warp_words);
+  for (int env = blockIdx.x * ly.wpc + warp; env < ly.N; env += gridDim.x * ly.wpc) {
+    float* rec = state + (size_t)env * ly.rec;
+    int cc = c, status = 0;
+    Masks mk;
+    load_env(ly, rec, w, lane, head, cc, mk);
+    if (flags & F_OBS0) record_rb(ly, rec, w, lane, env, head, 0, 0.f, 0.f, 0.f, io, mk);
+    if (flags & F_PUSH) cc = push_env(ly, rec, w, lane, env, head, cc, io, mk);
+    const int s = build_support(ly, w, lane, cc, mk.ps, mk.ls);
+    if (iters > 0 || (flags & F_COV)) {
+      int nLR = 0;
+      const int total = symbolic(ly, w, lane, cc, mk, s, nLR);
+      for (int it = 0; it < iters; ++it) {
+        assemble(ly, pr, rec, w, lane, head, cc, mk, s, total);
+        __syncwarp();
+        status |= cholesky(ly, w, lane, nLR);
+        back_substitute(ly, w, lane);
+        status |= apply_update(ly, w, lane, cc, mk);
+      }
+      if (flags & F_COV) {
+        assemble(ly, pr, rec, w, lane, head, cc, mk, s, total);
+        __syncwarp();
+        status |= cholesky(ly, w, lane, nLR);
+        covariance(ly, w, lane, env, cc, io);
+        __syncwarp();
+      }
+    }
+    if (io.last_pose && lane == 0) {  // newest pose in global coordinates: a (+) e_{c-1}
+      float sn, cn;
+      sincosf(w.st[2], &sn, &cn);
+      const float* e = w.st + st_pose(cc - 1);
+      io.last_pose[env] = w.st[0] + cn * e[0] - sn * e[1];
+      io.last_pose[(size_t)ly.N + env] = w.st[1] + sn * e[0] + cn * e[1];
+      io.last_pose[2 * (size_t)ly.N + env] = wrapf(w.st[2] + e[2]);
+    }
+    if (flags & F_MARG) status |= marginalize(ly, pr, rec, w, lane, head, cc, mk, s);
+    store_state(ly, rec, w, lane, head, cc, mk);
+    if (status && lane == 0) reinterpret_cast<int*>(rec)[ly.o_status] |= status;
+    __syncwarp();
+  }
+}
+
+// reset: one warp per environment
+__global__ void slam_reset_kernel(Layout ly, Params pr, float* state, const float* init_pose) {
+  const int env = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (env >= ly.N) return;
+  float* rec = state + (size_t)env * ly.rec;
+  int* reci = reinterpret_cast<int*>(rec);
+  for (int i = lane; i < ly.o_lam + 8; i += 32) rec[i] = 0.f;
+  __syncwarp();
+  for (int k = lane; k < ly.W; k += 32) reci[ly.o_lct + k] = -1;
+  if (lane < 3) {
+    const float a = init_pose ? init_pose[(size_t)lane * ly.N + env] : 0.f;
+    rec[ly.o_a + lane] = a;
+    rec[ly.o_vbar + lane] = a;
+    rec[ly.o_lam + (lane * (lane + 1) / 2) + lane] = pr.om_prior[lane];
+  }
+}
+
+// poses[3][W][N] = a (+) e_k for k < c, else 0
+__global__ void slam_poses_kernel(Layout ly, const float* state, int head, int c, float* poses) {
+  const int env = blockIdx.x * blockDim.x + threadIdx.x;
+  if (env >= ly.N) return;
+  const float* rec = state + (size_t)env * ly.rec;
+  const float ax = rec[ly.o_a], ay = rec[ly.o_a + 1], at = rec[ly.o_a + 2];
+  float sn, cn;
+  sincosf(at, &sn, &cn);
+  for (int k = 0; k < ly.W; ++k) {
+    float x = 0.f, y = 0.f, t = 0.f;
+    if (k < c) {
+      const int r = ring_of(k, head, ly.W);
+      const float ex = k ? rec[ly.o_e + 3 * r] : 0.f, ey = k ? rec[ly.o_e + 3 * r + 1] : 0.f, et = k ? rec[ly.o_e + 3 * r + 2] : 0.f;
+      x = ax + cn * ex - sn * ey; y = ay + sn * ex + cn * ey; t = wrapf(at + et);
+    }
+    poses[((size_t)0 * ly.W + k) * ly.N + env] = x;
+    poses[((size_t)1 * ly.W + k) * ly.N + env] = y;
+    poses[((size_t)2 * ly.W + k) * ly.N + env] = t;
+  }
+}
+
+__global__ void slam_landmarks_kernel(Layout ly, const float* state, float* lm, uint32_t* active) {
+  const int env = blockIdx.x * blockDim.x + threadIdx.x;
+  if (env >= ly.N) return;
+  const float* rec = state + (size_t)env * ly.rec;
+  const uint32_t* recu = reinterpret_cast<const uint32_t*>(rec);
+  const float ax = rec[ly.o_a], ay = rec[ly.o_a + 1], at = rec[ly.o_a + 2];
+  float sn, cn;
+  sincosf(at, &sn, &cn);
+  for (int q = 0; q < ly.nw; ++q) active[(size_t)q * ly.N + env] = recu[ly.o_act + q];
+  for (int l = 0; l < ly.L; ++l) {
+    const bool act = (recu[ly.o_act + (l >> 5)] >> (l & 31)) & 1u;
+    const float mx = rec[ly.o_m + 2 * l], my = rec[ly.o_m + 2 * l + 1];
+    lm[((size_t)0 * ly.L + l) * ly.N + env] = act ? ax + cn * mx - sn * my : 0.f;
+    lm[((size_t)1 * ly.L + l) * ly.N + env] = act ? ay + sn * mx + cn * my : 0.f;
+  }
+}
+
+__global__ void slam_status_kernel(Layout ly, const float* state, int32_t* status) {
+  const int env = blockIdx.x * blockDim.x + threadIdx.x;
+  if (env < ly.N) status[env] = reinterpret_cast<const int*>(state + (size_t)env * ly.rec)[ly.o_status];
+}
+
+__global__ void slam_copycov_kernel(int N, const float* cache, float* cov, float* logdet, float* dopt) {
+  const int env = blockIdx.x * blockDim.x + threadIdx.x;
+  if (env >= N) return;
+  if (cov)
+    for (int k = 0; k < 9; ++k) cov[(size_t)k * N + env] = cache[(size_t)k * N + env];
+  const float ld = cache[(size_t)9 * N + env];
+  if (logdet) logdet[env] = ld;
+  if (dopt) dopt[env] = expf(ld * (1.0f / 3.0f));
+}
+
+// ------------------------------------------------------------------ host object
+struct slam_ctx {
+  Layout ly;
+  Params pr;
+  cudaStream_t stream;
+  float* state;
+  float* cov_cache;
+  // device staging for slam_step_host
+  float *st_odom, *st_lc_meas, *st_rb_meas, *st_cov, *st_logdet, *st_pose;
+  int32_t* st_lc_back;
+  uint32_t* st_rb_mask;
+  int head, count;
+  bool cov_valid;
+  long long launches;
+  int grid, smem_bytes, ctas_per_sm;
+  char err[256];
+};
+
+static int fail(slam_ctx* c, int code, const char* msg) {
+  if (c) snprintf(c->err, sizeof(c->err), "%s", msg);
+  return code;
+}
+static int check_cuda(slam_ctx* c, const char* what) {
+  const cudaError_t e = cudaGetLastError();
+  if (e == cudaSuccess) return SLAM_OK;
+  if (c) snprintf(c->err, sizeof(c->err), "%s: %s", what, cudaGetErrorString(e));
+  return SLAM_ECUDA;
+}
+static size_t al256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+static bool sizes_ok(int batch, int window, int landmarks) {
+  return batch >= 1 && window >= 2 && window <= SLAM_MAX_WINDOW && landmarks >= 0 && landmarks <= SLAM_MAX_LANDMARKS;
+}
+
+static int pick_wpc(int W, int L) {
+  const Layout t = make_layout(1, W, L, -1, 1);
+  const size_t wb = (size_t)t.warp_words * 4;
+  int wpc = (int)((size_t)227 * 1024 / wb);
+  if (wpc > 8) wpc = 8;
+  return wpc;  // 0 if one environment does not fit
+}
+
+struct WsPlan { size_t state, cache, odom, lcb, lcm, rbk, rbm, cov, ld, pose, total; };
+static WsPlan plan(const Layout& ly) {
+  WsPlan p;
+  size_t o = 0;
+  const size_t N = (size_t)ly.N;
+  p.state = o; o = al256(o + N * ly.rec * 4);
+  p.cache = o; o = al256(o + N * 10 * 4);
+  p.odom = o; o = al256(o + N * 3 * 4);
+  p.lcb = o; o = al256(o + N * 4);
+  p.lcm = o; o = al256(o + N * 3 * 4);
+  p.rbk = o; o = al256(o + N * (size_t)(ly.nw ? ly.nw : 1) * 4);
+  p.rbm = o; o = al256(o + N * (size_t)(ly.L ? 2 * ly.L : 1) * 4);
+  p.cov = o; o = al256(o + N * 9 * 4);
+  p.ld = o; o = al256(o + N * 4);
+  p.pose = o; o = al256(o + N * 3 * 4);
+  p.total = o;
+  return p;
+}
+
+extern "C" {
+
+void slam_default_config(slam_config* cfg) {
+  if (!cfg) return;
+  const float p[3] = {0.01f, 0.01f, 0.005f}, o[3] = {0.05f, 0.05f, 0.02f}, l[3] = {0.10f, 0.10f, 0.03f};
+  for (int k = 0; k < 3; ++k) { cfg->prior_sigma[k] = p[k]; cfg->odo_sigma[k] = o[k]; cfg->lc_sigma[k] = l[k]; }
+  cfg->rb_sigma[0] = 0.05f; cfg->rb_sigma[1] = 0.01f;
+}
+
+size_t slam_workspace_bytes(int batch, int window, int landmarks) {
+  if (!sizes_ok(batch, window, landmarks)) return 0;
+  const int wpc = pick_wpc(window, landmarks);
+  if (wpc < 1) return 0;
+  return plan(make_layout(batch, window, landmarks, -1, wpc)).total;
+}
+
+int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam_config* cfg, void* workspace,
+                size_t workspace_bytes, void* cuda_stream) {
+  if (!out) return SLAM_EINVAL;
+  *out = nullptr;
+  if (!sizes_ok(batch, window, landmarks) || !workspace || ((uintptr_t)workspace & 255)) return SLAM_EINVAL;
+  const int wpc = pick_wpc(window, landmarks);
+  if (wpc < 1) return SLAM_EINVAL;
+  slam_config dc;
+  slam_default_config(&dc);
+  if (!cfg) cfg = &dc;
+  for (int k = 0; k < 3; ++k)
+    if (!(cfg->prior_sigma[k] > 0.f) || !(cfg->odo_sigma[k] > 0.f) || !(cfg->lc_sigma[k] > 0.f)) return SLAM_EINVAL;
+  if (!(cfg->rb_sigma[0] > 0.f) || !(cfg->rb_sigma[1] > 0.f)) return SLAM_EINVAL;
+  slam_ctx* c = new (std::nothrow) slam_ctx();
+  if (!c) return SLAM_ENOMEM;
+  c->ly = make_layout(batch, window, landmarks, -1, wpc);
+  const WsPlan p = plan(c->ly);
+  if (workspace_bytes < p.total) { delete c; return SLAM_EINVAL; }
+  for (int k = 0; k < 3; ++k) {
+    c->pr.om_prior[k] = 1.0f / (cfg->prior_sigma[k] * cfg->prior_sigma[k]);
+    c->pr.om_odo[k] = 1.0f / (cfg->odo_sigma[k] * cfg->odo_sigma[k]);
+    c->pr.om_lc[k] = 1.0f / (cfg->lc_sigma[k] * cfg->lc_sigma[k]);
+  }
+  c->pr.om_rb[0] = 1.0f / (cfg->rb_sigma[0] * cfg->rb_sigma[0]);
+  c->pr.om_rb[1] = 1.0f / (cfg->rb_sigma[1] * cfg->rb_sigma[1]);
+  c->stream = (cudaStream_t)cuda_stream;
+  char* base = (char*)workspace;
+  c->state = (float*)(base + p.state);
+  c->cov_cache = (float*)(base + p.cache);
+  c->st_odom = (float*)(base + p.odom);
+  c->st_lc_back = (int32_t*)(base + p.lcb);
+  c->st_lc_meas = (float*)(base + p.lcm);
+  c->st_rb_mask = (uint32_t*)(base + p.rbk);
+  c->st_rb_meas = (float*)(base + p.rbm);
+  c->st_cov = (float*)(base + p.cov);
+  c->st_logdet = (float*)(base + p.ld);
+  c->st_pose = (float*)(base + p.pose);
+  c->launches = 0;
+  c->err[0] = 0;
+  c->smem_bytes = c->ly.warp_words * 4 * wpc;
+  if (cudaFuncSetAttribute(slam_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_bytes) != cudaSuccess) {
+    cudaGetLastError();
+    delete c;
+    return SLAM_ECUDA;
+  }
+  int dev = 0, sms = 0, occ = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, slam_step_kernel, wpc * 32, c->smem_bytes);
+  if (occ < 1 || sms < 1) { cudaGetLastError(); delete c; return SLAM_ECUDA; }
+  c->ctas_per_sm = occ;
+  const int need = (batch + wpc - 1) / wpc;
+  c->grid = need < sms * occ ? need : sms * occ;
+  *out = c;
+  const int rc = slam_reset(c, nullptr);
+  if (rc != SLAM_OK) { *out = nullptr; delete c; }
+  return rc;
+}
+
+void slam_destroy(slam_ctx* ctx) { delete ctx; }
+
+int slam_reset(slam_ctx* c, const float* init_pose) {
+  if (!c) return SLAM_EINVAL;
+  const int threads = 256, blocks = (int)(((size_t)c->ly.N * 32 + threads - 1) / threads);
+  slam_reset_kernel<<<blocks, threads, 0, c->stream>>>(c->ly, c->pr, c->state, init_pose);
+  c->launches++;
+  c->head = 0; c->count = 1; c->cov_valid = false;
+  return check_cuda(c, "slam_reset");
+}
+
+static int launch_step(slam_ctx* c, int flags, int iters, const StepIO& io) {
+  slam_step_kernel<<<c->grid, c->ly.wpc * 32, c->smem_bytes, c->stream>>>(c->ly, c->pr, c->state, c->head, c->count, flags,
+                                                                        iters, io);
+  c->launches++;
+  return check_cuda(c, "slam_step_kernel");
+}
+
+static int check_push_args(slam_ctx* c, const float* odom, const int32_t* lc_back, const float* lc_meas,
+                           const uint32_t* rb_mask, const float* rb_meas) {
+  if (!odom) return fail(c, SLAM_EINVAL, "odom is NULL");
+  if (lc_back && !lc_meas) return fail(c, SLAM_EINVAL, "lc_back given without lc_meas");
+  if (c->ly.L > 0 && (!rb_mask || !rb_meas)) return fail(c, SLAM_EINVAL, "rb_mask/rb_meas required when landmarks > 0");
+  if (c->count >= c->ly.W) return fail(c, SLAM_ESTATE, "push on a full window: marginalize first");
+  return SLAM_OK;
+}
+
+int slam_push_step(slam_ctx* c, const float* odom, const int32_t* lc_back, const float* lc_meas, const uint32_t* rb_mask,
+                   const float* rb_meas) {
+  if (!c) return SLAM_EINVAL;
+  int rc = check_push_args(c, odom, lc_back, lc_meas, rb_mask, rb_meas);
+  if (rc) return rc;
+  StepIO io = {odom, lc_back, lc_meas, rb_mask, rb_meas, nullptr, nullptr, nullptr, nullptr, c->cov_cache};
+  rc = launch_step(c, F_PUSH, 0, io);
+  if (rc) return rc;
+  c->count++; c->cov_valid = false;
+  return SLAM_OK;
+}
+
+int slam_observe_first(slam_ctx* c, const uint32_t* rb_mask, const float* rb_meas) {
+  if (!c) return SLAM_EINVAL;
+  if (c->ly.L == 0) return SLAM_OK;
+  if (!rb_mask || !rb_meas) return fail(c, SLAM_EINVAL, "rb_mask/rb_meas are NULL");
+  if (c->count != 1) return fail(c, SLAM_ESTATE, "observe_first is only valid right after reset");
+  StepIO io = {nullptr, nullptr, nullptr, rb_mask, rb_meas, nullptr, nullptr, nullptr, nullptr, c->cov_cache};
+  c->cov_valid = false;
+  return launch_step(c, F_OBS0, 0, io);
+}
+
+int slam_solve(slam_ctx* c, int iters) {
+  if (!c) return SLAM_EINVAL;
+  if (iters < 0) return fail(c, SLAM_EINVAL, "iters < 0");
+  if (iters == 0) return SLAM_OK;
+  StepIO io = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, c->cov_cache};
+  c->cov_valid = false;
+  return launch_step(c, 0, iters, io);
+}
+
+static int cov_call(slam_ctx* c, float* cov, float* logdet, float* dopt) {
+  if (c->cov_valid) {
+    const int threads = 256, blocks = (c->ly.N + threads - 1) / threads;
+    slam_copycov_kernel<<<blocks, threads, 0, c->stream>>>(c->ly.N, c->cov_cache, cov, logdet, dopt);
+    c->launches++;
+    return check_cuda(c, "slam_copycov_kernel");
+  }
+  StepIO io = {nullptr, nullptr, nullptr, nullptr, nullptr, cov, logdet, dopt, nullptr, c->cov_cache};
+  const int rc = launch_step(c, F_COV, 0, io);
+  if (rc == SLAM_OK) c->cov_valid = true;
+  return rc;
+}
+
+int slam_marginal_cov(slam_ctx* c, float* cov) {
+  if (!c) return SLAM_EINVAL;
+  if (!cov) return fail(c, SLAM_EINVAL, "cov is NULL");
+  return cov_call(c, cov, nullptr, nullptr);
+}
+
+int slam_dopt(slam_ctx* c, float* logdet, float* dopt) {
+  if (!c) return SLAM_EINVAL;
+  if (!logdet && !dopt) return fail(c, SLAM_EINVAL, "logdet and dopt are both NULL");
+  return cov_call(c, nullptr, logdet, dopt);
+}
+
+int slam_marginalize_oldest(slam_ctx* c) {
+  if (!c) return SLAM_EINVAL;
+  if (c->count < 2) return fail(c, SLAM_ESTATE, "marginalize needs count >= 2");
+  StepIO io = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, c->cov_cache};
+  const int rc = launch_step(c, F_MARG, 0, io);
+  if (rc) return rc;
+  c->head = (c->head + 1) % c->ly.W;
+  c->count--;
+  c->cov_valid = false;
+  return SLAM_OK;
+}
+
+int slam_step(slam_ctx* c, const float* odom, const int32_t* lc_back, const float* lc_meas, const uint32_t* rb_mask,
+              const float* rb_meas, int iters, float* cov, float* logdet, float* last_pose) {
+  if (!c) return SLAM_EINVAL;
+  if (iters < 0) return fail(c, SLAM_EINVAL, "iters < 0");
+  int rc = check_push_args(c, odom, lc_back, lc_meas, rb_mask, rb_meas);
+  if (rc) return rc;
+  const bool marg = (c->count + 1 == c->ly.W);
+  StepIO io = {odom, lc_back, lc_meas, rb_mask, rb_meas, cov, logdet, nullptr, last_pose, c->cov_cache};
+  rc = launch_step(c, F_PUSH | F_COV | (marg ? F_MARG : 0), iters, io);
+  if (rc) return rc;
+  c->count++;
+  c->cov_valid = !marg;
+  if (marg) { c->head = (c->head + 1) % c->ly.W; c->count--; }
+  return SLAM_OK;
+}
+
+int slam_step_host(slam_ctx* c, const float* odom, const int32_t* lc_back, const float* lc_meas, const uint32_t* rb_mask,
+                   const float* rb_meas, int iters, float* cov, float* logdet, float* last_pose) {
+  if (!c) return SLAM_EINVAL;
+  int rc = check_push_args(c, odom, lc_back, lc_meas, rb_mask, rb_meas);
+  if (rc) return rc;
+  const size_t N = (size_t)c->ly.N;
+  cudaMemcpyAsync(c->st_odom, odom, N * 3 * 4, cudaMemcpyHostToDevice, c->stream);
+  if (lc_back) {
+    cudaMemcpyAsync(c->st_lc_back, lc_back, N * 4, cudaMemcpyHostToDevice, c->stream);
+    cudaMemcpyAsync(c->st_lc_meas, lc_meas, N * 3 * 4, cudaMemcpyHostToDevice, c->stream);
+  }
+  if (c->ly.L > 0) {
+    cudaMemcpyAsync(c->st_rb_mask, rb_mask, N * c->ly.nw * 4, cudaMemcpyHostToDevice, c->stream);
+    cudaMemcpyAsync(c->st_rb_meas, rb_meas, N * 2 * c->ly.L * 4, cudaMemcpyHostToDevice, c->stream);
+  }
+  rc = slam_step(c, c->st_odom, lc_back ? c->st_lc_back : nullptr, lc_back ? c->st_lc_meas : nullptr,
+                 c->ly.L > 0 ? c->st_rb_mask : nullptr, c->ly.L > 0 ? c->st_rb_meas : nullptr, iters,
+                 cov ? c->st_cov : nullptr, logdet ? c->st_logdet : nullptr, last_pose ? c->st_pose : nullptr);
+  if (rc) return rc;
+  if (cov) cudaMemcpyAsync(cov, c->st_cov, N * 9 * 4, cudaMemcpyDeviceToHost, c->stream);
+  if (logdet) cudaMemcpyAsync(logdet, c->st_logdet, N * 4, cudaMemcpyDeviceToHost, c->stream);
+  if (last_pose) cudaMemcpyAsync(last_pose, c->st_pose, N * 3 * 4, cudaMemcpyDeviceToHost, c->stream);
+  return check_cuda(c, "slam_step_host copies");
+}
+
+int slam_get_poses(slam_ctx* c, float* poses) {
+  if (!c || !poses) return SLAM_EINVAL;
+  const int threads = 128, blocks = (c->ly.N + threads - 1) / threads;
+  slam_poses_kernel<<<blocks, threads, 0, c->stream>>>(c->ly, c->state, c->head, c->count, poses);
+  c->launches++;
+  return check_cuda(c, "slam_poses_kernel");
+}
+
+int slam_get_landmarks(slam_ctx* c, float* lm, uint32_t* active) {
+  if (!c) return SLAM_EINVAL;
+  if (c->ly.L == 0) return SLAM_OK;
+  if (!lm || !active) return fail(c, SLAM_EINVAL, "lm/active are NULL");
+  const int threads = 128, blocks = (c->ly.N + threads - 1) / threads;
+  slam_landmarks_kernel<<<blocks, threads, 0, c->stream>>>(c->ly, c->state, lm, active);
+  c->launches++;
+  return check_cuda(c, "slam_landmarks_kernel");
+}
+
+int slam_get_status(slam_ctx* c, int32_t* status) {
+  if (!c || !status) return SLAM_EINVAL;
+  const int threads = 128, blocks = (c->ly.N + threads - 1) / threads;
+  slam_status_kernel<<<blocks, threads, 0, c->stream>>>(c->ly, c->state, status);
+  c->launches++;
+  return check_cuda(c, "slam_status_kernel");
+}
+
+int slam_count(const slam_ctx* c) { return c ? c->count : -1; }
+long long slam_launch_count(const slam_ctx* c) { return c ? c->launches : -1; }
+const char* slam_last_error(const slam_ctx* c) { return c ? c->err : "null context"; }
+
+int slam_kernel_info(const slam_ctx* c, int* smem_bytes_per_cta, int* warps_per_cta, int* ctas_per_sm) {
+  if (!c) return SLAM_EINVAL;
+  if (smem_bytes_per_cta) *smem_bytes_per_cta = c->smem_bytes;
+  if (warps_per_cta) *warps_per_cta = c->ly.wpc;
+  if (ctas_per_sm) *ctas_per_sm = c->ctas_per_sm;
+  return SLAM_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,1037 @@
+// Hand-written sm_100a kernels of the batched fixed-lag SE(2) smoother (one WARP per environment).
+//
+// Hot path: per environment and per step
+//   S0 push        dead-reckoned guess + factor bookkeeping
+//   S1 linearise   residuals + SE(2) Jacobians of every live factor              (eq. (5))
+//   S2 assemble    H = Lambda + sum J'Omega J, b, in shared memory, envelope (skyline) storage
+//   S3 factor      left-looking envelope Cholesky, lanes over rows; the rhs rides along as an extra
+//                  row (forward solve for free); back substitution; additive update
+//   S4 covariance  trailing 6x6 of L -> Sigma_t (global coords), ln det      (eq. (6))
+//   S5 marginalise re-anchor + Schur complement of the oldest pose on the prior's support
+//
+// Elimination order of the window variables (scalar offsets):
+//   [ e_1 .. e_{W-2} (chain, 3 each) | m_0 .. m_{L-1} (2 each) | newest pose e_{c-1} (3) | anchor a (3) ]
+// so that the covariance read-out needs only the trailing 6x6 of L, and the weakly determined
+// global anchor `a` (touched by the prior only) is never added into the well determined relative
+// blocks.  Row n (= 3W+2L) of the envelope storage is the right-hand side b.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "slam_layout.h"
+
+namespace slamk {
+
+enum { F_PUSH = 1, F_OBS0 = 2, F_COV = 4, F_MARG = 8, F_COPYCOV = 16 };
+enum { ENV_NOT_PD = 1, ENV_NONFINITE = 2 };
+
+struct StepIO {
+  const float* odom; const int32_t* lc_back; const float* lc_meas; const uint32_t* rb_mask; const float* rb_meas;
+  float* cov; float* logdet; float* dopt; float* last_pose;
+  float* cov_cache;  // [10][N]: 9 covariance entries + logdet
+};
+
+struct WS {  // per-warp views into shared memory
+  float* st; float* zodo; float* zlc; int* lct; float* cs; uint32_t* rbm;
+  int* first; int* rbase; int* LR; int* ssup; int* sidx; float* sds; float* H;
+};
+
+__device__ __forceinline__ WS make_ws(const Layout& ly, float* base) {
+  WS w;
+  w.st = base + ly.s_st; w.zodo = base + ly.s_zodo; w.zlc = base + ly.s_zlc;
+  w.lct = (int*)(base + ly.s_lct); w.cs = base + ly.s_cs; w.rbm = (uint32_t*)(base + ly.s_rbm);
+  w.first = (int*)(base + ly.s_first); w.rbase = (int*)(base + ly.s_rbase); w.LR = (int*)(base + ly.s_lr);
+  w.ssup = (int*)(base + ly.s_ssup); w.sidx = (int*)(base + ly.s_sidx); w.sds = base + ly.s_sds;
+  w.H = base + ly.s_H;
+  return w;
+}
+
+// ------------------------------------------------------------------ small helpers
+#define FULLMASK 0xffffffffu
+
+__device__ __forceinline__ float wrapf(float x) {  // to [-pi, pi], 2*pi split hi/lo
+  const float k = rintf(x * 0.15915494309189535f);
+  x = fmaf(-k, 6.2831854820251465f, x);
+  return fmaf(-k, -1.7484555e-7f, x);
+}
+__device__ __forceinline__ uint64_t lowmask(int k) { return k >= 64 ? ~0ull : ((1ull << k) - 1ull); }
+__device__ __forceinline__ uint64_t ring_to_slot(uint64_t ring, int head, int W) {
+  const uint64_t mW = lowmask(W);
+  ring &= mW;
+  if (head == 0) return ring;
+  return ((ring >> head) | (ring << (W - head))) & mW;
+}
+__device__ __forceinline__ uint64_t slot_to_ring(uint64_t slot, int head, int W) {
+  const uint64_t mW = lowmask(W);
+  slot &= mW;
+  if (head == 0) return slot;
+  return ((slot << head) | (slot >> (W - head))) & mW;
+}
+__device__ __forceinline__ int nth_set_bit(uint64_t m, int k) {  // k-th (0-based) set bit
+  const uint32_t lo = (uint32_t)m, hi = (uint32_t)(m >> 32);
+  const int plo = __popc(lo);
+  return k < plo ? (int)__fns(lo, 0, k + 1) : 32 + (int)__fns(hi, 0, k - plo + 1);
+}
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULLMASK, v, o);
+  return v;
+}
+
+__device__ __forceinline__ int ring_of(int slot, int head, int W) { int r = head + slot; return r >= W ? r - W : r; }
+// state array index
+__device__ __forceinline__ int st_pose(int k) { return 3 + 3 * k; }
+__device__ __forceinline__ int st_lm(const Layout& ly, int l) { return 3 + 3 * ly.W + 2 * l; }
+// elimination offsets
+__device__ __forceinline__ int off_new(const Layout& ly) { return 3 * (ly.W - 2) + 2 * ly.L; }
+__device__ __forceinline__ int off_a(const Layout& ly) { return 3 * (ly.W - 2) + 2 * ly.L + 3; }
+__device__ __forceinline__ int off_lm(const Layout& ly, int l) { return 3 * (ly.W - 2) + 2 * l; }
+__device__ __forceinline__ int off_slot(const Layout& ly, int k, int c) { return k == c - 1 ? off_new(ly) : 3 * (k - 1); }
+
+struct Masks {  // warp-uniform
+  uint64_t ps;   // prior support, pose SLOTS (bit k = slot k)
+  uint64_t ls;   // prior support, landmarks
+  uint64_t act;  // active landmarks
+};
+
+// ------------------------------------------------------------------ load / store of the record
+__device__ void load_env(const Layout& ly, const float* rec, const WS& w, int lane, int head, int c, Masks& mk) {
+  const int W = ly.W, L = ly.L;
+  const int* reci = (const int*)rec;
+  const uint32_t* recu = (const uint32_t*)rec;
+  if (lane < 3) w.st[lane] = rec[ly.o_a + lane];
+  for (int i = lane; i < 3 * W; i += 32) {
+    const int k = i / 3, j = i - 3 * k, r = ring_of(k, head, W);
+    const bool live = k < c;
+    w.st[3 + i] = (live && k > 0) ? rec[ly.o_e + 3 * r + j] : 0.0f;
+    w.zodo[i] = live ? rec[ly.o_zodo + 3 * r + j] : 0.0f;
+    w.zlc[i] = live ? rec[ly.o_zlc + 3 * r + j] : 0.0f;
+  }
+  for (int k = lane; k < W; k += 32) {
+    const int r = ring_of(k, head, W);
+    const int t = (k < c) ? reci[ly.o_lct + r] : -1;
+    int ts = -1;
+    if (t >= 0) { ts = t - head; if (ts < 0) ts += W; }
+    w.lct[k] = ts;
+    for (int q = 0; q < ly.nw; ++q) w.rbm[k * ly.nw + q] = (k < c) ? recu[ly.o_rbm + r * ly.nw + q] : 0u;
+  }
+  for (int i = lane; i < 2 * L; i += 32) w.st[3 + 3 * W + i] = rec[ly.o_m + i];
+  const uint64_t pm = (uint64_t)recu[ly.o_pm] | ((uint64_t)recu[ly.o_pm + 1] << 32);
+  mk.ps = ring_to_slot(pm, head, W);
+  mk.ls = (uint64_t)recu[ly.o_lm] | ((uint64_t)recu[ly.o_lm + 1] << 32);
+  mk.act = (uint64_t)recu[ly.o_act] | ((uint64_t)recu[ly.o_act + 1] << 32);
+  __syncwarp();
+}
+
+// writes a, e (ring positions of the CURRENT head), m, active mask
+__device__ void store_state(const Layout& ly, float* rec, const WS& w, int lane, int head, int c, const Masks& mk) {
+  const int W = ly.W, L = ly.L;
+  uint32_t* recu = (uint32_t*)rec;
+  if (lane < 3) rec[ly.o_a + lane] = w.st[lane];
+  for (int i = lane; i < 3 * c; i += 32) {
+    const int k = i / 3, j = i - 3 * k, r = ring_of(k, head, W);
+    rec[ly.o_e + 3 * r + j] = w.st[3 + i];
+  }
+  for (int i = lane; i < 2 * L; i += 32) rec[ly.o_m + i] = w.st[3 + 3 * W + i];
+  if (lane == 0) { recu[ly.o_act] = (uint32_t)mk.act; recu[ly.o_act + 1] = (uint32_t)(mk.act >> 32); }
+}
+
+// ------------------------------------------------------------------ S0 push / observe
+// Range-bearing bookkeeping for the pose in `slot` (pose px,py,pth in the anchor frame).
+__device__ void record_rb(const Layout& ly, float* rec, const WS& w, int lane, int env, int head, int slot,
+                          float px, float py, float pth, const StepIO& io, Masks& mk) {
+  const int L = ly.L, N = ly.N, r = ring_of(slot, head, ly.W);
+  uint32_t* recu = (uint32_t*)rec;
+  uint64_t act = mk.act;
+  for (int base = 0; base < L; base += 32) {
+    const int l = base + lane;
+    const uint32_t word = io.rb_mask[(size_t)(base >> 5) * N + env];
+    const bool vis = l < L && ((word >> lane) & 1u);
+    if (l < L) {
+      const float zr = io.rb_meas[(size_t)l * N + env];
+      const float zb = io.rb_meas[(size_t)(L + l) * N + env];
+      rec[ly.o_zrb + (r * 2 + 0) * L + l] = zr;
+      rec[ly.o_zrb + (r * 2 + 1) * L + l] = zb;
+      if (vis && !((act >> l) & 1ull)) {  // R6: inverse projection from the observing pose's guess
+        float sn, cn;
+        sincosf(pth + zb, &sn, &cn);
+        w.st[st_lm(ly, l)] = px + zr * cn;
+        w.st[st_lm(ly, l) + 1] = py + zr * sn;
+      }
+    }
+    const uint64_t wm = (uint64_t)(L - base >= 32 ? word : (word & ((1u << (L - base)) - 1u)));
+    if (lane == 0) {
+      w.rbm[slot * ly.nw + (base >> 5)] = (uint32_t)wm;
+      recu[ly.o_rbm + r * ly.nw + (base >> 5)] = (uint32_t)wm;
+    }
+    act |= wm << base;
+  }
+  mk.act = act;
+  __syncwarp();
+}
+
+// Appends slot c (count before the push).  Returns the new count.
+__device__ int push_env(const Layout& ly, float* rec, const WS& w, int lane, int env, int head, int c,
+                        const StepIO& io, Masks& mk) {
+  const int W = ly.W, N = ly.N, r = ring_of(c, head, W);
+  int* reci = (int*)rec;
+  const float zx = io.odom[env], zy = io.odom[(size_t)N + env], zt = io.odom[2 * (size_t)N + env];
+  const float* p = w.st + st_pose(c - 1);  // slot 0 is stored as zeros
+  const float pxo = p[0], pyo = p[1], pto = p[2];
+  float sn, cn;
+  sincosf(pto, &sn, &cn);
+  const float nx = pxo + cn * zx - sn * zy, ny = pyo + sn * zx + cn * zy, nt = wrapf(pto + zt);
+  int back = io.lc_back ? io.lc_back[env] : 0;
+  const int tgt = (back >= 1 && back <= c) ? c - back : -1;  // R11
+  __syncwarp();
+  if (lane == 0) {
+    float* q = w.st + st_pose(c);
+    q[0] = nx; q[1] = ny; q[2] = nt;
+    w.lct[c] = tgt;
+    reci[ly.o_lct + r] = tgt < 0 ? -1 : ring_of(tgt, head, W);
+  }
+  if (lane < 3) {
+    const float z = lane == 0 ? zx : (lane == 1 ? zy : zt);
+    w.zodo[3 * c + lane] = z;
+    rec[ly.o_zodo + 3 * r + lane] = z;
+    const float zl = io.lc_meas ? io.lc_meas[(size_t)lane * N + env] : 0.0f;
+    w.zlc[3 * c + lane] = zl;
+    rec[ly.o_zlc + 3 * r + lane] = zl;
+  }
+  __syncwarp();
+  if (ly.L > 0) record_rb(ly, rec, w, lane, env, head, c, nx, ny, nt, io, mk);
+  return c + 1;
+}
+
+// ------------------------------------------------------------------ prior support tables
+// For support scalar p (canonical order [a | poses by slot | landmarks]): elimination offset in
+// ssup[p], state index in sidx[p] (bit 16 set for angle components).  Returns the support dimension.
+__device__ int build_support(const Layout& ly, const WS& w, int lane, int c, uint64_t ps, uint64_t ls) {
+  const int npo = __popcll(ps), nlo = __popcll(ls);
+  const int s = 3 + 3 * npo + 2 * nlo;
+  for (int p = lane; p < s; p += 32) {
+    int off, idx;
+    if (p < 3) { off = off_a(ly) + p; idx = p | (p == 2 ? 0x10000 : 0); }
+    else if (p < 3 + 3 * npo) {
+      const int b = (p - 3) / 3, j = (p - 3) - 3 * b, k = nth_set_bit(ps, b);
+      off = off_slot(ly, k, c) + j; idx = (st_pose(k) + j) | (j == 2 ? 0x10000 : 0);
+    } else {
+      const int q = p - 3 - 3 * npo, b = q >> 1, j = q & 1, l = nth_set_bit(ls, b);
+      off = off_lm(ly, l) + j; idx = st_lm(ly, l) + j;
+    }
+    w.ssup[p] = off; w.sidx[p] = idx;
+  }
+  __syncwarp();
+  return s;
+}
+
+// ------------------------------------------------------------------ symbolic phase: envelope of H
+// first[i] = first column of row i inside the envelope; rbase[i] + j addresses H(i,j), j >= first[i];
+// LR = sorted list of "long" rows (i - first[i] > 5, plus the rhs row n).  Returns total words used.
+__device__ int symbolic(const Layout& ly, const WS& w, int lane, int c, const Masks& mk, int s, int& nLR) {
+  const int W = ly.W, L = ly.L, n = ly.n;
+  const int oN = off_new(ly), oA = off_a(ly), oL = off_lm(ly, 0);
+  // own block offsets
+  for (int i = lane; i <= n; i += 32) {
+    int f;
+    if (i < oL) f = (i / 3) * 3;
+    else if (i < oN) f = oL + ((i - oL) >> 1) * 2;
+    else if (i < oA) f = oN;
+    else if (i < n) f = oA;
+    else f = 0;
+    w.first[i] = f;
+  }
+  __syncwarp();
+  // pose rows
+  for (int k = 1 + lane; k < c; k += 32) {
+    const int o = off_slot(ly, k, c);
+    int f = o;
+    if (k >= 2) f = min(f, off_slot(ly, k - 1, c));
+    const int t = w.lct[k];
+    if (t >= 1) f = min(f, off_slot(ly, t, c));
+    if (k == c - 1 && L > 0) {  // newest pose comes after the landmarks it observes
+      uint64_t m = (uint64_t)w.rbm[k * ly.nw];
+      if (ly.nw > 1) m |= (uint64_t)w.rbm[k * ly.nw + 1] << 32;
+      if (m) f = min(f, off_lm(ly, __ffsll((long long)m) - 1));
+    }
+    w.first[o] = f; w.first[o + 1] = f; w.first[o + 2] = f;
+  }
+  // landmark rows: first chain pose (slots 1..c-2) that observes them
+  for (int l = lane; l < L; l += 32) {
+    const int o = off_lm(ly, l);
+    int f = o;
+    for (int k = 1; k <= c - 2; ++k)
+      if ((w.rbm[k * ly.nw + (l >> 5)] >> (l & 31)) & 1u) { f = 3 * (k - 1); break; }
+    w.first[o] = f; w.first[o + 1] = f;
+  }
+  __syncwarp();
+  // prior: all support blocks are mutually coupled
+  if (s > 3) {
+    int fs = n;
+    for (int p = 3 + lane; p < s; p += 32) fs = min(fs, w.ssup[p]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) fs = min(fs, __shfl_xor_sync(FULLMASK, fs, o));
+    for (int p = lane; p < s; p += 32) { const int i = w.ssup[p]; w.first[i] = min(w.first[i], fs); }
+  }
+  __syncwarp();
+  // rows of a block must share `first` (min over the block) -- they do by construction, except
+  // that support scalars were updated one by one with the same fs, which keeps them equal.
+  // prefix sum of row lengths -> rbase; long-row list
+  int run = 0, cnt = 0;
+  for (int base = 0; base <= n; base += 32) {
+    const int i = base + lane;
+    const int f = (i <= n) ? w.first[i] : 0;
+    const int len = (i <= n) ? (i - f + 1) : 0;
+    int x = len;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(FULLMASK, x, o); if (lane >= o) x += y; }
+    if (i <= n) w.rbase[i] = run + x - len - f;
+    const bool lng = (i <= n) && ((i - f > 5) || i == n);
+    const uint32_t bal = __ballot_sync(FULLMASK, lng);
+    if (lng) w.LR[cnt + __popc(bal & ((1u << lane) - 1u))] = i;
+    cnt += __popc(bal);
+    run += __shfl_sync(FULLMASK, x, 31);
+  }
+  nLR = cnt;
+  __syncwarp();
+  return run;
+}
+
+// ------------------------------------------------------------------ S1 + S2: linearise and assemble
+struct Between {  // residual and the pieces of J_i, J_j of a between factor (A.2)
+  float r[3], c, s, hx, hy;
+};
+__device__ __forceinline__ Between between_eval(const float* pi, float ci, float si, const float* pj, const float* z) {
+  Between b;
+  const float dx = pj[0] - pi[0], dy = pj[1] - pi[1];
+  b.c = ci; b.s = si;
+  b.hx = ci * dx + si * dy; b.hy = -si * dx + ci * dy;
+  b.r[0] = b.hx - z[0]; b.r[1] = b.hy - z[1]; b.r[2] = wrapf(pj[2] - pi[2] - z[2]);
+  return b;
+}
+// J_j = [[c,s,0],[-s,c,0],[0,0,1]],  J_i = [[-c,-s,hy],[s,-c,-hx],[0,0,-1]]
+__device__ __forceinline__ void between_jac(const Between& b, float Ji[3][3], float Jj[3][3]) {
+  Jj[0][0] = b.c; Jj[0][1] = b.s; Jj[0][2] = 0.f;
+  Jj[1][0] = -b.s; Jj[1][1] = b.c; Jj[1][2] = 0.f;
+  Jj[2][0] = 0.f; Jj[2][1] = 0.f; Jj[2][2] = 1.f;
+  Ji[0][0] = -b.c; Ji[0][1] = -b.s; Ji[0][2] = b.hy;
+  Ji[1][0] = b.s; Ji[1][1] = -b.c; Ji[1][2] = -b.hx;
+  Ji[2][0] = 0.f; Ji[2][1] = 0.f; Ji[2][2] = -1.f;
+}
+
+// H(rowblock oj, colblock oi) += Jj' Om Ji (full 3x3), H(oj,oj) += Jj' Om Jj (lower), b(oj) -= Jj' Om r
+__device__ __forceinline__ void add_j_side(const WS& w, int n, int oj, int oi, const float Ji[3][3], const float Jj[3][3],
+                                           const float* om, const float* r, bool has_i) {
+  float* rhs = w.H + w.rbase[n];
+#pragma unroll
+  for (int x = 0; x < 3; ++x) {
+    float* row = w.H + w.rbase[oj + x];
+    float g = 0.f;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) g = fmaf(Jj[k][x] * om[k], r[k], g);
+    rhs[oj + x] -= g;
+#pragma unroll
+    for (int y = 0; y <= x; ++y) {
+      float h = 0.f;
+#pragma unroll
+      for (int k = 0; k < 3; ++k) h = fmaf(Jj[k][x] * om[k], Jj[k][y], h);
+      row[oj + y] += h;
+    }
+    if (has_i) {
+#pragma unroll
+      for (int y = 0; y < 3; ++y) {
+        float h = 0.f;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) h = fmaf(Jj[k][x] * om[k], Ji[k][y], h);
+        row[oi + y] += h;
+      }
+    }
+  }
+}
+__device__ __forceinline__ void acc_i_side(const float Ji[3][3], const float* om, const float* r, float Hii[6], float gi[3]) {
+  int t = 0;
+#pragma unroll
+  for (int x = 0; x < 3; ++x) {
+#pragma unroll
+    for (int k = 0; k < 3; ++k) gi[x] = fmaf(Ji[k][x] * om[k], r[k], gi[x]);
+#pragma unroll
+    for (int y = 0; y <= x; ++y) {
+#pragma unroll
+      for (int k = 0; k < 3; ++k) Hii[t] = fmaf(Ji[k][x] * om[k], Ji[k][y], Hii[t]);
+      ++t;
+    }
+  }
+}
+__device__ __forceinline__ void add_i_side(const WS& w, int n, int oi, const float Hii[6], const float gi[3]) {
+  float* rhs = w.H + w.rbase[n];
+  int t = 0;
+#pragma unroll
+  for (int x = 0; x < 3; ++x) {
+    float* row = w.H + w.rbase[oi + x];
+    rhs[oi + x] -= gi[x];
+#pragma unroll
+    for (int y = 0; y <= x; ++y) row[oi + y] += Hii[t++];
+  }
+}
+
+// Builds H and b (row n) at the current state.  `s` = prior support dimension.
+__device__ void assemble(const Layout& ly, const Params& pr, const float* rec, const WS& w, int lane, int head, int c,
+                         const Masks& mk, int s, int total) {
+  const int W = ly.W, L = ly.L, n = ly.n;
+  for (int t = lane; t < total; t += 32) w.H[t] = 0.f;
+  // cos/sin of every live pose (slot 0 is the frame itself)
+  for (int k = lane; k < c; k += 32) {
+    float sn = 0.f, cn = 1.f;
+    if (k > 0) sincosf(w.st[st_pose(k) + 2], &sn, &cn);
+    w.cs[2 * k] = cn; w.cs[2 * k + 1] = sn;
+  }
+  // prior displacement d = v - vbar on the support (angles wrapped)
+  for (int p = lane; p < s; p += 32) {
+    const int id = w.sidx[p];
+    float d = w.st[id & 0xffff] - rec[ly.o_vbar + p];
+    if (id & 0x10000) d = wrapf(d);
+    w.sds[p] = d;
+  }
+  __syncwarp();
+  // identity rows for unused chain slots, the unused newest slot (c == 1) and inactive landmarks
+  for (int i = lane; i < n; i += 32) {
+    bool unused;
+    if (i < 3 * (W - 2)) unused = (i / 3 + 1) > c - 2;
+    else if (i < off_new(ly)) unused = !((mk.act >> ((i - 3 * (W - 2)) >> 1)) & 1ull);
+    else if (i < off_a(ly)) unused = c < 2;
+    else unused = false;
+    if (unused) w.H[w.rbase[i] + i] = 1.0f;
+  }
+  // prior: H += Lambda (row by row, coalesced over the packed lower triangle)
+  {
+    const float* lam = rec + ly.o_lam;
+    for (int p = 0; p < s; ++p) {
+      const int ip = w.ssup[p];
+      const float* lrow = lam + (p * (p + 1) >> 1);
+      for (int q = lane; q <= p; q += 32) {
+        const int iq = w.ssup[q];
+        const float v = lrow[q];
+        const int hi = max(ip, iq), lo = min(ip, iq);
+        w.H[w.rbase[hi] + lo] += v;
+      }
+    }
+    // b -= Lambda d + g
+    float* rhs = w.H + w.rbase[n];
+    for (int p = lane; p < s; p += 32) {
+      float acc = rec[ly.o_g + p];
+      const float* lrow = lam + (p * (p + 1) >> 1);
+      for (int q = 0; q <= p; ++q) acc = fmaf(lrow[q], w.sds[q], acc);
+      for (int q = p + 1; q < s; ++q) acc = fmaf(lam[(q * (q + 1) >> 1) + p], w.sds[q], acc);
+      rhs[w.ssup[p]] -= acc;
+    }
+  }
+  __syncwarp();
+  // odometry factors k-1 -> k: phase A (j side), phase B (i side)
+  for (int pass = 0; pass < 2; ++pass) {
+    for (int k = 1 + lane; k < c; k += 32) {
+      const float* pi = w.st + st_pose(k - 1);
+      const float* pj = w.st + st_pose(k);
+      const Between b = between_eval(pi, w.cs[2 * (k - 1)], w.cs[2 * (k - 1) + 1], pj, w.zodo + 3 * k);
+      float Ji[3][3], Jj[3][3];
+      between_jac(b, Ji, Jj);
+      if (pass == 0) {
+        add_j_side(w, n, off_slot(ly, k, c), k >= 2 ? off_slot(ly, k - 1, c) : 0, Ji, Jj, pr.om_odo, b.r, k >= 2);
+      } else if (k >= 2) {
+        float Hii[6] = {0, 0, 0, 0, 0, 0}, gi[3] = {0, 0, 0};
+        acc_i_side(Ji, pr.om_odo, b.r, Hii, gi);
+        add_i_side(w, n, off_slot(ly, k - 1, c), Hii, gi);
+      }
+    }
+    __syncwarp();
+  }
+  // loop closures t -> k: phase C (j side: at most one per k), phase D (i side: lane per target)
+  for (int k = 1 + lane; k < c; k += 32) {
+    const int t = w.lct[k];
+    if (t < 0) continue;
+    const Between b = between_eval(w.st + st_pose(t), w.cs[2 * t], w.cs[2 * t + 1], w.st + st_pose(k), w.zlc + 3 * k);
+    float Ji[3][3], Jj[3][3];
+    between_jac(b, Ji, Jj);
+    add_j_side(w, n, off_slot(ly, k, c), t >= 1 ? off_slot(ly, t, c) : 0, Ji, Jj, pr.om_lc, b.r, t >= 1);
+  }
+  __syncwarp();
+  for (int t = 1 + lane; t < c - 1; t += 32) {
+    float Hii[6] = {0, 0, 0, 0, 0, 0}, gi[3] = {0, 0, 0};
+    bool any = false;
+    for (int k = t + 1; k < c; ++k) {
+      if (w.lct[k] != t) continue;
+      const Between b = between_eval(w.st + st_pose(t), w.cs[2 * t], w.cs[2 * t + 1], w.st + st_pose(k), w.zlc + 3 * k);
+      float Ji[3][3], Jj[3][3];
+      between_jac(b, Ji, Jj);
+      acc_i_side(Ji, pr.om_lc, b.r, Hii, gi);
+      any = true;
+    }
+    if (any) add_i_side(w, n, off_slot(ly, t, c), Hii, gi);
+  }
+  __syncwarp();
+  // range-bearing factors: lanes over landmarks, loop over slots; pose-side sums by warp shuffles
+  if (L > 0) {
+    float* rhs = w.H + w.rbase[n];
+    const float w0 = pr.om_rb[0], w1 = pr.om_rb[1];
+    for (int base = 0; base < L; base += 32) {
+      const int l = base + lane;
+      const bool inl = l < L;
+      const float mx = inl ? w.st[st_lm(ly, l)] : 0.f, my = inl ? w.st[st_lm(ly, l) + 1] : 0.f;
+      float Lxx = 0.f, Lxy = 0.f, Lyy = 0.f, gx = 0.f, gy = 0.f;
+      const int ol = off_lm(ly, inl ? l : 0);
+      for (int k = 0; k < c; ++k) {
+        const uint32_t word = w.rbm[k * ly.nw + (base >> 5)];
+        if (word == 0u) continue;  // warp-uniform
+        const bool vis = inl && ((word >> lane) & 1u);
+        const int r = ring_of(k, head, W);
+        float P[6] = {0, 0, 0, 0, 0, 0}, gp[3] = {0, 0, 0};
+        if (vis) {
+          const float zr = rec[ly.o_zrb + (r * 2 + 0) * L + l], zb = rec[ly.o_zrb + (r * 2 + 1) * L + l];
+          const float* p = w.st + st_pose(k);
+          const float dx = mx - p[0], dy = my - p[1];
+          const float q = dx * dx + dy * dy, irho = rsqrtf(q), rho = q * irho, iq = irho * irho;
+          const float r0 = rho - zr, r1 = wrapf(atan2f(dy, dx) - p[2] - zb);
+          // J_l = [[ux, uy], [-dy/q, dx/q]],  J_p = [[-ux, -uy, 0], [dy/q, -dx/q, -1]]
+          const float ux = dx * irho, uy = dy * irho, vx = -dy * iq, vy = dx * iq;
+          const float a0 = w0 * ux, a1 = w0 * uy, b0 = w1 * vx, b1 = w1 * vy;
+          Lxx += a0 * ux + b0 * vx; Lxy += a0 * uy + b0 * vy; Lyy += a1 * uy + b1 * vy;
+          gx += a0 * r0 + b0 * r1; gy += a1 * r0 + b1 * r1;
+          if (k > 0) {
+            // cross block J_l' Om J_p (2x3): rows landmark (x,y), cols pose (x,y,th)
+            const float c00 = -(a0 * ux + b0 * vx), c01 = -(a0 * uy + b0 * vy), c02 = -b0;
+            const float c10 = -(a1 * ux + b1 * vx), c11 = -(a1 * uy + b1 * vy), c12 = -b1;
+            const int op = off_slot(ly, k, c);
+            if (op < ol) {  // chain pose: landmark rows, pose columns
+              float* r0p = w.H + w.rbase[ol];
+              float* r1p = w.H + w.rbase[ol + 1];
+              r0p[op] += c00; r0p[op + 1] += c01; r0p[op + 2] += c02;
+              r1p[op] += c10; r1p[op + 1] += c11; r1p[op + 2] += c12;
+            } else {        // newest pose: pose rows, landmark columns
+              w.H[w.rbase[op] + ol] += c00; w.H[w.rbase[op] + ol + 1] += c10;
+              w.H[w.rbase[op + 1] + ol] += c01; w.H[w.rbase[op + 1] + ol + 1] += c11;
+              w.H[w.rbase[op + 2] + ol] += c02; w.H[w.rbase[op + 2] + ol + 1] += c12;
+            }
+            // pose diagonal J_p' Om J_p (lower: xx, yx, yy, tx, ty, tt) and gradient
+            P[0] = a0 * ux + b0 * vx; P[1] = a1 * ux + b1 * vx; P[2] = a1 * uy + b1 * vy;
+            P[3] = b0; P[4] = b1; P[5] = w1;
+            gp[0] = -(a0 * r0 + b0 * r1); gp[1] = -(a1 * r0 + b1 * r1); gp[2] = -w1 * r1;
+          }
+        }
+        if (k > 0) {
+#pragma unroll
+          for (int t = 0; t < 6; ++t) P[t] = warp_sum(P[t]);
+#pragma unroll
+          for (int t = 0; t < 3; ++t) gp[t] = warp_sum(gp[t]);
+          if (lane == 0) {
+            const int op = off_slot(ly, k, c);
+            float* q0 = w.H + w.rbase[op];
+            float* q1 = w.H + w.rbase[op + 1];
+            float* q2 = w.H + w.rbase[op + 2];
+            q0[op] += P[0]; q1[op] += P[1]; q1[op + 1] += P[2];
+            q2[op] += P[3]; q2[op + 1] += P[4]; q2[op + 2] += P[5];
+            rhs[op] -= gp[0]; rhs[op + 1] -= gp[1]; rhs[op + 2] -= gp[2];
+          }
+        }
+        __syncwarp();
+      }
+      if (inl && ((mk.act >> l) & 1ull)) {
+        float* r0p = w.H + w.rbase[ol];
+        float* r1p = w.H + w.rbase[ol + 1];
+        r0p[ol] += Lxx; r1p[ol] += Lxy; r1p[ol + 1] += Lyy;
+        rhs[ol] -= gx; rhs[ol + 1] -= gy;
+      }
+      __syncwarp();
+    }
+  }
+}
+
+// ------------------------------------------------------------------ S3: envelope Cholesky + solves
+// Left-looking by columns, lanes over the rows of the column's structure: lane 0 owns the diagonal
+// row j, lanes 1..5 the short rows j+1..j+5, lanes 6..31 the long rows (LR) below j.  The diagonal
+// slot stores 1/L_jj.  Row n carries b, so on exit row n holds y = L^{-1} b.
+__device__ int cholesky(const Layout& ly, const WS& w, int lane, int nLR) {
+  const int n = ly.n;
+  int flag = 0;
+  int p = 0;  // first LR entry with row > j
+  for (int j = 0; j < n; ++j) {
+    const int fj = w.first[j];
+    const float* rowj = w.H + w.rbase[j];
+    while (p < nLR && w.LR[p] <= j) ++p;
+    float dj = 0.f;
+    for (int q0 = p - 6; q0 < nLR; q0 += 32) {  // first pass: lanes 0..5 near rows, 6.. long rows
+      int i = -1;
+      const bool first_pass = (q0 == p - 6);
+      if (first_pass && lane < 6) {
+        const int ii = j + lane;
+        if (ii < n) {
+          const int fi = w.first[ii];
+          if (lane == 0 || (ii - fi <= 5 && fi <= j)) i = ii;
+        }
+      } else {
+        const int q = q0 + lane;
+        if (q >= p && q < nLR) { const int ii = w.LR[q]; if (w.first[ii] <= j) i = ii; }
+      }
+      float acc = 0.f;
+      float* rowi = nullptr;
+      if (i >= 0) {
+        rowi = w.H + w.rbase[i];
+        acc = rowi[j];
+        const int k0 = max(w.first[i], fj);
+        for (int k = k0; k < j; ++k) acc = fmaf(-rowi[k], rowj[k], acc);
+      }
+      if (first_pass) {
+        const float dg = __shfl_sync(FULLMASK, acc, 0);
+        if (!(dg > 0.f)) { flag |= ENV_NOT_PD; dj = 1.0f; }
+        else dj = rsqrtf(dg);
+      }
+      __syncwarp();
+      if (i >= 0) rowi[j] = (first_pass && lane == 0) ? dj : acc * dj;
+    }
+    __syncwarp();
+  }
+  return flag;
+}
+
+// Solves L' delta = y in place in row n (column-oriented: lanes over the row being eliminated).
+__device__ void back_substitute(const Layout& ly, const WS& w, int lane) {
+  const int n = ly.n;
+  float* y = w.H + w.rbase[n];
+  for (int i = n - 1; i >= 0; --i) {
+    const float* rowi = w.H + w.rbase[i];
+    const float d = y[i] * rowi[i];
+    __syncwarp();
+    if (lane == 0) y[i] = d;
+    for (int k = w.first[i] + lane; k < i; k += 32) y[k] = fmaf(-rowi[k], d, y[k]);
+    __syncwarp();
+  }
+}
+
+// v <- v + delta (R1: additive, angles wrapped).  Returns ENV_NONFINITE if the update is not finite.
+__device__ int apply_update(const Layout& ly, const WS& w, int lane, int c, const Masks& mk) {
+  const int W = ly.W, L = ly.L, n = ly.n;
+  const float* dl = w.H + w.rbase[n];
+  int bad = 0;
+  if (lane < 3) {
+    const float d = dl[off_a(ly) + lane];
+    bad |= !isfinite(d);
+    const float v = w.st[lane] + d;
+    w.st[lane] = lane == 2 ? wrapf(v) : v;
+  }
+  for (int i = lane; i < 3 * (c - 1); i += 32) {
+    const int k = 1 + i / 3, j = i - 3 * (k - 1);
+    const float d = dl[off_slot(ly, k, c) + j];
+    bad |= !isfinite(d);
+    const float v = w.st[st_pose(k) + j] + d;
+    w.st[st_pose(k) + j] = j == 2 ? wrapf(v) : v;
+  }
+  for (int i = lane; i < 2 * L; i += 32) {
+    if (!((mk.act >> (i >> 1)) & 1ull)) continue;
+    const float d = dl[off_lm(ly, 0) + i];
+    bad |= !isfinite(d);
+    w.st[3 + 3 * W + i] += d;
+  }
+  bad = __any_sync(FULLMASK, bad);
+  __syncwarp();
+  return bad ? ENV_NONFINITE : 0;
+}
+
+// ------------------------------------------------------------------ S4: covariance of the newest pose
+// Sigma_6 = (L_t L_t')^{-1} from the trailing 6x6 of L (variables: newest pose e, anchor a), then
+// Sigma_t = J Sigma_6 J' with x = a (+) e (A.4).  O(1) per environment, done in fp64 by lane 0.
+__device__ void covariance(const Layout& ly, const WS& w, int lane, int env, int c, const StepIO& io) {
+  if (lane != 0) return;
+  const int n = ly.n, N = ly.N;
+  double S[3][3];
+  if (c == 1) {
+    // only the anchor exists: Sigma = (L_a L_a')^{-1}
+    double Li[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+    double Lm[3][3];
+    for (int x = 0; x < 3; ++x) {
+      const int i = n - 3 + x;
+      for (int y = 0; y <= x; ++y) Lm[x][y] = (y == x) ? 1.0 / (double)w.H[w.rbase[i] + i] : (double)w.H[w.rbase[i] + n - 3 + y];
+    }
+    for (int col = 0; col < 3; ++col)
+      for (int x = col; x < 3; ++x) {
+        double sum = (x == col) ? 1.0 : 0.0;
+        for (int k = col; k < x; ++k) sum -= Lm[x][k] * Li[k][col];
+        Li[x][col] = sum / Lm[x][x];
+      }
+    for (int x = 0; x < 3; ++x)
+      for (int y = 0; y < 3; ++y) {
+        double sum = 0.0;
+        for (int k = 0; k < 3; ++k) sum += Li[k][x] * Li[k][y];
+        S[x][y] = sum;
+      }
+  } else {
+    double Lm[6][6], Li[6][6];
+    for (int x = 0; x < 6; ++x) {
+      const int i = n - 6 + x;
+      const int fi = w.first[i];
+      for (int y = 0; y < 6; ++y) { Lm[x][y] = 0.0; Li[x][y] = 0.0; }
+      for (int y = 0; y <= x; ++y) {
+        const int j = n - 6 + y;
+        if (y == x) Lm[x][y] = 1.0 / (double)w.H[w.rbase[i] + i];
+        else if (j >= fi) Lm[x][y] = (double)w.H[w.rbase[i] + j];
+      }
+    }
+    for (int col = 0; col < 6; ++col)
+      for (int x = col; x < 6; ++x) {
+        double sum = (x == col) ? 1.0 : 0.0;
+        for (int k = col; k < x; ++k) sum -= Lm[x][k] * Li[k][col];
+        Li[x][col] = sum / Lm[x][x];
+      }
+    double S6[6][6];
+    for (int x = 0; x < 6; ++x)
+      for (int y = 0; y < 6; ++y) {
+        double sum = 0.0;
+        for (int k = (x > y ? x : y); k < 6; ++k) sum += Li[k][x] * Li[k][y];
+        S6[x][y] = sum;
+      }
+    // J = [J_e | J_a], J_e = blockdiag(Rot(a_th), 1), J_a = [[1,0,-dy],[0,1,dx],[0,0,1]], d = Rot(a_th) t_e
+    const double ath = (double)w.st[2];
+    const double ca = cos(ath), sa = sin(ath);
+    const float* e = w.st + st_pose(c - 1);
+    const double dx = ca * e[0] - sa * e[1], dy = sa * e[0] + ca * e[1];
+    double J[3][6] = {{ca, -sa, 0, 1, 0, -dy}, {sa, ca, 0, 0, 1, dx}, {0, 0, 1, 0, 0, 1}};
+    for (int x = 0; x < 3; ++x)
+      for (int y = 0; y < 3; ++y) {
+        double sum = 0.0;
+        for (int p2 = 0; p2 < 6; ++p2) {
+          double t = 0.0;
+          for (int q = 0; q < 6; ++q) t += S6[p2][q] * J[y][q];
+          sum += J[x][p2] * t;
+        }
+        S[x][y] = sum;
+      }
+  }
+  for (int x = 0; x < 3; ++x)  // R20
+    for (int y = x + 1; y < 3; ++y) { const double t = 0.5 * (S[x][y] + S[y][x]); S[x][y] = t; S[y][x] = t; }
+  const double det = S[0][0] * (S[1][1] * S[2][2] - S[1][2] * S[2][1]) - S[0][1] * (S[1][0] * S[2][2] - S[1][2] * S[2][0]) +
+                     S[0][2] * (S[1][0] * S[2][1] - S[1][1] * S[2][0]);
+  const double ld = log(det);
+  for (int x = 0; x < 3; ++x)
+    for (int y = 0; y < 3; ++y) {
+      const float v = (float)S[x][y];
+      io.cov_cache[(size_t)(3 * x + y) * N + env] = v;
+      if (io.cov) io.cov[(size_t)(3 * x + y) * N + env] = v;
+    }
+  io.cov_cache[(size_t)9 * N + env] = (float)ld;
+  if (io.logdet) io.logdet[env] = (float)ld;
+  if (io.dopt) io.dopt[env] = (float)exp(ld / 3.0);
+}
+
+// ------------------------------------------------------------------ S5: marginalise the oldest pose
+// Works on the SUPPORT of the sub-problem only (old prior + factors touching slot 0), dimension s:
+//   H_s, gamma_s  ->  congruence with N = dv/du = E + X P_w'  (E block diagonal, X the w-column)
+//   ->  Schur complement over w = e_1  ->  (Lambda', g', vbar') on the support without w.
+// Block order of the support: [a | pose slots ascending (slot 1 = w first) | landmarks ascending].
+struct Etype { float p, q, u, v; };  // E = [[p,-q,u],[q,p,v],[0,0,1]]
+
+__device__ __forceinline__ int tri(int i, int j) { return (i * (i + 1) >> 1) + j; }  // i >= j
+__device__ __forceinline__ float sym_get(const float* Hs, int i, int j) { return i >= j ? Hs[tri(i, j)] : Hs[tri(j, i)]; }
+
+__device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const WS& w, int lane, int head, int c,
+                           Masks& mk, int s_old) {
+  const int W = ly.W, L = ly.L;
+  int* reci = (int*)rec;
+  uint32_t* recu = (uint32_t*)rec;
+  // --- A. new support masks
+  uint64_t lc0 = 0ull;
+  for (int base = 0; base < c; base += 32) {
+    const int k = base + lane;
+    const uint32_t bal = __ballot_sync(FULLMASK, k >= 1 && k < c && w.lct[k] == 0);
+    lc0 |= (uint64_t)bal << base;
+  }
+  uint64_t rb0 = 0ull;
+  if (L > 0) { rb0 = (uint64_t)w.rbm[0]; if (ly.nw > 1) rb0 |= (uint64_t)w.rbm[1] << 32; }
+  const uint64_t nps = mk.ps | 2ull | lc0, nls = mk.ls | rb0;
+  const int npn = __popcll(nps), nln = __popcll(nls);
+  const int s = 3 + 3 * npn + 2 * nln, nbk = 1 + npn + nln;
+  const int npo = __popcll(mk.ps);
+  if ((s * (s + 1) >> 1) + 8 * s > ly.cap) return 4;  // cannot happen with the dense capacity
+  float* Hs = w.H;
+  float* gam = Hs + (s * (s + 1) >> 1);
+  float* X = gam + s;
+  float* Q = X + 3 * s;
+  int* omap = (int*)(Q + 3 * s);
+  int* nidx = w.ssup;  // elimination offsets are dead from here on
+
+  // --- B. old displacement d, old -> new scalar map, new state-index table
+  for (int p = lane; p < s_old; p += 32) {
+    const int id = w.sidx[p];
+    float d = w.st[id & 0xffff] - rec[ly.o_vbar + p];
+    if (id & 0x10000) d = wrapf(d);
+    w.sds[p] = d;
+    int P;
+    if (p < 3) P = p;
+    else if (p < 3 + 3 * npo) {
+      const int b = (p - 3) / 3, j = (p - 3) - 3 * b, k = nth_set_bit(mk.ps, b);
+      P = 3 + 3 * __popcll(nps & lowmask(k)) + j;
+    } else {
+      const int q = p - 3 - 3 * npo, b = q >> 1, j = q & 1, l = nth_set_bit(mk.ls, b);
+      P = 3 + 3 * npn + 2 * __popcll(nls & lowmask(l)) + j;
+    }
+    omap[p] = P;
+  }
+  for (int t = lane; t < (s * (s + 1) >> 1) + s; t += 32) Hs[t] = 0.f;  // Hs and gam
+  __syncwarp();
+  const float a_th = w.st[2];
+  float sa, ca;
+  sincosf(a_th, &sa, &ca);
+  const float x1 = w.st[st_pose(1)], y1 = w.st[st_pose(1) + 1], th1 = w.st[st_pose(1) + 2];
+  float s1, c1;
+  sincosf(th1, &s1, &c1);
+  const float ddx = ca * x1 - sa * y1, ddy = sa * x1 + ca * y1;  // d = Rot(a_th) t_1
+  // new tables + X rows (step E)
+  for (int p = lane; p < s; p += 32) {
+    int id;
+    float X0, X1, X2;
+    if (p < 3) {
+      id = p | (p == 2 ? 0x10000 : 0);
+      // B = da/dw = [[-ca, sa, -dy], [-sa, -ca, dx], [0, 0, -1]]
+      X0 = p == 0 ? -ca : (p == 1 ? -sa : 0.f);
+      X1 = p == 0 ? sa : (p == 1 ? -ca : 0.f);
+      X2 = p == 0 ? -ddy : (p == 1 ? ddx : -1.f);
+    } else if (p < 3 + 3 * npn) {
+      const int b = (p - 3) / 3, j = (p - 3) - 3 * b, k = nth_set_bit(nps, b);
+      id = (st_pose(k) + j) | (j == 2 ? 0x10000 : 0);
+      if (k == 1) { X0 = 0.f; X1 = 0.f; X2 = 0.f; }
+      else {  // C_k = de_k/dw = [[1,0,-(y_k-y_1)],[0,1,x_k-x_1],[0,0,1]]
+        X0 = j == 0 ? 1.f : 0.f; X1 = j == 1 ? 1.f : 0.f;
+        X2 = j == 0 ? -(w.st[st_pose(k) + 1] - y1) : (j == 1 ? (w.st[st_pose(k)] - x1) : 1.f);
+      }
+    } else {
+      const int q = p - 3 - 3 * npn, b = q >> 1, j = q & 1, l = nth_set_bit(nls, b);
+      id = st_lm(ly, l) + j;
+      X0 = j == 0 ? 1.f : 0.f; X1 = j == 1 ? 1.f : 0.f;
+      X2 = j == 0 ? -(w.st[st_lm(ly, l) + 1] - y1) : (w.st[st_lm(ly, l)] - x1);
+    }
+    nidx[p] = id;
+    X[3 * p] = X0; X[3 * p + 1] = X1; X[3 * p + 2] = X2;
+  }
+  __syncwarp();
+  // --- C. scatter the old prior
+  {
+    const float* lam = rec + ly.o_lam;
+    for (int p = 0; p < s_old; ++p) {
+      const int P = omap[p];
+      const float* lrow = lam + (p * (p + 1) >> 1);
+      for (int q = lane; q <= p; q += 32) Hs[tri(P, omap[q])] = lrow[q];
+    }
+    for (int p = lane; p < s_old; p += 32) {
+      float acc = rec[ly.o_g + p];
+      const float* lrow = lam + (p * (p + 1) >> 1);
+      for (int q = 0; q <= p; ++q) acc = fmaf(lrow[q], w.sds[q], acc);
+      for (int q = p + 1; q < s_old; ++q) acc = fmaf(lam[(q * (q + 1) >> 1) + p], w.sds[q], acc);
+      gam[omap[p]] = acc;
+    }
+  }
+  __syncwarp();
+  // --- D. factors touching slot 0 (the frame): J_j = I for between factors
+  if (lane < 3) {
+    float r = w.st[st_pose(1) + lane] - w.zodo[3 + lane];
+    if (lane == 2) r = wrapf(r);
+    Hs[tri(3 + lane, 3 + lane)] += pr.om_odo[lane];
+    gam[3 + lane] += pr.om_odo[lane] * r;
+  }
+  __syncwarp();
+  for (int base = 0; base < c; base += 32) {
+    const int k = base + lane;
+    if (k >= 1 && k < c && w.lct[k] == 0) {
+      const int P = 3 + 3 * __popcll(nps & lowmask(k));
+      for (int x = 0; x < 3; ++x) {
+        float r = w.st[st_pose(k) + x] - w.zlc[3 * k + x];
+        if (x == 2) r = wrapf(r);
+        Hs[tri(P + x, P + x)] += pr.om_lc[x];
+        gam[P + x] += pr.om_lc[x] * r;
+      }
+    }
+  }
+  for (int base = 0; base < L; base += 32) {
+    const int l = base + lane;
+    if (l < L && ((rb0 >> l) & 1ull)) {
+      const float zr = rec[ly.o_zrb + (head * 2 + 0) * L + l], zb = rec[ly.o_zrb + (head * 2 + 1) * L + l];
+      const float dx = w.st[st_lm(ly, l)], dy = w.st[st_lm(ly, l) + 1];
+      const float q = dx * dx + dy * dy, irho = rsqrtf(q), rho = q * irho, iq = irho * irho;
+      const float r0 = rho - zr, r1 = wrapf(atan2f(dy, dx) - zb);
+      const float ux = dx * irho, uy = dy * irho, vx = -dy * iq, vy = dx * iq;
+      const float a0 = pr.om_rb[0] * ux, a1 = pr.om_rb[0] * uy, b0 = pr.om_rb[1] * vx, b1 = pr.om_rb[1] * vy;
+      const int P = 3 + 3 * npn + 2 * __popcll(nls & lowmask(l));
+      Hs[tri(P, P)] += a0 * ux + b0 * vx;
+      Hs[tri(P + 1, P)] += a1 * ux + b1 * vx;
+      Hs[tri(P + 1, P + 1)] += a1 * uy + b1 * vy;
+      gam[P] += a0 * r0 + b0 * r1;
+      gam[P + 1] += a1 * r0 + b1 * r1;
+    }
+  }
+  __syncwarp();
+  // --- F. Q = H_s X;  Y = X'Q;  gx = X'gamma
+  float Y[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0}, gx[3] = {0, 0, 0};
+  for (int base = 0; base < s; base += 32) {
+    const int p = base + lane;
+    float q0 = 0.f, q1 = 0.f, q2 = 0.f;
+    if (p < s) {
+      for (int q = 0; q < s; ++q) {
+        const float h = sym_get(Hs, p, q);
+        q0 = fmaf(h, X[3 * q], q0); q1 = fmaf(h, X[3 * q + 1], q1); q2 = fmaf(h, X[3 * q + 2], q2);
+      }
+      Q[3 * p] = q0; Q[3 * p + 1] = q1; Q[3 * p + 2] = q2;
+      const float xa = X[3 * p], xb = X[3 * p + 1], xc = X[3 * p + 2], gp = gam[p];
+      Y[0] += xa * q0; Y[1] += xa * q1; Y[2] += xa * q2;
+      Y[3] += xb * q0; Y[4] += xb * q1; Y[5] += xb * q2;
+      Y[6] += xc * q0; Y[7] += xc * q1; Y[8] += xc * q2;
+      gx[0] += xa * gp; gx[1] += xb * gp; gx[2] += xc * gp;
+    }
+  }
+#pragma unroll
+  for (int t = 0; t < 9; ++t) Y[t] = warp_sum(Y[t]);
+#pragma unroll
+  for (int t = 0; t < 3; ++t) gx[t] = warp_sum(gx[t]);
+  __syncwarp();
+  // --- G. G = E' H_s E block by block (in place);  T_b = E_b' Q_b;  gamma_b = E_b' gamma_b
+  auto etype = [&](int b) -> Etype {
+    if (b == 0) return Etype{1.f, 0.f, ddy, -ddx};          // A = da/da'
+    if (b == 1) return Etype{1.f, 0.f, 0.f, 0.f};           // w: identity
+    return Etype{c1, s1, 0.f, 0.f};                         // blockdiag(Rot(th_1), 1) / Rot(th_1)
+  };
+  auto bpos = [&](int b) -> int { return b == 0 ? 0 : (b <= npn ? 3 + 3 * (b - 1) : 3 + 3 * npn + 2 * (b - 1 - npn)); };
+  const int npairs = nbk * (nbk + 1) >> 1;
+  for (int t = lane; t < npairs; t += 32) {
+    int bi = (int)((sqrtf(8.f * (float)t + 1.f) - 1.f) * 0.5f);
+    while ((bi + 1) * (bi + 2) / 2 <= t) ++bi;
+    while (bi * (bi + 1) / 2 > t) --bi;
+    const int bj = t - bi * (bi + 1) / 2;
+    const int pi = bpos(bi), pj = bpos(bj), di = bi <= npn ? 3 : 2, dj = bj <= npn ? 3 : 2;
+    const Etype Ei = etype(bi), Ej = etype(bj);
+    float M[3][3];
+#pragma unroll
+    for (int x = 0; x < 3; ++x)
+#pragma unroll
+      for (int y = 0; y < 3; ++y) M[x][y] = (x < di && y < dj) ? sym_get(Hs, pi + x, pj + y) : 0.f;
+    float T[3][3];
+#pragma unroll
+    for (int x = 0; x < 3; ++x) {
+      T[x][0] = M[x][0] * Ej.p + M[x][1] * Ej.q;
+      T[x][1] = -M[x][0] * Ej.q + M[x][1] * Ej.p;
+      T[x][2] = M[x][0] * Ej.u + M[x][1] * Ej.v + M[x][2];
+    }
+#pragma unroll
+    for (int y = 0; y < 3; ++y) {
+      M[0][y] = Ei.p * T[0][y] + Ei.q * T[1][y];
+      M[1][y] = -Ei.q * T[0][y] + Ei.p * T[1][y];
+      M[2][y] = Ei.u * T[0][y] + Ei.v * T[1][y] + T[2][y];
+    }
+#pragma unroll
+    for (int x = 0; x < 3; ++x)
+#pragma unroll
+      for (int y = 0; y < 3; ++y)
+        if (x < di && y < dj && (bi != bj || y <= x)) Hs[tri(pi + x, pj + y)] = M[x][y];
+  }
+  for (int b = lane; b < nbk; b += 32) {
+    const int pb = bpos(b), db = b <= npn ? 3 : 2;
+    const Etype E = etype(b);
+    float t0[3], t1[3], t2[3] = {0, 0, 0};
+#pragma unroll
+    for (int y = 0; y < 3; ++y) { t0[y] = Q[3 * pb + y]; t1[y] = Q[3 * (pb + 1) + y]; if (db == 3) t2[y] = Q[3 * (pb + 2) + y]; }
+    const float g0 = gam[pb], g1 = gam[pb + 1], g2 = db == 3 ? gam[pb + 2] : 0.f;
+#pragma unroll
+    for (int y = 0; y < 3; ++y) {
+      Q[3 * pb + y] = E.p * t0[y] + E.q * t1[y];
+      Q[3 * (pb + 1) + y] = -E.q * t0[y] + E.p * t1[y];
+      if (db == 3) Q[3 * (pb + 2) + y] = E.u * t0[y] + E.v * t1[y] + t2[y];
+    }
+    gam[pb] = E.p * g0 + E.q * g1;
+    gam[pb + 1] = -E.q * g0 + E.p * g1;
+    if (db == 3) gam[pb + 2] = E.u * g0 + E.v * g1 + g2;
+  }
+  __syncwarp();
+  // --- I. H_ww, gamma_w (every lane redundantly), K = G[:,w] + T (into Q), KW = K H_ww^{-1} (into X)
+  float Hw[3][3], gw[3];
+#pragma unroll
+  for (int x = 0; x < 3; ++x) {
+    gw[x] = gam[3 + x] + gx[x];
+#pragma unroll
+    for (int y = 0; y < 3; ++y) Hw[x][y] = sym_get(Hs, 3 + x, 3 + y) + Q[3 * (3 + x) + y] + Q[3 * (3 + y) + x] + Y[3 * x + y];
+  }
+  float Wi[3][3];
+  {
+    const float c00 = Hw[1][1] * Hw[2][2] - Hw[1][2] * Hw[2][1];
+    const float c01 = Hw[1][2] * Hw[2][0] - Hw[1][0] * Hw[2][2];
+    const float c02 = Hw[1][0] * Hw[2][1] - Hw[1][1] * Hw[2][0];
+    const float det = Hw[0][0] * c00 + Hw[0][1] * c01 + Hw[0][2] * c02;
+    const float id = 1.0f / det;
+    Wi[0][0] = c00 * id; Wi[1][0] = c01 * id; Wi[2][0] = c02 * id;
+    Wi[0][1] = (Hw[0][2] * Hw[2][1] - Hw[0][1] * Hw[2][2]) * id;
+    Wi[1][1] = (Hw[0][0] * Hw[2][2] - Hw[0][2] * Hw[2][0]) * id;
+    Wi[2][1] = (Hw[0][1] * Hw[2][0] - Hw[0][0] * Hw[2][1]) * id;
+    Wi[0][2] = (Hw[0][1] * Hw[1][2] - Hw[0][2] * Hw[1][1]) * id;
+    Wi[1][2] = (Hw[0][2] * Hw[1][0] - Hw[0][0] * Hw[1][2]) * id;
+    Wi[2][2] = (Hw[0][0] * Hw[1][1] - Hw[0][1] * Hw[1][0]) * id;
+  }
+  __syncwarp();
+  for (int r = lane; r < s; r += 32) {
+    if (r >= 3 && r < 6) continue;
+    float K[3];
+#pragma unroll
+    for (int y = 0; y < 3; ++y) K[y] = Q[3 * r + y] + sym_get(Hs, r, 3 + y);
+#pragma unroll
+    for (int y = 0; y < 3; ++y) {
+      Q[3 * r + y] = K[y];
+      X[3 * r + y] = K[0] * Wi[0][y] + K[1] * Wi[1][y] + K[2] * Wi[2][y];
+    }
+  }
+  __syncwarp();
+  // --- 6. re-anchor the state (A.5 step 6); slot k keeps its ring position, slot 1 becomes the frame
+  {
+    const float nax = w.st[0] + ddx, nay = w.st[1] + ddy, nat = wrapf(a_th + th1);
+    for (int k = 2 + lane; k < c; k += 32) {
+      float* e = w.st + st_pose(k);
+      const float ex = e[0] - x1, ey = e[1] - y1;
+      e[0] = c1 * ex + s1 * ey; e[1] = -s1 * ex + c1 * ey; e[2] = wrapf(e[2] - th1);
+    }
+    for (int l = lane; l < L; l += 32) {
+      if (!((mk.act >> l) & 1ull)) continue;
+      float* m = w.st + st_lm(ly, l);
+      const float ex = m[0] - x1, ey = m[1] - y1;
+      m[0] = c1 * ex + s1 * ey; m[1] = -s1 * ex + c1 * ey;
+    }
+    __syncwarp();
+    if (lane == 0) { w.st[0] = nax; w.st[1] = nay; w.st[2] = nat; }
+    if (lane < 3) w.st[st_pose(1) + lane] = 0.f;
+    __syncwarp();
+  }
+  // --- J. write (Lambda', g', vbar') on the support without w, packed lower, canonical order
+  {
+    float* lam = rec + ly.o_lam;
+    for (int r = 0; r < s; ++r) {
+      if (r >= 3 && r < 6) continue;
+      const int R = r < 3 ? r : r - 3;
+      const float k0 = X[3 * r], k1 = X[3 * r + 1], k2 = X[3 * r + 2];
+      float* lrow = lam + (R * (R + 1) >> 1);
+      for (int q = lane; q <= r; q += 32) {
+        if (q >= 3 && q < 6) continue;
+        const int Qn = q < 3 ? q : q - 3;
+        lrow[Qn] = Hs[tri(r, q)] - (k0 * Q[3 * q] + k1 * Q[3 * q + 1] + k2 * Q[3 * q + 2]);
+      }
+    }
+    for (int r = lane; r < s; r += 32) {
+      if (r >= 3 && r < 6) continue;
+      const int R = r < 3 ? r : r - 3;
+      rec[ly.o_g + R] = gam[r] - (X[3 * r] * gw[0] + X[3 * r + 1] * gw[1] + X[3 * r + 2] * gw[2]);
+      rec[ly.o_vbar + R] = w.st[nidx[r] & 0xffff];
+    }
+  }
+  // --- K. bookkeeping: loop closures to the old slot 0 now live in the prior; new support masks
+  for (int k = 1 + lane; k < c; k += 32)
+    if (w.lct[k] == 0) reci[ly.o_lct + ring_of(k, head, W)] = -1;
+  mk.ps = nps & ~2ull;  // still indexed by the OLD slots; converted with the old head
+  mk.ls = nls;
+  if (lane == 0) {
+    const uint64_t pm = slot_to_ring(mk.ps, head, W);
+    recu[ly.o_pm] = (uint32_t)pm; recu[ly.o_pm + 1] = (uint32_t)(pm >> 32);
+    recu[ly.o_lm] = (uint32_t)nls; recu[ly.o_lm + 1] = (uint32_t)(nls >> 32);
+  }
+  __syncwarp();
+  return 0;
+}
+
+}  // namespace slamk

@@ -1,0 +1,80 @@
+// Device-memory and shared-memory layout of one environment (host + device).
+//
+// HBM: one contiguous, 16-byte aligned RECORD per environment ("array of per-environment
+// structures of arrays"), so that the warp that owns an environment reads and writes coalesced,
+// contiguous runs and the whole record can be staged by bulk copies.  Slot arrays are RING BUFFERS
+// indexed by ring position r = (head + slot) % W: marginalisation advances `head` and never moves
+// factor data (north_star "ring-buffer window shift").
+//
+// The marginalisation prior is stored on its SUPPORT only: two 64-bit masks (pose ring positions,
+// landmarks) name the support blocks in canonical order [anchor a | poses by ascending slot |
+// landmarks by ascending index]; Lambda is packed lower-triangular over that order.
+#pragma once
+#include <stdint.h>
+
+namespace slamk {
+
+struct Layout {
+  int N, W, L, n, nw;  // n = 3W + 2L state dimension, nw = ceil(L/32) mask words
+  // record (32-bit words)
+  int rec;             // record stride
+  int o_status, o_pm, o_lm, o_act, o_a, o_e, o_m, o_zodo, o_lct, o_zlc, o_rbm, o_zrb, o_vbar, o_g, o_lam;
+  // shared memory per warp (32-bit words)
+  int s_st, s_zodo, s_zlc, s_lct, s_cs, s_rbm, s_first, s_rbase, s_lr, s_ssup, s_sidx, s_sds, s_H;
+  int cap;             // words available for H (envelope + rhs row) / marginalisation scratch
+  int warp_words;      // total shared words per warp
+  int wpc;             // warps per CTA
+};
+
+struct Params {
+  float om_prior[3], om_odo[3], om_lc[3], om_rb[2];  // information = 1 / sigma^2
+};
+
+static inline int pad4(int x) { return (x + 3) & ~3; }
+
+// Fills every offset.  `cap` < 0 selects the dense capacity (always sufficient).
+static inline Layout make_layout(int N, int W, int L, int cap, int wpc) {
+  Layout y;
+  y.N = N; y.W = W; y.L = L; y.n = 3 * W + 2 * L; y.nw = (L + 31) / 32;
+  int n = y.n, o = 0;
+  y.o_status = o; o += 1;
+  y.o_pm = o; o += 2;
+  y.o_lm = o; o += 2;
+  y.o_act = o; o += 2;
+  o = pad4(o + 1);
+  y.o_a = o; o += 4;
+  y.o_e = o; o = pad4(o + 3 * W);
+  y.o_m = o; o = pad4(o + 2 * L);
+  y.o_zodo = o; o = pad4(o + 3 * W);
+  y.o_lct = o; o = pad4(o + W);
+  y.o_zlc = o; o = pad4(o + 3 * W);
+  y.o_rbm = o; o = pad4(o + W * y.nw);
+  y.o_zrb = o; o = pad4(o + W * 2 * L);
+  y.o_vbar = o; o = pad4(o + n);
+  y.o_g = o; o = pad4(o + n);
+  y.o_lam = o; o = pad4(o + n * (n + 1) / 2);
+  y.rec = (o + 31) & ~31;  // 128-byte multiple
+
+  int s = 0;
+  y.s_st = s; s = pad4(s + n + 3);
+  y.s_zodo = s; s = pad4(s + 3 * W);
+  y.s_zlc = s; s = pad4(s + 3 * W);
+  y.s_lct = s; s = pad4(s + W);
+  y.s_cs = s; s = pad4(s + 2 * W);
+  y.s_rbm = s; s = pad4(s + W * y.nw);
+  y.s_first = s; s = pad4(s + n + 1);
+  y.s_rbase = s; s = pad4(s + n + 2);
+  y.s_lr = s; s = pad4(s + n + 2);
+  y.s_ssup = s; s = pad4(s + n);
+  y.s_sidx = s; s = pad4(s + n);
+  y.s_sds = s; s = pad4(s + n);
+  y.s_H = s;
+  int dense = n * (n + 1) / 2 + 8 * n + 16;
+  y.cap = pad4(cap < 0 ? dense : cap);
+  s += y.cap;
+  y.warp_words = pad4(s);
+  y.wpc = wpc;
+  return y;
+}
+
+}  // namespace slamk
