@@ -55,7 +55,7 @@ def lib():
         L.orc_cost.restype = C.c_double
         L.orc_cost.argtypes = [C.c_void_p]
         L.orc_between_factor.argtypes = [_dp, _dp, _dp, C.c_int, _dp, _dp, _dp]
-        L.orc_rb_factor.argtypes = [_dp, _dp, _dp, C.c_int, _dp, _dp, _dp]
+        L.orc_rb_factor.argtypes = [_dp, _dp, _dp, _dp, C.c_int, _dp, _dp, _dp, _dp]
         L.orc_reanchor_map.argtypes = [C.c_void_p, _dp, _dp]
         L.orc_reanchor_jac.argtypes = [C.c_void_p, _dp]
         L.orc_run_batch.restype = C.c_int
@@ -186,10 +186,11 @@ def between_factor(ei, ej, z, i_is_frame=False):
     return r, Ji.reshape(3, 3), Jj.reshape(3, 3)
 
 
-def rb_factor(ek, ml, z, k_is_frame=False):
-    r, Jp, Jl = np.zeros(2), np.zeros(6), np.zeros(4)
-    lib().orc_rb_factor(_p(_d(ek)), _p(_d(ml)), _p(_d(z)), int(k_is_frame), _p(r), _p(Jp), _p(Jl))
-    return r, Jp.reshape(2, 3), Jl.reshape(2, 2)
+def rb_factor(a, ek, gl, z, k_is_frame=False):
+    """Range-bearing factor, landmark gl global, observing pose a (+) ek: returns r, Ja (2x3), Jp (2x3), Jg (2x2)."""
+    r, Ja, Jp, Jg = np.zeros(2), np.zeros(6), np.zeros(6), np.zeros(4)
+    lib().orc_rb_factor(_p(_d(a)), _p(_d(ek)), _p(_d(gl)), _p(_d(z)), int(k_is_frame), _p(r), _p(Ja), _p(Jp), _p(Jg))
+    return r, Ja.reshape(2, 3), Jp.reshape(2, 3), Jg.reshape(2, 2)
 
 
 def max_threads() -> int:

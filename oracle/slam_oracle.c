@@ -21,7 +21,7 @@ struct orc {
   double sig[11];
   double a[3];      /* global pose of the anchor (slot 0) */
   double* e;        /* [W][3] slot poses in the anchor frame, e[0] == 0 */
-  double* m;        /* [L][2] landmarks in the anchor frame */
+  double* m;        /* [L][2] landmarks g_l in GLOBAL coordinates (reading R17b) */
   int* active;      /* [L] */
   double *Lam, *g, *vbar; /* prior: 0.5 d'Lam d + g'd, d = v - vbar */
   double* z_odo;    /* [W][3]  z_odo[k]: slot k-1 -> k */
@@ -136,50 +136,60 @@ static void between_factor(int linear, const double* ei, const double* ej, const
   }
 }
 
-/* Range-bearing factor from pose k to landmark l (anchor frame).  R4:
- * r = [ |m - t| - z_r ; wrap(atan2(dy,dx) - th - z_b) ].  Jp is 2x3, Jl is 2x2. */
-static void rb_factor(const double* ek, const double* ml, const double* z, int k_is_frame,
-                      double* r, double* Jp, double* Jl) {
+/* Range-bearing factor from the pose in slot k to landmark l.  The landmark g is kept in GLOBAL
+ * coordinates (reading R17b); the observing pose is x = a (+) e_k (x = a if k is the anchor slot).
+ * R4: r = [ |g - t_x| - z_r ; wrap(atan2(dy,dx) - th_x - z_b) ].
+ * Jacobians by the chain rule through x: Ja (2x3, wrt the anchor a), Jp (2x3, wrt e_k; zero if
+ * k_is_frame), Jg (2x2, wrt the landmark). */
+static void rb_factor(const double* a, const double* ek, const double* gl, const double* z, int k_is_frame,
+                      double* r, double* Ja, double* Jp, double* Jg) {
   double zero[3] = {0, 0, 0};
-  const double* p = k_is_frame ? zero : ek;
-  double dx = ml[0] - p[0], dy = ml[1] - p[1];
+  const double* e = k_is_frame ? zero : ek;
+  double x[3];
+  compose(0, a, e, x);
+  double dx = gl[0] - x[0], dy = gl[1] - x[1];
   double q = dx * dx + dy * dy, rho = sqrt(q);
   r[0] = rho - z[0];
-  r[1] = wrap_pi(atan2(dy, dx) - p[2] - z[1]);
-  Jl[0] = dx / rho; Jl[1] = dy / rho;
-  Jl[2] = -dy / q;  Jl[3] = dx / q;
-  memset(Jp, 0, 6 * sizeof(double));
-  if (!k_is_frame) {
-    Jp[0] = -dx / rho; Jp[1] = -dy / rho; Jp[2] = 0;
-    Jp[3] = dy / q;    Jp[4] = -dx / q;   Jp[5] = -1;
-  }
+  r[1] = wrap_pi(atan2(dy, dx) - x[2] - z[1]);
+  /* wrt the global observing pose x and the landmark */
+  double Jx[6] = {-dx / rho, -dy / rho, 0, dy / q, -dx / q, -1};
+  Jg[0] = dx / rho; Jg[1] = dy / rho;
+  Jg[2] = -dy / q;  Jg[3] = dx / q;
+  /* x = a (+) e:  dx/da = [[1,0,-d_y],[0,1,d_x],[0,0,1]], d = Rot(a_th) t_e;  dx/de = blockdiag(Rot(a_th),1) */
+  double ca = cos(a[2]), sa = sin(a[2]);
+  double ddx = ca * e[0] - sa * e[1], ddy = sa * e[0] + ca * e[1];
+  double Xa[9] = {1, 0, -ddy, 0, 1, ddx, 0, 0, 1};
+  double Xe[9] = {ca, -sa, 0, sa, ca, 0, 0, 0, 1};
+  for (int i = 0; i < 2; ++i)
+    for (int j = 0; j < 3; ++j) {
+      double sa_ = 0.0, se_ = 0.0;
+      for (int k = 0; k < 3; ++k) { sa_ += Jx[i * 3 + k] * Xa[k * 3 + j]; se_ += Jx[i * 3 + k] * Xe[k * 3 + j]; }
+      Ja[i * 3 + j] = sa_;
+      Jp[i * 3 + j] = k_is_frame ? 0.0 : se_;
+    }
 }
 
 void orc_between_factor(const double* ei3, const double* ej3, const double* z3, int i_is_frame,
                         double* r3, double* Ji9, double* Jj9) {
   between_factor(0, ei3, ej3, z3, i_is_frame, r3, Ji9, Jj9);
 }
-void orc_rb_factor(const double* ek3, const double* ml2, const double* z2, int k_is_frame,
-                   double* r2, double* Jp6, double* Jl4) {
-  rb_factor(ek3, ml2, z2, k_is_frame, r2, Jp6, Jl4);
+void orc_rb_factor(const double* a3, const double* ek3, const double* gl2, const double* z2, int k_is_frame,
+                   double* r2, double* Ja6, double* Jp6, double* Jg4) {
+  rb_factor(a3, ek3, gl2, z2, k_is_frame, r2, Ja6, Jp6, Jg4);
 }
 
-/* Accumulate one factor with up to two variable blocks into the normal equations:
+/* Accumulate one factor with up to three variable blocks into the normal equations:
  *   H += J' Omega J,  grad += J' Omega r      (Omega diagonal, rdim rows)
- * block A: index ia, width wa, Jacobian JA (rdim x wa), skipped if ia < 0; same for B. */
-static void add_factor(double* H, double* grad, double* cost, int n, int rdim, const double* r,
-                       const double* omega, int ia, int wa, const double* JA, int ib, int wb,
-                       const double* JB) {
-  const int idx[2] = {ia, ib};
-  const int wid[2] = {wa, wb};
-  const double* J[2] = {JA, JB};
-  for (int p = 0; p < 2; ++p) {
+ * block p: index idx[p] (skipped if < 0), width wid[p], Jacobian J[p] (rdim x wid[p], row-major). */
+static void add_factor_n(double* H, double* grad, double* cost, int n, int rdim, const double* r,
+                         const double* omega, int nblk, const int* idx, const int* wid, const double* const* J) {
+  for (int p = 0; p < nblk; ++p) {
     if (idx[p] < 0) continue;
     for (int x = 0; x < wid[p]; ++x) {
       double s = 0.0;
       for (int k = 0; k < rdim; ++k) s += J[p][k * wid[p] + x] * omega[k] * r[k];
       if (grad) grad[idx[p] + x] += s;
-      for (int q = 0; q < 2; ++q) {
+      for (int q = 0; q < nblk; ++q) {
         if (idx[q] < 0) continue;
         for (int y = 0; y < wid[q]; ++y) {
           double h = 0.0;
@@ -190,6 +200,14 @@ static void add_factor(double* H, double* grad, double* cost, int n, int rdim, c
     }
   }
   if (cost) for (int k = 0; k < rdim; ++k) *cost += 0.5 * r[k] * omega[k] * r[k];
+}
+static void add_factor(double* H, double* grad, double* cost, int n, int rdim, const double* r,
+                       const double* omega, int ia, int wa, const double* JA, int ib, int wb,
+                       const double* JB) {
+  const int idx[2] = {ia, ib};
+  const int wid[2] = {wa, wb};
+  const double* J[2] = {JA, JB};
+  add_factor_n(H, grad, cost, n, rdim, r, omega, 2, idx, wid, J);
 }
 
 /* ------------------------------------------------------------------ object */
@@ -258,14 +276,15 @@ void orc_reset(orc* o, const double* init_pose3) {
 }
 
 static void record_rb(orc* o, int slot, const int* rb_valid, const double* rb_meas) {
-  const double* p = o->e + 3 * slot; /* e[0] == 0: the frame itself */
+  double p[3]; /* global pose of the observing slot, x = a (+) e_slot (e[0] == 0) */
+  compose(0, o->a, o->e + 3 * slot, p);
   for (int l = 0; l < o->L; ++l) {
     int v = rb_valid ? (rb_valid[l] != 0) : 0;
     o->rb_valid[slot * o->L + l] = v;
     if (!v) continue;
     o->z_rb[(slot * o->L + l) * 2 + 0] = rb_meas[2 * l + 0];
     o->z_rb[(slot * o->L + l) * 2 + 1] = rb_meas[2 * l + 1];
-    if (!o->active[l]) { /* R6: inverse projection from the observing pose's current estimate */
+    if (!o->active[l]) { /* R6: inverse projection from the observing pose's current estimate (global) */
       double r = rb_meas[2 * l], beta = rb_meas[2 * l + 1];
       o->m[2 * l + 0] = p[0] + r * cos(p[2] + beta);
       o->m[2 * l + 1] = p[1] + r * sin(p[2] + beta);
@@ -342,7 +361,7 @@ static void build_system(const orc* o, int only_slot0, double* H, double* grad, 
   }
   free(d);
 
-  double r[3], Ji[9], Jj[9], Jp[6], Jl[4];
+  double r[3], Ji[9], Jj[9], Ja[6], Jp[6], Jg[4];
   for (int k = 1; k < c; ++k) { /* odometry k-1 -> k */
     int i = k - 1;
     if (only_slot0 && i != 0) continue;
@@ -360,8 +379,11 @@ static void build_system(const orc* o, int only_slot0, double* H, double* grad, 
     if (only_slot0 && k != 0) continue;
     for (int l = 0; l < L; ++l) {
       if (!o->rb_valid[k * L + l]) continue;
-      rb_factor(o->e + 3 * k, o->m + 2 * l, o->z_rb + (k * L + l) * 2, k == 0, r, Jp, Jl);
-      add_factor(H, grad, cost, n, 2, r, om_rb, k == 0 ? -1 : idx_e(k), 3, Jp, idx_m(o, l), 2, Jl);
+      rb_factor(o->a, o->e + 3 * k, o->m + 2 * l, o->z_rb + (k * L + l) * 2, k == 0, r, Ja, Jp, Jg);
+      const int idx[3] = {0, k == 0 ? -1 : idx_e(k), idx_m(o, l)};
+      const int wid[3] = {3, 3, 2};
+      const double* J[3] = {Ja, Jp, Jg};
+      add_factor_n(H, grad, cost, n, 2, r, om_rb, 3, idx, wid, J);
     }
   }
 }
@@ -473,17 +495,16 @@ void orc_get_poses(const orc* o, double* poses) {
 }
 
 void orc_get_landmarks(const orc* o, double* lm, int* active) {
-  double ca = cos(o->a[2]), sa = sin(o->a[2]);
   for (int l = 0; l < o->L; ++l) {
     active[l] = o->active[l];
-    lm[2 * l + 0] = o->active[l] ? o->a[0] + ca * o->m[2 * l] - sa * o->m[2 * l + 1] : 0.0;
-    lm[2 * l + 1] = o->active[l] ? o->a[1] + sa * o->m[2 * l] + ca * o->m[2 * l + 1] : 0.0;
+    lm[2 * l + 0] = o->active[l] ? o->m[2 * l] : 0.0;
+    lm[2 * l + 1] = o->active[l] ? o->m[2 * l + 1] : 0.0;
   }
 }
 
 /* ------------------------------------------------------------------ marginalization (A.5) */
 
-/* step 2: new coordinates u(v) = (a' = a (+) e_1, w = e_1, e'_k = between(e_1, e_k), m'_l).
+/* step 2: new coordinates u(v) = (a' = a (+) e_1, w = e_1, e'_k = between(e_1, e_k), g_l unchanged).
  * u is indexed like v: a' at 0, w where e_1 sits, e'_k where e_k sits, m'_l where m_l sits. */
 void orc_reanchor_map(const orc* o, const double* v, double* u) {
   int W = o->W, L = o->L, c = o->c;
@@ -492,14 +513,7 @@ void orc_reanchor_map(const orc* o, const double* v, double* u) {
   const double* e1 = v + 3;
   compose(o->linear, a, e1, u);                   /* a' */
   for (int k = 2; k < c; ++k) between(o->linear, e1, v + 3 * k, u + 3 * k);
-  for (int l = 0; l < L; ++l) {
-    if (!o->active[l]) continue;
-    const double* ml = v + 3 * W + 2 * l;
-    double c1 = cos(e1[2]), s1 = sin(e1[2]);
-    double dx = ml[0] - e1[0], dy = ml[1] - e1[1];
-    u[3 * W + 2 * l + 0] = c1 * dx + s1 * dy;
-    u[3 * W + 2 * l + 1] = -s1 * dx + c1 * dy;
-  }
+  (void)W; (void)L; /* landmarks are global: unchanged by re-anchoring */
 }
 
 /* step 3: M = du/dv at the current estimate (analytic; pinned by finite differences) */
@@ -533,17 +547,7 @@ void orc_reanchor_jac(const orc* o, double* M) {
         M[(3 * k + x) * n + 3 * k + y] = Jj[x * 3 + y];
       }
   }
-  double c1 = cos(e1[2]), s1 = sin(e1[2]);
-  for (int l = 0; l < L; ++l) {
-    if (!o->active[l]) continue;
-    int im = 3 * W + 2 * l;
-    double mx = o->m[2 * l] - e1[0], my = o->m[2 * l + 1] - e1[1];
-    double px = c1 * mx + s1 * my, py = -s1 * mx + c1 * my;            /* m'_l */
-    M[im * n + 3] = -c1; M[im * n + 4] = -s1; M[im * n + 5] = py;
-    M[(im + 1) * n + 3] = s1; M[(im + 1) * n + 4] = -c1; M[(im + 1) * n + 5] = -px;
-    M[im * n + im] = c1; M[im * n + im + 1] = s1;
-    M[(im + 1) * n + im] = -s1; M[(im + 1) * n + im + 1] = c1;
-  }
+  (void)W; (void)L; /* dg/dg = I */
 }
 
 int orc_marginalize(orc* o) {
@@ -632,13 +636,6 @@ int orc_marginalize(orc* o) {
   for (int k = 2; k < c; ++k) { between(o->linear, e1, o->e + 3 * k, v); memcpy(o->e + 3 * (k - 1), v, sizeof(v)); }
   for (int k = c - 1; k < W; ++k) memset(o->e + 3 * k, 0, 3 * sizeof(double));
   memset(o->e, 0, 3 * sizeof(double));
-  double c1 = cos(e1[2]), s1 = sin(e1[2]);
-  for (int l = 0; l < L; ++l) {
-    if (!o->active[l]) continue;
-    double mx = o->m[2 * l] - e1[0], my = o->m[2 * l + 1] - e1[1];
-    o->m[2 * l] = c1 * mx + s1 * my;
-    o->m[2 * l + 1] = -s1 * mx + c1 * my;
-  }
   for (int k = 2; k < c; ++k) {
     memcpy(o->z_odo + 3 * (k - 1), o->z_odo + 3 * k, 3 * sizeof(double));
     int t = o->lc_tgt[k] - 1;          /* targets that were slot 0 now live in the prior */

@@ -15,7 +15,10 @@
  *   marginalize  re-anchor + explicit Schur complement of the oldest pose (dense)
  *
  * Variable vector (natural order, NOT the GPU's elimination order):
- *   v = [ a(3) ; e_1(3) ... e_{W-1}(3) ; m_0(2) ... m_{L-1}(2) ],  n = 3W + 2L
+ *   v = [ a(3) ; e_1(3) ... e_{W-1}(3) ; g_0(2) ... g_{L-1}(2) ],  n = 3W + 2L
+ *   a = global pose of the oldest window pose (anchor), e_k = pose k in the anchor frame,
+ *   g_l = landmark l in GLOBAL coordinates (reading R17b: anchor-frame landmarks make the information
+ *   matrix couple the weakly known anchor to strongly known landmarks -- unusable in fp32).
  *   index(a)=0, index(e_k)=3k, index(m_l)=3W+2l.
  *
  * Pins (tests/test_oracle_pins.py): finite-difference Jacobians, noise-free exact recovery, the
@@ -63,8 +66,9 @@ double orc_cost(const orc*);   /* 0.5*sum r'Omega r + 0.5 d'Lam d + g'd at the c
 /* residual and Jacobians of one between factor in the anchor frame; i_is_frame: pose i is the anchor */
 void orc_between_factor(const double* ei3, const double* ej3, const double* z3, int i_is_frame,
                         double* r3, double* Ji9, double* Jj9);
-void orc_rb_factor(const double* ek3, const double* ml2, const double* z2, int k_is_frame,
-                   double* r2, double* Jp6, double* Jl4);
+/* landmark gl in global coordinates, observing pose x = a (+) ek (x = a if k_is_frame) */
+void orc_rb_factor(const double* a3, const double* ek3, const double* gl2, const double* z2, int k_is_frame,
+                   double* r2, double* Ja6, double* Jp6, double* Jg4);
 /* re-anchoring map u(v) of A.5 step 2 and its Jacobian M = du/dv at the current state */
 void orc_reanchor_map(const orc*, const double* v, double* u);
 void orc_reanchor_jac(const orc*, double* M /* [n*n] */);

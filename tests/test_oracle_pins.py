@@ -67,16 +67,27 @@ def test_between_factor_jacobians_fd():
 def test_rb_factor_jacobians_fd():
     rng = np.random.default_rng(2)
     for _ in range(20):
+        a = rng.normal(size=3) * [5, 5, 1]
         ek = rng.normal(size=3)
-        ml = ek[:2] + rng.uniform(0.5, 8.0) * np.array([np.cos(1.3), np.sin(1.3)]) + rng.normal(size=2) * 0.1
+        x = synth.compose(a[:, None], ek[:, None])[:, 0]                 # global observing pose
+        gl = x[:2] + rng.uniform(0.5, 8.0) * np.array([np.cos(1.3), np.sin(1.3)]) + rng.normal(size=2) * 0.1
         z = np.array([rng.uniform(0.5, 8), rng.uniform(-3, 3)])
-        r, Jp, Jl = oracle.rb_factor(ek, ml, z)
-        assert np.allclose(Jp, fd_jac(lambda x: oracle.rb_factor(x, ml, z)[0], ek), atol=1e-6)
-        assert np.allclose(Jl, fd_jac(lambda x: oracle.rb_factor(ek, x, z)[0], ml), atol=1e-6)
-    # definition (R4): a landmark at range 2, bearing 0.5 from pose (1,2,0.3)
+        r, Ja, Jp, Jg = oracle.rb_factor(a, ek, gl, z)
+        assert np.allclose(Ja, fd_jac(lambda q: oracle.rb_factor(q, ek, gl, z)[0], a), atol=1e-6)
+        assert np.allclose(Jp, fd_jac(lambda q: oracle.rb_factor(a, q, gl, z)[0], ek), atol=1e-6)
+        assert np.allclose(Jg, fd_jac(lambda q: oracle.rb_factor(a, ek, q, z)[0], gl), atol=1e-6)
+        # the anchor slot observes from x = a: no e block
+        r0, Ja0, Jp0, Jg0 = oracle.rb_factor(a, ek, gl, z, k_is_frame=True)
+        assert np.allclose(r0, oracle.rb_factor(a, np.zeros(3), gl, z)[0]) and np.allclose(Jp0, 0)
+        assert np.allclose(Ja0, fd_jac(lambda q: oracle.rb_factor(q, ek, gl, z, True)[0], a), atol=1e-6)
+    # definition (R4): a landmark at range 2, bearing 0.5 from the global pose (1,2,0.3)
     p = np.array([1.0, 2.0, 0.3])
     l = p[:2] + 2.0 * np.array([np.cos(0.8), np.sin(0.8)])
-    assert np.allclose(oracle.rb_factor(p, l, [2.0, 0.5])[0], 0, atol=1e-14)
+    assert np.allclose(oracle.rb_factor(p, np.zeros(3), l, [2.0, 0.5], True)[0], 0, atol=1e-14)
+    a, e = np.array([0.4, -0.3, 0.9]), np.array([0.2, 0.1, -0.5])
+    x = synth.compose(a[:, None], e[:, None])[:, 0]
+    l = x[:2] + 3.0 * np.array([np.cos(x[2] - 0.7), np.sin(x[2] - 0.7)])
+    assert np.allclose(oracle.rb_factor(a, e, l, [3.0, -0.7])[0], 0, atol=1e-14)
 
 
 def _random_window(W=6, L=3, seed=3):
@@ -107,6 +118,7 @@ def test_reanchor_jacobian_fd():
         g_old = synth.compose(v[:3, None], v[3 * k:3 * k + 3, None])[:, 0]
         g_new = synth.compose(a2[:, None], u[3 * k:3 * k + 3, None])[:, 0]
         assert np.allclose(g_old, g_new, atol=1e-12)
+    assert np.array_equal(u[3 * o.W:], v[3 * o.W:])        # landmarks are global: untouched (R17b)
 
 
 def test_gradient_and_hessian_of_cost_fd():
