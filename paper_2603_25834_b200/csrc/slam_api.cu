@@ -107,15 +107,12 @@ __global__ void slam_landmarks_kernel(Layout ly, const float* state, float* lm, 
   if (env >= ly.N) return;
   const float* rec = state + (size_t)env * ly.rec;
   const uint32_t* recu = reinterpret_cast<const uint32_t*>(rec);
-  const float ax = rec[ly.o_a], ay = rec[ly.o_a + 1], at = rec[ly.o_a + 2];
-  float sn, cn;
-  sincosf(at, &sn, &cn);
   for (int q = 0; q < ly.nw; ++q) active[(size_t)q * ly.N + env] = recu[ly.o_act + q];
   for (int l = 0; l < ly.L; ++l) {
     const bool act = (recu[ly.o_act + (l >> 5)] >> (l & 31)) & 1u;
     const float mx = rec[ly.o_m + 2 * l], my = rec[ly.o_m + 2 * l + 1];
-    lm[((size_t)0 * ly.L + l) * ly.N + env] = act ? ax + cn * mx - sn * my : 0.f;
-    lm[((size_t)1 * ly.L + l) * ly.N + env] = act ? ay + sn * mx + cn * my : 0.f;
+    lm[((size_t)0 * ly.L + l) * ly.N + env] = act ? mx : 0.f;  // landmarks are stored in global coordinates
+    lm[((size_t)1 * ly.L + l) * ly.N + env] = act ? my : 0.f;
   }
 }
 

@@ -137,7 +137,8 @@ __device__ void store_state(const Layout& ly, float* rec, const WS& w, int lane,
 }
 
 // ------------------------------------------------------------------ S0 push / observe
-// Range-bearing bookkeeping for the pose in `slot` (pose px,py,pth in the anchor frame).
+// Range-bearing bookkeeping for the pose in `slot` (pose px,py,pth in the anchor frame; landmarks are
+// kept in GLOBAL coordinates, reading R17b).
 __device__ void record_rb(const Layout& ly, float* rec, const WS& w, int lane, int env, int head, int slot,
                           float px, float py, float pth, const StepIO& io, Masks& mk) {
   const int L = ly.L, N = ly.N, r = ring_of(slot, head, ly.W);
@@ -152,11 +153,13 @@ __device__ void record_rb(const Layout& ly, float* rec, const WS& w, int lane, i
       const float zb = io.rb_meas[(size_t)(L + l) * N + env];
       rec[ly.o_zrb + (r * 2 + 0) * L + l] = zr;
       rec[ly.o_zrb + (r * 2 + 1) * L + l] = zb;
-      if (vis && !((act >> l) & 1ull)) {  // R6: inverse projection from the observing pose's guess
-        float sn, cn;
-        sincosf(pth + zb, &sn, &cn);
-        w.st[st_lm(ly, l)] = px + zr * cn;
-        w.st[st_lm(ly, l) + 1] = py + zr * sn;
+      if (vis && !((act >> l) & 1ull)) {  // R6: inverse projection from the observing pose's guess (global)
+        float sa, ca, sn, cn;
+        sincosf(w.st[2], &sa, &ca);
+        const float gx = w.st[0] + ca * px - sa * py, gy = w.st[1] + sa * px + ca * py;
+        sincosf(w.st[2] + pth + zb, &sn, &cn);
+        w.st[st_lm(ly, l)] = gx + zr * cn;
+        w.st[st_lm(ly, l) + 1] = gy + zr * sn;
       }
     }
     const uint64_t wm = (uint64_t)(L - base >= 32 ? word : (word & ((1u << (L - base)) - 1u)));
@@ -274,8 +277,23 @@ __device__ int symbolic(const Layout& ly, const WS& w, int lane, int c, const Ma
     for (int p = lane; p < s; p += 32) { const int i = w.ssup[p]; w.first[i] = min(w.first[i], fs); }
   }
   __syncwarp();
-  // rows of a block must share `first` (min over the block) -- they do by construction, except
-  // that support scalars were updated one by one with the same fs, which keeps them equal.
+  // landmarks are global: every range-bearing factor also touches the anchor, whose rows therefore
+  // reach back to the first observing chain pose and the first observed landmark
+  if (L > 0) {
+    int fa = oA;
+    for (int k = lane; k < c; k += 32) {
+      uint64_t m = (uint64_t)w.rbm[k * ly.nw];
+      if (ly.nw > 1) m |= (uint64_t)w.rbm[k * ly.nw + 1] << 32;
+      if (m) {
+        if (k >= 1) fa = min(fa, off_slot(ly, k, c));
+        fa = min(fa, off_lm(ly, __ffsll((long long)m) - 1));
+      }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) fa = min(fa, __shfl_xor_sync(FULLMASK, fa, o));
+    if (lane < 3) w.first[oA + lane] = min(w.first[oA + lane], fa);
+  }
+  __syncwarp();
   // prefix sum of row lengths -> rbase; long-row list
   int run = 0, cnt = 0;
   for (int base = 0; base <= n; base += 32) {
@@ -468,79 +486,123 @@ __device__ void assemble(const Layout& ly, const Params& pr, const float* rec, c
     if (any) add_i_side(w, n, off_slot(ly, t, c), Hii, gi);
   }
   __syncwarp();
-  // range-bearing factors: lanes over landmarks, loop over slots; pose-side sums by warp shuffles
+  // range-bearing factors: lanes over landmarks, loop over slots.  Landmarks g are global, so each
+  // factor has three blocks: anchor a, observing pose e_k (k >= 1), landmark g.  With the anchor-frame
+  // landmark m = Rot(a_th)'(g - a_t), D = m - t_k:  J_e = [-J_l | (0,-1)'],  J_g = J_l Rot(a_th)',
+  // J_a = [-J_g | -J_l S m].  Pose- and anchor-side sums over landmarks go through warp shuffles.
   if (L > 0) {
     float* rhs = w.H + w.rbase[n];
     const float w0 = pr.om_rb[0], w1 = pr.om_rb[1];
+    const int oA = off_a(ly);
+    float sa, ca;
+    sincosf(w.st[2], &sa, &ca);
+    const float ax = w.st[0], ay = w.st[1];
+    float A[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};  // sums over all factors: gg(3), <a2,g0>, <a2,g1>, <a2,a2>, <g0,r>, <g1,r>, <a2,r>
     for (int base = 0; base < L; base += 32) {
       const int l = base + lane;
       const bool inl = l < L;
-      const float mx = inl ? w.st[st_lm(ly, l)] : 0.f, my = inl ? w.st[st_lm(ly, l) + 1] : 0.f;
-      float Lxx = 0.f, Lxy = 0.f, Lyy = 0.f, gx = 0.f, gy = 0.f;
+      const float gxl = inl ? w.st[st_lm(ly, l)] - ax : 0.f, gyl = inl ? w.st[st_lm(ly, l) + 1] - ay : 0.f;
+      const float mx = ca * gxl + sa * gyl, my = -sa * gxl + ca * gyl;
+      float Lxx = 0.f, Lxy = 0.f, Lyy = 0.f, bgx = 0.f, bgy = 0.f, ag0 = 0.f, ag1 = 0.f;
       const int ol = off_lm(ly, inl ? l : 0);
       for (int k = 0; k < c; ++k) {
         const uint32_t word = w.rbm[k * ly.nw + (base >> 5)];
         if (word == 0u) continue;  // warp-uniform
         const bool vis = inl && ((word >> lane) & 1u);
         const int r = ring_of(k, head, W);
-        float P[6] = {0, 0, 0, 0, 0, 0}, gp[3] = {0, 0, 0};
+        float R[18];  // per-pose sums: ee (6), b_e (3), ae (9)
+#pragma unroll
+        for (int t = 0; t < 18; ++t) R[t] = 0.f;
         if (vis) {
           const float zr = rec[ly.o_zrb + (r * 2 + 0) * L + l], zb = rec[ly.o_zrb + (r * 2 + 1) * L + l];
           const float* p = w.st + st_pose(k);
           const float dx = mx - p[0], dy = my - p[1];
           const float q = dx * dx + dy * dy, irho = rsqrtf(q), rho = q * irho, iq = irho * irho;
           const float r0 = rho - zr, r1 = wrapf(atan2f(dy, dx) - p[2] - zb);
-          // J_l = [[ux, uy], [-dy/q, dx/q]],  J_p = [[-ux, -uy, 0], [dy/q, -dx/q, -1]]
-          const float ux = dx * irho, uy = dy * irho, vx = -dy * iq, vy = dx * iq;
-          const float a0 = w0 * ux, a1 = w0 * uy, b0 = w1 * vx, b1 = w1 * vy;
-          Lxx += a0 * ux + b0 * vx; Lxy += a0 * uy + b0 * vy; Lyy += a1 * uy + b1 * vy;
-          gx += a0 * r0 + b0 * r1; gy += a1 * r0 + b1 * r1;
+          const float ux = dx * irho, uy = dy * irho, vx = -dy * iq, vy = dx * iq;     // J_l rows
+          const float Ux = ca * ux - sa * uy, Uy = sa * ux + ca * uy;                  // J_g rows
+          const float Vx = ca * vx - sa * vy, Vy = sa * vx + ca * vy;
+          const float j0 = ux * my - uy * mx, j1 = vx * my - vy * mx;                  // J_a theta column
+          // weighted columns
+          const float wg0a = w0 * Ux, wg0b = w1 * Vx, wg1a = w0 * Uy, wg1b = w1 * Vy, wa2a = w0 * j0, wa2b = w1 * j1;
+          const float gg00 = wg0a * Ux + wg0b * Vx, gg01 = wg0a * Uy + wg0b * Vy, gg11 = wg1a * Uy + wg1b * Vy;
+          const float a2g0 = wa2a * Ux + wa2b * Vx, a2g1 = wa2a * Uy + wa2b * Vy, a2a2 = wa2a * j0 + wa2b * j1;
+          const float g0r = wg0a * r0 + wg0b * r1, g1r = wg1a * r0 + wg1b * r1, a2r = wa2a * r0 + wa2b * r1;
+          Lxx += gg00; Lxy += gg01; Lyy += gg11; bgx += g0r; bgy += g1r; ag0 += a2g0; ag1 += a2g1;
+          A[0] += gg00; A[1] += gg01; A[2] += gg11; A[3] += a2g0; A[4] += a2g1; A[5] += a2a2;
+          A[6] += g0r; A[7] += g1r; A[8] += a2r;
           if (k > 0) {
-            // cross block J_l' Om J_p (2x3): rows landmark (x,y), cols pose (x,y,th)
-            const float c00 = -(a0 * ux + b0 * vx), c01 = -(a0 * uy + b0 * vy), c02 = -b0;
-            const float c10 = -(a1 * ux + b1 * vx), c11 = -(a1 * uy + b1 * vy), c12 = -b1;
+            // pose columns e0 = (-ux,-vx), e1 = (-uy,-vy), e2 = (0,-1)
+            const float ge00 = -(wg0a * ux + wg0b * vx), ge01 = -(wg0a * uy + wg0b * vy), ge02 = -wg0b;
+            const float ge10 = -(wg1a * ux + wg1b * vx), ge11 = -(wg1a * uy + wg1b * vy), ge12 = -wg1b;
             const int op = off_slot(ly, k, c);
             if (op < ol) {  // chain pose: landmark rows, pose columns
               float* r0p = w.H + w.rbase[ol];
               float* r1p = w.H + w.rbase[ol + 1];
-              r0p[op] += c00; r0p[op + 1] += c01; r0p[op + 2] += c02;
-              r1p[op] += c10; r1p[op + 1] += c11; r1p[op + 2] += c12;
+              r0p[op] += ge00; r0p[op + 1] += ge01; r0p[op + 2] += ge02;
+              r1p[op] += ge10; r1p[op + 1] += ge11; r1p[op + 2] += ge12;
             } else {        // newest pose: pose rows, landmark columns
-              w.H[w.rbase[op] + ol] += c00; w.H[w.rbase[op] + ol + 1] += c10;
-              w.H[w.rbase[op + 1] + ol] += c01; w.H[w.rbase[op + 1] + ol + 1] += c11;
-              w.H[w.rbase[op + 2] + ol] += c02; w.H[w.rbase[op + 2] + ol + 1] += c12;
+              w.H[w.rbase[op] + ol] += ge00; w.H[w.rbase[op] + ol + 1] += ge10;
+              w.H[w.rbase[op + 1] + ol] += ge01; w.H[w.rbase[op + 1] + ol + 1] += ge11;
+              w.H[w.rbase[op + 2] + ol] += ge02; w.H[w.rbase[op + 2] + ol + 1] += ge12;
             }
-            // pose diagonal J_p' Om J_p (lower: xx, yx, yy, tx, ty, tt) and gradient
-            P[0] = a0 * ux + b0 * vx; P[1] = a1 * ux + b1 * vx; P[2] = a1 * uy + b1 * vy;
-            P[3] = b0; P[4] = b1; P[5] = w1;
-            gp[0] = -(a0 * r0 + b0 * r1); gp[1] = -(a1 * r0 + b1 * r1); gp[2] = -w1 * r1;
+            const float e0a = w0 * ux, e0b = w1 * vx, e1a = w0 * uy, e1b = w1 * vy;
+            // pose diagonal (lower: xx, yx, yy, tx, ty, tt) and gradient
+            R[0] = e0a * ux + e0b * vx; R[1] = e1a * ux + e1b * vx; R[2] = e1a * uy + e1b * vy;
+            R[3] = e0b; R[4] = e1b; R[5] = w1;
+            R[6] = -(e0a * r0 + e0b * r1); R[7] = -(e1a * r0 + e1b * r1); R[8] = -w1 * r1;
+            // anchor rows x pose columns: <a_i, e_j>, a0 = -g0, a1 = -g1, a2 = (j0, j1)
+            R[9] = -ge00; R[10] = -ge01; R[11] = -ge02;
+            R[12] = -ge10; R[13] = -ge11; R[14] = -ge12;
+            R[15] = -(wa2a * ux + wa2b * vx); R[16] = -(wa2a * uy + wa2b * vy); R[17] = -wa2b;
           }
         }
         if (k > 0) {
 #pragma unroll
-          for (int t = 0; t < 6; ++t) P[t] = warp_sum(P[t]);
-#pragma unroll
-          for (int t = 0; t < 3; ++t) gp[t] = warp_sum(gp[t]);
+          for (int t = 0; t < 18; ++t) R[t] = warp_sum(R[t]);
           if (lane == 0) {
             const int op = off_slot(ly, k, c);
             float* q0 = w.H + w.rbase[op];
             float* q1 = w.H + w.rbase[op + 1];
             float* q2 = w.H + w.rbase[op + 2];
-            q0[op] += P[0]; q1[op] += P[1]; q1[op + 1] += P[2];
-            q2[op] += P[3]; q2[op + 1] += P[4]; q2[op + 2] += P[5];
-            rhs[op] -= gp[0]; rhs[op + 1] -= gp[1]; rhs[op + 2] -= gp[2];
+            q0[op] += R[0]; q1[op] += R[1]; q1[op + 1] += R[2];
+            q2[op] += R[3]; q2[op + 1] += R[4]; q2[op + 2] += R[5];
+            rhs[op] -= R[6]; rhs[op + 1] -= R[7]; rhs[op + 2] -= R[8];
+#pragma unroll
+            for (int i = 0; i < 3; ++i) {
+              float* qa = w.H + w.rbase[oA + i];
+              qa[op] += R[9 + 3 * i]; qa[op + 1] += R[10 + 3 * i]; qa[op + 2] += R[11 + 3 * i];
+            }
           }
         }
-        __syncwarp();
       }
       if (inl && ((mk.act >> l) & 1ull)) {
         float* r0p = w.H + w.rbase[ol];
         float* r1p = w.H + w.rbase[ol + 1];
         r0p[ol] += Lxx; r1p[ol] += Lxy; r1p[ol + 1] += Lyy;
-        rhs[ol] -= gx; rhs[ol + 1] -= gy;
+        rhs[ol] -= bgx; rhs[ol + 1] -= bgy;
+        if (Lxx != 0.f || Lyy != 0.f) {  // anchor rows x landmark columns: a0 = -g0, a1 = -g1, a2
+          float* qa0 = w.H + w.rbase[oA];
+          float* qa1 = w.H + w.rbase[oA + 1];
+          float* qa2 = w.H + w.rbase[oA + 2];
+          qa0[ol] -= Lxx; qa0[ol + 1] -= Lxy;
+          qa1[ol] -= Lxy; qa1[ol + 1] -= Lyy;
+          qa2[ol] += ag0; qa2[ol + 1] += ag1;
+        }
       }
       __syncwarp();
     }
+#pragma unroll
+    for (int t = 0; t < 9; ++t) A[t] = warp_sum(A[t]);
+    if (lane == 0) {  // anchor diagonal block and gradient
+      float* qa0 = w.H + w.rbase[oA];
+      float* qa1 = w.H + w.rbase[oA + 1];
+      float* qa2 = w.H + w.rbase[oA + 2];
+      qa0[oA] += A[0]; qa1[oA] += A[1]; qa1[oA + 1] += A[2];
+      qa2[oA] -= A[3]; qa2[oA + 1] -= A[4]; qa2[oA + 2] += A[5];
+      rhs[oA] += A[6]; rhs[oA + 1] += A[7]; rhs[oA + 2] -= A[8];
+    }
+    __syncwarp();
   }
 }
 
@@ -802,8 +864,7 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
     } else {
       const int q = p - 3 - 3 * npn, b = q >> 1, j = q & 1, l = nth_set_bit(nls, b);
       id = st_lm(ly, l) + j;
-      X0 = j == 0 ? 1.f : 0.f; X1 = j == 1 ? 1.f : 0.f;
-      X2 = j == 0 ? -(w.st[st_lm(ly, l) + 1] - y1) : (w.st[st_lm(ly, l)] - x1);
+      X0 = 0.f; X1 = 0.f; X2 = 0.f;  // landmarks are global: untouched by re-anchoring
     }
     nidx[p] = id;
     X[3 * p] = X0; X[3 * p + 1] = X1; X[3 * p + 2] = X2;
@@ -846,21 +907,40 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
       }
     }
   }
-  for (int base = 0; base < L; base += 32) {
-    const int l = base + lane;
-    if (l < L && ((rb0 >> l) & 1ull)) {
-      const float zr = rec[ly.o_zrb + (head * 2 + 0) * L + l], zb = rec[ly.o_zrb + (head * 2 + 1) * L + l];
-      const float dx = w.st[st_lm(ly, l)], dy = w.st[st_lm(ly, l) + 1];
-      const float q = dx * dx + dy * dy, irho = rsqrtf(q), rho = q * irho, iq = irho * irho;
-      const float r0 = rho - zr, r1 = wrapf(atan2f(dy, dx) - zb);
-      const float ux = dx * irho, uy = dy * irho, vx = -dy * iq, vy = dx * iq;
-      const float a0 = pr.om_rb[0] * ux, a1 = pr.om_rb[0] * uy, b0 = pr.om_rb[1] * vx, b1 = pr.om_rb[1] * vy;
-      const int P = 3 + 3 * npn + 2 * __popcll(nls & lowmask(l));
-      Hs[tri(P, P)] += a0 * ux + b0 * vx;
-      Hs[tri(P + 1, P)] += a1 * ux + b1 * vx;
-      Hs[tri(P + 1, P + 1)] += a1 * uy + b1 * vy;
-      gam[P] += a0 * r0 + b0 * r1;
-      gam[P + 1] += a1 * r0 + b1 * r1;
+  if (L > 0 && rb0) {  // range-bearing from slot 0 (observing pose x = a): blocks a and g
+    float A[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+    for (int base = 0; base < L; base += 32) {
+      const int l = base + lane;
+      if (l < L && ((rb0 >> l) & 1ull)) {
+        const float zr = rec[ly.o_zrb + (head * 2 + 0) * L + l], zb = rec[ly.o_zrb + (head * 2 + 1) * L + l];
+        const float gxl = w.st[st_lm(ly, l)] - w.st[0], gyl = w.st[st_lm(ly, l) + 1] - w.st[1];
+        const float dx = ca * gxl + sa * gyl, dy = -sa * gxl + ca * gyl;  // m = Rot(a_th)'(g - a_t)
+        const float q = dx * dx + dy * dy, irho = rsqrtf(q), rho = q * irho, iq = irho * irho;
+        const float r0 = rho - zr, r1 = wrapf(atan2f(dy, dx) - zb);
+        const float ux = dx * irho, uy = dy * irho, vx = -dy * iq, vy = dx * iq;
+        const float Ux = ca * ux - sa * uy, Uy = sa * ux + ca * uy, Vx = ca * vx - sa * vy, Vy = sa * vx + ca * vy;
+        const float j0 = ux * dy - uy * dx, j1 = vx * dy - vy * dx;       // = 0, -1 (kept in the general form)
+        const float wg0a = pr.om_rb[0] * Ux, wg0b = pr.om_rb[1] * Vx, wg1a = pr.om_rb[0] * Uy, wg1b = pr.om_rb[1] * Vy;
+        const float wa2a = pr.om_rb[0] * j0, wa2b = pr.om_rb[1] * j1;
+        const float gg00 = wg0a * Ux + wg0b * Vx, gg01 = wg0a * Uy + wg0b * Vy, gg11 = wg1a * Uy + wg1b * Vy;
+        const float a2g0 = wa2a * Ux + wa2b * Vx, a2g1 = wa2a * Uy + wa2b * Vy, a2a2 = wa2a * j0 + wa2b * j1;
+        const float g0r = wg0a * r0 + wg0b * r1, g1r = wg1a * r0 + wg1b * r1, a2r = wa2a * r0 + wa2b * r1;
+        const int P = 3 + 3 * npn + 2 * __popcll(nls & lowmask(l));
+        Hs[tri(P, P)] += gg00; Hs[tri(P + 1, P)] += gg01; Hs[tri(P + 1, P + 1)] += gg11;
+        gam[P] += g0r; gam[P + 1] += g1r;
+        // landmark rows x anchor columns: <g_i, a_j>, a0 = -g0, a1 = -g1, a2 = (j0, j1)
+        Hs[tri(P, 0)] -= gg00; Hs[tri(P, 1)] -= gg01; Hs[tri(P, 2)] += a2g0;
+        Hs[tri(P + 1, 0)] -= gg01; Hs[tri(P + 1, 1)] -= gg11; Hs[tri(P + 1, 2)] += a2g1;
+        A[0] += gg00; A[1] += gg01; A[2] += gg11; A[3] += a2g0; A[4] += a2g1; A[5] += a2a2;
+        A[6] += g0r; A[7] += g1r; A[8] += a2r;
+      }
+    }
+#pragma unroll
+    for (int t = 0; t < 9; ++t) A[t] = warp_sum(A[t]);
+    if (lane == 0) {
+      Hs[tri(0, 0)] += A[0]; Hs[tri(1, 0)] += A[1]; Hs[tri(1, 1)] += A[2];
+      Hs[tri(2, 0)] -= A[3]; Hs[tri(2, 1)] -= A[4]; Hs[tri(2, 2)] += A[5];
+      gam[0] -= A[6]; gam[1] -= A[7]; gam[2] += A[8];
     }
   }
   __syncwarp();
@@ -890,8 +970,8 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
   // --- G. G = E' H_s E block by block (in place);  T_b = E_b' Q_b;  gamma_b = E_b' gamma_b
   auto etype = [&](int b) -> Etype {
     if (b == 0) return Etype{1.f, 0.f, ddy, -ddx};          // A = da/da'
-    if (b == 1) return Etype{1.f, 0.f, 0.f, 0.f};           // w: identity
-    return Etype{c1, s1, 0.f, 0.f};                         // blockdiag(Rot(th_1), 1) / Rot(th_1)
+    if (b == 1 || b > npn) return Etype{1.f, 0.f, 0.f, 0.f};  // w and the (global) landmarks: identity
+    return Etype{c1, s1, 0.f, 0.f};                           // blockdiag(Rot(th_1), 1)
   };
   auto bpos = [&](int b) -> int { return b == 0 ? 0 : (b <= npn ? 3 + 3 * (b - 1) : 3 + 3 * npn + 2 * (b - 1 - npn)); };
   const int npairs = nbk * (nbk + 1) >> 1;
@@ -987,12 +1067,6 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
       float* e = w.st + st_pose(k);
       const float ex = e[0] - x1, ey = e[1] - y1;
       e[0] = c1 * ex + s1 * ey; e[1] = -s1 * ex + c1 * ey; e[2] = wrapf(e[2] - th1);
-    }
-    for (int l = lane; l < L; l += 32) {
-      if (!((mk.act >> l) & 1ull)) continue;
-      float* m = w.st + st_lm(ly, l);
-      const float ex = m[0] - x1, ey = m[1] - y1;
-      m[0] = c1 * ex + s1 * ey; m[1] = -s1 * ex + c1 * ey;
     }
     __syncwarp();
     if (lane == 0) { w.st[0] = nax; w.st[1] = nay; w.st[2] = nat; }
