@@ -32,19 +32,18 @@ __global__ void __launch_bounds__(256) slam_step_kernel(Layout ly, Params pr, fl
     if (flags & F_PUSH) cc = push_env(ly, rec, w, lane, env, head, cc, io, mk);
     const int s = build_support(ly, w, lane, cc, mk.ps, mk.ls);
     if (iters > 0 || (flags & F_COV)) {
-      int nLR = 0;
-      const int total = symbolic(ly, w, lane, cc, mk, s, nLR);
+      const int total = symbolic(ly, w, lane, cc, mk, s);
       for (int it = 0; it < iters; ++it) {
         assemble(ly, pr, rec, w, lane, head, cc, mk, s, total);
         __syncwarp();
-        status |= cholesky(ly, w, lane, nLR);
+        status |= cholesky(ly, w, lane);
         back_substitute(ly, w, lane);
         status |= apply_update(ly, w, lane, cc, mk);
       }
       if (flags & F_COV) {
         assemble(ly, pr, rec, w, lane, head, cc, mk, s, total);
         __syncwarp();
-        status |= cholesky(ly, w, lane, nLR);
+        status |= cholesky(ly, w, lane);
         covariance(ly, w, lane, env, cc, io);
         __syncwarp();
       }

@@ -10,10 +10,12 @@
 //   S5 marginalise re-anchor + Schur complement of the oldest pose on the prior's support
 //
 // Elimination order of the window variables (scalar offsets):
-//   [ e_1 .. e_{W-2} (chain, 3 each) | m_0 .. m_{L-1} (2 each) | newest pose e_{c-1} (3) | anchor a (3) ]
+//   [ e_1 .. e_{W-2} (chain, 3 each) | g_0 .. g_{L-1} (2 each) | pad | newest pose e_{c-1} (3) | anchor a (3) ]
+// (pad = 0..3 dummy identity rows so that the dimension np is a multiple of 4: the factorisation
+// works on 4-column blocks with 128-bit shared-memory loads)
 // so that the covariance read-out needs only the trailing 6x6 of L, and the weakly determined
 // global anchor `a` (touched by the prior only) is never added into the well determined relative
-// blocks.  Row n (= 3W+2L) of the envelope storage is the right-hand side b.
+// blocks.  Row np of the envelope storage is the right-hand side b (row np+1 is its zero twin).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -33,14 +35,14 @@ struct StepIO {
 
 struct WS {  // per-warp views into shared memory
   float* st; float* zodo; float* zlc; int* lct; float* cs; uint32_t* rbm;
-  int* first; int* rbase; int* LR; int* ssup; int* sidx; float* sds; float* H;
+  int* first; int* rbase; int* ssup; int* sidx; float* sds; float* H;
 };
 
 __device__ __forceinline__ WS make_ws(const Layout& ly, float* base) {
   WS w;
   w.st = base + ly.s_st; w.zodo = base + ly.s_zodo; w.zlc = base + ly.s_zlc;
   w.lct = (int*)(base + ly.s_lct); w.cs = base + ly.s_cs; w.rbm = (uint32_t*)(base + ly.s_rbm);
-  w.first = (int*)(base + ly.s_first); w.rbase = (int*)(base + ly.s_rbase); w.LR = (int*)(base + ly.s_lr);
+  w.first = (int*)(base + ly.s_first); w.rbase = (int*)(base + ly.s_rbase);
   w.ssup = (int*)(base + ly.s_ssup); w.sidx = (int*)(base + ly.s_sidx); w.sds = base + ly.s_sds;
   w.H = base + ly.s_H;
   return w;
@@ -83,8 +85,8 @@ __device__ __forceinline__ int ring_of(int slot, int head, int W) { int r = head
 __device__ __forceinline__ int st_pose(int k) { return 3 + 3 * k; }
 __device__ __forceinline__ int st_lm(const Layout& ly, int l) { return 3 + 3 * ly.W + 2 * l; }
 // elimination offsets
-__device__ __forceinline__ int off_new(const Layout& ly) { return 3 * (ly.W - 2) + 2 * ly.L; }
-__device__ __forceinline__ int off_a(const Layout& ly) { return 3 * (ly.W - 2) + 2 * ly.L + 3; }
+__device__ __forceinline__ int off_new(const Layout& ly) { return 3 * (ly.W - 2) + 2 * ly.L + ly.pad; }
+__device__ __forceinline__ int off_a(const Layout& ly) { return 3 * (ly.W - 2) + 2 * ly.L + ly.pad + 3; }
 __device__ __forceinline__ int off_lm(const Layout& ly, int l) { return 3 * (ly.W - 2) + 2 * l; }
 __device__ __forceinline__ int off_slot(const Layout& ly, int k, int c) { return k == c - 1 ? off_new(ly) : 3 * (k - 1); }
 
@@ -229,18 +231,21 @@ __device__ int build_support(const Layout& ly, const WS& w, int lane, int c, uin
 }
 
 // ------------------------------------------------------------------ symbolic phase: envelope of H
-// first[i] = first column of row i inside the envelope; rbase[i] + j addresses H(i,j), j >= first[i];
-// LR = sorted list of "long" rows (i - first[i] > 5, plus the rhs row n).  Returns total words used.
-__device__ int symbolic(const Layout& ly, const WS& w, int lane, int c, const Masks& mk, int s, int& nLR) {
-  const int W = ly.W, L = ly.L, n = ly.n;
-  const int oN = off_new(ly), oA = off_a(ly), oL = off_lm(ly, 0);
+// Rows are grouped in fours; all rows of group g store the columns [first, 4g+3] (whole 4x4 tiles,
+// first a multiple of 4), so every tile row is one aligned 128-bit word.  first[i] = first column
+// of row i; rbase[i] + j addresses H(i,j).  Rows np (rhs) and np+1 (zero twin) span [0, np).
+// Returns the total words used.
+__device__ int symbolic(const Layout& ly, const WS& w, int lane, int c, const Masks& mk, int s) {
+  const int L = ly.L, np = ly.np;
+  const int oN = off_new(ly), oA = off_a(ly), oL = off_lm(ly, 0), oP = oL + 2 * L;
   // own block offsets
-  for (int i = lane; i <= n; i += 32) {
+  for (int i = lane; i < np + 2; i += 32) {
     int f;
     if (i < oL) f = (i / 3) * 3;
-    else if (i < oN) f = oL + ((i - oL) >> 1) * 2;
+    else if (i < oP) f = oL + ((i - oL) >> 1) * 2;
+    else if (i < oN) f = i;
     else if (i < oA) f = oN;
-    else if (i < n) f = oA;
+    else if (i < np) f = oA;
     else f = 0;
     w.first[i] = f;
   }
@@ -270,7 +275,7 @@ __device__ int symbolic(const Layout& ly, const WS& w, int lane, int c, const Ma
   __syncwarp();
   // prior: all support blocks are mutually coupled
   if (s > 3) {
-    int fs = n;
+    int fs = np;
     for (int p = 3 + lane; p < s; p += 32) fs = min(fs, w.ssup[p]);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) fs = min(fs, __shfl_xor_sync(FULLMASK, fs, o));
@@ -294,23 +299,25 @@ __device__ int symbolic(const Layout& ly, const WS& w, int lane, int c, const Ma
     if (lane < 3) w.first[oA + lane] = min(w.first[oA + lane], fa);
   }
   __syncwarp();
-  // prefix sum of row lengths -> rbase; long-row list
-  int run = 0, cnt = 0;
-  for (int base = 0; base <= n; base += 32) {
+  // group rows in fours (shared first, aligned down to 4); prefix sum of the row lengths -> rbase
+  int run = 0;
+  for (int base = 0; base < np + 2; base += 32) {
     const int i = base + lane;
-    const int f = (i <= n) ? w.first[i] : 0;
-    const int len = (i <= n) ? (i - f + 1) : 0;
+    int f = 0, len = 0;
+    if (i < np) {
+      const int g4 = i & ~3;
+      f = min(min(w.first[g4], w.first[g4 + 1]), min(w.first[g4 + 2], w.first[g4 + 3])) & ~3;
+      len = g4 + 4 - f;
+    } else if (i < np + 2) {
+      len = np;
+    }
     int x = len;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(FULLMASK, x, o); if (lane >= o) x += y; }
-    if (i <= n) w.rbase[i] = run + x - len - f;
-    const bool lng = (i <= n) && ((i - f > 5) || i == n);
-    const uint32_t bal = __ballot_sync(FULLMASK, lng);
-    if (lng) w.LR[cnt + __popc(bal & ((1u << lane) - 1u))] = i;
-    cnt += __popc(bal);
+    __syncwarp();
+    if (i < np + 2) { w.first[i] = f; w.rbase[i] = run + x - len - f; }
     run += __shfl_sync(FULLMASK, x, 31);
   }
-  nLR = cnt;
   __syncwarp();
   return run;
 }
@@ -395,7 +402,7 @@ __device__ __forceinline__ void add_i_side(const WS& w, int n, int oi, const flo
 // Builds H and b (row n) at the current state.  `s` = prior support dimension.
 __device__ void assemble(const Layout& ly, const Params& pr, const float* rec, const WS& w, int lane, int head, int c,
                          const Masks& mk, int s, int total) {
-  const int W = ly.W, L = ly.L, n = ly.n;
+  const int W = ly.W, L = ly.L, n = ly.np;  // n: row index of the rhs
   for (int t = lane; t < total; t += 32) w.H[t] = 0.f;
   // cos/sin of every live pose (slot 0 is the frame itself)
   for (int k = lane; k < c; k += 32) {
@@ -411,11 +418,12 @@ __device__ void assemble(const Layout& ly, const Params& pr, const float* rec, c
     w.sds[p] = d;
   }
   __syncwarp();
-  // identity rows for unused chain slots, the unused newest slot (c == 1) and inactive landmarks
+  // identity rows for unused chain slots, the unused newest slot (c == 1), inactive landmarks, padding
   for (int i = lane; i < n; i += 32) {
     bool unused;
     if (i < 3 * (W - 2)) unused = (i / 3 + 1) > c - 2;
-    else if (i < off_new(ly)) unused = !((mk.act >> ((i - 3 * (W - 2)) >> 1)) & 1ull);
+    else if (i < 3 * (W - 2) + 2 * L) unused = !((mk.act >> ((i - 3 * (W - 2)) >> 1)) & 1ull);
+    else if (i < off_new(ly)) unused = true;
     else if (i < off_a(ly)) unused = c < 2;
     else unused = false;
     if (unused) w.H[w.rbase[i] + i] = 1.0f;
@@ -607,70 +615,131 @@ __device__ void assemble(const Layout& ly, const Params& pr, const float* rec, c
 }
 
 // ------------------------------------------------------------------ S3: envelope Cholesky + solves
-// Left-looking by columns, lanes over the rows of the column's structure: lane 0 owns the diagonal
-// row j, lanes 1..5 the short rows j+1..j+5, lanes 6..31 the long rows (LR) below j.  The diagonal
-// slot stores 1/L_jj.  Row n carries b, so on exit row n holds y = L^{-1} b.
-__device__ int cholesky(const Layout& ly, const WS& w, int lane, int nLR) {
-  const int n = ly.n;
+// Left-looking by 4-column blocks.  For block column J every lane owns a PAIR of rows below it (lane q
+// of pass p: rows 4J + 2(q + 32p), +1) and accumulates its 2x4 strip S = H - sum_K L(i,K) L(J,K)' with
+// 128-bit shared-memory loads (own rows: 2 loads, the four rows of block J: 4 broadcast loads, 32 FMA).
+// The 4x4 diagonal tile (lanes 0 and 1 of pass 0) is shuffled to every lane, factorised redundantly in
+// registers, and each lane finishes its rows by a 4-term forward substitution.  Diagonal slots store
+// 1/L_jj.  Rows np (rhs b) and np+1 ride along, so on exit row np holds y = L^{-1} b.
+__device__ __forceinline__ float4 ld4(const float* p) { return *reinterpret_cast<const float4*>(p); }
+__device__ __forceinline__ void st4(float* p, float4 v) { *reinterpret_cast<float4*>(p) = v; }
+#define FMA4(ACC, XV, BV)                                                                    \
+  ACC = fmaf(-XV.x, BV.x, ACC); ACC = fmaf(-XV.y, BV.y, ACC); ACC = fmaf(-XV.z, BV.z, ACC); \
+  ACC = fmaf(-XV.w, BV.w, ACC);
+
+__device__ int cholesky(const Layout& ly, const WS& w, int lane) {
+  const int np = ly.np, G = np >> 2;
   int flag = 0;
-  int p = 0;  // first LR entry with row > j
-  for (int j = 0; j < n; ++j) {
-    const int fj = w.first[j];
-    const float* rowj = w.H + w.rbase[j];
-    while (p < nLR && w.LR[p] <= j) ++p;
-    float dj = 0.f;
-    for (int q0 = p - 6; q0 < nLR; q0 += 32) {  // first pass: lanes 0..5 near rows, 6.. long rows
-      int i = -1;
-      const bool first_pass = (q0 == p - 6);
-      if (first_pass && lane < 6) {
-        const int ii = j + lane;
-        if (ii < n) {
-          const int fi = w.first[ii];
-          if (lane == 0 || (ii - fi <= 5 && fi <= j)) i = ii;
+  for (int J = 0; J < G; ++J) {
+    const int c0 = 4 * J;
+    const int fJ = w.first[c0];
+    const float* rJ0 = w.H + w.rbase[c0];
+    const float* rJ1 = w.H + w.rbase[c0 + 1];
+    const float* rJ2 = w.H + w.rbase[c0 + 2];
+    const float* rJ3 = w.H + w.rbase[c0 + 3];
+    float d0 = 1.f, d1 = 1.f, d2 = 1.f, d3 = 1.f, l10 = 0.f, l20 = 0.f, l21 = 0.f, l30 = 0.f, l31 = 0.f, l32 = 0.f;
+    for (int i0 = c0 + 2 * lane; i0 - 2 * lane < np + 2; i0 += 64) {
+      const bool first_pass = (i0 - 2 * lane == c0);
+      const bool act = i0 < np + 2 && w.first[i0] <= c0;
+      float4 a0 = make_float4(0.f, 0.f, 0.f, 0.f), a1 = a0;
+      float* p0 = nullptr;
+      float* p1 = nullptr;
+      if (act) {
+        p0 = w.H + w.rbase[i0];
+        p1 = w.H + w.rbase[i0 + 1];
+        a0 = ld4(p0 + c0);
+        a1 = ld4(p1 + c0);
+        for (int k = max(w.first[i0], fJ); k < c0; k += 4) {
+          const float4 x0 = ld4(p0 + k), x1 = ld4(p1 + k);
+          const float4 b0 = ld4(rJ0 + k), b1 = ld4(rJ1 + k), b2 = ld4(rJ2 + k), b3 = ld4(rJ3 + k);
+          FMA4(a0.x, x0, b0) FMA4(a0.y, x0, b1) FMA4(a0.z, x0, b2) FMA4(a0.w, x0, b3)
+          FMA4(a1.x, x1, b0) FMA4(a1.y, x1, b1) FMA4(a1.z, x1, b2) FMA4(a1.w, x1, b3)
         }
-      } else {
-        const int q = q0 + lane;
-        if (q >= p && q < nLR) { const int ii = w.LR[q]; if (w.first[ii] <= j) i = ii; }
       }
-      float acc = 0.f;
-      float* rowi = nullptr;
-      if (i >= 0) {
-        rowi = w.H + w.rbase[i];
-        acc = rowi[j];
-        const int k0 = max(w.first[i], fj);
-        for (int k = k0; k < j; ++k) acc = fmaf(-rowi[k], rowj[k], acc);
+      if (first_pass) {  // diagonal tile: lane 0 holds rows c0, c0+1; lane 1 rows c0+2, c0+3
+        const float s00 = __shfl_sync(FULLMASK, a0.x, 0);
+        const float s10 = __shfl_sync(FULLMASK, a1.x, 0), s11 = __shfl_sync(FULLMASK, a1.y, 0);
+        const float s20 = __shfl_sync(FULLMASK, a0.x, 1), s21 = __shfl_sync(FULLMASK, a0.y, 1), s22 = __shfl_sync(FULLMASK, a0.z, 1);
+        const float s30 = __shfl_sync(FULLMASK, a1.x, 1), s31 = __shfl_sync(FULLMASK, a1.y, 1), s32 = __shfl_sync(FULLMASK, a1.z, 1);
+        const float s33 = __shfl_sync(FULLMASK, a1.w, 1);
+        bool bad = !(s00 > 0.f);
+        d0 = rsqrtf(s00);
+        l10 = s10 * d0; l20 = s20 * d0; l30 = s30 * d0;
+        const float t11 = fmaf(-l10, l10, s11);
+        bad |= !(t11 > 0.f);
+        d1 = rsqrtf(t11);
+        l21 = fmaf(-l20, l10, s21) * d1; l31 = fmaf(-l30, l10, s31) * d1;
+        const float t22 = fmaf(-l21, l21, fmaf(-l20, l20, s22));
+        bad |= !(t22 > 0.f);
+        d2 = rsqrtf(t22);
+        l32 = fmaf(-l31, l21, fmaf(-l30, l20, s32)) * d2;
+        const float t33 = fmaf(-l32, l32, fmaf(-l31, l31, fmaf(-l30, l30, s33)));
+        bad |= !(t33 > 0.f);
+        d3 = rsqrtf(t33);
+        if (bad) {
+          flag |= ENV_NOT_PD;
+          if (!(s00 > 0.f)) d0 = 1.f;
+          if (!(t11 > 0.f)) d1 = 1.f;
+          if (!(t22 > 0.f)) d2 = 1.f;
+          if (!(t33 > 0.f)) d3 = 1.f;
+        }
       }
-      if (first_pass) {
-        const float dg = __shfl_sync(FULLMASK, acc, 0);
-        if (!(dg > 0.f)) { flag |= ENV_NOT_PD; dj = 1.0f; }
-        else dj = rsqrtf(dg);
+      if (act) {
+        if (first_pass && lane < 2) {
+          if (lane == 0) { a0 = make_float4(d0, 0.f, 0.f, 0.f); a1 = make_float4(l10, d1, 0.f, 0.f); }
+          else { a0 = make_float4(l20, l21, d2, 0.f); a1 = make_float4(l30, l31, l32, d3); }
+        } else {
+          a0.x *= d0; a0.y = fmaf(-a0.x, l10, a0.y) * d1;
+          a0.z = fmaf(-a0.y, l21, fmaf(-a0.x, l20, a0.z)) * d2;
+          a0.w = fmaf(-a0.z, l32, fmaf(-a0.y, l31, fmaf(-a0.x, l30, a0.w))) * d3;
+          a1.x *= d0; a1.y = fmaf(-a1.x, l10, a1.y) * d1;
+          a1.z = fmaf(-a1.y, l21, fmaf(-a1.x, l20, a1.z)) * d2;
+          a1.w = fmaf(-a1.z, l32, fmaf(-a1.y, l31, fmaf(-a1.x, l30, a1.w))) * d3;
+        }
+        st4(p0 + c0, a0);
+        st4(p1 + c0, a1);
       }
-      __syncwarp();
-      if (i >= 0) rowi[j] = (first_pass && lane == 0) ? dj : acc * dj;
     }
     __syncwarp();
   }
   return flag;
 }
 
-// Solves L' delta = y in place in row n (column-oriented: lanes over the row being eliminated).
+// Solves L' delta = y in place in row np, by 4-row blocks from the bottom: delta_I from the diagonal
+// tile (every lane redundantly), then y_K -= L(I,K)' delta_I with lanes over the column blocks K.
 __device__ void back_substitute(const Layout& ly, const WS& w, int lane) {
-  const int n = ly.n;
-  float* y = w.H + w.rbase[n];
-  for (int i = n - 1; i >= 0; --i) {
-    const float* rowi = w.H + w.rbase[i];
-    const float d = y[i] * rowi[i];
+  const int np = ly.np, G = np >> 2;
+  float* y = w.H + w.rbase[np];
+  for (int I = G - 1; I >= 0; --I) {
+    const int c0 = 4 * I;
+    const float* r0 = w.H + w.rbase[c0];
+    const float* r1 = w.H + w.rbase[c0 + 1];
+    const float* r2 = w.H + w.rbase[c0 + 2];
+    const float* r3 = w.H + w.rbase[c0 + 3];
+    const float4 yy = ld4(y + c0), t0 = ld4(r0 + c0), t1 = ld4(r1 + c0), t2 = ld4(r2 + c0), t3 = ld4(r3 + c0);
+    const float e3 = yy.w * t3.w;
+    const float e2 = fmaf(-t3.z, e3, yy.z) * t2.z;
+    const float e1 = fmaf(-t3.y, e3, fmaf(-t2.y, e2, yy.y)) * t1.y;
+    const float e0 = fmaf(-t3.x, e3, fmaf(-t2.x, e2, fmaf(-t1.x, e1, yy.x))) * t0.x;
     __syncwarp();
-    if (lane == 0) y[i] = d;
-    for (int k = w.first[i] + lane; k < i; k += 32) y[k] = fmaf(-rowi[k], d, y[k]);
+    if (lane == 0) st4(y + c0, make_float4(e0, e1, e2, e3));
+    for (int k = w.first[c0] + 4 * lane; k < c0; k += 128) {
+      const float4 x0 = ld4(r0 + k), x1 = ld4(r1 + k), x2 = ld4(r2 + k), x3 = ld4(r3 + k);
+      float4 v = ld4(y + k);
+      v.x = fmaf(-x3.x, e3, fmaf(-x2.x, e2, fmaf(-x1.x, e1, fmaf(-x0.x, e0, v.x))));
+      v.y = fmaf(-x3.y, e3, fmaf(-x2.y, e2, fmaf(-x1.y, e1, fmaf(-x0.y, e0, v.y))));
+      v.z = fmaf(-x3.z, e3, fmaf(-x2.z, e2, fmaf(-x1.z, e1, fmaf(-x0.z, e0, v.z))));
+      v.w = fmaf(-x3.w, e3, fmaf(-x2.w, e2, fmaf(-x1.w, e1, fmaf(-x0.w, e0, v.w))));
+      st4(y + k, v);
+    }
     __syncwarp();
   }
 }
 
 // v <- v + delta (R1: additive, angles wrapped).  Returns ENV_NONFINITE if the update is not finite.
 __device__ int apply_update(const Layout& ly, const WS& w, int lane, int c, const Masks& mk) {
-  const int W = ly.W, L = ly.L, n = ly.n;
-  const float* dl = w.H + w.rbase[n];
+  const int W = ly.W, L = ly.L;
+  const float* dl = w.H + w.rbase[ly.np];
   int bad = 0;
   if (lane < 3) {
     const float d = dl[off_a(ly) + lane];
@@ -701,7 +770,7 @@ __device__ int apply_update(const Layout& ly, const WS& w, int lane, int c, cons
 // Sigma_t = J Sigma_6 J' with x = a (+) e (A.4).  O(1) per environment, done in fp64 by lane 0.
 __device__ void covariance(const Layout& ly, const WS& w, int lane, int env, int c, const StepIO& io) {
   if (lane != 0) return;
-  const int n = ly.n, N = ly.N;
+  const int n = ly.np, N = ly.N;
   double S[3][3];
   if (c == 1) {
     // only the anchor exists: Sigma = (L_a L_a')^{-1}

@@ -16,11 +16,12 @@ namespace slamk {
 
 struct Layout {
   int N, W, L, n, nw;  // n = 3W + 2L state dimension, nw = ceil(L/32) mask words
+  int np, pad;         // matrix dimension padded to a multiple of 4 (pad dummy rows before the newest pose)
   // record (32-bit words)
   int rec;             // record stride
   int o_status, o_pm, o_lm, o_act, o_a, o_e, o_m, o_zodo, o_lct, o_zlc, o_rbm, o_zrb, o_vbar, o_g, o_lam;
   // shared memory per warp (32-bit words)
-  int s_st, s_zodo, s_zlc, s_lct, s_cs, s_rbm, s_first, s_rbase, s_lr, s_ssup, s_sidx, s_sds, s_H;
+  int s_st, s_zodo, s_zlc, s_lct, s_cs, s_rbm, s_first, s_rbase, s_ssup, s_sidx, s_sds, s_H;
   int cap;             // words available for H (envelope + rhs row) / marginalisation scratch
   int warp_words;      // total shared words per warp
   int wpc;             // warps per CTA
@@ -36,6 +37,7 @@ static inline int pad4(int x) { return (x + 3) & ~3; }
 static inline Layout make_layout(int N, int W, int L, int cap, int wpc) {
   Layout y;
   y.N = N; y.W = W; y.L = L; y.n = 3 * W + 2 * L; y.nw = (L + 31) / 32;
+  y.np = (y.n + 3) & ~3; y.pad = y.np - y.n;
   int n = y.n, o = 0;
   y.o_status = o; o += 1;
   y.o_pm = o; o += 2;
@@ -62,14 +64,17 @@ static inline Layout make_layout(int N, int W, int L, int cap, int wpc) {
   y.s_lct = s; s = pad4(s + W);
   y.s_cs = s; s = pad4(s + 2 * W);
   y.s_rbm = s; s = pad4(s + W * y.nw);
-  y.s_first = s; s = pad4(s + n + 1);
-  y.s_rbase = s; s = pad4(s + n + 2);
-  y.s_lr = s; s = pad4(s + n + 2);
+  y.s_first = s; s = pad4(s + y.np + 2);
+  y.s_rbase = s; s = pad4(s + y.np + 2);
   y.s_ssup = s; s = pad4(s + n);
   y.s_sidx = s; s = pad4(s + n);
   y.s_sds = s; s = pad4(s + n);
   y.s_H = s;
-  int dense = n * (n + 1) / 2 + 8 * n + 16;
+  // dense capacity: full 4x4 tiles of the lower triangle + two rhs rows; or the marginalisation scratch
+  const int G = y.np / 4;
+  int dense = 8 * G * (G + 1) + 2 * y.np;
+  const int marg = n * (n + 1) / 2 + 8 * n + 16;
+  if (marg > dense) dense = marg;
   y.cap = pad4(cap < 0 ? dense : cap);
   s += y.cap;
   y.warp_words = pad4(s);
