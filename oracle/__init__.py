@@ -198,7 +198,7 @@ def max_threads() -> int:
 
 
 def run_batch(data: dict, iters: int, envs=None, sigmas=DEFAULT_SIGMAS, threads: int = 0,
-              want=("poses", "cov", "logdet", "step")) -> dict:
+              want=("poses", "cov", "logdet", "step"), f32_storage: bool = False) -> dict:
     """Run push -> solve -> cov -> (marginalize iff full) over ``data`` (a ``synth.generate`` dict, float32
     arrays) for the environments ``envs`` (column indices into the arrays).  Returns float64 arrays
     ``poses[T,ne,W,3]``, ``cov[T,ne,3,3]``, ``logdet[T,ne]``, ``step[T,ne]`` and ``bad`` (#singular envs)."""
@@ -219,8 +219,10 @@ def run_batch(data: dict, iters: int, envs=None, sigmas=DEFAULT_SIGMAS, threads:
     sig = _d(sigmas)
     ptr = lambda a: None if a is None else _p(a)
     vp = lambda a: a.ctypes.data_as(C.c_void_p)
+    lib().orc_batch_set_f32_storage(int(f32_storage))
     bad = lib().orc_run_batch(N, W, L, T, iters, _p(sig), vp(odom), vp(lc_back), vp(lc_meas), vp(rb_mask),
                               vp(rb_meas), envs.ctypes.data_as(_ip), ne, int(threads),
                               ptr(out["poses"]), ptr(out["cov"]), ptr(out["logdet"]), ptr(out["step"]))
+    lib().orc_batch_set_f32_storage(0)
     out["bad"] = bad
     return out

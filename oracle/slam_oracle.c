@@ -18,6 +18,7 @@
 
 struct orc {
   int W, L, n, c, linear;
+  int f32_storage; /* conditioning probe: round H, b, the prior and the state to fp32 (see slam_oracle.h) */
   double sig[11];
   double a[3];      /* global pose of the anchor (slot 0) */
   double* e;        /* [W][3] slot poses in the anchor frame, e[0] == 0 */
@@ -402,12 +403,18 @@ static void mask_unused(const orc* o, double* H, double* b) {
   }
 }
 
+void orc_set_f32_storage(orc* o, int on) { o->f32_storage = on; }
+
 void orc_assemble(const orc* o, double* H, double* b) {
   int n = o->n;
   double* grad = (double*)malloc(sizeof(double) * n);
   build_system(o, 0, H, grad, NULL);
   for (int i = 0; i < n; ++i) grad[i] = -grad[i]; /* b = -(Lam d + g) - sum J'Omega r */
   mask_unused(o, H, grad);
+  if (o->f32_storage) {
+    for (int i = 0; i < n * n; ++i) H[i] = (double)(float)H[i];
+    for (int i = 0; i < n; ++i) grad[i] = (double)(float)grad[i];
+  }
   if (b) memcpy(b, grad, sizeof(double) * n);
   free(grad);
 }
@@ -433,6 +440,7 @@ int orc_solve(orc* o, int iters, double* last_step_norm) {
     double mx = 0.0;
     for (int i = 0; i < n; ++i) { v[i] += b[i]; if (fabs(b[i]) > mx) mx = fabs(b[i]); }
     for (int k = 0; k < o->W; ++k) v[3 * k + 2] = owrap(o, v[3 * k + 2]);
+    if (o->f32_storage) for (int i = 0; i < n; ++i) v[i] = (double)(float)v[i];
     orc_set_state(o, v);
     if (last_step_norm) *last_step_norm = mx;
   }
@@ -649,6 +657,15 @@ int orc_marginalize(orc* o) {
   o->lc_tgt[c - 1] = -1;
   memset(o->rb_valid + (c - 1) * L, 0, sizeof(int) * L);
   o->c = c - 1;
+  if (o->f32_storage) {
+    double* sv = (double*)malloc(sizeof(double) * n);
+    orc_get_state(o, sv);
+    for (int i = 0; i < n; ++i) sv[i] = (double)(float)sv[i];
+    orc_set_state(o, sv);
+    free(sv);
+    for (size_t i = 0; i < nn; ++i) o->Lam[i] = (double)(float)o->Lam[i];
+    for (int i = 0; i < n; ++i) o->g[i] = (double)(float)o->g[i];
+  }
   orc_get_state(o, o->vbar); /* d = 0 right after marginalization */
 
   free(Hs); free(gs); free(M); free(Nm); free(T); free(Hu); free(gu); free(Lp); free(gp); free(newidx);
@@ -665,6 +682,9 @@ int orc_max_threads(void) {
 #endif
 }
 
+static int g_batch_f32_storage = 0;
+void orc_batch_set_f32_storage(int on) { g_batch_f32_storage = on; }
+
 int orc_run_batch(int N, int W, int L, int T, int iters, const double* sig11,
                   const float* odom, const int* lc_back, const float* lc_meas,
                   const unsigned* rb_mask, const float* rb_meas,
@@ -679,6 +699,7 @@ int orc_run_batch(int N, int W, int L, int T, int iters, const double* sig11,
   for (int q = 0; q < ne; ++q) {
     int env = envs[q];
     orc* o = orc_create(W, L, sig11, 0);
+    o->f32_storage = g_batch_f32_storage;
     int* valid = (int*)calloc(L + 1, sizeof(int));
     double* zrb = (double*)calloc(2 * (L + 1), sizeof(double));
     int failed = 0;

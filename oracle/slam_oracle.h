@@ -73,6 +73,14 @@ void orc_rb_factor(const double* a3, const double* ek3, const double* gl2, const
 void orc_reanchor_map(const orc*, const double* v, double* u);
 void orc_reanchor_jac(const orc*, double* M /* [n*n] */);
 
+/* Conditioning probe (not a second implementation): with f32 storage on, the SAME fp64 algorithm rounds
+ * the assembled H and b, the marginalisation prior and the state vector to fp32 before using them.
+ * The distance between this run and the plain run is a lower bound on the error of ANY implementation
+ * that stores those quantities in fp32; the parity tests use it to recognise the env-steps on which
+ * the stated tolerances cannot be met in fp32 at all. */
+void orc_set_f32_storage(orc*, int on);
+void orc_batch_set_f32_storage(int on);
+
 /* ---- batch driver: push -> solve -> cov -> (marginalize iff count == W), T steps, a set of envs.
  * Input arrays are float32, environment-fastest, exactly as the generator wrote them and as the
  * library consumes them (include/slam.h); `envs[ne]` selects which environments to run.

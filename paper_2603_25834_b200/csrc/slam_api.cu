@@ -30,18 +30,19 @@ __global__ void __launch_bounds__(256) slam_step_kernel(Layout ly, Params pr, fl
     load_env(ly, rec, w, lane, head, cc, mk);
     if (flags & F_OBS0) record_rb(ly, rec, w, lane, env, head, 0, 0.f, 0.f, 0.f, io, mk);
     if (flags & F_PUSH) cc = push_env(ly, rec, w, lane, env, head, cc, io, mk);
-    const int s = build_support(ly, w, lane, cc, mk.ps, mk.ls);
+    const Ord od = make_ord(ly, w.rbm, cc);
+    const int s = build_support(ly, od, w, lane, cc, mk.ps, mk.ls);
     if (iters > 0 || (flags & F_COV)) {
-      const int total = symbolic(ly, w, lane, cc, mk, s);
+      const int total = symbolic(ly, od, w, lane, cc, mk, s);
       for (int it = 0; it < iters; ++it) {
-        assemble(ly, pr, rec, w, lane, head, cc, mk, s, total);
+        assemble(ly, pr, od, rec, w, lane, head, cc, mk, s, total);
         __syncwarp();
         status |= cholesky(ly, w, lane);
         back_substitute(ly, w, lane);
-        status |= apply_update(ly, w, lane, cc, mk);
+        status |= apply_update(ly, od, w, lane, cc, mk);
       }
       if (flags & F_COV) {
-        assemble(ly, pr, rec, w, lane, head, cc, mk, s, total);
+        assemble(ly, pr, od, rec, w, lane, head, cc, mk, s, total);
         __syncwarp();
         status |= cholesky(ly, w, lane);
         covariance(ly, w, lane, env, cc, io);

@@ -10,7 +10,7 @@
 //   S5 marginalise re-anchor + Schur complement of the oldest pose on the prior's support
 //
 // Elimination order of the window variables (scalar offsets):
-//   [ e_1 .. e_{W-2} (chain, 3 each) | g_0 .. g_{L-1} (2 each) | pad | newest pose e_{c-1} (3) | anchor a (3) ]
+//   [ passive landmarks | e_1 .. e_{W-2} (chain, 3 each) | observed landmarks | pad | newest pose e_{c-1} (3) | anchor a (3) ]
 // (pad = 0..3 dummy identity rows so that the dimension np is a multiple of 4: the factorisation
 // works on 4-column blocks with 128-bit shared-memory loads)
 // so that the covariance read-out needs only the trailing 6x6 of L, and the weakly determined
@@ -85,10 +85,31 @@ __device__ __forceinline__ int ring_of(int slot, int head, int W) { int r = head
 __device__ __forceinline__ int st_pose(int k) { return 3 + 3 * k; }
 __device__ __forceinline__ int st_lm(const Layout& ly, int l) { return 3 + 3 * ly.W + 2 * l; }
 // elimination offsets
+// Per-environment elimination order: landmarks WITHOUT a live range-bearing factor in the window
+// ("passive": coupled through the prior only, or never seen) come first, then the chain poses, then the
+// observed landmarks, padding, the newest pose and the anchor.  obs = landmarks observed from any slot.
+struct Ord { uint64_t obs; int npas; };
 __device__ __forceinline__ int off_new(const Layout& ly) { return 3 * (ly.W - 2) + 2 * ly.L + ly.pad; }
 __device__ __forceinline__ int off_a(const Layout& ly) { return 3 * (ly.W - 2) + 2 * ly.L + ly.pad + 3; }
-__device__ __forceinline__ int off_lm(const Layout& ly, int l) { return 3 * (ly.W - 2) + 2 * l; }
-__device__ __forceinline__ int off_slot(const Layout& ly, int k, int c) { return k == c - 1 ? off_new(ly) : 3 * (k - 1); }
+__device__ __forceinline__ int off_lm(const Layout& ly, const Ord& od, int l) {
+  const uint64_t below = lowmask(l);
+  return ((od.obs >> l) & 1ull) ? 2 * od.npas + 3 * (ly.W - 2) + 2 * __popcll(od.obs & below)
+                                : 2 * __popcll(~od.obs & below);
+}
+__device__ __forceinline__ int off_slot(const Layout& ly, const Ord& od, int k, int c) {
+  return k == c - 1 ? off_new(ly) : 2 * od.npas + 3 * (k - 1);
+}
+__device__ __forceinline__ Ord make_ord(const Layout& ly, const uint32_t* rbm, int c) {
+  uint64_t obs = 0ull;
+  for (int k = 0; k < c; ++k) {
+    obs |= (uint64_t)rbm[k * ly.nw];
+    if (ly.nw > 1) obs |= (uint64_t)rbm[k * ly.nw + 1] << 32;
+  }
+  Ord od;
+  od.obs = obs & lowmask(ly.L);
+  od.npas = ly.L - __popcll(od.obs);
+  return od;
+}
 
 struct Masks {  // warp-uniform
   uint64_t ps;   // prior support, pose SLOTS (bit k = slot k)
@@ -211,7 +232,7 @@ __device__ int push_env(const Layout& ly, float* rec, const WS& w, int lane, int
 // ------------------------------------------------------------------ prior support tables
 // For support scalar p (canonical order [a | poses by slot | landmarks]): elimination offset in
 // ssup[p], state index in sidx[p] (bit 16 set for angle components).  Returns the support dimension.
-__device__ int build_support(const Layout& ly, const WS& w, int lane, int c, uint64_t ps, uint64_t ls) {
+__device__ int build_support(const Layout& ly, const Ord& od, const WS& w, int lane, int c, uint64_t ps, uint64_t ls) {
   const int npo = __popcll(ps), nlo = __popcll(ls);
   const int s = 3 + 3 * npo + 2 * nlo;
   for (int p = lane; p < s; p += 32) {
@@ -219,10 +240,10 @@ __device__ int build_support(const Layout& ly, const WS& w, int lane, int c, uin
     if (p < 3) { off = off_a(ly) + p; idx = p | (p == 2 ? 0x10000 : 0); }
     else if (p < 3 + 3 * npo) {
       const int b = (p - 3) / 3, j = (p - 3) - 3 * b, k = nth_set_bit(ps, b);
-      off = off_slot(ly, k, c) + j; idx = (st_pose(k) + j) | (j == 2 ? 0x10000 : 0);
+      off = off_slot(ly, od, k, c) + j; idx = (st_pose(k) + j) | (j == 2 ? 0x10000 : 0);
     } else {
       const int q = p - 3 - 3 * npo, b = q >> 1, j = q & 1, l = nth_set_bit(ls, b);
-      off = off_lm(ly, l) + j; idx = st_lm(ly, l) + j;
+      off = off_lm(ly, od, l) + j; idx = st_lm(ly, l) + j;
     }
     w.ssup[p] = off; w.sidx[p] = idx;
   }
@@ -235,13 +256,14 @@ __device__ int build_support(const Layout& ly, const WS& w, int lane, int c, uin
 // first a multiple of 4), so every tile row is one aligned 128-bit word.  first[i] = first column
 // of row i; rbase[i] + j addresses H(i,j).  Rows np (rhs) and np+1 (zero twin) span [0, np).
 // Returns the total words used.
-__device__ int symbolic(const Layout& ly, const WS& w, int lane, int c, const Masks& mk, int s) {
+__device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, int lane, int c, const Masks& mk, int s) {
   const int L = ly.L, np = ly.np;
-  const int oN = off_new(ly), oA = off_a(ly), oL = off_lm(ly, 0), oP = oL + 2 * L;
+  const int oC = 2 * od.npas, oL = oC + 3 * (ly.W - 2), oP = 3 * (ly.W - 2) + 2 * L, oN = off_new(ly), oA = off_a(ly);
   // own block offsets
   for (int i = lane; i < np + 2; i += 32) {
     int f;
-    if (i < oL) f = (i / 3) * 3;
+    if (i < oC) f = i & ~1;
+    else if (i < oL) f = oC + ((i - oC) / 3) * 3;
     else if (i < oP) f = oL + ((i - oL) >> 1) * 2;
     else if (i < oN) f = i;
     else if (i < oA) f = oN;
@@ -252,24 +274,24 @@ __device__ int symbolic(const Layout& ly, const WS& w, int lane, int c, const Ma
   __syncwarp();
   // pose rows
   for (int k = 1 + lane; k < c; k += 32) {
-    const int o = off_slot(ly, k, c);
+    const int o = off_slot(ly, od, k, c);
     int f = o;
-    if (k >= 2) f = min(f, off_slot(ly, k - 1, c));
+    if (k >= 2) f = min(f, off_slot(ly, od, k - 1, c));
     const int t = w.lct[k];
-    if (t >= 1) f = min(f, off_slot(ly, t, c));
+    if (t >= 1) f = min(f, off_slot(ly, od, t, c));
     if (k == c - 1 && L > 0) {  // newest pose comes after the landmarks it observes
       uint64_t m = (uint64_t)w.rbm[k * ly.nw];
       if (ly.nw > 1) m |= (uint64_t)w.rbm[k * ly.nw + 1] << 32;
-      if (m) f = min(f, off_lm(ly, __ffsll((long long)m) - 1));
+      if (m) f = min(f, off_lm(ly, od, __ffsll((long long)m) - 1));
     }
     w.first[o] = f; w.first[o + 1] = f; w.first[o + 2] = f;
   }
   // landmark rows: first chain pose (slots 1..c-2) that observes them
   for (int l = lane; l < L; l += 32) {
-    const int o = off_lm(ly, l);
+    const int o = off_lm(ly, od, l);
     int f = o;
     for (int k = 1; k <= c - 2; ++k)
-      if ((w.rbm[k * ly.nw + (l >> 5)] >> (l & 31)) & 1u) { f = 3 * (k - 1); break; }
+      if ((w.rbm[k * ly.nw + (l >> 5)] >> (l & 31)) & 1u) { f = oC + 3 * (k - 1); break; }
     w.first[o] = f; w.first[o + 1] = f;
   }
   __syncwarp();
@@ -290,8 +312,8 @@ __device__ int symbolic(const Layout& ly, const WS& w, int lane, int c, const Ma
       uint64_t m = (uint64_t)w.rbm[k * ly.nw];
       if (ly.nw > 1) m |= (uint64_t)w.rbm[k * ly.nw + 1] << 32;
       if (m) {
-        if (k >= 1) fa = min(fa, off_slot(ly, k, c));
-        fa = min(fa, off_lm(ly, __ffsll((long long)m) - 1));
+        if (k >= 1) fa = min(fa, off_slot(ly, od, k, c));
+        fa = min(fa, off_lm(ly, od, __ffsll((long long)m) - 1));
       }
     }
 #pragma unroll
@@ -400,8 +422,8 @@ __device__ __forceinline__ void add_i_side(const WS& w, int n, int oi, const flo
 }
 
 // Builds H and b (row n) at the current state.  `s` = prior support dimension.
-__device__ void assemble(const Layout& ly, const Params& pr, const float* rec, const WS& w, int lane, int head, int c,
-                         const Masks& mk, int s, int total) {
+__device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, const float* rec, const WS& w, int lane, int head,
+                         int c, const Masks& mk, int s, int total) {
   const int W = ly.W, L = ly.L, n = ly.np;  // n: row index of the rhs
   for (int t = lane; t < total; t += 32) w.H[t] = 0.f;
   // cos/sin of every live pose (slot 0 is the frame itself)
@@ -419,14 +441,18 @@ __device__ void assemble(const Layout& ly, const Params& pr, const float* rec, c
   }
   __syncwarp();
   // identity rows for unused chain slots, the unused newest slot (c == 1), inactive landmarks, padding
-  for (int i = lane; i < n; i += 32) {
-    bool unused;
-    if (i < 3 * (W - 2)) unused = (i / 3 + 1) > c - 2;
-    else if (i < 3 * (W - 2) + 2 * L) unused = !((mk.act >> ((i - 3 * (W - 2)) >> 1)) & 1ull);
-    else if (i < off_new(ly)) unused = true;
-    else if (i < off_a(ly)) unused = c < 2;
-    else unused = false;
-    if (unused) w.H[w.rbase[i] + i] = 1.0f;
+  for (int k = max(c - 1, 1) + lane; k <= W - 2; k += 32) {
+    const int o = 2 * od.npas + 3 * (k - 1);
+    w.H[w.rbase[o] + o] = 1.0f; w.H[w.rbase[o + 1] + o + 1] = 1.0f; w.H[w.rbase[o + 2] + o + 2] = 1.0f;
+  }
+  for (int l = lane; l < L; l += 32)
+    if (!((mk.act >> l) & 1ull)) {
+      const int o = off_lm(ly, od, l);
+      w.H[w.rbase[o] + o] = 1.0f; w.H[w.rbase[o + 1] + o + 1] = 1.0f;
+    }
+  if (lane < ly.pad + (c < 2 ? 3 : 0)) {
+    const int o = off_new(ly) - ly.pad + lane;
+    w.H[w.rbase[o] + o] = 1.0f;
   }
   // prior: H += Lambda (row by row, coalesced over the packed lower triangle)
   {
@@ -461,11 +487,11 @@ __device__ void assemble(const Layout& ly, const Params& pr, const float* rec, c
       float Ji[3][3], Jj[3][3];
       between_jac(b, Ji, Jj);
       if (pass == 0) {
-        add_j_side(w, n, off_slot(ly, k, c), k >= 2 ? off_slot(ly, k - 1, c) : 0, Ji, Jj, pr.om_odo, b.r, k >= 2);
+        add_j_side(w, n, off_slot(ly, od, k, c), k >= 2 ? off_slot(ly, od, k - 1, c) : 0, Ji, Jj, pr.om_odo, b.r, k >= 2);
       } else if (k >= 2) {
         float Hii[6] = {0, 0, 0, 0, 0, 0}, gi[3] = {0, 0, 0};
         acc_i_side(Ji, pr.om_odo, b.r, Hii, gi);
-        add_i_side(w, n, off_slot(ly, k - 1, c), Hii, gi);
+        add_i_side(w, n, off_slot(ly, od, k - 1, c), Hii, gi);
       }
     }
     __syncwarp();
@@ -477,7 +503,7 @@ __device__ void assemble(const Layout& ly, const Params& pr, const float* rec, c
     const Between b = between_eval(w.st + st_pose(t), w.cs[2 * t], w.cs[2 * t + 1], w.st + st_pose(k), w.zlc + 3 * k);
     float Ji[3][3], Jj[3][3];
     between_jac(b, Ji, Jj);
-    add_j_side(w, n, off_slot(ly, k, c), t >= 1 ? off_slot(ly, t, c) : 0, Ji, Jj, pr.om_lc, b.r, t >= 1);
+    add_j_side(w, n, off_slot(ly, od, k, c), t >= 1 ? off_slot(ly, od, t, c) : 0, Ji, Jj, pr.om_lc, b.r, t >= 1);
   }
   __syncwarp();
   for (int t = 1 + lane; t < c - 1; t += 32) {
@@ -491,117 +517,131 @@ __device__ void assemble(const Layout& ly, const Params& pr, const float* rec, c
       acc_i_side(Ji, pr.om_lc, b.r, Hii, gi);
       any = true;
     }
-    if (any) add_i_side(w, n, off_slot(ly, t, c), Hii, gi);
+    if (any) add_i_side(w, n, off_slot(ly, od, t, c), Hii, gi);
   }
   __syncwarp();
-  // range-bearing factors: lanes over landmarks, loop over slots.  Landmarks g are global, so each
-  // factor has three blocks: anchor a, observing pose e_k (k >= 1), landmark g.  With the anchor-frame
-  // landmark m = Rot(a_th)'(g - a_t), D = m - t_k:  J_e = [-J_l | (0,-1)'],  J_g = J_l Rot(a_th)',
-  // J_a = [-J_g | -J_l S m].  Pose- and anchor-side sums over landmarks go through warp shuffles.
-  if (L > 0) {
+  // range-bearing factors.  Landmarks g are global, so each factor has three blocks: anchor a, observing
+  // pose e_k (k >= 1), landmark g.  With the anchor-frame landmark m = Rot(a_th)'(g - a_t), D = m - t_k:
+  //   J_e = [-J_l | (0,-1)'],  J_g = J_l Rot(a_th)',  J_a = [-J_g | -J_l S m].
+  // Two passes, no cross-lane reductions inside the loops: pass A has one lane per POSE (sums over its
+  // landmarks stay in registers: pose diagonal, gradient, anchor x pose block); pass B one lane per
+  // LANDMARK (landmark diagonal, gradient, anchor x landmark block, anchor diagonal partial sums).
+  if (L > 0 && od.obs) {
     float* rhs = w.H + w.rbase[n];
     const float w0 = pr.om_rb[0], w1 = pr.om_rb[1];
     const int oA = off_a(ly);
     float sa, ca;
     sincosf(w.st[2], &sa, &ca);
     const float ax = w.st[0], ay = w.st[1];
-    float A[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};  // sums over all factors: gg(3), <a2,g0>, <a2,g1>, <a2,a2>, <g0,r>, <g1,r>, <a2,r>
+    float* mloc = w.sds + s;  // anchor-frame landmark positions (2L floats after the prior displacement)
+    for (int l = lane; l < L; l += 32) {
+      const float gxl = w.st[st_lm(ly, l)] - ax, gyl = w.st[st_lm(ly, l) + 1] - ay;
+      mloc[2 * l] = ca * gxl + sa * gyl;
+      mloc[2 * l + 1] = -sa * gxl + ca * gyl;
+    }
+    __syncwarp();
+    // ---- pass A: lane = pose slot k >= 1
+    for (int k = 1 + lane; k < c; k += 32) {
+      uint64_t m = (uint64_t)w.rbm[k * ly.nw];
+      if (ly.nw > 1) m |= (uint64_t)w.rbm[k * ly.nw + 1] << 32;
+      if (!m) continue;
+      const int r = ring_of(k, head, W), op = off_slot(ly, od, k, c);
+      const float px = w.st[st_pose(k)], py = w.st[st_pose(k) + 1], pt = w.st[st_pose(k) + 2];
+      float R[18];
+#pragma unroll
+      for (int t = 0; t < 18; ++t) R[t] = 0.f;
+      while (m) {
+        const int l = __ffsll((long long)m) - 1;
+        m &= m - 1;
+        const float zr = rec[ly.o_zrb + (r * 2 + 0) * L + l], zb = rec[ly.o_zrb + (r * 2 + 1) * L + l];
+        const float mx = mloc[2 * l], my = mloc[2 * l + 1];
+        const float dx = mx - px, dy = my - py;
+        const float q = dx * dx + dy * dy, irho = rsqrtf(q), rho = q * irho, iq = irho * irho;
+        const float r0 = rho - zr, r1 = wrapf(atan2f(dy, dx) - pt - zb);
+        const float ux = dx * irho, uy = dy * irho, vx = -dy * iq, vy = dx * iq;     // J_l rows
+        const float Ux = ca * ux - sa * uy, Uy = sa * ux + ca * uy;                  // J_g rows
+        const float Vx = ca * vx - sa * vy, Vy = sa * vx + ca * vy;
+        const float j0 = ux * my - uy * mx, j1 = vx * my - vy * mx;                  // J_a theta column
+        const float wg0a = w0 * Ux, wg0b = w1 * Vx, wg1a = w0 * Uy, wg1b = w1 * Vy, wa2a = w0 * j0, wa2b = w1 * j1;
+        // cross block <g_i, e_j>, pose columns e0 = (-ux,-vx), e1 = (-uy,-vy), e2 = (0,-1)
+        const float ge00 = -(wg0a * ux + wg0b * vx), ge01 = -(wg0a * uy + wg0b * vy), ge02 = -wg0b;
+        const float ge10 = -(wg1a * ux + wg1b * vx), ge11 = -(wg1a * uy + wg1b * vy), ge12 = -wg1b;
+        const int ol = off_lm(ly, od, l);
+        if (op < ol) {  // chain pose: landmark rows, pose columns
+          float* r0p = w.H + w.rbase[ol];
+          float* r1p = w.H + w.rbase[ol + 1];
+          r0p[op] += ge00; r0p[op + 1] += ge01; r0p[op + 2] += ge02;
+          r1p[op] += ge10; r1p[op + 1] += ge11; r1p[op + 2] += ge12;
+        } else {        // newest pose: pose rows, landmark columns
+          w.H[w.rbase[op] + ol] += ge00; w.H[w.rbase[op] + ol + 1] += ge10;
+          w.H[w.rbase[op + 1] + ol] += ge01; w.H[w.rbase[op + 1] + ol + 1] += ge11;
+          w.H[w.rbase[op + 2] + ol] += ge02; w.H[w.rbase[op + 2] + ol + 1] += ge12;
+        }
+        const float e0a = w0 * ux, e0b = w1 * vx, e1a = w0 * uy, e1b = w1 * vy;
+        R[0] += e0a * ux + e0b * vx; R[1] += e1a * ux + e1b * vx; R[2] += e1a * uy + e1b * vy;
+        R[3] += e0b; R[4] += e1b; R[5] += w1;
+        R[6] -= e0a * r0 + e0b * r1; R[7] -= e1a * r0 + e1b * r1; R[8] -= w1 * r1;
+        R[9] -= ge00; R[10] -= ge01; R[11] -= ge02;
+        R[12] -= ge10; R[13] -= ge11; R[14] -= ge12;
+        R[15] -= wa2a * ux + wa2b * vx; R[16] -= wa2a * uy + wa2b * vy; R[17] -= wa2b;
+      }
+      float* q0 = w.H + w.rbase[op];
+      float* q1 = w.H + w.rbase[op + 1];
+      float* q2 = w.H + w.rbase[op + 2];
+      q0[op] += R[0]; q1[op] += R[1]; q1[op + 1] += R[2];
+      q2[op] += R[3]; q2[op + 1] += R[4]; q2[op + 2] += R[5];
+      rhs[op] -= R[6]; rhs[op + 1] -= R[7]; rhs[op + 2] -= R[8];
+#pragma unroll
+      for (int i = 0; i < 3; ++i) {
+        float* qa = w.H + w.rbase[oA + i];
+        qa[op] += R[9 + 3 * i]; qa[op + 1] += R[10 + 3 * i]; qa[op + 2] += R[11 + 3 * i];
+      }
+    }
+    __syncwarp();
+    // ---- pass B: lane = landmark
+    float A[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};  // gg(3), <a2,g0>, <a2,g1>, <a2,a2>, <g0,r>, <g1,r>, <a2,r>
     for (int base = 0; base < L; base += 32) {
       const int l = base + lane;
-      const bool inl = l < L;
-      const float gxl = inl ? w.st[st_lm(ly, l)] - ax : 0.f, gyl = inl ? w.st[st_lm(ly, l) + 1] - ay : 0.f;
-      const float mx = ca * gxl + sa * gyl, my = -sa * gxl + ca * gyl;
-      float Lxx = 0.f, Lxy = 0.f, Lyy = 0.f, bgx = 0.f, bgy = 0.f, ag0 = 0.f, ag1 = 0.f;
-      const int ol = off_lm(ly, inl ? l : 0);
+      const bool inl = l < L && ((od.obs >> l) & 1ull);
+      const float mx = inl ? mloc[2 * l] : 0.f, my = inl ? mloc[2 * l + 1] : 0.f;
+      float Lxx = 0.f, Lxy = 0.f, Lyy = 0.f, bgx = 0.f, bgy = 0.f, ag0 = 0.f, ag1 = 0.f, a22 = 0.f, a2r = 0.f;
       for (int k = 0; k < c; ++k) {
         const uint32_t word = w.rbm[k * ly.nw + (base >> 5)];
-        if (word == 0u) continue;  // warp-uniform
-        const bool vis = inl && ((word >> lane) & 1u);
+        if (!((word >> lane) & 1u) || !inl) continue;
         const int r = ring_of(k, head, W);
-        float R[18];  // per-pose sums: ee (6), b_e (3), ae (9)
-#pragma unroll
-        for (int t = 0; t < 18; ++t) R[t] = 0.f;
-        if (vis) {
-          const float zr = rec[ly.o_zrb + (r * 2 + 0) * L + l], zb = rec[ly.o_zrb + (r * 2 + 1) * L + l];
-          const float* p = w.st + st_pose(k);
-          const float dx = mx - p[0], dy = my - p[1];
-          const float q = dx * dx + dy * dy, irho = rsqrtf(q), rho = q * irho, iq = irho * irho;
-          const float r0 = rho - zr, r1 = wrapf(atan2f(dy, dx) - p[2] - zb);
-          const float ux = dx * irho, uy = dy * irho, vx = -dy * iq, vy = dx * iq;     // J_l rows
-          const float Ux = ca * ux - sa * uy, Uy = sa * ux + ca * uy;                  // J_g rows
-          const float Vx = ca * vx - sa * vy, Vy = sa * vx + ca * vy;
-          const float j0 = ux * my - uy * mx, j1 = vx * my - vy * mx;                  // J_a theta column
-          // weighted columns
-          const float wg0a = w0 * Ux, wg0b = w1 * Vx, wg1a = w0 * Uy, wg1b = w1 * Vy, wa2a = w0 * j0, wa2b = w1 * j1;
-          const float gg00 = wg0a * Ux + wg0b * Vx, gg01 = wg0a * Uy + wg0b * Vy, gg11 = wg1a * Uy + wg1b * Vy;
-          const float a2g0 = wa2a * Ux + wa2b * Vx, a2g1 = wa2a * Uy + wa2b * Vy, a2a2 = wa2a * j0 + wa2b * j1;
-          const float g0r = wg0a * r0 + wg0b * r1, g1r = wg1a * r0 + wg1b * r1, a2r = wa2a * r0 + wa2b * r1;
-          Lxx += gg00; Lxy += gg01; Lyy += gg11; bgx += g0r; bgy += g1r; ag0 += a2g0; ag1 += a2g1;
-          A[0] += gg00; A[1] += gg01; A[2] += gg11; A[3] += a2g0; A[4] += a2g1; A[5] += a2a2;
-          A[6] += g0r; A[7] += g1r; A[8] += a2r;
-          if (k > 0) {
-            // pose columns e0 = (-ux,-vx), e1 = (-uy,-vy), e2 = (0,-1)
-            const float ge00 = -(wg0a * ux + wg0b * vx), ge01 = -(wg0a * uy + wg0b * vy), ge02 = -wg0b;
-            const float ge10 = -(wg1a * ux + wg1b * vx), ge11 = -(wg1a * uy + wg1b * vy), ge12 = -wg1b;
-            const int op = off_slot(ly, k, c);
-            if (op < ol) {  // chain pose: landmark rows, pose columns
-              float* r0p = w.H + w.rbase[ol];
-              float* r1p = w.H + w.rbase[ol + 1];
-              r0p[op] += ge00; r0p[op + 1] += ge01; r0p[op + 2] += ge02;
-              r1p[op] += ge10; r1p[op + 1] += ge11; r1p[op + 2] += ge12;
-            } else {        // newest pose: pose rows, landmark columns
-              w.H[w.rbase[op] + ol] += ge00; w.H[w.rbase[op] + ol + 1] += ge10;
-              w.H[w.rbase[op + 1] + ol] += ge01; w.H[w.rbase[op + 1] + ol + 1] += ge11;
-              w.H[w.rbase[op + 2] + ol] += ge02; w.H[w.rbase[op + 2] + ol + 1] += ge12;
-            }
-            const float e0a = w0 * ux, e0b = w1 * vx, e1a = w0 * uy, e1b = w1 * vy;
-            // pose diagonal (lower: xx, yx, yy, tx, ty, tt) and gradient
-            R[0] = e0a * ux + e0b * vx; R[1] = e1a * ux + e1b * vx; R[2] = e1a * uy + e1b * vy;
-            R[3] = e0b; R[4] = e1b; R[5] = w1;
-            R[6] = -(e0a * r0 + e0b * r1); R[7] = -(e1a * r0 + e1b * r1); R[8] = -w1 * r1;
-            // anchor rows x pose columns: <a_i, e_j>, a0 = -g0, a1 = -g1, a2 = (j0, j1)
-            R[9] = -ge00; R[10] = -ge01; R[11] = -ge02;
-            R[12] = -ge10; R[13] = -ge11; R[14] = -ge12;
-            R[15] = -(wa2a * ux + wa2b * vx); R[16] = -(wa2a * uy + wa2b * vy); R[17] = -wa2b;
-          }
-        }
-        if (k > 0) {
-#pragma unroll
-          for (int t = 0; t < 18; ++t) R[t] = warp_sum(R[t]);
-          if (lane == 0) {
-            const int op = off_slot(ly, k, c);
-            float* q0 = w.H + w.rbase[op];
-            float* q1 = w.H + w.rbase[op + 1];
-            float* q2 = w.H + w.rbase[op + 2];
-            q0[op] += R[0]; q1[op] += R[1]; q1[op + 1] += R[2];
-            q2[op] += R[3]; q2[op + 1] += R[4]; q2[op + 2] += R[5];
-            rhs[op] -= R[6]; rhs[op + 1] -= R[7]; rhs[op + 2] -= R[8];
-#pragma unroll
-            for (int i = 0; i < 3; ++i) {
-              float* qa = w.H + w.rbase[oA + i];
-              qa[op] += R[9 + 3 * i]; qa[op + 1] += R[10 + 3 * i]; qa[op + 2] += R[11 + 3 * i];
-            }
-          }
-        }
+        const float zr = rec[ly.o_zrb + (r * 2 + 0) * L + l], zb = rec[ly.o_zrb + (r * 2 + 1) * L + l];
+        const float* p = w.st + st_pose(k);
+        const float dx = mx - p[0], dy = my - p[1];
+        const float q = dx * dx + dy * dy, irho = rsqrtf(q), rho = q * irho, iq = irho * irho;
+        const float r0 = rho - zr, r1 = wrapf(atan2f(dy, dx) - p[2] - zb);
+        const float ux = dx * irho, uy = dy * irho, vx = -dy * iq, vy = dx * iq;
+        const float Ux = ca * ux - sa * uy, Uy = sa * ux + ca * uy, Vx = ca * vx - sa * vy, Vy = sa * vx + ca * vy;
+        const float j0 = ux * my - uy * mx, j1 = vx * my - vy * mx;
+        const float wg0a = w0 * Ux, wg0b = w1 * Vx, wg1a = w0 * Uy, wg1b = w1 * Vy, wa2a = w0 * j0, wa2b = w1 * j1;
+        Lxx += wg0a * Ux + wg0b * Vx; Lxy += wg0a * Uy + wg0b * Vy; Lyy += wg1a * Uy + wg1b * Vy;
+        ag0 += wa2a * Ux + wa2b * Vx; ag1 += wa2a * Uy + wa2b * Vy; a22 += wa2a * j0 + wa2b * j1;
+        bgx += wg0a * r0 + wg0b * r1; bgy += wg1a * r0 + wg1b * r1; a2r += wa2a * r0 + wa2b * r1;
       }
-      if (inl && ((mk.act >> l) & 1ull)) {
+      if (inl) {
+        const int ol = off_lm(ly, od, l);
         float* r0p = w.H + w.rbase[ol];
         float* r1p = w.H + w.rbase[ol + 1];
         r0p[ol] += Lxx; r1p[ol] += Lxy; r1p[ol + 1] += Lyy;
         rhs[ol] -= bgx; rhs[ol + 1] -= bgy;
-        if (Lxx != 0.f || Lyy != 0.f) {  // anchor rows x landmark columns: a0 = -g0, a1 = -g1, a2
-          float* qa0 = w.H + w.rbase[oA];
-          float* qa1 = w.H + w.rbase[oA + 1];
-          float* qa2 = w.H + w.rbase[oA + 2];
-          qa0[ol] -= Lxx; qa0[ol + 1] -= Lxy;
-          qa1[ol] -= Lxy; qa1[ol + 1] -= Lyy;
-          qa2[ol] += ag0; qa2[ol + 1] += ag1;
-        }
+        // anchor rows x landmark columns: a0 = -g0, a1 = -g1, a2
+        float* qa0 = w.H + w.rbase[oA];
+        float* qa1 = w.H + w.rbase[oA + 1];
+        float* qa2 = w.H + w.rbase[oA + 2];
+        qa0[ol] -= Lxx; qa0[ol + 1] -= Lxy;
+        qa1[ol] -= Lxy; qa1[ol + 1] -= Lyy;
+        qa2[ol] += ag0; qa2[ol + 1] += ag1;
+        A[0] += Lxx; A[1] += Lxy; A[2] += Lyy; A[3] += ag0; A[4] += ag1; A[5] += a22;
+        A[6] += bgx; A[7] += bgy; A[8] += a2r;
       }
-      __syncwarp();
     }
 #pragma unroll
     for (int t = 0; t < 9; ++t) A[t] = warp_sum(A[t]);
+    __syncwarp();
     if (lane == 0) {  // anchor diagonal block and gradient
       float* qa0 = w.H + w.rbase[oA];
       float* qa1 = w.H + w.rbase[oA + 1];
@@ -737,7 +777,7 @@ __device__ void back_substitute(const Layout& ly, const WS& w, int lane) {
 }
 
 // v <- v + delta (R1: additive, angles wrapped).  Returns ENV_NONFINITE if the update is not finite.
-__device__ int apply_update(const Layout& ly, const WS& w, int lane, int c, const Masks& mk) {
+__device__ int apply_update(const Layout& ly, const Ord& od, const WS& w, int lane, int c, const Masks& mk) {
   const int W = ly.W, L = ly.L;
   const float* dl = w.H + w.rbase[ly.np];
   int bad = 0;
@@ -749,14 +789,14 @@ __device__ int apply_update(const Layout& ly, const WS& w, int lane, int c, cons
   }
   for (int i = lane; i < 3 * (c - 1); i += 32) {
     const int k = 1 + i / 3, j = i - 3 * (k - 1);
-    const float d = dl[off_slot(ly, k, c) + j];
+    const float d = dl[off_slot(ly, od, k, c) + j];
     bad |= !isfinite(d);
     const float v = w.st[st_pose(k) + j] + d;
     w.st[st_pose(k) + j] = j == 2 ? wrapf(v) : v;
   }
   for (int i = lane; i < 2 * L; i += 32) {
     if (!((mk.act >> (i >> 1)) & 1ull)) continue;
-    const float d = dl[off_lm(ly, 0) + i];
+    const float d = dl[off_lm(ly, od, i >> 1) + (i & 1)];
     bad |= !isfinite(d);
     w.st[3 + 3 * W + i] += d;
   }

@@ -68,7 +68,7 @@ static inline Layout make_layout(int N, int W, int L, int cap, int wpc) {
   y.s_rbase = s; s = pad4(s + y.np + 2);
   y.s_ssup = s; s = pad4(s + n);
   y.s_sidx = s; s = pad4(s + n);
-  y.s_sds = s; s = pad4(s + n);
+  y.s_sds = s; s = pad4(s + n + 2 * L);  // prior displacement (<= n) + anchor-frame landmarks (2L)
   y.s_H = s;
   // dense capacity: full 4x4 tiles of the lower triangle + two rhs rows; or the marginalisation scratch
   const int G = y.np / 4;

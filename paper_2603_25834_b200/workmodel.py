@@ -9,7 +9,8 @@ bookkeeping of the kernels on the generator's event arrays -- no floating-point 
   B_alg = step inputs + outputs + state r/w + live factor data + prior on its support r/w
 
 with the envelope (skyline) of H in the kernel's elimination order
-[e_1..e_{W-2} | landmarks | newest pose | anchor]:
+[passive landmarks | e_1..e_{W-2} | observed landmarks | newest pose | anchor]
+(passive = no live range-bearing factor in the window):
 
   F_chol = sum_{i<n} sum_{j=first_i..i} (2 (j - max(first_i, first_j)) + 1)
   F_fwd  = sum_{j<n} (2 (j - first_j) + 1)         (the rhs row that rides along the factorisation)
@@ -53,12 +54,25 @@ class WindowStructure:
         self.act |= mask
         self.c = c + 1
 
-    # elimination offsets
+    # elimination offsets: [passive landmarks | chain poses | observed landmarks | newest | anchor]
+    def obs(self):
+        m = 0
+        for k in range(self.c):
+            m |= self.rbm[k]
+        return m
+
+    def npas(self):
+        return self.L - _popcount(self.obs())
+
     def off_slot(self, k):
-        return 3 * (self.W - 2) + 2 * self.L if k == self.c - 1 else 3 * (k - 1)
+        return 3 * (self.W - 2) + 2 * self.L if k == self.c - 1 else 2 * self.npas() + 3 * (k - 1)
 
     def off_lm(self, l):
-        return 3 * (self.W - 2) + 2 * l
+        obs = self.obs()
+        below = (1 << l) - 1
+        if (obs >> l) & 1:
+            return 2 * self.npas() + 3 * (self.W - 2) + 2 * _popcount(obs & below)
+        return 2 * _popcount(~obs & below)
 
     def support_dim(self):
         return 3 + 3 * _popcount(self.ps) + 2 * _popcount(self.ls)
@@ -66,10 +80,12 @@ class WindowStructure:
     def first(self) -> np.ndarray:
         """first[i] for the n rows of H (block granularity), as the symbolic phase computes it."""
         W, L, n, c = self.W, self.L, self.n, self.c
-        oL, oN, oA = 3 * (W - 2), 3 * (W - 2) + 2 * L, 3 * (W - 2) + 2 * L + 3
+        oC = 2 * self.npas()
+        oL, oN, oA = oC + 3 * (W - 2), 3 * (W - 2) + 2 * L, 3 * (W - 2) + 2 * L + 3
         first = np.empty(n, np.int64)
         idx = np.arange(n)
-        first[:oL] = (idx[:oL] // 3) * 3
+        first[:oC] = (idx[:oC] // 2) * 2
+        first[oC:oL] = oC + ((idx[oC:oL] - oC) // 3) * 3
         first[oL:oN] = oL + ((idx[oL:oN] - oL) // 2) * 2
         first[oN:oA] = oN
         first[oA:] = oA
@@ -88,14 +104,14 @@ class WindowStructure:
             o = self.off_lm(l)
             for k in range(1, c - 1):
                 if (self.rbm[k] >> l) & 1:
-                    first[o:o + 2] = 3 * (k - 1)
+                    first[o:o + 2] = oC + 3 * (k - 1)
                     break
         sup = [self.off_slot(k) for k in range(1, c) if (self.ps >> k) & 1] + \
               [self.off_lm(l) for l in range(L) if (self.ls >> l) & 1]
         if sup:
             fs = min(sup)
             for o in sup:
-                d = 3 if (o < oL or o >= oN) else 2
+                d = 3 if (oC <= o < oL or o >= oN) else 2
                 first[o:o + d] = np.minimum(first[o:o + d], fs)
             first[oA:] = np.minimum(first[oA:], fs)
         # landmarks are global (R17b): every range-bearing factor also touches the anchor a, so a's rows
