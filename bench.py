@@ -28,7 +28,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from paper_2603_25834_b200 import synth, workmodel  # noqa: E402
+from paper_2603_25834_b200 import replicas, synth, workmodel  # noqa: E402
 
 SM_COUNT, LANES = 148, 128
 L2_BYTES = 126 * 2 ** 20
@@ -174,7 +174,7 @@ def main():
     device = torch.device(f"cuda:{local}")
 
     base = parse_config(args.config)
-    cfg = synth.Config(base.name, base.N, base.W, base.L, base.iters, base.T, base.p_lc, seed=base.seed + rank)
+    cfg = synth.Config(base.name, base.N, base.W, base.L, base.iters, base.T, base.p_lc, seed=replicas.rank_seed(base.seed, rank))
     K = args.steps or cfg.T
     Wm = max(args.warmup, 0)
     N, W, L, nw = cfg.N, cfg.W, cfg.L, (cfg.L + 31) // 32
@@ -212,9 +212,7 @@ def main():
     launches0 = slam.launch_count
 
     def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+        replicas.barrier(world)
 
     barrier()
     with ClockSampler(local) as clk:
@@ -259,11 +257,8 @@ def main():
         e2e = {"seconds": e2e_s, "h2d": N * 4 * (3 + 1 + 3 + nw + 2 * L), "d2h": N * 4 * 10}
 
     # max over ranks (device-timed)
-    tt = torch.tensor([ms, e2e["seconds"] if e2e else 0.0], device=device, dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    ms_max, e2e_s_max = float(tt[0]), float(tt[1])
-    value = world * N * K / (ms_max * 1e-3)
+    ms_max, e2e_s_max = replicas.max_over_ranks([ms, e2e["seconds"] if e2e else 0.0], world, device)
+    value = replicas.whole_job_rate(N * K, world, ms_max * 1e-3)
 
     if rank == 0:
         peaks = measured_peaks()
@@ -296,7 +291,7 @@ def main():
             "status_flagged_envs": status_bad, "outputs_finite": finite, "kernel_info": slam.kernel_info(),
         }
         if e2e:
-            out["e2e"] = {"value": world * N * K / e2e_s_max, "unit": "env-steps/s",
+            out["e2e"] = {"value": replicas.whole_job_rate(N * K, world, e2e_s_max), "unit": "env-steps/s",
                           "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"]}
         if not args.no_cpu_baseline and world == 1:
             cb, envs, res = cpu_oracle_leg(data, cfg, K)
@@ -305,11 +300,13 @@ def main():
             g_ld = logdet[:, torch.from_numpy(envs.astype(np.int64)).to(device)].cpu().numpy().astype(np.float64)
             e_ld = np.abs(g_ld - res["logdet"])
             p_ld = np.abs(res["probe_logdet"] - res["logdet"])          # error of fp32 STORAGE alone (oracle probe)
-            bound = np.maximum(1e-3, 12.0 * p_ld)
+            forked = np.maximum.accumulate(p_ld > 1e-3 / 12.0, axis=0)  # per env: from its first ill-conditioned step on
             out["parity_sampled"] = {"envs": int(len(envs)), "env_steps": int(e_ld.size), "tol_abs_logdet": 1e-3,
-                                     "frac_within_tol": float((e_ld <= 1e-3).mean()), "max_abs_logdet_err": float(e_ld.max()),
-                                     "ill_conditioned_env_steps": int((12.0 * p_ld > 1e-3).sum()),
-                                     "all_within_conditioned_bound": bool((e_ld <= bound).all())}
+                                     "frac_within_tol": float((e_ld <= 1e-3).mean()),
+                                     "strict_coverage": float((~forked).mean()),
+                                     "max_err_well_conditioned": float(e_ld[~forked].max()) if (~forked).any() else None,
+                                     "max_err_forked": float(e_ld[forked].max()) if forked.any() else 0.0,
+                                     "probe_max_err": float(p_ld.max())}
         print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
