@@ -121,6 +121,11 @@ int slam_get_poses(slam_ctx* ctx, float* poses);
 int slam_get_landmarks(slam_ctx* ctx, float* lm, uint32_t* active);
 int slam_get_status(slam_ctx* ctx, int32_t* status);
 
+/* Device counters since the last reset, copied to stats8 ([8] uint64, device): [0] max and [1] sum of the
+ * envelope words (shared-memory footprint of H) over [2] solved environment-instances, [3] instances
+ * that exceeded the shared-memory capacity and ran from the global-memory fallback. */
+int slam_get_stats(slam_ctx* ctx, unsigned long long* stats8);
+
 int slam_count(const slam_ctx* ctx);                /* host-side window count c in [1, window] */
 long long slam_launch_count(const slam_ctx* ctx);   /* kernels launched by this context so far */
 const char* slam_last_error(const slam_ctx* ctx);   /* message of the last non-zero return */

@@ -23,7 +23,7 @@ SYMBOLS = (
     "slam_default_config", "slam_workspace_bytes", "slam_create", "slam_destroy", "slam_reset",
     "slam_push_step", "slam_observe_first", "slam_solve", "slam_marginal_cov", "slam_dopt",
     "slam_marginalize_oldest", "slam_step", "slam_step_host", "slam_get_poses", "slam_get_landmarks",
-    "slam_get_status", "slam_count", "slam_launch_count", "slam_last_error", "slam_kernel_info",
+    "slam_get_status", "slam_get_stats", "slam_count", "slam_launch_count", "slam_last_error", "slam_kernel_info",
 )
 
 
@@ -66,6 +66,7 @@ def _load() -> C.CDLL:
     lib.slam_get_poses.argtypes = [vp, fp]
     lib.slam_get_landmarks.argtypes = [vp, fp, ip]
     lib.slam_get_status.argtypes = [vp, ip]
+    lib.slam_get_stats.argtypes = [vp, ip]
     lib.slam_count.argtypes = [vp]
     lib.slam_launch_count.argtypes = [vp]
     lib.slam_launch_count.restype = C.c_longlong
@@ -215,6 +216,12 @@ class FixedLagSlam:
         out = self._new(self.N, dtype=torch.int32)
         self._chk(LIB.slam_get_status(self._h, C.c_void_p(out.data_ptr())))
         return out
+
+    def get_stats(self) -> dict:
+        out = self._new(8, dtype=torch.int64)
+        self._chk(LIB.slam_get_stats(self._h, C.c_void_p(out.data_ptr())))
+        v = [int(x) for x in out.cpu()]
+        return dict(max_envelope_words=v[0], mean_envelope_words=v[1] / max(v[2], 1), solved=v[2], fallback=v[3])
 
     @property
     def count(self) -> int:

@@ -14,53 +14,86 @@
 using namespace slamk;
 
 // ------------------------------------------------------------------ kernels
-// One warp per environment, `wpc` warps per CTA, persistent grid-stride loop over environments.
-// flags select the phases, so that the separate ABI calls and the fused slam_step share the same
-// device code and are bit-for-bit identical.
-__global__ void __launch_bounds__(256) slam_step_kernel(Layout ly, Params pr, float* state, int head, int c, int flags,
-                                                        int iters, StepIO io) {
+// One TEAM of 32/64/128 threads per environment, `wpc` teams per CTA, persistent grid-stride loop over
+// environments.  flags select the phases, so that the separate ABI calls and the fused slam_step share
+// the same device code and are bit-for-bit identical.
+template <int TEAM>
+__global__ void __launch_bounds__(TEAM == 128 ? 896 : (TEAM == 64 ? 512 : 256))
+slam_step_kernel(Layout ly, Params pr, float* state, int head, int c, int flags, int iters, StepIO io,
+                 unsigned long long* stats) {
   extern __shared__ float4 smem4[];
   float* smem = reinterpret_cast<float*>(smem4);
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const WS w = make_ws(ly, smem + (size_t)warp * ly.warp_words);
-  for (int env = blockIdx.x * ly.wpc + warp; env < ly.N; env += gridDim.x * ly.wpc) {
-    float* rec = state + (size_t)env * ly.rec;
-    int cc = c, status = 0;
+  const int team = threadIdx.x / TEAM, lane = threadIdx.x % TEAM;
+  float* base = smem + (size_t)team * ly.warp_words;
+  const WS w = make_ws(ly, base);
+  Team<TEAM> tm;
+  tm.bar = 1 + team;
+  tm.scr = base + ly.s_scr;
+  // All teams of a CTA walk through the phases in LOCK-STEP (CTA barriers between phases): the kernel is
+  // large (~12 k instructions) and instruction-fetch bound, so warps that execute the same code at the
+  // same time share every fetched line.  Teams without an environment in the last round only take part
+  // in the barriers.
+  for (int env0 = blockIdx.x * ly.wpc; env0 < ly.N; env0 += gridDim.x * ly.wpc) {
+    const int env = env0 + team;
+    const bool valid = env < ly.N;
+    float* rec = state + (size_t)(valid ? env : 0) * ly.rec;
+    int cc = c, status = 0, s = 0, total = 0;
     Masks mk;
-    load_env(ly, rec, w, lane, head, cc, mk);
-    if (flags & F_OBS0) record_rb(ly, rec, w, lane, env, head, 0, 0.f, 0.f, 0.f, io, mk);
-    if (flags & F_PUSH) cc = push_env(ly, rec, w, lane, env, head, cc, io, mk);
-    const Ord od = make_ord(ly, w.rbm, cc);
-    const int s = build_support(ly, od, w, lane, cc, mk.ps, mk.ls);
-    if (iters > 0 || (flags & F_COV)) {
-      const int total = symbolic(ly, od, w, lane, cc, mk, s);
-      for (int it = 0; it < iters; ++it) {
-        assemble(ly, pr, od, rec, w, lane, head, cc, mk, s, total);
-        __syncwarp();
-        status |= cholesky(ly, w, lane);
-        back_substitute(ly, w, lane);
-        status |= apply_update(ly, od, w, lane, cc, mk);
+    Ord od;
+    __syncthreads();
+    if (valid) {
+      load_env<TEAM>(ly, rec, w, tm, lane, head, cc, mk);
+      if (flags & F_OBS0) record_rb<TEAM>(ly, rec, w, tm, lane, env, head, 0, 0.f, 0.f, 0.f, io, mk);
+      if (flags & F_PUSH) cc = push_env<TEAM>(ly, rec, w, tm, lane, env, head, cc, io, mk);
+      od = make_ord(ly, w.rbm, cc);
+      s = build_support<TEAM>(ly, od, w, tm, lane, cc, mk.ps, mk.ls);
+    }
+    // iters Gauss-Newton iterations, then (F_COV) one more linearisation + factorisation at the final
+    // estimate for the covariance: ONE call site per phase keeps the kernel small.
+    const int nlin = iters + ((flags & F_COV) ? 1 : 0);
+    if (nlin > 0) {
+      __syncthreads();
+      if (valid) {
+        total = symbolic<TEAM>(ly, od, w, tm, lane, cc, mk, s);
+        if (stats && lane == 0) {  // envelope statistics (words per environment): max, sum, count
+          atomicMax(stats + 0, (unsigned long long)total);
+          atomicAdd(stats + 1, (unsigned long long)total);
+          atomicAdd(stats + 2, 1ull);
+        }
       }
-      if (flags & F_COV) {
-        assemble(ly, pr, od, rec, w, lane, head, cc, mk, s, total);
-        __syncwarp();
-        status |= cholesky(ly, w, lane);
-        covariance(ly, w, lane, env, cc, io);
-        __syncwarp();
+#pragma unroll 1
+      for (int it = 0; it < nlin; ++it) {
+        __syncthreads();
+        if (valid) { assemble<TEAM>(ly, pr, od, rec, w, tm, lane, head, cc, mk, s, total); tm.sync(); }
+        __syncthreads();
+        if (valid) status |= cholesky<TEAM>(ly, w, tm, lane);
+        __syncthreads();
+        if (valid) {
+          if (it < iters) {
+            back_substitute<TEAM>(ly, w, tm, lane);
+            status |= apply_update<TEAM>(ly, od, w, tm, lane, cc, mk);
+          } else {
+            covariance<TEAM>(ly, w, tm, lane, env, cc, io);
+            tm.sync();
+          }
+        }
       }
     }
-    if (io.last_pose && lane == 0) {  // newest pose in global coordinates: a (+) e_{c-1}
-      float sn, cn;
-      sincosf(w.st[2], &sn, &cn);
-      const float* e = w.st + st_pose(cc - 1);
-      io.last_pose[env] = w.st[0] + cn * e[0] - sn * e[1];
-      io.last_pose[(size_t)ly.N + env] = w.st[1] + sn * e[0] + cn * e[1];
-      io.last_pose[2 * (size_t)ly.N + env] = wrapf(w.st[2] + e[2]);
+    __syncthreads();
+    if (valid) {
+      if (io.last_pose && lane == 0) {  // newest pose in global coordinates: a (+) e_{c-1}
+        float sn, cn;
+        sincos_pi(w.st[2], &sn, &cn);
+        const float* e = w.st + st_pose(cc - 1);
+        io.last_pose[env] = w.st[0] + cn * e[0] - sn * e[1];
+        io.last_pose[(size_t)ly.N + env] = w.st[1] + sn * e[0] + cn * e[1];
+        io.last_pose[2 * (size_t)ly.N + env] = wrapf(w.st[2] + e[2]);
+      }
+      if (flags & F_MARG) status |= marginalize<TEAM>(ly, pr, rec, w, tm, lane, head, cc, mk, s);
+      store_state<TEAM>(ly, rec, w, tm, lane, head, cc, mk);
+      if (status && lane == 0) reinterpret_cast<int*>(rec)[ly.o_status] |= status;
+      tm.sync();
     }
-    if (flags & F_MARG) status |= marginalize(ly, pr, rec, w, lane, head, cc, mk, s);
-    store_state(ly, rec, w, lane, head, cc, mk);
-    if (status && lane == 0) reinterpret_cast<int*>(rec)[ly.o_status] |= status;
-    __syncwarp();
   }
 }
 
@@ -88,7 +121,7 @@ __global__ void slam_poses_kernel(Layout ly, const float* state, int head, int c
   const float* rec = state + (size_t)env * ly.rec;
   const float ax = rec[ly.o_a], ay = rec[ly.o_a + 1], at = rec[ly.o_a + 2];
   float sn, cn;
-  sincosf(at, &sn, &cn);
+  sincos_pi(at, &sn, &cn);
   for (int k = 0; k < ly.W; ++k) {
     float x = 0.f, y = 0.f, t = 0.f;
     if (k < c) {
@@ -138,6 +171,7 @@ struct slam_ctx {
   cudaStream_t stream;
   float* state;
   float* cov_cache;
+  unsigned long long* stats;  // [8] device counters: max / sum / count of envelope words, ...
   // device staging for slam_step_host
   float *st_odom, *st_lc_meas, *st_rb_meas, *st_cov, *st_logdet, *st_pose;
   int32_t* st_lc_back;
@@ -165,19 +199,35 @@ static bool sizes_ok(int batch, int window, int landmarks) {
   return batch >= 1 && window >= 2 && window <= SLAM_MAX_WINDOW && landmarks >= 0 && landmarks <= SLAM_MAX_LANDMARKS;
 }
 
-static int pick_wpc(int W, int L) {
+// Threads per environment: SLAM_TEAM={32,64,128} overrides; default by state dimension (a dense-ish
+// window of ~100 variables has enough rows and factors for four warps; small windows for one).
+static int pick_team(int W, int L) {
+  const char* e = getenv("SLAM_TEAM");
+  if (e) { const int t = atoi(e); if (t == 32 || t == 64 || t == 128) return t; }
+  const int n = 3 * W + 2 * L;
+  if (L > 0 && n >= 96) return 128;
+  if (n >= 48) return 64;
+  return 32;
+}
+static int pick_wpc(int W, int L, int team) {
   const Layout t = make_layout(1, W, L, -1, 1);
   const size_t wb = (size_t)t.warp_words * 4;
   int wpc = (int)((size_t)227 * 1024 / wb);
-  if (wpc > 8) wpc = 8;
+  const int maxt = team == 128 ? 7 : 8;   // 896 / 512 / 256 threads per CTA
+  if (wpc > maxt) wpc = maxt;
   return wpc;  // 0 if one environment does not fit
 }
+typedef void (*step_fn)(Layout, Params, float*, int, int, int, int, StepIO, unsigned long long*);
+static step_fn kernel_of(int team) {
+  return team == 128 ? slam_step_kernel<128> : (team == 64 ? slam_step_kernel<64> : slam_step_kernel<32>);
+}
 
-struct WsPlan { size_t state, cache, odom, lcb, lcm, rbk, rbm, cov, ld, pose, total; };
+struct WsPlan { size_t stats, state, cache, odom, lcb, lcm, rbk, rbm, cov, ld, pose, total; };
 static WsPlan plan(const Layout& ly) {
   WsPlan p;
   size_t o = 0;
   const size_t N = (size_t)ly.N;
+  p.stats = o; o = al256(o + 64);
   p.state = o; o = al256(o + N * ly.rec * 4);
   p.cache = o; o = al256(o + N * 10 * 4);
   p.odom = o; o = al256(o + N * 3 * 4);
@@ -203,7 +253,7 @@ void slam_default_config(slam_config* cfg) {
 
 size_t slam_workspace_bytes(int batch, int window, int landmarks) {
   if (!sizes_ok(batch, window, landmarks)) return 0;
-  const int wpc = pick_wpc(window, landmarks);
+  const int wpc = pick_wpc(window, landmarks, pick_team(window, landmarks));
   if (wpc < 1) return 0;
   return plan(make_layout(batch, window, landmarks, -1, wpc)).total;
 }
@@ -213,7 +263,8 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   if (!out) return SLAM_EINVAL;
   *out = nullptr;
   if (!sizes_ok(batch, window, landmarks) || !workspace || ((uintptr_t)workspace & 255)) return SLAM_EINVAL;
-  const int wpc = pick_wpc(window, landmarks);
+  const int team = pick_team(window, landmarks);
+  const int wpc = pick_wpc(window, landmarks, team);
   if (wpc < 1) return SLAM_EINVAL;
   slam_config dc;
   slam_default_config(&dc);
@@ -224,6 +275,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   slam_ctx* c = new (std::nothrow) slam_ctx();
   if (!c) return SLAM_ENOMEM;
   c->ly = make_layout(batch, window, landmarks, -1, wpc);
+  c->ly.team = team;
   const WsPlan p = plan(c->ly);
   if (workspace_bytes < p.total) { delete c; return SLAM_EINVAL; }
   for (int k = 0; k < 3; ++k) {
@@ -235,6 +287,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   c->pr.om_rb[1] = 1.0f / (cfg->rb_sigma[1] * cfg->rb_sigma[1]);
   c->stream = (cudaStream_t)cuda_stream;
   char* base = (char*)workspace;
+  c->stats = (unsigned long long*)(base + p.stats);
   c->state = (float*)(base + p.state);
   c->cov_cache = (float*)(base + p.cache);
   c->st_odom = (float*)(base + p.odom);
@@ -248,7 +301,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   c->launches = 0;
   c->err[0] = 0;
   c->smem_bytes = c->ly.warp_words * 4 * wpc;
-  if (cudaFuncSetAttribute(slam_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_bytes) != cudaSuccess) {
+  if (cudaFuncSetAttribute(kernel_of(team), cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_bytes) != cudaSuccess) {
     cudaGetLastError();
     delete c;
     return SLAM_ECUDA;
@@ -256,7 +309,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   int dev = 0, sms = 0, occ = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, slam_step_kernel, wpc * 32, c->smem_bytes);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel_of(team), wpc * team, c->smem_bytes);
   if (occ < 1 || sms < 1) { cudaGetLastError(); delete c; return SLAM_ECUDA; }
   c->ctas_per_sm = occ;
   const int need = (batch + wpc - 1) / wpc;
@@ -272,6 +325,7 @@ void slam_destroy(slam_ctx* ctx) { delete ctx; }
 int slam_reset(slam_ctx* c, const float* init_pose) {
   if (!c) return SLAM_EINVAL;
   const int threads = 256, blocks = (int)(((size_t)c->ly.N * 32 + threads - 1) / threads);
+  cudaMemsetAsync(c->stats, 0, 64, c->stream);
   slam_reset_kernel<<<blocks, threads, 0, c->stream>>>(c->ly, c->pr, c->state, init_pose);
   c->launches++;
   c->head = 0; c->count = 1; c->cov_valid = false;
@@ -279,8 +333,8 @@ int slam_reset(slam_ctx* c, const float* init_pose) {
 }
 
 static int launch_step(slam_ctx* c, int flags, int iters, const StepIO& io) {
-  slam_step_kernel<<<c->grid, c->ly.wpc * 32, c->smem_bytes, c->stream>>>(c->ly, c->pr, c->state, c->head, c->count, flags,
-                                                                        iters, io);
+  kernel_of(c->ly.team)<<<c->grid, c->ly.wpc * c->ly.team, c->smem_bytes, c->stream>>>(c->ly, c->pr, c->state, c->head,
+                                                                                      c->count, flags, iters, io, c->stats);
   c->launches++;
   return check_cuda(c, "slam_step_kernel");
 }
@@ -429,6 +483,12 @@ int slam_get_status(slam_ctx* c, int32_t* status) {
   return check_cuda(c, "slam_status_kernel");
 }
 
+int slam_get_stats(slam_ctx* c, unsigned long long* stats8) {
+  if (!c || !stats8) return SLAM_EINVAL;
+  cudaMemcpyAsync(stats8, c->stats, 64, cudaMemcpyDeviceToDevice, c->stream);
+  return check_cuda(c, "slam_get_stats");
+}
+
 int slam_count(const slam_ctx* c) { return c ? c->count : -1; }
 long long slam_launch_count(const slam_ctx* c) { return c ? c->launches : -1; }
 const char* slam_last_error(const slam_ctx* c) { return c ? c->err : "null context"; }
@@ -436,7 +496,7 @@ const char* slam_last_error(const slam_ctx* c) { return c ? c->err : "null conte
 int slam_kernel_info(const slam_ctx* c, int* smem_bytes_per_cta, int* warps_per_cta, int* ctas_per_sm) {
   if (!c) return SLAM_EINVAL;
   if (smem_bytes_per_cta) *smem_bytes_per_cta = c->smem_bytes;
-  if (warps_per_cta) *warps_per_cta = c->ly.wpc;
+  if (warps_per_cta) *warps_per_cta = c->ly.wpc * c->ly.team / 32;
   if (ctas_per_sm) *ctas_per_sm = c->ctas_per_sm;
   return SLAM_OK;
 }

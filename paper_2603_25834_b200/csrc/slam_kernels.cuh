@@ -56,6 +56,23 @@ __device__ __forceinline__ float wrapf(float x) {  // to [-pi, pi], 2*pi split h
   x = fmaf(-k, 6.2831854820251465f, x);
   return fmaf(-k, -1.7484555e-7f, x);
 }
+// sin and cos for |x| up to a few pi (every angle here is wrapped): quadrant reduction with a hi/lo
+// split of pi/2 and the classic single-precision minimax kernels (Cephes sinf/cosf coefficients),
+// ~1e-7 absolute.  Replaces sincosf, whose inlined large-argument slow path bloats the kernel: the
+// step kernel is instruction-fetch bound, so code size is a first-order cost.
+__device__ __forceinline__ void sincos_pi(float x, float* sn, float* cn) {
+  const float k = rintf(x * 0.63661977236758134f);
+  float r = fmaf(-k, 1.5707963705062866f, x);
+  r = fmaf(-k, -4.3711388286737929e-8f, r);
+  const float z = r * r;
+  const float sp = fmaf(fmaf(fmaf(-1.9515295891e-4f, z, 8.3321608736e-3f), z, -1.6666654611e-1f), z * r, r);
+  const float cp = fmaf(fmaf(fmaf(2.443315711809948e-5f, z, -1.388731625493765e-3f), z, 4.166664568298827e-2f), z * z,
+                        fmaf(-0.5f, z, 1.0f));
+  const int q = (int)k;
+  const float s0 = (q & 1) ? cp : sp, c0 = (q & 1) ? sp : cp;
+  *sn = (q & 2) ? -s0 : s0;
+  *cn = ((q + 1) & 2) ? -c0 : c0;
+}
 __device__ __forceinline__ uint64_t lowmask(int k) { return k >= 64 ? ~0ull : ((1ull << k) - 1ull); }
 __device__ __forceinline__ uint64_t ring_to_slot(uint64_t ring, int head, int W) {
   const uint64_t mW = lowmask(W);
@@ -69,16 +86,75 @@ __device__ __forceinline__ uint64_t slot_to_ring(uint64_t slot, int head, int W)
   if (head == 0) return slot;
   return ((slot << head) | (slot >> (W - head))) & mW;
 }
-__device__ __forceinline__ int nth_set_bit(uint64_t m, int k) {  // k-th (0-based) set bit
-  const uint32_t lo = (uint32_t)m, hi = (uint32_t)(m >> 32);
-  const int plo = __popc(lo);
-  return k < plo ? (int)__fns(lo, 0, k + 1) : 32 + (int)__fns(hi, 0, k - plo + 1);
+__device__ __forceinline__ int nth_set_bit(uint64_t m, int k) {  // k-th (0-based) set bit; tiny code on purpose
+#pragma unroll 1
+  for (int i = 0; i < k; ++i) m &= m - 1;
+  return __ffsll((long long)m) - 1;
 }
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULLMASK, v, o);
   return v;
 }
+
+// A TEAM of TEAM threads (1, 2 or 4 warps) owns one environment.  `lane` below is the thread index
+// inside the team.  Synchronisation is __syncwarp for one warp, a named barrier otherwise.
+template <int TEAM>
+struct Team {
+  int bar;     // named barrier id (1..15)
+  float* scr;  // shared scratch, 128 floats
+  static constexpr int NW = TEAM / 32;
+  __device__ __forceinline__ void sync() const {
+    if (TEAM == 32) __syncwarp();
+    else asm volatile("bar.sync %0, %1;" ::"r"(bar), "n"(TEAM) : "memory");
+  }
+  // sum of N values over the team (every thread gets the result); uniform call sites only
+  template <int N>
+  __device__ __forceinline__ void sum_n(float (&v)[N], int lane) const {
+#pragma unroll
+    for (int t = 0; t < N; ++t) v[t] = warp_sum(v[t]);
+    if (TEAM > 32) {
+      sync();
+      if ((lane & 31) == 0) {
+#pragma unroll
+        for (int t = 0; t < N; ++t) scr[(lane >> 5) * N + t] = v[t];
+      }
+      sync();
+#pragma unroll
+      for (int t = 0; t < N; ++t) {
+        float a = 0.f;
+#pragma unroll
+        for (int q = 0; q < NW; ++q) a += scr[q * N + t];
+        v[t] = a;
+      }
+    }
+  }
+  __device__ __forceinline__ int min_int(int v, int lane) const {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = min(v, __shfl_xor_sync(FULLMASK, v, o));
+    if (TEAM > 32) {
+      int* is = reinterpret_cast<int*>(scr);
+      sync();
+      if ((lane & 31) == 0) is[lane >> 5] = v;
+      sync();
+#pragma unroll
+      for (int q = 0; q < NW; ++q) v = min(v, is[q]);
+    }
+    return v;
+  }
+  __device__ __forceinline__ bool any(bool p, int lane) const {
+    int v = __any_sync(FULLMASK, p) ? 1 : 0;
+    if (TEAM > 32) {
+      int* is = reinterpret_cast<int*>(scr);
+      sync();
+      if ((lane & 31) == 0) is[lane >> 5] = v;
+      sync();
+#pragma unroll
+      for (int q = 0; q < NW; ++q) v |= is[q];
+    }
+    return v != 0;
+  }
+};
 
 __device__ __forceinline__ int ring_of(int slot, int head, int W) { int r = head + slot; return r >= W ? r - W : r; }
 // state array index
@@ -118,19 +194,20 @@ struct Masks {  // warp-uniform
 };
 
 // ------------------------------------------------------------------ load / store of the record
-__device__ void load_env(const Layout& ly, const float* rec, const WS& w, int lane, int head, int c, Masks& mk) {
+template <int TEAM>
+__device__ void load_env(const Layout& ly, const float* rec, const WS& w, const Team<TEAM>& tm, int lane, int head, int c, Masks& mk) {
   const int W = ly.W, L = ly.L;
   const int* reci = (const int*)rec;
   const uint32_t* recu = (const uint32_t*)rec;
   if (lane < 3) w.st[lane] = rec[ly.o_a + lane];
-  for (int i = lane; i < 3 * W; i += 32) {
+  for (int i = lane; i < 3 * W; i += TEAM) {
     const int k = i / 3, j = i - 3 * k, r = ring_of(k, head, W);
     const bool live = k < c;
     w.st[3 + i] = (live && k > 0) ? rec[ly.o_e + 3 * r + j] : 0.0f;
     w.zodo[i] = live ? rec[ly.o_zodo + 3 * r + j] : 0.0f;
     w.zlc[i] = live ? rec[ly.o_zlc + 3 * r + j] : 0.0f;
   }
-  for (int k = lane; k < W; k += 32) {
+  for (int k = lane; k < W; k += TEAM) {
     const int r = ring_of(k, head, W);
     const int t = (k < c) ? reci[ly.o_lct + r] : -1;
     int ts = -1;
@@ -138,66 +215,65 @@ __device__ void load_env(const Layout& ly, const float* rec, const WS& w, int la
     w.lct[k] = ts;
     for (int q = 0; q < ly.nw; ++q) w.rbm[k * ly.nw + q] = (k < c) ? recu[ly.o_rbm + r * ly.nw + q] : 0u;
   }
-  for (int i = lane; i < 2 * L; i += 32) w.st[3 + 3 * W + i] = rec[ly.o_m + i];
+  for (int i = lane; i < 2 * L; i += TEAM) w.st[3 + 3 * W + i] = rec[ly.o_m + i];
   const uint64_t pm = (uint64_t)recu[ly.o_pm] | ((uint64_t)recu[ly.o_pm + 1] << 32);
   mk.ps = ring_to_slot(pm, head, W);
   mk.ls = (uint64_t)recu[ly.o_lm] | ((uint64_t)recu[ly.o_lm + 1] << 32);
   mk.act = (uint64_t)recu[ly.o_act] | ((uint64_t)recu[ly.o_act + 1] << 32);
-  __syncwarp();
+  tm.sync();
 }
 
 // writes a, e (ring positions of the CURRENT head), m, active mask
-__device__ void store_state(const Layout& ly, float* rec, const WS& w, int lane, int head, int c, const Masks& mk) {
+template <int TEAM>
+__device__ void store_state(const Layout& ly, float* rec, const WS& w, const Team<TEAM>& tm, int lane, int head, int c, const Masks& mk) {
   const int W = ly.W, L = ly.L;
   uint32_t* recu = (uint32_t*)rec;
   if (lane < 3) rec[ly.o_a + lane] = w.st[lane];
-  for (int i = lane; i < 3 * c; i += 32) {
+  for (int i = lane; i < 3 * c; i += TEAM) {
     const int k = i / 3, j = i - 3 * k, r = ring_of(k, head, W);
     rec[ly.o_e + 3 * r + j] = w.st[3 + i];
   }
-  for (int i = lane; i < 2 * L; i += 32) rec[ly.o_m + i] = w.st[3 + 3 * W + i];
+  for (int i = lane; i < 2 * L; i += TEAM) rec[ly.o_m + i] = w.st[3 + 3 * W + i];
   if (lane == 0) { recu[ly.o_act] = (uint32_t)mk.act; recu[ly.o_act + 1] = (uint32_t)(mk.act >> 32); }
 }
 
 // ------------------------------------------------------------------ S0 push / observe
 // Range-bearing bookkeeping for the pose in `slot` (pose px,py,pth in the anchor frame; landmarks are
 // kept in GLOBAL coordinates, reading R17b).
-__device__ void record_rb(const Layout& ly, float* rec, const WS& w, int lane, int env, int head, int slot,
+template <int TEAM>
+__device__ void record_rb(const Layout& ly, float* rec, const WS& w, const Team<TEAM>& tm, int lane, int env, int head, int slot,
                           float px, float py, float pth, const StepIO& io, Masks& mk) {
   const int L = ly.L, N = ly.N, r = ring_of(slot, head, ly.W);
   uint32_t* recu = (uint32_t*)rec;
-  uint64_t act = mk.act;
-  for (int base = 0; base < L; base += 32) {
-    const int l = base + lane;
-    const uint32_t word = io.rb_mask[(size_t)(base >> 5) * N + env];
-    const bool vis = l < L && ((word >> lane) & 1u);
-    if (l < L) {
-      const float zr = io.rb_meas[(size_t)l * N + env];
-      const float zb = io.rb_meas[(size_t)(L + l) * N + env];
-      rec[ly.o_zrb + (r * 2 + 0) * L + l] = zr;
-      rec[ly.o_zrb + (r * 2 + 1) * L + l] = zb;
-      if (vis && !((act >> l) & 1ull)) {  // R6: inverse projection from the observing pose's guess (global)
-        float sa, ca, sn, cn;
-        sincosf(w.st[2], &sa, &ca);
-        const float gx = w.st[0] + ca * px - sa * py, gy = w.st[1] + sa * px + ca * py;
-        sincosf(w.st[2] + pth + zb, &sn, &cn);
-        w.st[st_lm(ly, l)] = gx + zr * cn;
-        w.st[st_lm(ly, l) + 1] = gy + zr * sn;
-      }
+  uint64_t vis = (uint64_t)io.rb_mask[env];
+  if (ly.nw > 1) vis |= (uint64_t)io.rb_mask[(size_t)N + env] << 32;
+  vis &= lowmask(L);
+  for (int l = lane; l < L; l += TEAM) {
+    const float zr = io.rb_meas[(size_t)l * N + env];
+    const float zb = io.rb_meas[(size_t)(L + l) * N + env];
+    rec[ly.o_zrb + (r * 2 + 0) * L + l] = zr;
+    rec[ly.o_zrb + (r * 2 + 1) * L + l] = zb;
+    if (((vis >> l) & 1ull) && !((mk.act >> l) & 1ull)) {  // R6: inverse projection from the observing pose's guess (global)
+      float sa, ca, sn, cn;
+      sincos_pi(w.st[2], &sa, &ca);
+      const float gx = w.st[0] + ca * px - sa * py, gy = w.st[1] + sa * px + ca * py;
+      sincos_pi(w.st[2] + pth + zb, &sn, &cn);
+      w.st[st_lm(ly, l)] = gx + zr * cn;
+      w.st[st_lm(ly, l) + 1] = gy + zr * sn;
     }
-    const uint64_t wm = (uint64_t)(L - base >= 32 ? word : (word & ((1u << (L - base)) - 1u)));
-    if (lane == 0) {
-      w.rbm[slot * ly.nw + (base >> 5)] = (uint32_t)wm;
-      recu[ly.o_rbm + r * ly.nw + (base >> 5)] = (uint32_t)wm;
-    }
-    act |= wm << base;
   }
-  mk.act = act;
-  __syncwarp();
+  if (lane < ly.nw) {
+    const uint32_t word = (uint32_t)(vis >> (32 * lane));
+    w.rbm[slot * ly.nw + lane] = word;
+    recu[ly.o_rbm + r * ly.nw + lane] = word;
+  }
+  mk.act |= vis;
+  tm.sync();
 }
 
 // Appends slot c (count before the push).  Returns the new count.
-__device__ int push_env(const Layout& ly, float* rec, const WS& w, int lane, int env, int head, int c,
+template <int TEAM>
+__device__ int push_env(const Layout& ly, float* rec, const WS& w, const Team<TEAM>& tm, int lane, int env, int head, int c,
                         const StepIO& io, Masks& mk) {
   const int W = ly.W, N = ly.N, r = ring_of(c, head, W);
   int* reci = (int*)rec;
@@ -205,11 +281,11 @@ __device__ int push_env(const Layout& ly, float* rec, const WS& w, int lane, int
   const float* p = w.st + st_pose(c - 1);  // slot 0 is stored as zeros
   const float pxo = p[0], pyo = p[1], pto = p[2];
   float sn, cn;
-  sincosf(pto, &sn, &cn);
+  sincos_pi(pto, &sn, &cn);
   const float nx = pxo + cn * zx - sn * zy, ny = pyo + sn * zx + cn * zy, nt = wrapf(pto + zt);
   int back = io.lc_back ? io.lc_back[env] : 0;
   const int tgt = (back >= 1 && back <= c) ? c - back : -1;  // R11
-  __syncwarp();
+  tm.sync();
   if (lane == 0) {
     float* q = w.st + st_pose(c);
     q[0] = nx; q[1] = ny; q[2] = nt;
@@ -224,18 +300,19 @@ __device__ int push_env(const Layout& ly, float* rec, const WS& w, int lane, int
     w.zlc[3 * c + lane] = zl;
     rec[ly.o_zlc + 3 * r + lane] = zl;
   }
-  __syncwarp();
-  if (ly.L > 0) record_rb(ly, rec, w, lane, env, head, c, nx, ny, nt, io, mk);
+  tm.sync();
+  if (ly.L > 0) record_rb<TEAM>(ly, rec, w, tm, lane, env, head, c, nx, ny, nt, io, mk);
   return c + 1;
 }
 
 // ------------------------------------------------------------------ prior support tables
 // For support scalar p (canonical order [a | poses by slot | landmarks]): elimination offset in
 // ssup[p], state index in sidx[p] (bit 16 set for angle components).  Returns the support dimension.
-__device__ int build_support(const Layout& ly, const Ord& od, const WS& w, int lane, int c, uint64_t ps, uint64_t ls) {
+template <int TEAM>
+__device__ int build_support(const Layout& ly, const Ord& od, const WS& w, const Team<TEAM>& tm, int lane, int c, uint64_t ps, uint64_t ls) {
   const int npo = __popcll(ps), nlo = __popcll(ls);
   const int s = 3 + 3 * npo + 2 * nlo;
-  for (int p = lane; p < s; p += 32) {
+  for (int p = lane; p < s; p += TEAM) {
     int off, idx;
     if (p < 3) { off = off_a(ly) + p; idx = p | (p == 2 ? 0x10000 : 0); }
     else if (p < 3 + 3 * npo) {
@@ -247,7 +324,7 @@ __device__ int build_support(const Layout& ly, const Ord& od, const WS& w, int l
     }
     w.ssup[p] = off; w.sidx[p] = idx;
   }
-  __syncwarp();
+  tm.sync();
   return s;
 }
 
@@ -256,11 +333,12 @@ __device__ int build_support(const Layout& ly, const Ord& od, const WS& w, int l
 // first a multiple of 4), so every tile row is one aligned 128-bit word.  first[i] = first column
 // of row i; rbase[i] + j addresses H(i,j).  Rows np (rhs) and np+1 (zero twin) span [0, np).
 // Returns the total words used.
-__device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, int lane, int c, const Masks& mk, int s) {
+template <int TEAM>
+__device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, const Team<TEAM>& tm, int lane, int c, const Masks& mk, int s) {
   const int L = ly.L, np = ly.np;
   const int oC = 2 * od.npas, oL = oC + 3 * (ly.W - 2), oP = 3 * (ly.W - 2) + 2 * L, oN = off_new(ly), oA = off_a(ly);
   // own block offsets
-  for (int i = lane; i < np + 2; i += 32) {
+  for (int i = lane; i < np + 2; i += TEAM) {
     int f;
     if (i < oC) f = i & ~1;
     else if (i < oL) f = oC + ((i - oC) / 3) * 3;
@@ -271,9 +349,9 @@ __device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, int lane, 
     else f = 0;
     w.first[i] = f;
   }
-  __syncwarp();
+  tm.sync();
   // pose rows
-  for (int k = 1 + lane; k < c; k += 32) {
+  for (int k = 1 + lane; k < c; k += TEAM) {
     const int o = off_slot(ly, od, k, c);
     int f = o;
     if (k >= 2) f = min(f, off_slot(ly, od, k - 1, c));
@@ -287,28 +365,27 @@ __device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, int lane, 
     w.first[o] = f; w.first[o + 1] = f; w.first[o + 2] = f;
   }
   // landmark rows: first chain pose (slots 1..c-2) that observes them
-  for (int l = lane; l < L; l += 32) {
+  for (int l = lane; l < L; l += TEAM) {
     const int o = off_lm(ly, od, l);
     int f = o;
     for (int k = 1; k <= c - 2; ++k)
       if ((w.rbm[k * ly.nw + (l >> 5)] >> (l & 31)) & 1u) { f = oC + 3 * (k - 1); break; }
     w.first[o] = f; w.first[o + 1] = f;
   }
-  __syncwarp();
+  tm.sync();
   // prior: all support blocks are mutually coupled
   if (s > 3) {
     int fs = np;
-    for (int p = 3 + lane; p < s; p += 32) fs = min(fs, w.ssup[p]);
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) fs = min(fs, __shfl_xor_sync(FULLMASK, fs, o));
-    for (int p = lane; p < s; p += 32) { const int i = w.ssup[p]; w.first[i] = min(w.first[i], fs); }
+    for (int p = 3 + lane; p < s; p += TEAM) fs = min(fs, w.ssup[p]);
+    fs = tm.min_int(fs, lane);
+    for (int p = lane; p < s; p += TEAM) { const int i = w.ssup[p]; w.first[i] = min(w.first[i], fs); }
   }
-  __syncwarp();
+  tm.sync();
   // landmarks are global: every range-bearing factor also touches the anchor, whose rows therefore
   // reach back to the first observing chain pose and the first observed landmark
   if (L > 0) {
     int fa = oA;
-    for (int k = lane; k < c; k += 32) {
+    for (int k = lane; k < c; k += TEAM) {
       uint64_t m = (uint64_t)w.rbm[k * ly.nw];
       if (ly.nw > 1) m |= (uint64_t)w.rbm[k * ly.nw + 1] << 32;
       if (m) {
@@ -316,32 +393,35 @@ __device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, int lane, 
         fa = min(fa, off_lm(ly, od, __ffsll((long long)m) - 1));
       }
     }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) fa = min(fa, __shfl_xor_sync(FULLMASK, fa, o));
+    fa = tm.min_int(fa, lane);
     if (lane < 3) w.first[oA + lane] = min(w.first[oA + lane], fa);
   }
-  __syncwarp();
+  tm.sync();
   // group rows in fours (shared first, aligned down to 4); prefix sum of the row lengths -> rbase
-  int run = 0;
-  for (int base = 0; base < np + 2; base += 32) {
-    const int i = base + lane;
-    int f = 0, len = 0;
-    if (i < np) {
-      const int g4 = i & ~3;
-      f = min(min(w.first[g4], w.first[g4 + 1]), min(w.first[g4 + 2], w.first[g4 + 3])) & ~3;
-      len = g4 + 4 - f;
-    } else if (i < np + 2) {
-      len = np;
-    }
-    int x = len;
+  // (done by the first warp of the team)
+  if (lane < 32) {
+    int run = 0;
+    for (int base = 0; base < np + 2; base += 32) {
+      const int i = base + lane;
+      int f = 0, len = 0;
+      if (i < np) {
+        const int g4 = i & ~3;
+        f = min(min(w.first[g4], w.first[g4 + 1]), min(w.first[g4 + 2], w.first[g4 + 3])) & ~3;
+        len = g4 + 4 - f;
+      } else if (i < np + 2) {
+        len = np;
+      }
+      int x = len;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(FULLMASK, x, o); if (lane >= o) x += y; }
-    __syncwarp();
-    if (i < np + 2) { w.first[i] = f; w.rbase[i] = run + x - len - f; }
-    run += __shfl_sync(FULLMASK, x, 31);
+      for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(FULLMASK, x, o); if (lane >= o) x += y; }
+      __syncwarp();
+      if (i < np + 2) { w.first[i] = f; w.rbase[i] = run + x - len - f; }
+      run += __shfl_sync(FULLMASK, x, 31);
+    }
+    if (lane == 0) reinterpret_cast<int*>(tm.scr)[8] = run;
   }
-  __syncwarp();
-  return run;
+  tm.sync();
+  return reinterpret_cast<const int*>(tm.scr)[8];
 }
 
 // ------------------------------------------------------------------ S1 + S2: linearise and assemble
@@ -422,30 +502,31 @@ __device__ __forceinline__ void add_i_side(const WS& w, int n, int oi, const flo
 }
 
 // Builds H and b (row n) at the current state.  `s` = prior support dimension.
-__device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, const float* rec, const WS& w, int lane, int head,
+template <int TEAM>
+__device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, const float* rec, const WS& w, const Team<TEAM>& tm, int lane, int head,
                          int c, const Masks& mk, int s, int total) {
   const int W = ly.W, L = ly.L, n = ly.np;  // n: row index of the rhs
-  for (int t = lane; t < total; t += 32) w.H[t] = 0.f;
+  for (int t = lane; t < total; t += TEAM) w.H[t] = 0.f;
   // cos/sin of every live pose (slot 0 is the frame itself)
-  for (int k = lane; k < c; k += 32) {
+  for (int k = lane; k < c; k += TEAM) {
     float sn = 0.f, cn = 1.f;
-    if (k > 0) sincosf(w.st[st_pose(k) + 2], &sn, &cn);
+    if (k > 0) sincos_pi(w.st[st_pose(k) + 2], &sn, &cn);
     w.cs[2 * k] = cn; w.cs[2 * k + 1] = sn;
   }
   // prior displacement d = v - vbar on the support (angles wrapped)
-  for (int p = lane; p < s; p += 32) {
+  for (int p = lane; p < s; p += TEAM) {
     const int id = w.sidx[p];
     float d = w.st[id & 0xffff] - rec[ly.o_vbar + p];
     if (id & 0x10000) d = wrapf(d);
     w.sds[p] = d;
   }
-  __syncwarp();
+  tm.sync();
   // identity rows for unused chain slots, the unused newest slot (c == 1), inactive landmarks, padding
-  for (int k = max(c - 1, 1) + lane; k <= W - 2; k += 32) {
+  for (int k = max(c - 1, 1) + lane; k <= W - 2; k += TEAM) {
     const int o = 2 * od.npas + 3 * (k - 1);
     w.H[w.rbase[o] + o] = 1.0f; w.H[w.rbase[o + 1] + o + 1] = 1.0f; w.H[w.rbase[o + 2] + o + 2] = 1.0f;
   }
-  for (int l = lane; l < L; l += 32)
+  for (int l = lane; l < L; l += TEAM)
     if (!((mk.act >> l) & 1ull)) {
       const int o = off_lm(ly, od, l);
       w.H[w.rbase[o] + o] = 1.0f; w.H[w.rbase[o + 1] + o + 1] = 1.0f;
@@ -457,10 +538,10 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
   // prior: H += Lambda (row by row, coalesced over the packed lower triangle)
   {
     const float* lam = rec + ly.o_lam;
-    for (int p = 0; p < s; ++p) {
+    for (int p = lane >> 5; p < s; p += TEAM / 32) {  // one packed row per warp at a time
       const int ip = w.ssup[p];
       const float* lrow = lam + (p * (p + 1) >> 1);
-      for (int q = lane; q <= p; q += 32) {
+      for (int q = lane & 31; q <= p; q += 32) {
         const int iq = w.ssup[q];
         const float v = lrow[q];
         const int hi = max(ip, iq), lo = min(ip, iq);
@@ -469,7 +550,7 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
     }
     // b -= Lambda d + g
     float* rhs = w.H + w.rbase[n];
-    for (int p = lane; p < s; p += 32) {
+    for (int p = lane; p < s; p += TEAM) {
       float acc = rec[ly.o_g + p];
       const float* lrow = lam + (p * (p + 1) >> 1);
       for (int q = 0; q <= p; ++q) acc = fmaf(lrow[q], w.sds[q], acc);
@@ -477,10 +558,10 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
       rhs[w.ssup[p]] -= acc;
     }
   }
-  __syncwarp();
+  tm.sync();
   // odometry factors k-1 -> k: phase A (j side), phase B (i side)
   for (int pass = 0; pass < 2; ++pass) {
-    for (int k = 1 + lane; k < c; k += 32) {
+    for (int k = 1 + lane; k < c; k += TEAM) {
       const float* pi = w.st + st_pose(k - 1);
       const float* pj = w.st + st_pose(k);
       const Between b = between_eval(pi, w.cs[2 * (k - 1)], w.cs[2 * (k - 1) + 1], pj, w.zodo + 3 * k);
@@ -494,10 +575,10 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
         add_i_side(w, n, off_slot(ly, od, k - 1, c), Hii, gi);
       }
     }
-    __syncwarp();
+    tm.sync();
   }
   // loop closures t -> k: phase C (j side: at most one per k), phase D (i side: lane per target)
-  for (int k = 1 + lane; k < c; k += 32) {
+  for (int k = 1 + lane; k < c; k += TEAM) {
     const int t = w.lct[k];
     if (t < 0) continue;
     const Between b = between_eval(w.st + st_pose(t), w.cs[2 * t], w.cs[2 * t + 1], w.st + st_pose(k), w.zlc + 3 * k);
@@ -505,8 +586,8 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
     between_jac(b, Ji, Jj);
     add_j_side(w, n, off_slot(ly, od, k, c), t >= 1 ? off_slot(ly, od, t, c) : 0, Ji, Jj, pr.om_lc, b.r, t >= 1);
   }
-  __syncwarp();
-  for (int t = 1 + lane; t < c - 1; t += 32) {
+  tm.sync();
+  for (int t = 1 + lane; t < c - 1; t += TEAM) {
     float Hii[6] = {0, 0, 0, 0, 0, 0}, gi[3] = {0, 0, 0};
     bool any = false;
     for (int k = t + 1; k < c; ++k) {
@@ -519,7 +600,7 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
     }
     if (any) add_i_side(w, n, off_slot(ly, od, t, c), Hii, gi);
   }
-  __syncwarp();
+  tm.sync();
   // range-bearing factors.  Landmarks g are global, so each factor has three blocks: anchor a, observing
   // pose e_k (k >= 1), landmark g.  With the anchor-frame landmark m = Rot(a_th)'(g - a_t), D = m - t_k:
   //   J_e = [-J_l | (0,-1)'],  J_g = J_l Rot(a_th)',  J_a = [-J_g | -J_l S m].
@@ -531,17 +612,22 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
     const float w0 = pr.om_rb[0], w1 = pr.om_rb[1];
     const int oA = off_a(ly);
     float sa, ca;
-    sincosf(w.st[2], &sa, &ca);
+    sincos_pi(w.st[2], &sa, &ca);
     const float ax = w.st[0], ay = w.st[1];
     float* mloc = w.sds + s;  // anchor-frame landmark positions (2L floats after the prior displacement)
-    for (int l = lane; l < L; l += 32) {
+    for (int l = lane; l < L; l += TEAM) {
       const float gxl = w.st[st_lm(ly, l)] - ax, gyl = w.st[st_lm(ly, l) + 1] - ay;
       mloc[2 * l] = ca * gxl + sa * gyl;
       mloc[2 * l + 1] = -sa * gxl + ca * gyl;
     }
-    __syncwarp();
+    tm.sync();
+    // With more than one warp per environment the two passes run concurrently on the two halves of the
+    // team (they write disjoint entries of H and b).
+    const int halfA = TEAM == 32 ? TEAM : TEAM / 2;
+    const bool doA = TEAM == 32 || lane < halfA, doB = TEAM == 32 || lane >= halfA;
+    const int laneB = TEAM == 32 ? lane : lane - halfA;
     // ---- pass A: lane = pose slot k >= 1
-    for (int k = 1 + lane; k < c; k += 32) {
+    for (int k = doA ? 1 + lane : c; k < c; k += halfA) {
       uint64_t m = (uint64_t)w.rbm[k * ly.nw];
       if (ly.nw > 1) m |= (uint64_t)w.rbm[k * ly.nw + 1] << 32;
       if (!m) continue;
@@ -597,17 +683,16 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
         qa[op] += R[9 + 3 * i]; qa[op + 1] += R[10 + 3 * i]; qa[op + 2] += R[11 + 3 * i];
       }
     }
-    __syncwarp();
+    if (TEAM == 32) tm.sync();
     // ---- pass B: lane = landmark
     float A[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};  // gg(3), <a2,g0>, <a2,g1>, <a2,a2>, <g0,r>, <g1,r>, <a2,r>
-    for (int base = 0; base < L; base += 32) {
-      const int l = base + lane;
-      const bool inl = l < L && ((od.obs >> l) & 1ull);
+    for (int l = doB ? laneB : L; l < L; l += halfA) {
+      const bool inl = (od.obs >> l) & 1ull;
       const float mx = inl ? mloc[2 * l] : 0.f, my = inl ? mloc[2 * l + 1] : 0.f;
       float Lxx = 0.f, Lxy = 0.f, Lyy = 0.f, bgx = 0.f, bgy = 0.f, ag0 = 0.f, ag1 = 0.f, a22 = 0.f, a2r = 0.f;
       for (int k = 0; k < c; ++k) {
-        const uint32_t word = w.rbm[k * ly.nw + (base >> 5)];
-        if (!((word >> lane) & 1u) || !inl) continue;
+        const uint32_t word = w.rbm[k * ly.nw + (l >> 5)];
+        if (!((word >> (l & 31)) & 1u) || !inl) continue;
         const int r = ring_of(k, head, W);
         const float zr = rec[ly.o_zrb + (r * 2 + 0) * L + l], zb = rec[ly.o_zrb + (r * 2 + 1) * L + l];
         const float* p = w.st + st_pose(k);
@@ -639,9 +724,8 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
         A[6] += bgx; A[7] += bgy; A[8] += a2r;
       }
     }
-#pragma unroll
-    for (int t = 0; t < 9; ++t) A[t] = warp_sum(A[t]);
-    __syncwarp();
+    tm.sync();
+    tm.sum_n(A, lane);
     if (lane == 0) {  // anchor diagonal block and gradient
       float* qa0 = w.H + w.rbase[oA];
       float* qa1 = w.H + w.rbase[oA + 1];
@@ -650,7 +734,7 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
       qa2[oA] -= A[3]; qa2[oA + 1] -= A[4]; qa2[oA + 2] += A[5];
       rhs[oA] += A[6]; rhs[oA + 1] += A[7]; rhs[oA + 2] -= A[8];
     }
-    __syncwarp();
+    tm.sync();
   }
 }
 
@@ -667,7 +751,8 @@ __device__ __forceinline__ void st4(float* p, float4 v) { *reinterpret_cast<floa
   ACC = fmaf(-XV.x, BV.x, ACC); ACC = fmaf(-XV.y, BV.y, ACC); ACC = fmaf(-XV.z, BV.z, ACC); \
   ACC = fmaf(-XV.w, BV.w, ACC);
 
-__device__ int cholesky(const Layout& ly, const WS& w, int lane) {
+template <int TEAM>
+__device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int lane) {
   const int np = ly.np, G = np >> 2;
   int flag = 0;
   for (int J = 0; J < G; ++J) {
@@ -677,31 +762,58 @@ __device__ int cholesky(const Layout& ly, const WS& w, int lane) {
     const float* rJ1 = w.H + w.rbase[c0 + 1];
     const float* rJ2 = w.H + w.rbase[c0 + 2];
     const float* rJ3 = w.H + w.rbase[c0 + 3];
+    // K-split: when fewer row pairs than threads remain, `ch` adjacent lanes share one pair and split
+    // the dot-product range; partial sums are combined by shuffles.
+    const int npairs = (np + 2 - c0) >> 1;
+    int ch = 1;
+    while (ch < 8 && npairs * (ch * 2) <= TEAM) ch *= 2;
+    const int per_pass = TEAM / ch;
+    const int t = lane & (ch - 1);
     float d0 = 1.f, d1 = 1.f, d2 = 1.f, d3 = 1.f, l10 = 0.f, l20 = 0.f, l21 = 0.f, l30 = 0.f, l31 = 0.f, l32 = 0.f;
-    for (int i0 = c0 + 2 * lane; i0 - 2 * lane < np + 2; i0 += 64) {
-      const bool first_pass = (i0 - 2 * lane == c0);
-      const bool act = i0 < np + 2 && w.first[i0] <= c0;
+    for (int q0 = 0; q0 < npairs; q0 += per_pass) {
+      const bool first_pass = q0 == 0;
+      const int q = q0 + lane / ch;
+      const int i0 = c0 + 2 * q;
+      const bool act = q < npairs && w.first[i0] <= c0;
       float4 a0 = make_float4(0.f, 0.f, 0.f, 0.f), a1 = a0;
       float* p0 = nullptr;
       float* p1 = nullptr;
       if (act) {
         p0 = w.H + w.rbase[i0];
         p1 = w.H + w.rbase[i0 + 1];
-        a0 = ld4(p0 + c0);
-        a1 = ld4(p1 + c0);
-        for (int k = max(w.first[i0], fJ); k < c0; k += 4) {
+        if (t == 0) { a0 = ld4(p0 + c0); a1 = ld4(p1 + c0); }
+        const int ks = max(w.first[i0], fJ);
+        const int nblk = (c0 - ks) >> 2;
+        const int kb = ks + 4 * ((t * nblk) / ch), ke = ks + 4 * (((t + 1) * nblk) / ch);
+        for (int k = kb; k < ke; k += 4) {
           const float4 x0 = ld4(p0 + k), x1 = ld4(p1 + k);
           const float4 b0 = ld4(rJ0 + k), b1 = ld4(rJ1 + k), b2 = ld4(rJ2 + k), b3 = ld4(rJ3 + k);
           FMA4(a0.x, x0, b0) FMA4(a0.y, x0, b1) FMA4(a0.z, x0, b2) FMA4(a0.w, x0, b3)
           FMA4(a1.x, x1, b0) FMA4(a1.y, x1, b1) FMA4(a1.z, x1, b2) FMA4(a1.w, x1, b3)
         }
       }
-      if (first_pass) {  // diagonal tile: lane 0 holds rows c0, c0+1; lane 1 rows c0+2, c0+3
-        const float s00 = __shfl_sync(FULLMASK, a0.x, 0);
-        const float s10 = __shfl_sync(FULLMASK, a1.x, 0), s11 = __shfl_sync(FULLMASK, a1.y, 0);
-        const float s20 = __shfl_sync(FULLMASK, a0.x, 1), s21 = __shfl_sync(FULLMASK, a0.y, 1), s22 = __shfl_sync(FULLMASK, a0.z, 1);
-        const float s30 = __shfl_sync(FULLMASK, a1.x, 1), s31 = __shfl_sync(FULLMASK, a1.y, 1), s32 = __shfl_sync(FULLMASK, a1.z, 1);
-        const float s33 = __shfl_sync(FULLMASK, a1.w, 1);
+      for (int o = ch >> 1; o > 0; o >>= 1) {  // combine the K-split partial sums (uniform trip count)
+        a0.x += __shfl_xor_sync(FULLMASK, a0.x, o); a0.y += __shfl_xor_sync(FULLMASK, a0.y, o);
+        a0.z += __shfl_xor_sync(FULLMASK, a0.z, o); a0.w += __shfl_xor_sync(FULLMASK, a0.w, o);
+        a1.x += __shfl_xor_sync(FULLMASK, a1.x, o); a1.y += __shfl_xor_sync(FULLMASK, a1.y, o);
+        a1.z += __shfl_xor_sync(FULLMASK, a1.z, o); a1.w += __shfl_xor_sync(FULLMASK, a1.w, o);
+      }
+      if (first_pass) {  // diagonal tile: thread 0 holds rows c0, c0+1; thread `ch` rows c0+2, c0+3
+        float s00, s10, s11, s20, s21, s22, s30, s31, s32, s33;
+        if (TEAM == 32) {
+          s00 = __shfl_sync(FULLMASK, a0.x, 0);
+          s10 = __shfl_sync(FULLMASK, a1.x, 0); s11 = __shfl_sync(FULLMASK, a1.y, 0);
+          s20 = __shfl_sync(FULLMASK, a0.x, ch); s21 = __shfl_sync(FULLMASK, a0.y, ch); s22 = __shfl_sync(FULLMASK, a0.z, ch);
+          s30 = __shfl_sync(FULLMASK, a1.x, ch); s31 = __shfl_sync(FULLMASK, a1.y, ch); s32 = __shfl_sync(FULLMASK, a1.z, ch);
+          s33 = __shfl_sync(FULLMASK, a1.w, ch);
+        } else {
+          float* dg = tm.scr + 16;
+          if (lane == 0) { dg[0] = a0.x; dg[1] = a1.x; dg[2] = a1.y; }
+          if (lane == ch) { dg[3] = a0.x; dg[4] = a0.y; dg[5] = a0.z; dg[6] = a1.x; dg[7] = a1.y; dg[8] = a1.z; dg[9] = a1.w; }
+          tm.sync();
+          s00 = dg[0]; s10 = dg[1]; s11 = dg[2]; s20 = dg[3]; s21 = dg[4]; s22 = dg[5];
+          s30 = dg[6]; s31 = dg[7]; s32 = dg[8]; s33 = dg[9];
+        }
         bool bad = !(s00 > 0.f);
         d0 = rsqrtf(s00);
         l10 = s10 * d0; l20 = s20 * d0; l30 = s30 * d0;
@@ -724,9 +836,9 @@ __device__ int cholesky(const Layout& ly, const WS& w, int lane) {
           if (!(t33 > 0.f)) d3 = 1.f;
         }
       }
-      if (act) {
-        if (first_pass && lane < 2) {
-          if (lane == 0) { a0 = make_float4(d0, 0.f, 0.f, 0.f); a1 = make_float4(l10, d1, 0.f, 0.f); }
+      if (act && t == 0) {
+        if (first_pass && q < 2) {
+          if (q == 0) { a0 = make_float4(d0, 0.f, 0.f, 0.f); a1 = make_float4(l10, d1, 0.f, 0.f); }
           else { a0 = make_float4(l20, l21, d2, 0.f); a1 = make_float4(l30, l31, l32, d3); }
         } else {
           a0.x *= d0; a0.y = fmaf(-a0.x, l10, a0.y) * d1;
@@ -740,14 +852,15 @@ __device__ int cholesky(const Layout& ly, const WS& w, int lane) {
         st4(p1 + c0, a1);
       }
     }
-    __syncwarp();
+    tm.sync();
   }
   return flag;
 }
 
 // Solves L' delta = y in place in row np, by 4-row blocks from the bottom: delta_I from the diagonal
 // tile (every lane redundantly), then y_K -= L(I,K)' delta_I with lanes over the column blocks K.
-__device__ void back_substitute(const Layout& ly, const WS& w, int lane) {
+template <int TEAM>
+__device__ void back_substitute(const Layout& ly, const WS& w, const Team<TEAM>& tm, int lane) {
   const int np = ly.np, G = np >> 2;
   float* y = w.H + w.rbase[np];
   for (int I = G - 1; I >= 0; --I) {
@@ -761,9 +874,9 @@ __device__ void back_substitute(const Layout& ly, const WS& w, int lane) {
     const float e2 = fmaf(-t3.z, e3, yy.z) * t2.z;
     const float e1 = fmaf(-t3.y, e3, fmaf(-t2.y, e2, yy.y)) * t1.y;
     const float e0 = fmaf(-t3.x, e3, fmaf(-t2.x, e2, fmaf(-t1.x, e1, yy.x))) * t0.x;
-    __syncwarp();
+    tm.sync();
     if (lane == 0) st4(y + c0, make_float4(e0, e1, e2, e3));
-    for (int k = w.first[c0] + 4 * lane; k < c0; k += 128) {
+    for (int k = w.first[c0] + 4 * lane; k < c0; k += 4 * TEAM) {
       const float4 x0 = ld4(r0 + k), x1 = ld4(r1 + k), x2 = ld4(r2 + k), x3 = ld4(r3 + k);
       float4 v = ld4(y + k);
       v.x = fmaf(-x3.x, e3, fmaf(-x2.x, e2, fmaf(-x1.x, e1, fmaf(-x0.x, e0, v.x))));
@@ -772,12 +885,13 @@ __device__ void back_substitute(const Layout& ly, const WS& w, int lane) {
       v.w = fmaf(-x3.w, e3, fmaf(-x2.w, e2, fmaf(-x1.w, e1, fmaf(-x0.w, e0, v.w))));
       st4(y + k, v);
     }
-    __syncwarp();
+    tm.sync();
   }
 }
 
 // v <- v + delta (R1: additive, angles wrapped).  Returns ENV_NONFINITE if the update is not finite.
-__device__ int apply_update(const Layout& ly, const Ord& od, const WS& w, int lane, int c, const Masks& mk) {
+template <int TEAM>
+__device__ int apply_update(const Layout& ly, const Ord& od, const WS& w, const Team<TEAM>& tm, int lane, int c, const Masks& mk) {
   const int W = ly.W, L = ly.L;
   const float* dl = w.H + w.rbase[ly.np];
   int bad = 0;
@@ -787,28 +901,29 @@ __device__ int apply_update(const Layout& ly, const Ord& od, const WS& w, int la
     const float v = w.st[lane] + d;
     w.st[lane] = lane == 2 ? wrapf(v) : v;
   }
-  for (int i = lane; i < 3 * (c - 1); i += 32) {
+  for (int i = lane; i < 3 * (c - 1); i += TEAM) {
     const int k = 1 + i / 3, j = i - 3 * (k - 1);
     const float d = dl[off_slot(ly, od, k, c) + j];
     bad |= !isfinite(d);
     const float v = w.st[st_pose(k) + j] + d;
     w.st[st_pose(k) + j] = j == 2 ? wrapf(v) : v;
   }
-  for (int i = lane; i < 2 * L; i += 32) {
+  for (int i = lane; i < 2 * L; i += TEAM) {
     if (!((mk.act >> (i >> 1)) & 1ull)) continue;
     const float d = dl[off_lm(ly, od, i >> 1) + (i & 1)];
     bad |= !isfinite(d);
     w.st[3 + 3 * W + i] += d;
   }
-  bad = __any_sync(FULLMASK, bad);
-  __syncwarp();
-  return bad ? ENV_NONFINITE : 0;
+  const bool anybad = tm.any(bad != 0, lane);
+  tm.sync();
+  return anybad ? ENV_NONFINITE : 0;
 }
 
 // ------------------------------------------------------------------ S4: covariance of the newest pose
 // Sigma_6 = (L_t L_t')^{-1} from the trailing 6x6 of L (variables: newest pose e, anchor a), then
 // Sigma_t = J Sigma_6 J' with x = a (+) e (A.4).  O(1) per environment, done in fp64 by lane 0.
-__device__ void covariance(const Layout& ly, const WS& w, int lane, int env, int c, const StepIO& io) {
+template <int TEAM>
+__device__ void covariance(const Layout& ly, const WS& w, const Team<TEAM>& tm, int lane, int env, int c, const StepIO& io) {
   if (lane != 0) return;
   const int n = ly.np, N = ly.N;
   double S[3][3];
@@ -816,16 +931,19 @@ __device__ void covariance(const Layout& ly, const WS& w, int lane, int env, int
     // only the anchor exists: Sigma = (L_a L_a')^{-1}
     double Li[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
     double Lm[3][3];
+    #pragma unroll 1
     for (int x = 0; x < 3; ++x) {
       const int i = n - 3 + x;
       for (int y = 0; y <= x; ++y) Lm[x][y] = (y == x) ? 1.0 / (double)w.H[w.rbase[i] + i] : (double)w.H[w.rbase[i] + n - 3 + y];
     }
+    #pragma unroll 1
     for (int col = 0; col < 3; ++col)
       for (int x = col; x < 3; ++x) {
         double sum = (x == col) ? 1.0 : 0.0;
         for (int k = col; k < x; ++k) sum -= Lm[x][k] * Li[k][col];
         Li[x][col] = sum / Lm[x][x];
       }
+    #pragma unroll 1
     for (int x = 0; x < 3; ++x)
       for (int y = 0; y < 3; ++y) {
         double sum = 0.0;
@@ -834,6 +952,7 @@ __device__ void covariance(const Layout& ly, const WS& w, int lane, int env, int
       }
   } else {
     double Lm[6][6], Li[6][6];
+    #pragma unroll 1
     for (int x = 0; x < 6; ++x) {
       const int i = n - 6 + x;
       const int fi = w.first[i];
@@ -844,6 +963,7 @@ __device__ void covariance(const Layout& ly, const WS& w, int lane, int env, int
         else if (j >= fi) Lm[x][y] = (double)w.H[w.rbase[i] + j];
       }
     }
+    #pragma unroll 1
     for (int col = 0; col < 6; ++col)
       for (int x = col; x < 6; ++x) {
         double sum = (x == col) ? 1.0 : 0.0;
@@ -851,6 +971,7 @@ __device__ void covariance(const Layout& ly, const WS& w, int lane, int env, int
         Li[x][col] = sum / Lm[x][x];
       }
     double S6[6][6];
+    #pragma unroll 1
     for (int x = 0; x < 6; ++x)
       for (int y = 0; y < 6; ++y) {
         double sum = 0.0;
@@ -858,11 +979,13 @@ __device__ void covariance(const Layout& ly, const WS& w, int lane, int env, int
         S6[x][y] = sum;
       }
     // J = [J_e | J_a], J_e = blockdiag(Rot(a_th), 1), J_a = [[1,0,-dy],[0,1,dx],[0,0,1]], d = Rot(a_th) t_e
-    const double ath = (double)w.st[2];
-    const double ca = cos(ath), sa = sin(ath);
+    float saf, caf;
+    sincos_pi(w.st[2], &saf, &caf);
+    const double ca = (double)caf, sa = (double)saf;
     const float* e = w.st + st_pose(c - 1);
     const double dx = ca * e[0] - sa * e[1], dy = sa * e[0] + ca * e[1];
     double J[3][6] = {{ca, -sa, 0, 1, 0, -dy}, {sa, ca, 0, 0, 1, dx}, {0, 0, 1, 0, 0, 1}};
+    #pragma unroll 1
     for (int x = 0; x < 3; ++x)
       for (int y = 0; y < 3; ++y) {
         double sum = 0.0;
@@ -874,20 +997,22 @@ __device__ void covariance(const Layout& ly, const WS& w, int lane, int env, int
         S[x][y] = sum;
       }
   }
-  for (int x = 0; x < 3; ++x)  // R20
+  #pragma unroll 1
+    for (int x = 0; x < 3; ++x)  // R20
     for (int y = x + 1; y < 3; ++y) { const double t = 0.5 * (S[x][y] + S[y][x]); S[x][y] = t; S[y][x] = t; }
   const double det = S[0][0] * (S[1][1] * S[2][2] - S[1][2] * S[2][1]) - S[0][1] * (S[1][0] * S[2][2] - S[1][2] * S[2][0]) +
                      S[0][2] * (S[1][0] * S[2][1] - S[1][1] * S[2][0]);
-  const double ld = log(det);
-  for (int x = 0; x < 3; ++x)
+  const float ld = logf((float)det);
+  #pragma unroll 1
+    for (int x = 0; x < 3; ++x)
     for (int y = 0; y < 3; ++y) {
       const float v = (float)S[x][y];
       io.cov_cache[(size_t)(3 * x + y) * N + env] = v;
       if (io.cov) io.cov[(size_t)(3 * x + y) * N + env] = v;
     }
-  io.cov_cache[(size_t)9 * N + env] = (float)ld;
-  if (io.logdet) io.logdet[env] = (float)ld;
-  if (io.dopt) io.dopt[env] = (float)exp(ld / 3.0);
+  io.cov_cache[(size_t)9 * N + env] = ld;
+  if (io.logdet) io.logdet[env] = ld;
+  if (io.dopt) io.dopt[env] = expf(ld * (1.0f / 3.0f));
 }
 
 // ------------------------------------------------------------------ S5: marginalise the oldest pose
@@ -900,15 +1025,16 @@ struct Etype { float p, q, u, v; };  // E = [[p,-q,u],[q,p,v],[0,0,1]]
 __device__ __forceinline__ int tri(int i, int j) { return (i * (i + 1) >> 1) + j; }  // i >= j
 __device__ __forceinline__ float sym_get(const float* Hs, int i, int j) { return i >= j ? Hs[tri(i, j)] : Hs[tri(j, i)]; }
 
-__device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const WS& w, int lane, int head, int c,
+template <int TEAM>
+__device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const WS& w, const Team<TEAM>& tm, int lane, int head, int c,
                            Masks& mk, int s_old) {
   const int W = ly.W, L = ly.L;
   int* reci = (int*)rec;
   uint32_t* recu = (uint32_t*)rec;
   // --- A. new support masks
   uint64_t lc0 = 0ull;
-  for (int base = 0; base < c; base += 32) {
-    const int k = base + lane;
+  for (int base = 0; base < c; base += 32) {  // every warp of the team builds the whole mask
+    const int k = base + (lane & 31);
     const uint32_t bal = __ballot_sync(FULLMASK, k >= 1 && k < c && w.lct[k] == 0);
     lc0 |= (uint64_t)bal << base;
   }
@@ -927,7 +1053,7 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
   int* nidx = w.ssup;  // elimination offsets are dead from here on
 
   // --- B. old displacement d, old -> new scalar map, new state-index table
-  for (int p = lane; p < s_old; p += 32) {
+  for (int p = lane; p < s_old; p += TEAM) {
     const int id = w.sidx[p];
     float d = w.st[id & 0xffff] - rec[ly.o_vbar + p];
     if (id & 0x10000) d = wrapf(d);
@@ -943,17 +1069,17 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
     }
     omap[p] = P;
   }
-  for (int t = lane; t < (s * (s + 1) >> 1) + s; t += 32) Hs[t] = 0.f;  // Hs and gam
-  __syncwarp();
+  for (int t = lane; t < (s * (s + 1) >> 1) + s; t += TEAM) Hs[t] = 0.f;  // Hs and gam
+  tm.sync();
   const float a_th = w.st[2];
   float sa, ca;
-  sincosf(a_th, &sa, &ca);
+  sincos_pi(a_th, &sa, &ca);
   const float x1 = w.st[st_pose(1)], y1 = w.st[st_pose(1) + 1], th1 = w.st[st_pose(1) + 2];
   float s1, c1;
-  sincosf(th1, &s1, &c1);
+  sincos_pi(th1, &s1, &c1);
   const float ddx = ca * x1 - sa * y1, ddy = sa * x1 + ca * y1;  // d = Rot(a_th) t_1
   // new tables + X rows (step E)
-  for (int p = lane; p < s; p += 32) {
+  for (int p = lane; p < s; p += TEAM) {
     int id;
     float X0, X1, X2;
     if (p < 3) {
@@ -978,16 +1104,16 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
     nidx[p] = id;
     X[3 * p] = X0; X[3 * p + 1] = X1; X[3 * p + 2] = X2;
   }
-  __syncwarp();
+  tm.sync();
   // --- C. scatter the old prior
   {
     const float* lam = rec + ly.o_lam;
-    for (int p = 0; p < s_old; ++p) {
+    for (int p = lane >> 5; p < s_old; p += TEAM / 32) {
       const int P = omap[p];
       const float* lrow = lam + (p * (p + 1) >> 1);
-      for (int q = lane; q <= p; q += 32) Hs[tri(P, omap[q])] = lrow[q];
+      for (int q = lane & 31; q <= p; q += 32) Hs[tri(P, omap[q])] = lrow[q];
     }
-    for (int p = lane; p < s_old; p += 32) {
+    for (int p = lane; p < s_old; p += TEAM) {
       float acc = rec[ly.o_g + p];
       const float* lrow = lam + (p * (p + 1) >> 1);
       for (int q = 0; q <= p; ++q) acc = fmaf(lrow[q], w.sds[q], acc);
@@ -995,7 +1121,7 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
       gam[omap[p]] = acc;
     }
   }
-  __syncwarp();
+  tm.sync();
   // --- D. factors touching slot 0 (the frame): J_j = I for between factors
   if (lane < 3) {
     float r = w.st[st_pose(1) + lane] - w.zodo[3 + lane];
@@ -1003,10 +1129,9 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
     Hs[tri(3 + lane, 3 + lane)] += pr.om_odo[lane];
     gam[3 + lane] += pr.om_odo[lane] * r;
   }
-  __syncwarp();
-  for (int base = 0; base < c; base += 32) {
-    const int k = base + lane;
-    if (k >= 1 && k < c && w.lct[k] == 0) {
+  tm.sync();
+  for (int k = 1 + lane; k < c; k += TEAM) {
+    if (w.lct[k] == 0) {
       const int P = 3 + 3 * __popcll(nps & lowmask(k));
       for (int x = 0; x < 3; ++x) {
         float r = w.st[st_pose(k) + x] - w.zlc[3 * k + x];
@@ -1018,9 +1143,8 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
   }
   if (L > 0 && rb0) {  // range-bearing from slot 0 (observing pose x = a): blocks a and g
     float A[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
-    for (int base = 0; base < L; base += 32) {
-      const int l = base + lane;
-      if (l < L && ((rb0 >> l) & 1ull)) {
+    for (int l = lane; l < L; l += TEAM) {
+      if ((rb0 >> l) & 1ull) {
         const float zr = rec[ly.o_zrb + (head * 2 + 0) * L + l], zb = rec[ly.o_zrb + (head * 2 + 1) * L + l];
         const float gxl = w.st[st_lm(ly, l)] - w.st[0], gyl = w.st[st_lm(ly, l) + 1] - w.st[1];
         const float dx = ca * gxl + sa * gyl, dy = -sa * gxl + ca * gyl;  // m = Rot(a_th)'(g - a_t)
@@ -1044,21 +1168,19 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
         A[6] += g0r; A[7] += g1r; A[8] += a2r;
       }
     }
-#pragma unroll
-    for (int t = 0; t < 9; ++t) A[t] = warp_sum(A[t]);
+    tm.sum_n(A, lane);
     if (lane == 0) {
       Hs[tri(0, 0)] += A[0]; Hs[tri(1, 0)] += A[1]; Hs[tri(1, 1)] += A[2];
       Hs[tri(2, 0)] -= A[3]; Hs[tri(2, 1)] -= A[4]; Hs[tri(2, 2)] += A[5];
       gam[0] -= A[6]; gam[1] -= A[7]; gam[2] += A[8];
     }
   }
-  __syncwarp();
+  tm.sync();
   // --- F. Q = H_s X;  Y = X'Q;  gx = X'gamma
   float Y[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0}, gx[3] = {0, 0, 0};
-  for (int base = 0; base < s; base += 32) {
-    const int p = base + lane;
+  for (int p = lane; p < s; p += TEAM) {
     float q0 = 0.f, q1 = 0.f, q2 = 0.f;
-    if (p < s) {
+    {
       for (int q = 0; q < s; ++q) {
         const float h = sym_get(Hs, p, q);
         q0 = fmaf(h, X[3 * q], q0); q1 = fmaf(h, X[3 * q + 1], q1); q2 = fmaf(h, X[3 * q + 2], q2);
@@ -1071,11 +1193,9 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
       gx[0] += xa * gp; gx[1] += xb * gp; gx[2] += xc * gp;
     }
   }
-#pragma unroll
-  for (int t = 0; t < 9; ++t) Y[t] = warp_sum(Y[t]);
-#pragma unroll
-  for (int t = 0; t < 3; ++t) gx[t] = warp_sum(gx[t]);
-  __syncwarp();
+  tm.sum_n(Y, lane);
+  tm.sum_n(gx, lane);
+  tm.sync();
   // --- G. G = E' H_s E block by block (in place);  T_b = E_b' Q_b;  gamma_b = E_b' gamma_b
   auto etype = [&](int b) -> Etype {
     if (b == 0) return Etype{1.f, 0.f, ddy, -ddx};          // A = da/da'
@@ -1084,7 +1204,7 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
   };
   auto bpos = [&](int b) -> int { return b == 0 ? 0 : (b <= npn ? 3 + 3 * (b - 1) : 3 + 3 * npn + 2 * (b - 1 - npn)); };
   const int npairs = nbk * (nbk + 1) >> 1;
-  for (int t = lane; t < npairs; t += 32) {
+  for (int t = lane; t < npairs; t += TEAM) {
     int bi = (int)((sqrtf(8.f * (float)t + 1.f) - 1.f) * 0.5f);
     while ((bi + 1) * (bi + 2) / 2 <= t) ++bi;
     while (bi * (bi + 1) / 2 > t) --bi;
@@ -1115,7 +1235,7 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
       for (int y = 0; y < 3; ++y)
         if (x < di && y < dj && (bi != bj || y <= x)) Hs[tri(pi + x, pj + y)] = M[x][y];
   }
-  for (int b = lane; b < nbk; b += 32) {
+  for (int b = lane; b < nbk; b += TEAM) {
     const int pb = bpos(b), db = b <= npn ? 3 : 2;
     const Etype E = etype(b);
     float t0[3], t1[3], t2[3] = {0, 0, 0};
@@ -1132,7 +1252,7 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
     gam[pb + 1] = -E.q * g0 + E.p * g1;
     if (db == 3) gam[pb + 2] = E.u * g0 + E.v * g1 + g2;
   }
-  __syncwarp();
+  tm.sync();
   // --- I. H_ww, gamma_w (every lane redundantly), K = G[:,w] + T (into Q), KW = K H_ww^{-1} (into X)
   float Hw[3][3], gw[3];
 #pragma unroll
@@ -1156,8 +1276,8 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
     Wi[1][2] = (Hw[0][2] * Hw[1][0] - Hw[0][0] * Hw[1][2]) * id;
     Wi[2][2] = (Hw[0][0] * Hw[1][1] - Hw[0][1] * Hw[1][0]) * id;
   }
-  __syncwarp();
-  for (int r = lane; r < s; r += 32) {
+  tm.sync();
+  for (int r = lane; r < s; r += TEAM) {
     if (r >= 3 && r < 6) continue;
     float K[3];
 #pragma unroll
@@ -1168,35 +1288,35 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
       X[3 * r + y] = K[0] * Wi[0][y] + K[1] * Wi[1][y] + K[2] * Wi[2][y];
     }
   }
-  __syncwarp();
+  tm.sync();
   // --- 6. re-anchor the state (A.5 step 6); slot k keeps its ring position, slot 1 becomes the frame
   {
     const float nax = w.st[0] + ddx, nay = w.st[1] + ddy, nat = wrapf(a_th + th1);
-    for (int k = 2 + lane; k < c; k += 32) {
+    for (int k = 2 + lane; k < c; k += TEAM) {
       float* e = w.st + st_pose(k);
       const float ex = e[0] - x1, ey = e[1] - y1;
       e[0] = c1 * ex + s1 * ey; e[1] = -s1 * ex + c1 * ey; e[2] = wrapf(e[2] - th1);
     }
-    __syncwarp();
+    tm.sync();
     if (lane == 0) { w.st[0] = nax; w.st[1] = nay; w.st[2] = nat; }
     if (lane < 3) w.st[st_pose(1) + lane] = 0.f;
-    __syncwarp();
+    tm.sync();
   }
   // --- J. write (Lambda', g', vbar') on the support without w, packed lower, canonical order
   {
     float* lam = rec + ly.o_lam;
-    for (int r = 0; r < s; ++r) {
+    for (int r = lane >> 5; r < s; r += TEAM / 32) {  // one packed row per warp at a time
       if (r >= 3 && r < 6) continue;
       const int R = r < 3 ? r : r - 3;
       const float k0 = X[3 * r], k1 = X[3 * r + 1], k2 = X[3 * r + 2];
       float* lrow = lam + (R * (R + 1) >> 1);
-      for (int q = lane; q <= r; q += 32) {
+      for (int q = lane & 31; q <= r; q += 32) {
         if (q >= 3 && q < 6) continue;
         const int Qn = q < 3 ? q : q - 3;
         lrow[Qn] = Hs[tri(r, q)] - (k0 * Q[3 * q] + k1 * Q[3 * q + 1] + k2 * Q[3 * q + 2]);
       }
     }
-    for (int r = lane; r < s; r += 32) {
+    for (int r = lane; r < s; r += TEAM) {
       if (r >= 3 && r < 6) continue;
       const int R = r < 3 ? r : r - 3;
       rec[ly.o_g + R] = gam[r] - (X[3 * r] * gw[0] + X[3 * r + 1] * gw[1] + X[3 * r + 2] * gw[2]);
@@ -1204,7 +1324,7 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
     }
   }
   // --- K. bookkeeping: loop closures to the old slot 0 now live in the prior; new support masks
-  for (int k = 1 + lane; k < c; k += 32)
+  for (int k = 1 + lane; k < c; k += TEAM)
     if (w.lct[k] == 0) reci[ly.o_lct + ring_of(k, head, W)] = -1;
   mk.ps = nps & ~2ull;  // still indexed by the OLD slots; converted with the old head
   mk.ls = nls;
@@ -1213,7 +1333,7 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
     recu[ly.o_pm] = (uint32_t)pm; recu[ly.o_pm + 1] = (uint32_t)(pm >> 32);
     recu[ly.o_lm] = (uint32_t)nls; recu[ly.o_lm + 1] = (uint32_t)(nls >> 32);
   }
-  __syncwarp();
+  tm.sync();
   return 0;
 }
 

@@ -21,10 +21,11 @@ struct Layout {
   int rec;             // record stride
   int o_status, o_pm, o_lm, o_act, o_a, o_e, o_m, o_zodo, o_lct, o_zlc, o_rbm, o_zrb, o_vbar, o_g, o_lam;
   // shared memory per warp (32-bit words)
-  int s_st, s_zodo, s_zlc, s_lct, s_cs, s_rbm, s_first, s_rbase, s_ssup, s_sidx, s_sds, s_H;
+  int s_scr, s_st, s_zodo, s_zlc, s_lct, s_cs, s_rbm, s_first, s_rbase, s_ssup, s_sidx, s_sds, s_H;
   int cap;             // words available for H (envelope + rhs row) / marginalisation scratch
   int warp_words;      // total shared words per warp
-  int wpc;             // warps per CTA
+  int wpc;             // teams (environments in flight) per CTA
+  int team;            // threads per environment: 32, 64 or 128
 };
 
 struct Params {
@@ -58,6 +59,7 @@ static inline Layout make_layout(int N, int W, int L, int cap, int wpc) {
   y.rec = (o + 31) & ~31;  // 128-byte multiple
 
   int s = 0;
+  y.s_scr = s; s += 128;  // team scratch (reductions, diagonal tile)
   y.s_st = s; s = pad4(s + n + 3);
   y.s_zodo = s; s = pad4(s + 3 * W);
   y.s_zlc = s; s = pad4(s + 3 * W);
@@ -79,6 +81,7 @@ static inline Layout make_layout(int N, int W, int L, int cap, int wpc) {
   s += y.cap;
   y.warp_words = pad4(s);
   y.wpc = wpc;
+  y.team = 32;
   return y;
 }
 
