@@ -20,7 +20,7 @@ using namespace slamk;
 template <int TEAM>
 __global__ void __launch_bounds__(TEAM == 128 ? 896 : (TEAM == 64 ? 512 : 256))
 slam_step_kernel(Layout ly, Params pr, float* state, int head, int c, int flags, int iters, StepIO io,
-                 unsigned long long* stats) {
+                 unsigned long long* stats, int mode, int* ovf) {
   extern __shared__ float4 smem4[];
   float* smem = reinterpret_cast<float*>(smem4);
   const int team = threadIdx.x / TEAM, lane = threadIdx.x % TEAM;
@@ -33,10 +33,15 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head, int c, int flags,
   // large (~12 k instructions) and instruction-fetch bound, so warps that execute the same code at the
   // same time share every fetched line.  Teams without an environment in the last round only take part
   // in the barriers.
-  for (int env0 = blockIdx.x * ly.wpc; env0 < ly.N; env0 += gridDim.x * ly.wpc) {
-    const int env = env0 + team;
-    const bool valid = env < ly.N;
-    float* rec = state + (size_t)(valid ? env : 0) * ly.rec;
+  // mode 0: every environment; one whose envelope (or marginalisation scratch) exceeds this launch's
+  // shared-memory capacity is appended to the overflow list ovf[1..] (count in ovf[0]) and left untouched.
+  // mode 1: the environments of that list (launched with the dense capacity).
+  const int nwork = mode == 0 ? ly.N : ovf[0];
+  for (int env0 = blockIdx.x * ly.wpc; env0 < nwork; env0 += gridDim.x * ly.wpc) {
+    const int widx = env0 + team;
+    bool valid = widx < nwork;
+    const int env = valid ? (mode == 0 ? widx : ovf[1 + widx]) : 0;
+    float* rec = state + (size_t)env * ly.rec;
     int cc = c, status = 0, s = 0, total = 0;
     Masks mk;
     Ord od;
@@ -48,6 +53,8 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head, int c, int flags,
       od = make_ord(ly, w.rbm, cc);
       s = build_support<TEAM>(ly, od, w, tm, lane, cc, mk.ps, mk.ls);
     }
+    int need = 0;
+    if (valid && (flags & F_MARG)) need = marg_need(ly, w, lane, cc, mk);
     // iters Gauss-Newton iterations, then (F_COV) one more linearisation + factorisation at the final
     // estimate for the covariance: ONE call site per phase keeps the kernel small.
     const int nlin = iters + ((flags & F_COV) ? 1 : 0);
@@ -55,12 +62,22 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head, int c, int flags,
       __syncthreads();
       if (valid) {
         total = symbolic<TEAM>(ly, od, w, tm, lane, cc, mk, s);
-        if (stats && lane == 0) {  // envelope statistics (words per environment): max, sum, count
+        need = max(need, total);
+        if (stats && lane == 0 && mode == 0) {  // envelope statistics (words per environment): max, sum, count
           atomicMax(stats + 0, (unsigned long long)total);
           atomicAdd(stats + 1, (unsigned long long)total);
           atomicAdd(stats + 2, 1ull);
         }
       }
+    }
+    if (valid && need > ly.cap) {  // does not fit this launch: hand over to the dense-capacity launch
+      if (lane == 0) {
+        if (mode == 0) { const int slot = atomicAdd(ovf, 1); ovf[1 + slot] = env; atomicAdd(stats + 3, 1ull); }
+        else reinterpret_cast<int*>(rec)[ly.o_status] |= 4;
+      }
+      valid = false;
+    }
+    if (nlin > 0) {
 #pragma unroll 1
       for (int it = 0; it < nlin; ++it) {
         __syncthreads();
@@ -179,7 +196,11 @@ struct slam_ctx {
   int head, count;
   bool cov_valid;
   long long launches;
-  int grid, smem_bytes, ctas_per_sm;
+  int grid, smem_bytes, ctas_per_sm;      // dense-capacity launch (the only one if !two_pass)
+  Layout ly_small;                        // first launch with a smaller shared-memory capacity
+  int grid_small, smem_small, ctas_small;
+  bool two_pass;
+  int* ovf;                               // [0] count, [1..N] environments that did not fit
   char err[256];
 };
 
@@ -205,29 +226,41 @@ static int pick_team(int W, int L) {
   const char* e = getenv("SLAM_TEAM");
   if (e) { const int t = atoi(e); if (t == 32 || t == 64 || t == 128) return t; }
   const int n = 3 * W + 2 * L;
-  if (L > 0 && n >= 96) return 128;
   if (n >= 48) return 64;
   return 32;
 }
-static int pick_wpc(int W, int L, int team) {
-  const Layout t = make_layout(1, W, L, -1, 1);
+// Shared-memory capacity (words) of the first launch.  Environments whose envelope does not fit are
+// re-run by a second launch with the dense capacity.  SLAM_CAP_FRAC (0..1] overrides.  Landmark windows
+// are nearly dense while the robot is among the landmarks, so they use the dense capacity directly.
+static int pick_cap(int W, int L) {
+  const Layout d = make_layout(1, W, L, -1, 1);
+  double frac = L > 0 ? 1.0 : 0.45;
+  const char* e = getenv("SLAM_CAP_FRAC");
+  if (e) { const double f = atof(e); if (f > 0.0 && f <= 1.0) frac = f; }
+  int cap = (int)(frac * d.cap);
+  if (cap < 256) cap = 256;
+  return cap >= d.cap ? -1 : cap;
+}
+static int pick_wpc(int W, int L, int team, int cap) {
+  const Layout t = make_layout(1, W, L, cap, 1);
   const size_t wb = (size_t)t.warp_words * 4;
   int wpc = (int)((size_t)227 * 1024 / wb);
   const int maxt = team == 128 ? 7 : 8;   // 896 / 512 / 256 threads per CTA
   if (wpc > maxt) wpc = maxt;
   return wpc;  // 0 if one environment does not fit
 }
-typedef void (*step_fn)(Layout, Params, float*, int, int, int, int, StepIO, unsigned long long*);
+typedef void (*step_fn)(Layout, Params, float*, int, int, int, int, StepIO, unsigned long long*, int, int*);
 static step_fn kernel_of(int team) {
   return team == 128 ? slam_step_kernel<128> : (team == 64 ? slam_step_kernel<64> : slam_step_kernel<32>);
 }
 
-struct WsPlan { size_t stats, state, cache, odom, lcb, lcm, rbk, rbm, cov, ld, pose, total; };
+struct WsPlan { size_t stats, ovf, state, cache, odom, lcb, lcm, rbk, rbm, cov, ld, pose, total; };
 static WsPlan plan(const Layout& ly) {
   WsPlan p;
   size_t o = 0;
   const size_t N = (size_t)ly.N;
   p.stats = o; o = al256(o + 64);
+  p.ovf = o; o = al256(o + (N + 1) * 4);
   p.state = o; o = al256(o + N * ly.rec * 4);
   p.cache = o; o = al256(o + N * 10 * 4);
   p.odom = o; o = al256(o + N * 3 * 4);
@@ -253,7 +286,7 @@ void slam_default_config(slam_config* cfg) {
 
 size_t slam_workspace_bytes(int batch, int window, int landmarks) {
   if (!sizes_ok(batch, window, landmarks)) return 0;
-  const int wpc = pick_wpc(window, landmarks, pick_team(window, landmarks));
+  const int wpc = pick_wpc(window, landmarks, pick_team(window, landmarks), -1);
   if (wpc < 1) return 0;
   return plan(make_layout(batch, window, landmarks, -1, wpc)).total;
 }
@@ -264,7 +297,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   *out = nullptr;
   if (!sizes_ok(batch, window, landmarks) || !workspace || ((uintptr_t)workspace & 255)) return SLAM_EINVAL;
   const int team = pick_team(window, landmarks);
-  const int wpc = pick_wpc(window, landmarks, team);
+  const int wpc = pick_wpc(window, landmarks, team, -1);
   if (wpc < 1) return SLAM_EINVAL;
   slam_config dc;
   slam_default_config(&dc);
@@ -288,6 +321,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   c->stream = (cudaStream_t)cuda_stream;
   char* base = (char*)workspace;
   c->stats = (unsigned long long*)(base + p.stats);
+  c->ovf = (int*)(base + p.ovf);
   c->state = (float*)(base + p.state);
   c->cov_cache = (float*)(base + p.cache);
   c->st_odom = (float*)(base + p.odom);
@@ -301,7 +335,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   c->launches = 0;
   c->err[0] = 0;
   c->smem_bytes = c->ly.warp_words * 4 * wpc;
-  if (cudaFuncSetAttribute(kernel_of(team), cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_bytes) != cudaSuccess) {
+  if (cudaFuncSetAttribute(kernel_of(team), cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) {
     cudaGetLastError();
     delete c;
     return SLAM_ECUDA;
@@ -314,6 +348,23 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   c->ctas_per_sm = occ;
   const int need = (batch + wpc - 1) / wpc;
   c->grid = need < sms * occ ? need : sms * occ;
+  // optional first launch with a smaller capacity (more environments in flight per SM)
+  c->two_pass = false;
+  const int cap = pick_cap(window, landmarks);
+  if (cap > 0) {
+    const int wpc_s = pick_wpc(window, landmarks, team, cap);
+    c->ly_small = make_layout(batch, window, landmarks, cap, wpc_s);
+    c->ly_small.team = team;
+    c->smem_small = c->ly_small.warp_words * 4 * wpc_s;
+    int occ_s = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_s, kernel_of(team), wpc_s * team, c->smem_small);
+    if (occ_s >= 1 && occ_s * wpc_s > occ * wpc) {
+      c->two_pass = true;
+      c->ctas_small = occ_s;
+      const int need_s = (batch + wpc_s - 1) / wpc_s;
+      c->grid_small = need_s < sms * occ_s ? need_s : sms * occ_s;
+    }
+  }
   *out = c;
   const int rc = slam_reset(c, nullptr);
   if (rc != SLAM_OK) { *out = nullptr; delete c; }
@@ -333,9 +384,19 @@ int slam_reset(slam_ctx* c, const float* init_pose) {
 }
 
 static int launch_step(slam_ctx* c, int flags, int iters, const StepIO& io) {
-  kernel_of(c->ly.team)<<<c->grid, c->ly.wpc * c->ly.team, c->smem_bytes, c->stream>>>(c->ly, c->pr, c->state, c->head,
-                                                                                      c->count, flags, iters, io, c->stats);
-  c->launches++;
+  const step_fn fn = kernel_of(c->ly.team);
+  if (c->two_pass) {
+    cudaMemsetAsync(c->ovf, 0, 4, c->stream);
+    fn<<<c->grid_small, c->ly_small.wpc * c->ly.team, c->smem_small, c->stream>>>(c->ly_small, c->pr, c->state, c->head, c->count,
+                                                                                   flags, iters, io, c->stats, 0, c->ovf);
+    fn<<<c->grid, c->ly.wpc * c->ly.team, c->smem_bytes, c->stream>>>(c->ly, c->pr, c->state, c->head, c->count, flags, iters,
+                                                                        io, c->stats, 1, c->ovf);
+    c->launches += 2;
+  } else {
+    fn<<<c->grid, c->ly.wpc * c->ly.team, c->smem_bytes, c->stream>>>(c->ly, c->pr, c->state, c->head, c->count, flags, iters,
+                                                                        io, c->stats, 0, c->ovf);
+    c->launches++;
+  }
   return check_cuda(c, "slam_step_kernel");
 }
 
@@ -495,9 +556,9 @@ const char* slam_last_error(const slam_ctx* c) { return c ? c->err : "null conte
 
 int slam_kernel_info(const slam_ctx* c, int* smem_bytes_per_cta, int* warps_per_cta, int* ctas_per_sm) {
   if (!c) return SLAM_EINVAL;
-  if (smem_bytes_per_cta) *smem_bytes_per_cta = c->smem_bytes;
-  if (warps_per_cta) *warps_per_cta = c->ly.wpc * c->ly.team / 32;
-  if (ctas_per_sm) *ctas_per_sm = c->ctas_per_sm;
+  if (smem_bytes_per_cta) *smem_bytes_per_cta = c->two_pass ? c->smem_small : c->smem_bytes;
+  if (warps_per_cta) *warps_per_cta = (c->two_pass ? c->ly_small.wpc : c->ly.wpc) * c->ly.team / 32;
+  if (ctas_per_sm) *ctas_per_sm = c->two_pass ? c->ctas_small : c->ctas_per_sm;
   return SLAM_OK;
 }
 

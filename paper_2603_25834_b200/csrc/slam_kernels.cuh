@@ -765,14 +765,15 @@ __device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int
     // K-split: when fewer row pairs than threads remain, `ch` adjacent lanes share one pair and split
     // the dot-product range; partial sums are combined by shuffles.
     const int npairs = (np + 2 - c0) >> 1;
-    int ch = 1;
-    while (ch < 8 && npairs * (ch * 2) <= TEAM) ch *= 2;
-    const int per_pass = TEAM / ch;
+    int lg = 0;  // ch = 1 << lg
+    while (lg < 3 && (npairs << (lg + 1)) <= TEAM) ++lg;
+    const int ch = 1 << lg;
+    const int per_pass = TEAM >> lg;
     const int t = lane & (ch - 1);
     float d0 = 1.f, d1 = 1.f, d2 = 1.f, d3 = 1.f, l10 = 0.f, l20 = 0.f, l21 = 0.f, l30 = 0.f, l31 = 0.f, l32 = 0.f;
     for (int q0 = 0; q0 < npairs; q0 += per_pass) {
       const bool first_pass = q0 == 0;
-      const int q = q0 + lane / ch;
+      const int q = q0 + (lane >> lg);
       const int i0 = c0 + 2 * q;
       const bool act = q < npairs && w.first[i0] <= c0;
       float4 a0 = make_float4(0.f, 0.f, 0.f, 0.f), a1 = a0;
@@ -784,7 +785,7 @@ __device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int
         if (t == 0) { a0 = ld4(p0 + c0); a1 = ld4(p1 + c0); }
         const int ks = max(w.first[i0], fJ);
         const int nblk = (c0 - ks) >> 2;
-        const int kb = ks + 4 * ((t * nblk) / ch), ke = ks + 4 * (((t + 1) * nblk) / ch);
+        const int kb = ks + 4 * ((t * nblk) >> lg), ke = ks + 4 * (((t + 1) * nblk) >> lg);
         for (int k = kb; k < ke; k += 4) {
           const float4 x0 = ld4(p0 + k), x1 = ld4(p1 + k);
           const float4 b0 = ld4(rJ0 + k), b1 = ld4(rJ1 + k), b2 = ld4(rJ2 + k), b3 = ld4(rJ3 + k);
@@ -1024,6 +1025,20 @@ struct Etype { float p, q, u, v; };  // E = [[p,-q,u],[q,p,v],[0,0,1]]
 
 __device__ __forceinline__ int tri(int i, int j) { return (i * (i + 1) >> 1) + j; }  // i >= j
 __device__ __forceinline__ float sym_get(const float* Hs, int i, int j) { return i >= j ? Hs[tri(i, j)] : Hs[tri(j, i)]; }
+
+// Shared-memory words the marginalisation of this environment needs (support of the sub-problem).
+__device__ __forceinline__ int marg_need(const Layout& ly, const WS& w, int lane, int c, const Masks& mk) {
+  uint64_t lc0 = 0ull;
+  for (int base = 0; base < c; base += 32) {
+    const int k = base + (lane & 31);
+    const uint32_t bal = __ballot_sync(FULLMASK, k >= 1 && k < c && w.lct[k] == 0);
+    lc0 |= (uint64_t)bal << base;
+  }
+  uint64_t rb0 = 0ull;
+  if (ly.L > 0) { rb0 = (uint64_t)w.rbm[0]; if (ly.nw > 1) rb0 |= (uint64_t)w.rbm[1] << 32; }
+  const int s = 3 + 3 * __popcll(mk.ps | 2ull | lc0) + 2 * __popcll(mk.ls | rb0);
+  return (s * (s + 1) >> 1) + 8 * s;
+}
 
 template <int TEAM>
 __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const WS& w, const Team<TEAM>& tm, int lane, int head, int c,
