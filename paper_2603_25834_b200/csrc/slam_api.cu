@@ -245,7 +245,9 @@ static int pick_wpc(int W, int L, int team, int cap) {
   const Layout t = make_layout(1, W, L, cap, 1);
   const size_t wb = (size_t)t.warp_words * 4;
   int wpc = (int)((size_t)227 * 1024 / wb);
-  const int maxt = team == 128 ? 7 : 8;   // 896 / 512 / 256 threads per CTA
+  int maxt = team == 128 ? 7 : 8;   // 896 / 512 / 256 threads per CTA
+  const char* e = getenv("SLAM_MAX_WPC");
+  if (e && atoi(e) >= 1 && atoi(e) < maxt) maxt = atoi(e);
   if (wpc > maxt) wpc = maxt;
   return wpc;  // 0 if one environment does not fit
 }
