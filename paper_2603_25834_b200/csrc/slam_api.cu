@@ -24,6 +24,7 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head, int c, int flags,
   extern __shared__ float4 smem4[];
   float* smem = reinterpret_cast<float*>(smem4);
   const int team = threadIdx.x / TEAM, lane = threadIdx.x % TEAM;
+  const int LOCK = ly.lock;
   float* base = smem + (size_t)team * ly.warp_words;
   const WS w = make_ws(ly, base);
   Team<TEAM> tm;
@@ -80,11 +81,11 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head, int c, int flags,
     if (nlin > 0) {
 #pragma unroll 1
       for (int it = 0; it < nlin; ++it) {
-        __syncthreads();
+        if (LOCK >= 1) __syncthreads();
         if (valid) { assemble<TEAM>(ly, pr, od, rec, w, tm, lane, head, cc, mk, s, total); tm.sync(); }
-        __syncthreads();
+        if (LOCK >= 2) __syncthreads();
         if (valid) status |= cholesky<TEAM>(ly, w, tm, lane);
-        __syncthreads();
+        if (LOCK >= 3) __syncthreads();
         if (valid) {
           if (it < iters) {
             back_substitute<TEAM>(ly, w, tm, lane);
@@ -311,6 +312,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   if (!c) return SLAM_ENOMEM;
   c->ly = make_layout(batch, window, landmarks, -1, wpc);
   c->ly.team = team;
+  { const char* e = getenv("SLAM_LOCK"); if (e) c->ly.lock = atoi(e); }
   const WsPlan p = plan(c->ly);
   if (workspace_bytes < p.total) { delete c; return SLAM_EINVAL; }
   for (int k = 0; k < 3; ++k) {
@@ -357,6 +359,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
     const int wpc_s = pick_wpc(window, landmarks, team, cap);
     c->ly_small = make_layout(batch, window, landmarks, cap, wpc_s);
     c->ly_small.team = team;
+    c->ly_small.lock = c->ly.lock;
     c->smem_small = c->ly_small.warp_words * 4 * wpc_s;
     int occ_s = 0;
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_s, kernel_of(team), wpc_s * team, c->smem_small);

@@ -102,7 +102,7 @@ __device__ __forceinline__ float warp_sum(float v) {
 template <int TEAM>
 struct Team {
   int bar;     // named barrier id (1..15)
-  float* scr;  // shared scratch, 128 floats
+  float* scr;  // shared scratch, 384 floats: [0,64) reductions / diagonal tile, [64,384) fp64 covariance tail
   static constexpr int NW = TEAM / 32;
   __device__ __forceinline__ void sync() const {
     if (TEAM == 32) __syncwarp();
@@ -925,95 +925,80 @@ __device__ int apply_update(const Layout& ly, const Ord& od, const WS& w, const 
 // Sigma_t = J Sigma_6 J' with x = a (+) e (A.4).  O(1) per environment, done in fp64 by lane 0.
 template <int TEAM>
 __device__ void covariance(const Layout& ly, const WS& w, const Team<TEAM>& tm, int lane, int env, int c, const StepIO& io) {
-  if (lane != 0) return;
+  if (lane >= 32) return;  // first warp of the team; stages separated by __syncwarp, fp64 scratch in shared memory
   const int n = ly.np, N = ly.N;
-  double S[3][3];
-  if (c == 1) {
-    // only the anchor exists: Sigma = (L_a L_a')^{-1}
-    double Li[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
-    double Lm[3][3];
-    #pragma unroll 1
-    for (int x = 0; x < 3; ++x) {
-      const int i = n - 3 + x;
-      for (int y = 0; y <= x; ++y) Lm[x][y] = (y == x) ? 1.0 / (double)w.H[w.rbase[i] + i] : (double)w.H[w.rbase[i] + n - 3 + y];
+  double* Lm = reinterpret_cast<double*>(tm.scr + 64);  // [6][6] trailing block of L (diagonal = 1/L_jj)
+  double* Li = Lm + 36;                                 // [6][6] its inverse
+  double* S6 = Li + 36;                                 // [6][6] Sigma_6 = Li' Li
+  double* T = S6 + 36;                                  // [6][3] Sigma_6 J'
+  double* S = T + 18;                                   // [3][3] Sigma_t
+  // J = [J_e | J_a], J_e = blockdiag(Rot(a_th), 1), J_a = [[1,0,-dy],[0,1,dx],[0,0,1]], d = Rot(a_th) t_e.
+  // With a single pose (c == 1) the newest-pose block is an identity placeholder: J_e = 0, J_a = I.
+  float saf, caf;
+  sincos_pi(w.st[2], &saf, &caf);
+  const double ca = (double)caf, sa = (double)saf, je = c >= 2 ? 1.0 : 0.0;
+  const float* e = w.st + st_pose(c >= 2 ? c - 1 : 0);
+  const double dx = ca * e[0] - sa * e[1], dy = sa * e[0] + ca * e[1];
+  const double J[3][6] = {{je * ca, -je * sa, 0, 1, 0, -dy}, {je * sa, je * ca, 0, 0, 1, dx}, {0, 0, je, 0, 0, 1}};
+  if (lane < 6) {  // row `lane` of the trailing block
+    const int i = n - 6 + lane, fi = w.first[i];
+    for (int y = 0; y < 6; ++y) {
+      const int j = n - 6 + y;
+      double v = 0.0;
+      if (y == lane) v = (double)w.H[w.rbase[i] + i];
+      else if (y < lane && j >= fi) v = (double)w.H[w.rbase[i] + j];
+      Lm[lane * 6 + y] = v;
+      Li[lane * 6 + y] = 0.0;
     }
-    #pragma unroll 1
-    for (int col = 0; col < 3; ++col)
-      for (int x = col; x < 3; ++x) {
-        double sum = (x == col) ? 1.0 : 0.0;
-        for (int k = col; k < x; ++k) sum -= Lm[x][k] * Li[k][col];
-        Li[x][col] = sum / Lm[x][x];
-      }
-    #pragma unroll 1
-    for (int x = 0; x < 3; ++x)
-      for (int y = 0; y < 3; ++y) {
-        double sum = 0.0;
-        for (int k = 0; k < 3; ++k) sum += Li[k][x] * Li[k][y];
-        S[x][y] = sum;
-      }
-  } else {
-    double Lm[6][6], Li[6][6];
-    #pragma unroll 1
-    for (int x = 0; x < 6; ++x) {
-      const int i = n - 6 + x;
-      const int fi = w.first[i];
-      for (int y = 0; y < 6; ++y) { Lm[x][y] = 0.0; Li[x][y] = 0.0; }
-      for (int y = 0; y <= x; ++y) {
-        const int j = n - 6 + y;
-        if (y == x) Lm[x][y] = 1.0 / (double)w.H[w.rbase[i] + i];
-        else if (j >= fi) Lm[x][y] = (double)w.H[w.rbase[i] + j];
-      }
-    }
-    #pragma unroll 1
-    for (int col = 0; col < 6; ++col)
-      for (int x = col; x < 6; ++x) {
-        double sum = (x == col) ? 1.0 : 0.0;
-        for (int k = col; k < x; ++k) sum -= Lm[x][k] * Li[k][col];
-        Li[x][col] = sum / Lm[x][x];
-      }
-    double S6[6][6];
-    #pragma unroll 1
-    for (int x = 0; x < 6; ++x)
-      for (int y = 0; y < 6; ++y) {
-        double sum = 0.0;
-        for (int k = (x > y ? x : y); k < 6; ++k) sum += Li[k][x] * Li[k][y];
-        S6[x][y] = sum;
-      }
-    // J = [J_e | J_a], J_e = blockdiag(Rot(a_th), 1), J_a = [[1,0,-dy],[0,1,dx],[0,0,1]], d = Rot(a_th) t_e
-    float saf, caf;
-    sincos_pi(w.st[2], &saf, &caf);
-    const double ca = (double)caf, sa = (double)saf;
-    const float* e = w.st + st_pose(c - 1);
-    const double dx = ca * e[0] - sa * e[1], dy = sa * e[0] + ca * e[1];
-    double J[3][6] = {{ca, -sa, 0, 1, 0, -dy}, {sa, ca, 0, 0, 1, dx}, {0, 0, 1, 0, 0, 1}};
-    #pragma unroll 1
-    for (int x = 0; x < 3; ++x)
-      for (int y = 0; y < 3; ++y) {
-        double sum = 0.0;
-        for (int p2 = 0; p2 < 6; ++p2) {
-          double t = 0.0;
-          for (int q = 0; q < 6; ++q) t += S6[p2][q] * J[y][q];
-          sum += J[x][p2] * t;
-        }
-        S[x][y] = sum;
-      }
   }
-  #pragma unroll 1
-    for (int x = 0; x < 3; ++x)  // R20
-    for (int y = x + 1; y < 3; ++y) { const double t = 0.5 * (S[x][y] + S[y][x]); S[x][y] = t; S[y][x] = t; }
-  const double det = S[0][0] * (S[1][1] * S[2][2] - S[1][2] * S[2][1]) - S[0][1] * (S[1][0] * S[2][2] - S[1][2] * S[2][0]) +
-                     S[0][2] * (S[1][0] * S[2][1] - S[1][1] * S[2][0]);
-  const float ld = logf((float)det);
-  #pragma unroll 1
-    for (int x = 0; x < 3; ++x)
-    for (int y = 0; y < 3; ++y) {
-      const float v = (float)S[x][y];
-      io.cov_cache[(size_t)(3 * x + y) * N + env] = v;
-      if (io.cov) io.cov[(size_t)(3 * x + y) * N + env] = v;
+  __syncwarp();
+  if (lane < 6) {  // column `lane` of L^{-1} by forward substitution
+    const int col = lane;
+    for (int x = col; x < 6; ++x) {
+      double sum = (x == col) ? 1.0 : 0.0;
+      for (int k = col; k < x; ++k) sum -= Lm[x * 6 + k] * Li[k * 6 + col];
+      Li[x * 6 + col] = sum * Lm[x * 6 + x];
     }
-  io.cov_cache[(size_t)9 * N + env] = ld;
-  if (io.logdet) io.logdet[env] = ld;
-  if (io.dopt) io.dopt[env] = expf(ld * (1.0f / 3.0f));
+  }
+  __syncwarp();
+  if (lane < 6) {  // row `lane` of Sigma_6 = Li' Li
+    for (int y = 0; y < 6; ++y) {
+      double sum = 0.0;
+      for (int k = (lane > y ? lane : y); k < 6; ++k) sum += Li[k * 6 + lane] * Li[k * 6 + y];
+      S6[lane * 6 + y] = sum;
+    }
+  }
+  __syncwarp();
+  if (lane < 6) {  // row `lane` of T = Sigma_6 J'
+    for (int j = 0; j < 3; ++j) {
+      double sum = 0.0;
+      for (int q = 0; q < 6; ++q) sum += S6[lane * 6 + q] * J[j][q];
+      T[lane * 3 + j] = sum;
+    }
+  }
+  __syncwarp();
+  if (lane < 9) {  // Sigma_t = J T
+    const int x = lane / 3, y = lane - 3 * x;
+    double sum = 0.0;
+    for (int p2 = 0; p2 < 6; ++p2) sum += J[x][p2] * T[p2 * 3 + y];
+    S[lane] = sum;
+  }
+  __syncwarp();
+  if (lane < 9) {  // R20: symmetrise; outputs
+    const int x = lane / 3, y = lane - 3 * x;
+    const float v = (float)(0.5 * (S[x * 3 + y] + S[y * 3 + x]));
+    io.cov_cache[(size_t)lane * N + env] = v;
+    if (io.cov) io.cov[(size_t)lane * N + env] = v;
+  }
+  if (lane == 0) {
+    const double s01 = 0.5 * (S[1] + S[3]), s02 = 0.5 * (S[2] + S[6]), s12 = 0.5 * (S[5] + S[7]);
+    const double det = S[0] * (S[4] * S[8] - s12 * s12) - s01 * (s01 * S[8] - s12 * s02) + s02 * (s01 * s12 - S[4] * s02);
+    const float ld = logf((float)det);
+    io.cov_cache[(size_t)9 * N + env] = ld;
+    if (io.logdet) io.logdet[env] = ld;
+    if (io.dopt) io.dopt[env] = expf(ld * (1.0f / 3.0f));
+  }
+  __syncwarp();
 }
 
 // ------------------------------------------------------------------ S5: marginalise the oldest pose

@@ -26,6 +26,7 @@ struct Layout {
   int warp_words;      // total shared words per warp
   int wpc;             // teams (environments in flight) per CTA
   int team;            // threads per environment: 32, 64 or 128
+  int lock;            // lock-step level: CTA barriers before assemble (1), + before Cholesky (2), + before the solve (3)
 };
 
 struct Params {
@@ -59,7 +60,7 @@ static inline Layout make_layout(int N, int W, int L, int cap, int wpc) {
   y.rec = (o + 31) & ~31;  // 128-byte multiple
 
   int s = 0;
-  y.s_scr = s; s += 128;  // team scratch (reductions, diagonal tile)
+  y.s_scr = s; s += 384;  // team scratch (reductions, diagonal tile, fp64 covariance tail)
   y.s_st = s; s = pad4(s + n + 3);
   y.s_zodo = s; s = pad4(s + 3 * W);
   y.s_zlc = s; s = pad4(s + 3 * W);
@@ -82,6 +83,7 @@ static inline Layout make_layout(int N, int W, int L, int cap, int wpc) {
   y.warp_words = pad4(s);
   y.wpc = wpc;
   y.team = 32;
+  y.lock = 0;
   return y;
 }
 
