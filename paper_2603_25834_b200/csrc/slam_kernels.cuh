@@ -35,14 +35,14 @@ struct StepIO {
 
 struct WS {  // per-warp views into shared memory
   float* st; float* zodo; float* zlc; int* lct; float* cs; uint32_t* rbm;
-  int* first; int* rbase; int* ssup; int* sidx; float* sds; float* H;
+  int* first; int* rbase; uint32_t* amask; int* ssup; int* sidx; float* sds; float* H;
 };
 
 __device__ __forceinline__ WS make_ws(const Layout& ly, float* base) {
   WS w;
   w.st = base + ly.s_st; w.zodo = base + ly.s_zodo; w.zlc = base + ly.s_zlc;
   w.lct = (int*)(base + ly.s_lct); w.cs = base + ly.s_cs; w.rbm = (uint32_t*)(base + ly.s_rbm);
-  w.first = (int*)(base + ly.s_first); w.rbase = (int*)(base + ly.s_rbase);
+  w.first = (int*)(base + ly.s_first); w.rbase = (int*)(base + ly.s_rbase); w.amask = (uint32_t*)(base + ly.s_amask);
   w.ssup = (int*)(base + ly.s_ssup); w.sidx = (int*)(base + ly.s_sidx); w.sds = base + ly.s_sds;
   w.H = base + ly.s_H;
   return w;
@@ -90,6 +90,16 @@ __device__ __forceinline__ int nth_set_bit(uint64_t m, int k) {  // k-th (0-base
 #pragma unroll 1
   for (int i = 0; i < k; ++i) m &= m - 1;
   return __ffsll((long long)m) - 1;
+}
+// index of the k-th (0-based) set bit of a 32-bit word, by bisection on popcounts (k < popc(m))
+__device__ __forceinline__ int nth_bit32(uint32_t m, int k) {
+  int r = 0;
+#pragma unroll
+  for (int h = 16; h > 0; h >>= 1) {
+    const int t = __popc(m & ((1u << h) - 1u));
+    if (k >= t) { k -= t; r += h; m >>= h; }
+  }
+  return r;
 }
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
@@ -419,6 +429,27 @@ __device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, const Team
       run += __shfl_sync(FULLMASK, x, 31);
     }
     if (lane == 0) reinterpret_cast<int*>(tm.scr)[8] = run;
+  }
+  tm.sync();
+  // active row pairs per 4-column block J: pair p (rows 2p, 2p+1; the rhs pair is p = np/2) takes part
+  // in column J iff first <= 4J <= 2p.  Compact lists: aoff[J] (16 bit) offsets into alist (8-bit pair
+  // indices, ascending, so the two diagonal pairs 2J and 2J+1 come first).  Built by the first warp.
+  if (lane < 32) {
+    const int G = np >> 2, NP = (np >> 1) + 1;
+    unsigned short* aoff = reinterpret_cast<unsigned short*>(w.amask);
+    unsigned char* alist = reinterpret_cast<unsigned char*>(aoff + G + 2);
+    int run = 0;
+    for (int J = 0; J < G; ++J) {
+      if (lane == 0) aoff[J] = (unsigned short)run;
+      for (int base = 2 * J; base < NP; base += 32) {
+        const int p = base + lane;
+        const bool on = p < NP && w.first[2 * p] <= 4 * J;
+        const uint32_t bal = __ballot_sync(FULLMASK, on);
+        if (on) alist[run + __popc(bal & ((1u << lane) - 1u))] = (unsigned char)p;
+        run += __popc(bal);
+      }
+    }
+    if (lane == 0) aoff[G] = (unsigned short)run;
   }
   tm.sync();
   return reinterpret_cast<const int*>(tm.scr)[8];
@@ -762,27 +793,36 @@ __device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int
     const float* rJ1 = w.H + w.rbase[c0 + 1];
     const float* rJ2 = w.H + w.rbase[c0 + 2];
     const float* rJ3 = w.H + w.rbase[c0 + 3];
-    // K-split: when fewer row pairs than threads remain, `ch` adjacent lanes share one pair and split
-    // the dot-product range; partial sums are combined by shuffles.
-    const int npairs = (np + 2 - c0) >> 1;
-    int lg = 0;  // ch = 1 << lg
-    while (lg < 3 && (npairs << (lg + 1)) <= TEAM) ++lg;
+    // The ACTIVE row pairs of this column (bit mask from the symbolic phase) are compacted onto the
+    // lowest threads.  K-split: when fewer pairs than threads, `ch` adjacent lanes share one pair and
+    // split the dot-product range; partial sums are combined by shuffles.
+    const unsigned short* aoff = reinterpret_cast<const unsigned short*>(w.amask);
+    const unsigned char* alist = reinterpret_cast<const unsigned char*>(aoff + G + 2) + aoff[J];
+    const int cnt = aoff[J + 1] - aoff[J];
+    int lg = 0;  // ch = 1 << lg; only worth it when the dot products are long
+    if (c0 - fJ >= 32) while (lg < 3 && (cnt << (lg + 1)) <= TEAM) ++lg;
     const int ch = 1 << lg;
     const int per_pass = TEAM >> lg;
     const int t = lane & (ch - 1);
     float d0 = 1.f, d1 = 1.f, d2 = 1.f, d3 = 1.f, l10 = 0.f, l20 = 0.f, l21 = 0.f, l30 = 0.f, l31 = 0.f, l32 = 0.f;
-    for (int q0 = 0; q0 < npairs; q0 += per_pass) {
+    for (int q0 = 0; q0 < cnt; q0 += per_pass) {
       const bool first_pass = q0 == 0;
       const int q = q0 + (lane >> lg);
-      const int i0 = c0 + 2 * q;
-      const bool act = q < npairs && w.first[i0] <= c0;
+      const bool act = q < cnt;
+      // a warp without any pair in this pass only takes part in the barriers
+      const bool warp_idle = TEAM > 32 && q0 + ((lane & ~31) >> lg) >= cnt;
+      if (warp_idle) {
+        if (first_pass) tm.sync();
+        continue;
+      }
+      const int i0 = act ? 2 * (int)alist[q] : c0;
       float4 a0 = make_float4(0.f, 0.f, 0.f, 0.f), a1 = a0;
       float* p0 = nullptr;
       float* p1 = nullptr;
       if (act) {
         p0 = w.H + w.rbase[i0];
         p1 = w.H + w.rbase[i0 + 1];
-        if (t == 0) { a0 = ld4(p0 + c0); a1 = ld4(p1 + c0); }
+        if (t == 0) { a0 = ld4(p0 + c0); a1 = ld4(p1 + c0); }  // (rows np, np+1 are the rhs pair)
         const int ks = max(w.first[i0], fJ);
         const int nblk = (c0 - ks) >> 2;
         const int kb = ks + 4 * ((t * nblk) >> lg), ke = ks + 4 * (((t + 1) * nblk) >> lg);

@@ -21,7 +21,8 @@ struct Layout {
   int rec;             // record stride
   int o_status, o_pm, o_lm, o_act, o_a, o_e, o_m, o_zodo, o_lct, o_zlc, o_rbm, o_zrb, o_vbar, o_g, o_lam;
   // shared memory per warp (32-bit words)
-  int s_scr, s_st, s_zodo, s_zlc, s_lct, s_cs, s_rbm, s_first, s_rbase, s_ssup, s_sidx, s_sds, s_H;
+  int s_scr, s_st, s_zodo, s_zlc, s_lct, s_cs, s_rbm, s_first, s_rbase, s_amask, s_ssup, s_sidx, s_sds, s_H;
+  int mw;              // 32-bit words of an active-row-pair mask (np/2 + 1 bits)
   int cap;             // words available for H (envelope + rhs row) / marginalisation scratch
   int warp_words;      // total shared words per warp
   int wpc;             // teams (environments in flight) per CTA
@@ -69,6 +70,12 @@ static inline Layout make_layout(int N, int W, int L, int cap, int wpc) {
   y.s_rbm = s; s = pad4(s + W * y.nw);
   y.s_first = s; s = pad4(s + y.np + 2);
   y.s_rbase = s; s = pad4(s + y.np + 2);
+  y.mw = (y.np / 2 + 1 + 31) / 32;
+  {  // active-pair lists: G+1 offsets (16 bit) then at most sum_J (NP - 2J) pair indices (8 bit)
+    const int G4 = y.np / 4, NPp = y.np / 2 + 1;
+    const int bytes = 2 * (G4 + 2) + G4 * NPp - G4 * (G4 - 1);
+    y.s_amask = s; s = pad4(s + (bytes + 3) / 4);
+  }
   y.s_ssup = s; s = pad4(s + n);
   y.s_sidx = s; s = pad4(s + n);
   y.s_sds = s; s = pad4(s + n + 2 * L);  // prior displacement (<= n) + anchor-frame landmarks (2L)

@@ -234,3 +234,28 @@ def test_step_host_matches_device_step():
                        pin(data["rb_mask"][t].view(np.int32)), pin(data["rb_meas"][t]), iters=cfg.iters, cov=cov, logdet=ld)
         torch.cuda.synchronize()
         assert np.array_equal(ld.numpy().astype(np.float64), a["logdet"][t - 1])
+
+
+def test_results_do_not_depend_on_capacity_or_team(monkeypatch):
+    """The shared-memory capacity only decides WHICH launch solves an environment (first launch or the
+    dense-capacity launch over the overflow list); the arithmetic is the same, so outputs are bit-equal.
+    Different team sizes change summation order in a few reductions: equal within the tolerances."""
+    cfg = synth.Config("cap", N=200, W=40, L=0, iters=3, T=70, p_lc=0.3, seed=11)
+    data = synth.generate(cfg)
+    monkeypatch.setenv("SLAM_CAP_FRAC", "1.0")
+    slam = _slam(cfg.N, cfg.W, cfg.L)
+    a = run_gpu(slam, data, cfg.iters, fused=True, want_poses=False)
+    assert slam.get_stats()["fallback"] == 0
+    monkeypatch.setenv("SLAM_CAP_FRAC", "0.3")
+    slam = _slam(cfg.N, cfg.W, cfg.L)
+    b = run_gpu(slam, data, cfg.iters, fused=True, want_poses=False)
+    st = slam.get_stats()
+    assert st["fallback"] > 0, st                       # the overflow path really ran
+    assert np.array_equal(a["cov"], b["cov"]) and np.array_equal(a["logdet"], b["logdet"])
+    assert (b["status"] == 0).all()
+    monkeypatch.delenv("SLAM_CAP_FRAC")
+    ref = oracle.run_batch(data, cfg.iters, envs=np.arange(0, cfg.N, 25, dtype=np.int32))
+    for team in ("32", "128"):
+        monkeypatch.setenv("SLAM_TEAM", team)
+        c = run_gpu(_slam(cfg.N, cfg.W, cfg.L), data, cfg.iters, fused=True, want_poses=False)
+        _check(_sub(c, np.arange(0, cfg.N, 25)), ref, what=("cov", "logdet"))
