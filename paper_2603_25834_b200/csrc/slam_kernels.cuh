@@ -101,6 +101,13 @@ __device__ __forceinline__ int nth_bit32(uint32_t m, int k) {
   }
   return r;
 }
+// (p, q) of the packed lower-triangular index t = p(p+1)/2 + q, q <= p
+__device__ __forceinline__ int tri_row(int t) {
+  int p = (int)((sqrtf(8.0f * (float)t + 1.0f) - 1.0f) * 0.5f);
+  if ((p + 1) * (p + 2) / 2 <= t) ++p;
+  if (p * (p + 1) / 2 > t) --p;
+  return p;
+}
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULLMASK, v, o);
@@ -569,15 +576,16 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
   // prior: H += Lambda (row by row, coalesced over the packed lower triangle)
   {
     const float* lam = rec + ly.o_lam;
-    for (int p = lane >> 5; p < s; p += TEAM / 32) {  // one packed row per warp at a time
-      const int ip = w.ssup[p];
-      const float* lrow = lam + (p * (p + 1) >> 1);
-      for (int q = lane & 31; q <= p; q += 32) {
-        const int iq = w.ssup[q];
-        const float v = lrow[q];
-        const int hi = max(ip, iq), lo = min(ip, iq);
-        w.H[w.rbase[hi] + lo] += v;
-      }
+    // flat over the packed triangle: coalesced, and every iteration is independent (memory-level
+    // parallelism: the loads of Lambda come from L2)
+    const int ntri = s * (s + 1) >> 1;
+#pragma unroll 4
+    for (int t = lane; t < ntri; t += TEAM) {
+      const int p = tri_row(t), q = t - (p * (p + 1) >> 1);
+      const float v = lam[t];
+      const int ip = w.ssup[p], iq = w.ssup[q];
+      const int hi = max(ip, iq), lo = min(ip, iq);
+      w.H[w.rbase[hi] + lo] += v;
     }
     // b -= Lambda d + g
     float* rhs = w.H + w.rbase[n];
@@ -667,10 +675,16 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
       float R[18];
 #pragma unroll
       for (int t = 0; t < 18; ++t) R[t] = 0.f;
+      int lnext = __ffsll((long long)m) - 1;  // measurements are prefetched one landmark ahead (they come from L2)
+      float zr_n = rec[ly.o_zrb + (r * 2 + 0) * L + lnext], zb_n = rec[ly.o_zrb + (r * 2 + 1) * L + lnext];
       while (m) {
-        const int l = __ffsll((long long)m) - 1;
+        const int l = lnext;
+        const float zr = zr_n, zb = zb_n;
         m &= m - 1;
-        const float zr = rec[ly.o_zrb + (r * 2 + 0) * L + l], zb = rec[ly.o_zrb + (r * 2 + 1) * L + l];
+        if (m) {
+          lnext = __ffsll((long long)m) - 1;
+          zr_n = rec[ly.o_zrb + (r * 2 + 0) * L + lnext]; zb_n = rec[ly.o_zrb + (r * 2 + 1) * L + lnext];
+        }
         const float mx = mloc[2 * l], my = mloc[2 * l + 1];
         const float dx = mx - px, dy = my - py;
         const float q = dx * dx + dy * dy, irho = rsqrtf(q), rho = q * irho, iq = irho * irho;
@@ -721,11 +735,21 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
       const bool inl = (od.obs >> l) & 1ull;
       const float mx = inl ? mloc[2 * l] : 0.f, my = inl ? mloc[2 * l + 1] : 0.f;
       float Lxx = 0.f, Lxy = 0.f, Lyy = 0.f, bgx = 0.f, bgy = 0.f, ag0 = 0.f, ag1 = 0.f, a22 = 0.f, a2r = 0.f;
-      for (int k = 0; k < c; ++k) {
-        const uint32_t word = w.rbm[k * ly.nw + (l >> 5)];
-        if (!((word >> (l & 31)) & 1u) || !inl) continue;
-        const int r = ring_of(k, head, W);
-        const float zr = rec[ly.o_zrb + (r * 2 + 0) * L + l], zb = rec[ly.o_zrb + (r * 2 + 1) * L + l];
+      uint64_t km = 0ull;  // slots that observe this landmark
+      if (inl)
+        for (int k = 0; k < c; ++k) km |= (uint64_t)((w.rbm[k * ly.nw + (l >> 5)] >> (l & 31)) & 1u) << k;
+      int knext = km ? __ffsll((long long)km) - 1 : 0;  // measurements prefetched one slot ahead (L2)
+      int rn = ring_of(knext, head, W);
+      float zr_n = km ? rec[ly.o_zrb + (rn * 2 + 0) * L + l] : 0.f, zb_n = km ? rec[ly.o_zrb + (rn * 2 + 1) * L + l] : 0.f;
+      while (km) {
+        const int k = knext;
+        const float zr = zr_n, zb = zb_n;
+        km &= km - 1;
+        if (km) {
+          knext = __ffsll((long long)km) - 1;
+          rn = ring_of(knext, head, W);
+          zr_n = rec[ly.o_zrb + (rn * 2 + 0) * L + l]; zb_n = rec[ly.o_zrb + (rn * 2 + 1) * L + l];
+        }
         const float* p = w.st + st_pose(k);
         const float dx = mx - p[0], dy = my - p[1];
         const float q = dx * dx + dy * dy, irho = rsqrtf(q), rho = q * irho, iq = irho * irho;
@@ -1148,10 +1172,11 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
   // --- C. scatter the old prior
   {
     const float* lam = rec + ly.o_lam;
-    for (int p = lane >> 5; p < s_old; p += TEAM / 32) {
-      const int P = omap[p];
-      const float* lrow = lam + (p * (p + 1) >> 1);
-      for (int q = lane & 31; q <= p; q += 32) Hs[tri(P, omap[q])] = lrow[q];
+    const int ntri = s_old * (s_old + 1) >> 1;
+#pragma unroll 4
+    for (int t = lane; t < ntri; t += TEAM) {
+      const int p = tri_row(t), q = t - (p * (p + 1) >> 1);
+      Hs[tri(omap[p], omap[q])] = lam[t];
     }
     for (int p = lane; p < s_old; p += TEAM) {
       float acc = rec[ly.o_g + p];
