@@ -80,6 +80,17 @@ int slam_reset(slam_ctx* ctx, const float* init_pose);
 int slam_push_step(slam_ctx* ctx, const float* odom, const int32_t* lc_back, const float* lc_meas,
                    const uint32_t* rb_mask, const float* rb_meas);
 
+/* NEXT-1: unary absolute-pose factor -- the paper's scan-match measurement, whose
+ * information matrix it scales by match score and ambiguity (formula not given, so the information
+ * is an input).  Registers a factor for the pose that the NEXT slam_push_step / slam_step appends:
+ *   pose  [3][N]  measured GLOBAL pose (x, y, theta) of that pose
+ *   info  [6][N]  symmetric 3x3 information in global coordinates, packed (xx, xy, yy, xt, yt, tt)
+ *   valid [N]     non-zero where the environment has a measurement; NULL = all
+ * Residual r = [x - z_x; y - z_y; wrap(theta - z_theta)].  The pointers are read by that next push
+ * (stream order) and must stay valid until then; pose = info = NULL cancels.  The factor leaves the
+ * window with its pose and is folded into the prior by marginalisation. */
+int slam_set_unary(slam_ctx* ctx, const float* pose, const float* info, const int32_t* valid);
+
 /* Landmark observations from pose 0; only valid right after reset (count == 1). */
 int slam_observe_first(slam_ctx* ctx, const uint32_t* rb_mask, const float* rb_meas);
 

@@ -58,6 +58,10 @@ def lib():
         L.orc_rb_factor.argtypes = [_dp, _dp, _dp, _dp, C.c_int, _dp, _dp, _dp, _dp]
         L.orc_reanchor_map.argtypes = [C.c_void_p, _dp, _dp]
         L.orc_reanchor_jac.argtypes = [C.c_void_p, _dp]
+        L.orc_add_unary.argtypes = [C.c_void_p, _dp, _dp]
+        L.orc_unary_factor.argtypes = [_dp, _dp, _dp, C.c_int, _dp, _dp, _dp]
+        L.orc_batch_set_unary.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_batch_set_unary.restype = None
         L.orc_run_batch.restype = C.c_int
         L.orc_run_batch.argtypes = [C.c_int] * 5 + [_dp, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                                     C.c_void_p, _ip, C.c_int, C.c_int, _dp, _dp, _dp, _dp]
@@ -116,6 +120,11 @@ class Oracle:
         v, z, vp, zp = self._rb(rb_valid, rb_meas)
         if lib().orc_observe_first(self._h, vp, zp) != 0:
             raise RuntimeError("observe_first after a push")
+
+    def add_unary(self, pose, info):
+        """Unary absolute-pose factor on the newest pose: measured global pose (3), 3x3 information."""
+        z, om = _d(pose), _d(np.asarray(info, float).reshape(3, 3))
+        lib().orc_add_unary(self._h, _p(z), _p(om))
 
     def solve(self, iters: int) -> float:
         s = C.c_double(0.0)
@@ -193,6 +202,12 @@ def rb_factor(a, ek, gl, z, k_is_frame=False):
     return r, Ja.reshape(2, 3), Jp.reshape(2, 3), Jg.reshape(2, 2)
 
 
+def unary_factor(a, ek, z, k_is_frame=False):
+    r, Ja, Je = np.zeros(3), np.zeros(9), np.zeros(9)
+    lib().orc_unary_factor(_p(_d(a)), _p(_d(ek)), _p(_d(z)), int(k_is_frame), _p(r), _p(Ja), _p(Je))
+    return r, Ja.reshape(3, 3), Je.reshape(3, 3)
+
+
 def max_threads() -> int:
     return lib().orc_max_threads()
 
@@ -219,10 +234,15 @@ def run_batch(data: dict, iters: int, envs=None, sigmas=DEFAULT_SIGMAS, threads:
     sig = _d(sigmas)
     ptr = lambda a: None if a is None else _p(a)
     vp = lambda a: a.ctypes.data_as(C.c_void_p)
+    keep = None
+    if data.get("un_valid") is not None:
+        keep = (np.ascontiguousarray(data["un_valid"], dtype=np.int32), f32(data["un_pose"]), f32(data["un_info"]))
+        lib().orc_batch_set_unary(vp(keep[0]), vp(keep[1]), vp(keep[2]))
     lib().orc_batch_set_f32_storage(int(f32_storage))
     bad = lib().orc_run_batch(N, W, L, T, iters, _p(sig), vp(odom), vp(lc_back), vp(lc_meas), vp(rb_mask),
                               vp(rb_meas), envs.ctypes.data_as(_ip), ne, int(threads),
                               ptr(out["poses"]), ptr(out["cov"]), ptr(out["logdet"]), ptr(out["step"]))
     lib().orc_batch_set_f32_storage(0)
+    lib().orc_batch_set_unary(None, None, None)
     out["bad"] = bad
     return out

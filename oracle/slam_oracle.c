@@ -30,6 +30,9 @@ struct orc {
   double* z_lc;     /* [W][3] */
   int* rb_valid;    /* [W][L] */
   double* z_rb;     /* [W][L][2] range, bearing */
+  int* un_valid;    /* [W]    unary absolute-pose factor on slot k (scan-match measurement) */
+  double* z_un;     /* [W][3] measured global pose */
+  double* om_un;    /* [W][9] its 3x3 information matrix (caller supplied, symmetric) */
 };
 
 /* ------------------------------------------------------------------ small helpers */
@@ -230,6 +233,9 @@ orc* orc_create(int W, int L, const double* sig11, int linear) {
   o->z_lc = (double*)calloc(3 * W, sizeof(double));
   o->rb_valid = (int*)calloc((size_t)W * (L + 1), sizeof(int));
   o->z_rb = (double*)calloc((size_t)W * (L + 1) * 2, sizeof(double));
+  o->un_valid = (int*)calloc(W, sizeof(int));
+  o->z_un = (double*)calloc(3 * W, sizeof(double));
+  o->om_un = (double*)calloc(9 * W, sizeof(double));
   orc_reset(o, NULL);
   return o;
 }
@@ -238,6 +244,7 @@ void orc_destroy(orc* o) {
   if (!o) return;
   free(o->e); free(o->m); free(o->active); free(o->Lam); free(o->g); free(o->vbar);
   free(o->z_odo); free(o->lc_tgt); free(o->z_lc); free(o->rb_valid); free(o->z_rb);
+  free(o->un_valid); free(o->z_un); free(o->om_un);
   free(o);
 }
 
@@ -273,6 +280,7 @@ void orc_reset(orc* o, const double* init_pose3) {
   for (int k = 0; k < 3; ++k) o->Lam[k * n + k] = 1.0 / (o->sig[k] * o->sig[k]);
   for (int k = 0; k < o->W; ++k) o->lc_tgt[k] = -1;
   memset(o->rb_valid, 0, sizeof(int) * o->W * (o->L + 1));
+  memset(o->un_valid, 0, sizeof(int) * o->W);
   orc_get_state(o, o->vbar);
 }
 
@@ -302,6 +310,42 @@ int orc_observe_first(orc* o, const int* rb_valid, const double* rb_meas) {
   return 0;
 }
 
+/* Unary absolute-pose factor on the NEWEST pose (NEXT-1; the paper's scan-match measurement with a
+ * caller-supplied information matrix).  x = a (+) e_k is the global pose of the slot:
+ *   r = [ x - z_x ; y - z_y ; wrap(th - z_th) ],  J_a = dx/da,  J_e = dx/de_k  (as for range-bearing). */
+int orc_add_unary(orc* o, const double* pose3, const double* info9) {
+  int k = o->c - 1;
+  o->un_valid[k] = 1;
+  for (int i = 0; i < 3; ++i) o->z_un[3 * k + i] = pose3[i];
+  for (int i = 0; i < 9; ++i) o->om_un[9 * k + i] = info9[i];
+  return 0;
+}
+
+static void unary_factor(int linear, const double* a, const double* ek, const double* z, int k_is_frame,
+                         double* r, double* Ja, double* Je) {
+  double zero[3] = {0, 0, 0};
+  const double* e = k_is_frame ? zero : ek;
+  double x[3];
+  compose(linear, a, e, x);
+  r[0] = x[0] - z[0];
+  r[1] = x[1] - z[1];
+  r[2] = linear ? x[2] - z[2] : wrap_pi(x[2] - z[2]);
+  memset(Ja, 0, 9 * sizeof(double));
+  memset(Je, 0, 9 * sizeof(double));
+  if (linear) {
+    for (int i = 0; i < 3; ++i) { Ja[i * 3 + i] = 1.0; if (!k_is_frame) Je[i * 3 + i] = 1.0; }
+    return;
+  }
+  double ca = cos(a[2]), sa = sin(a[2]);
+  double ddx = ca * e[0] - sa * e[1], ddy = sa * e[0] + ca * e[1];
+  Ja[0] = 1; Ja[2] = -ddy; Ja[4] = 1; Ja[5] = ddx; Ja[8] = 1;
+  if (!k_is_frame) { Je[0] = ca; Je[1] = -sa; Je[3] = sa; Je[4] = ca; Je[8] = 1; }
+}
+void orc_unary_factor(const double* a3, const double* ek3, const double* z3, int k_is_frame,
+                      double* r3, double* Ja9, double* Je9) {
+  unary_factor(0, a3, ek3, z3, k_is_frame, r3, Ja9, Je9);
+}
+
 /* push: e_c = e_{c-1} (+) z_odo (dead-reckoned initial guess, BASELINE.json cfg 0) */
 int orc_push(orc* o, const double* odom3, int lc_back, const double* lc_meas3,
              const int* rb_valid, const double* rb_meas) {
@@ -315,6 +359,7 @@ int orc_push(orc* o, const double* odom3, int lc_back, const double* lc_meas3,
     for (int k = 0; k < 3; ++k) o->z_lc[3 * c + k] = lc_meas3[k];
   }
   record_rb(o, c, rb_valid, rb_meas);
+  o->un_valid[c] = 0;
   o->c = c + 1;
   return 0;
 }
@@ -375,6 +420,35 @@ static void build_system(const orc* o, int only_slot0, double* H, double* grad, 
     if (only_slot0 && i != 0) continue;
     between_factor(o->linear, o->e + 3 * i, o->e + 3 * k, o->z_lc + 3 * k, i == 0, r, Ji, Jj);
     add_factor(H, grad, cost, n, 3, r, om_lc, i == 0 ? -1 : idx_e(i), 3, Ji, idx_e(k), 3, Jj);
+  }
+  for (int k = 0; k < c; ++k) { /* unary absolute-pose factors: full 3x3 information */
+    if (!o->un_valid[k]) continue;
+    if (only_slot0 && k != 0) continue;
+    double ru[3], Jua[9], Jue[9];
+    unary_factor(o->linear, o->a, o->e + 3 * k, o->z_un + 3 * k, k == 0, ru, Jua, Jue);
+    const double* Om = o->om_un + 9 * k;
+    const int idx[2] = {0, k == 0 ? -1 : idx_e(k)};
+    const double* J[2] = {Jua, Jue};
+    double Or[3];
+    for (int i = 0; i < 3; ++i) Or[i] = Om[i * 3] * ru[0] + Om[i * 3 + 1] * ru[1] + Om[i * 3 + 2] * ru[2];
+    for (int p = 0; p < 2; ++p) {
+      if (idx[p] < 0) continue;
+      for (int x = 0; x < 3; ++x) {
+        double sgrad = 0.0;
+        for (int i = 0; i < 3; ++i) sgrad += J[p][i * 3 + x] * Or[i];
+        if (grad) grad[idx[p] + x] += sgrad;
+        for (int q = 0; q < 2; ++q) {
+          if (idx[q] < 0) continue;
+          for (int y = 0; y < 3; ++y) {
+            double h = 0.0;
+            for (int i = 0; i < 3; ++i)
+              for (int j = 0; j < 3; ++j) h += J[p][i * 3 + x] * Om[i * 3 + j] * J[q][j * 3 + y];
+            if (H) H[(idx[p] + x) * n + idx[q] + y] += h;
+          }
+        }
+      }
+    }
+    if (cost) *cost += 0.5 * (ru[0] * Or[0] + ru[1] * Or[1] + ru[2] * Or[2]);
   }
   for (int k = 0; k < c; ++k) { /* range-bearing from slot k */
     if (only_slot0 && k != 0) continue;
@@ -654,6 +728,12 @@ int orc_marginalize(orc* o) {
     memcpy(o->rb_valid + (k - 1) * L, o->rb_valid + k * L, sizeof(int) * L);
     memcpy(o->z_rb + (size_t)(k - 1) * L * 2, o->z_rb + (size_t)k * L * 2, sizeof(double) * 2 * L);
   }
+  for (int k = 1; k < c; ++k) {
+    o->un_valid[k - 1] = o->un_valid[k];
+    memcpy(o->z_un + 3 * (k - 1), o->z_un + 3 * k, 3 * sizeof(double));
+    memcpy(o->om_un + 9 * (k - 1), o->om_un + 9 * k, 9 * sizeof(double));
+  }
+  o->un_valid[c - 1] = 0;
   o->lc_tgt[c - 1] = -1;
   memset(o->rb_valid + (c - 1) * L, 0, sizeof(int) * L);
   o->c = c - 1;
@@ -683,6 +763,11 @@ int orc_max_threads(void) {
 }
 
 static int g_batch_f32_storage = 0;
+/* optional unary factors of the batch run: un_valid[T][N] (int), un_pose[T][3][N], un_info[T][6][N] (xx,xy,yy,xt,yt,tt), float32 */
+static const int* g_un_valid = 0;
+static const float* g_un_pose = 0;
+static const float* g_un_info = 0;
+void orc_batch_set_unary(const int* valid, const float* pose, const float* info) { g_un_valid = valid; g_un_pose = pose; g_un_info = info; }
 void orc_batch_set_f32_storage(int on) { g_batch_f32_storage = on; }
 
 int orc_run_batch(int N, int W, int L, int T, int iters, const double* sig11,
@@ -719,6 +804,14 @@ int orc_run_batch(int N, int W, int L, int T, int iters, const double* sig11,
       }
       int back = lc_back ? lc_back[(size_t)(t - 1) * N + env] : 0;
       orc_push(o, od, back, zl, valid, zrb);
+      if (g_un_valid && g_un_valid[(size_t)(t - 1) * N + env]) {
+        double zp[3], I6[6], I9[9];
+        for (int k = 0; k < 3; ++k) zp[k] = g_un_pose[((size_t)(t - 1) * 3 + k) * N + env];
+        for (int k = 0; k < 6; ++k) I6[k] = g_un_info[((size_t)(t - 1) * 6 + k) * N + env];
+        I9[0] = I6[0]; I9[1] = I6[1]; I9[3] = I6[1]; I9[4] = I6[2];
+        I9[2] = I6[3]; I9[6] = I6[3]; I9[5] = I6[4]; I9[7] = I6[4]; I9[8] = I6[5];
+        orc_add_unary(o, zp, I9);
+      }
       double sn = 0.0, S[9], ld = 0.0;
       if (orc_solve(o, iters, &sn) != 0) failed = 1;
       if (orc_cov(o, S, &ld) != 0) failed = 1;

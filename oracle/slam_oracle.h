@@ -50,6 +50,13 @@ int  orc_dim(const orc*);
 int  orc_push(orc*, const double* odom3, int lc_back, const double* lc_meas3,
               const int* rb_valid, const double* rb_meas);
 int  orc_observe_first(orc*, const int* rb_valid, const double* rb_meas);
+/* NEXT-1: unary absolute-pose factor on the newest pose (the paper's scan-match measurement with its
+ * score-scaled information matrix; the scaling itself is not given, so the 3x3
+ * information is an input).  pose3 = measured GLOBAL pose, info9 = symmetric 3x3, row-major. */
+int  orc_add_unary(orc*, const double* pose3, const double* info9);
+void orc_unary_factor(const double* a3, const double* ek3, const double* z3, int k_is_frame,
+                      double* r3, double* Ja9, double* Je9);
+void orc_batch_set_unary(const int* valid, const float* pose, const float* info);
 /* returns 0, or -1 if H was singular.  last_step_norm (may be NULL) = max |delta| of the last iteration */
 int  orc_solve(orc*, int iters, double* last_step_norm);
 int  orc_cov(orc*, double* cov9, double* logdet);

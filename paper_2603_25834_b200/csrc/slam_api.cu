@@ -196,6 +196,8 @@ struct slam_ctx {
   uint32_t* st_rb_mask;
   int head, count;
   bool cov_valid;
+  const float *un_pose, *un_info;   // pending unary factor for the next pushed pose (NEXT-1)
+  const int32_t* un_valid;
   long long launches;
   int grid, smem_bytes, ctas_per_sm;      // dense-capacity launch (the only one if !two_pass)
   Layout ly_small;                        // first launch with a smaller shared-memory capacity
@@ -338,6 +340,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   c->st_pose = (float*)(base + p.pose);
   c->launches = 0;
   c->err[0] = 0;
+  c->un_pose = nullptr; c->un_info = nullptr; c->un_valid = nullptr;
   c->smem_bytes = c->ly.warp_words * 4 * wpc;
   if (cudaFuncSetAttribute(kernel_of(team), cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) {
     cudaGetLastError();
@@ -419,10 +422,19 @@ int slam_push_step(slam_ctx* c, const float* odom, const int32_t* lc_back, const
   if (!c) return SLAM_EINVAL;
   int rc = check_push_args(c, odom, lc_back, lc_meas, rb_mask, rb_meas);
   if (rc) return rc;
-  StepIO io = {odom, lc_back, lc_meas, rb_mask, rb_meas, nullptr, nullptr, nullptr, nullptr, c->cov_cache};
+  StepIO io = {odom, lc_back, lc_meas, rb_mask, rb_meas, nullptr, nullptr, nullptr, nullptr, c->cov_cache,
+               c->un_pose, c->un_info, c->un_valid};
+  c->un_pose = nullptr; c->un_info = nullptr; c->un_valid = nullptr;
   rc = launch_step(c, F_PUSH, 0, io);
   if (rc) return rc;
   c->count++; c->cov_valid = false;
+  return SLAM_OK;
+}
+
+int slam_set_unary(slam_ctx* c, const float* pose, const float* info, const int32_t* valid) {
+  if (!c) return SLAM_EINVAL;
+  if ((pose == nullptr) != (info == nullptr)) return fail(c, SLAM_EINVAL, "pose and info must both be given (or both NULL to cancel)");
+  c->un_pose = pose; c->un_info = info; c->un_valid = pose ? valid : nullptr;
   return SLAM_OK;
 }
 
@@ -489,7 +501,9 @@ int slam_step(slam_ctx* c, const float* odom, const int32_t* lc_back, const floa
   int rc = check_push_args(c, odom, lc_back, lc_meas, rb_mask, rb_meas);
   if (rc) return rc;
   const bool marg = (c->count + 1 == c->ly.W);
-  StepIO io = {odom, lc_back, lc_meas, rb_mask, rb_meas, cov, logdet, nullptr, last_pose, c->cov_cache};
+  StepIO io = {odom, lc_back, lc_meas, rb_mask, rb_meas, cov, logdet, nullptr, last_pose, c->cov_cache,
+               c->un_pose, c->un_info, c->un_valid};
+  c->un_pose = nullptr; c->un_info = nullptr; c->un_valid = nullptr;
   rc = launch_step(c, F_PUSH | F_COV | (marg ? F_MARG : 0), iters, io);
   if (rc) return rc;
   c->count++;

@@ -31,11 +31,13 @@ struct StepIO {
   const float* odom; const int32_t* lc_back; const float* lc_meas; const uint32_t* rb_mask; const float* rb_meas;
   float* cov; float* logdet; float* dopt; float* last_pose;
   float* cov_cache;  // [10][N]: 9 covariance entries + logdet
+  // NEXT-1: unary absolute-pose factor for the pose this push appends (NULL: none)
+  const float* un_pose; const float* un_info; const int32_t* un_valid;
 };
 
 struct WS {  // per-warp views into shared memory
   float* st; float* zodo; float* zlc; int* lct; float* cs; uint32_t* rbm;
-  int* first; int* rbase; uint32_t* amask; int* ssup; int* sidx; float* sds; float* H;
+  int* first; int* rbase; uint32_t* amask;  /* amask: active-pair lists per column block */ int* ssup; int* sidx; float* sds; float* H;
 };
 
 __device__ __forceinline__ WS make_ws(const Layout& ly, float* base) {
@@ -208,6 +210,7 @@ struct Masks {  // warp-uniform
   uint64_t ps;   // prior support, pose SLOTS (bit k = slot k)
   uint64_t ls;   // prior support, landmarks
   uint64_t act;  // active landmarks
+  uint64_t um;   // pose SLOTS with a unary absolute-pose factor
 };
 
 // ------------------------------------------------------------------ load / store of the record
@@ -237,6 +240,7 @@ __device__ void load_env(const Layout& ly, const float* rec, const WS& w, const 
   mk.ps = ring_to_slot(pm, head, W);
   mk.ls = (uint64_t)recu[ly.o_lm] | ((uint64_t)recu[ly.o_lm + 1] << 32);
   mk.act = (uint64_t)recu[ly.o_act] | ((uint64_t)recu[ly.o_act + 1] << 32);
+  mk.um = ring_to_slot((uint64_t)recu[ly.o_um] | ((uint64_t)recu[ly.o_um + 1] << 32), head, W) & lowmask(c);
   tm.sync();
 }
 
@@ -251,7 +255,11 @@ __device__ void store_state(const Layout& ly, float* rec, const WS& w, const Tea
     rec[ly.o_e + 3 * r + j] = w.st[3 + i];
   }
   for (int i = lane; i < 2 * L; i += TEAM) rec[ly.o_m + i] = w.st[3 + 3 * W + i];
-  if (lane == 0) { recu[ly.o_act] = (uint32_t)mk.act; recu[ly.o_act + 1] = (uint32_t)(mk.act >> 32); }
+  if (lane == 0) {
+    recu[ly.o_act] = (uint32_t)mk.act; recu[ly.o_act + 1] = (uint32_t)(mk.act >> 32);
+    const uint64_t um = slot_to_ring(mk.um, head, W);
+    recu[ly.o_um] = (uint32_t)um; recu[ly.o_um + 1] = (uint32_t)(um >> 32);
+  }
 }
 
 // ------------------------------------------------------------------ S0 push / observe
@@ -316,6 +324,12 @@ __device__ int push_env(const Layout& ly, float* rec, const WS& w, const Team<TE
     const float zl = io.lc_meas ? io.lc_meas[(size_t)lane * N + env] : 0.0f;
     w.zlc[3 * c + lane] = zl;
     rec[ly.o_zlc + 3 * r + lane] = zl;
+  }
+  mk.um &= ~(1ull << c);
+  if (io.un_pose && (io.un_valid == nullptr || io.un_valid[env] != 0)) {
+    if (lane < 3) rec[ly.o_zun + 3 * r + lane] = io.un_pose[(size_t)lane * N + env];
+    if (lane < 6) rec[ly.o_omun + 6 * r + lane] = io.un_info[(size_t)lane * N + env];
+    mk.um |= 1ull << c;
   }
   tm.sync();
   if (ly.L > 0) record_rb<TEAM>(ly, rec, w, tm, lane, env, head, c, nx, ny, nt, io, mk);
@@ -414,6 +428,11 @@ __device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, const Team
     if (lane < 3) w.first[oA + lane] = min(w.first[oA + lane], fa);
   }
   tm.sync();
+  if (mk.um >> 1) {  // unary factors couple the anchor to their pose (x_k = a (+) e_k)
+    const int kmin = __ffsll((long long)(mk.um >> 1));  // lowest slot >= 1
+    if (lane < 3) w.first[oA + lane] = min(w.first[oA + lane], off_slot(ly, od, kmin, c));
+    tm.sync();
+  }
   // group rows in fours (shared first, aligned down to 4); prefix sum of the row lengths -> rbase
   // (done by the first warp of the team)
   if (lane < 32) {
@@ -640,6 +659,68 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
     if (any) add_i_side(w, n, off_slot(ly, od, t, c), Hii, gi);
   }
   tm.sync();
+  // unary absolute-pose factors (NEXT-1): r = (a (+) e_k) - z, full 3x3 information,
+  // J_a = [[1,0,-dy],[0,1,dx],[0,0,1]] (d = Rot(a_th) t_k), J_e = blockdiag(Rot(a_th), 1); slot 0: x = a.
+  if (mk.um) {
+    float* rhs = w.H + w.rbase[n];
+    const int oA = off_a(ly);
+    float sa, ca;
+    sincos_pi(w.st[2], &sa, &ca);
+    float A[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};  // anchor block (lower 6) and gradient (3)
+    for (int k = lane; k < c; k += TEAM) {
+      if (!((mk.um >> k) & 1ull)) continue;
+      const int r = ring_of(k, head, W);
+      const float* e = w.st + st_pose(k);
+      const float dx = ca * e[0] - sa * e[1], dy = sa * e[0] + ca * e[1];
+      const float r0 = w.st[0] + dx - rec[ly.o_zun + 3 * r], r1 = w.st[1] + dy - rec[ly.o_zun + 3 * r + 1];
+      const float r2 = wrapf(w.st[2] + e[2] - rec[ly.o_zun + 3 * r + 2]);
+      const float* om = rec + ly.o_omun + 6 * r;
+      const float O[3][3] = {{om[0], om[1], om[3]}, {om[1], om[2], om[4]}, {om[3], om[4], om[5]}};
+      const float Ja[3][3] = {{1.f, 0.f, -dy}, {0.f, 1.f, dx}, {0.f, 0.f, 1.f}};
+      const float Je[3][3] = {{ca, -sa, 0.f}, {sa, ca, 0.f}, {0.f, 0.f, 1.f}};
+      float Or[3], OJa[3][3], OJe[3][3];
+#pragma unroll
+      for (int i = 0; i < 3; ++i) {
+        Or[i] = O[i][0] * r0 + O[i][1] * r1 + O[i][2] * r2;
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+          OJa[i][j] = O[i][0] * Ja[0][j] + O[i][1] * Ja[1][j] + O[i][2] * Ja[2][j];
+          OJe[i][j] = O[i][0] * Je[0][j] + O[i][1] * Je[1][j] + O[i][2] * Je[2][j];
+        }
+      }
+      int t = 0;
+#pragma unroll
+      for (int x = 0; x < 3; ++x) {
+#pragma unroll
+        for (int y = 0; y <= x; ++y) A[t++] += Ja[0][x] * OJa[0][y] + Ja[1][x] * OJa[1][y] + Ja[2][x] * OJa[2][y];
+        A[6 + x] += Ja[0][x] * Or[0] + Ja[1][x] * Or[1] + Ja[2][x] * Or[2];
+      }
+      if (k >= 1) {
+        const int op = off_slot(ly, od, k, c);
+#pragma unroll
+        for (int x = 0; x < 3; ++x) {
+          float* row = w.H + w.rbase[op + x];
+          float* arow = w.H + w.rbase[oA + x];
+#pragma unroll
+          for (int y = 0; y <= x; ++y) row[op + y] += Je[0][x] * OJe[0][y] + Je[1][x] * OJe[1][y] + Je[2][x] * OJe[2][y];
+#pragma unroll
+          for (int y = 0; y < 3; ++y) arow[op + y] += Ja[0][x] * OJe[0][y] + Ja[1][x] * OJe[1][y] + Ja[2][x] * OJe[2][y];
+          rhs[op + x] -= Je[0][x] * Or[0] + Je[1][x] * Or[1] + Je[2][x] * Or[2];
+        }
+      }
+    }
+    tm.sync();
+    tm.sum_n(A, lane);
+    if (lane == 0) {
+      float* qa0 = w.H + w.rbase[oA];
+      float* qa1 = w.H + w.rbase[oA + 1];
+      float* qa2 = w.H + w.rbase[oA + 2];
+      qa0[oA] += A[0]; qa1[oA] += A[1]; qa1[oA + 1] += A[2];
+      qa2[oA] += A[3]; qa2[oA + 1] += A[4]; qa2[oA + 2] += A[5];
+      rhs[oA] -= A[6]; rhs[oA + 1] -= A[7]; rhs[oA + 2] -= A[8];
+    }
+    tm.sync();
+  }
   // range-bearing factors.  Landmarks g are global, so each factor has three blocks: anchor a, observing
   // pose e_k (k >= 1), landmark g.  With the anchor-frame landmark m = Rot(a_th)'(g - a_t), D = m - t_k:
   //   J_e = [-J_l | (0,-1)'],  J_g = J_l Rot(a_th)',  J_a = [-J_g | -J_l S m].
@@ -817,8 +898,8 @@ __device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int
     const float* rJ1 = w.H + w.rbase[c0 + 1];
     const float* rJ2 = w.H + w.rbase[c0 + 2];
     const float* rJ3 = w.H + w.rbase[c0 + 3];
-    // The ACTIVE row pairs of this column (bit mask from the symbolic phase) are compacted onto the
-    // lowest threads.  K-split: when fewer pairs than threads, `ch` adjacent lanes share one pair and
+    // The ACTIVE row pairs of this column (compact list from the symbolic phase) sit on the lowest
+    // threads.  K-split: when fewer pairs than threads, `ch` adjacent lanes share one pair and
     // split the dot-product range; partial sums are combined by shuffles.
     const unsigned short* aoff = reinterpret_cast<const unsigned short*>(w.amask);
     const unsigned char* alist = reinterpret_cast<const unsigned char*>(aoff + G + 2) + aoff[J];
@@ -1206,6 +1287,17 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
       }
     }
   }
+  if ((mk.um & 1ull) && lane == 0) {  // unary factor of slot 0 (x = a, J_a = I)
+    const float* om = rec + ly.o_omun + 6 * head;
+    const float r0 = w.st[0] - rec[ly.o_zun + 3 * head], r1 = w.st[1] - rec[ly.o_zun + 3 * head + 1];
+    const float r2 = wrapf(w.st[2] - rec[ly.o_zun + 3 * head + 2]);
+    Hs[tri(0, 0)] += om[0]; Hs[tri(1, 0)] += om[1]; Hs[tri(1, 1)] += om[2];
+    Hs[tri(2, 0)] += om[3]; Hs[tri(2, 1)] += om[4]; Hs[tri(2, 2)] += om[5];
+    gam[0] += om[0] * r0 + om[1] * r1 + om[3] * r2;
+    gam[1] += om[1] * r0 + om[2] * r1 + om[4] * r2;
+    gam[2] += om[3] * r0 + om[4] * r1 + om[5] * r2;
+  }
+  tm.sync();
   if (L > 0 && rb0) {  // range-bearing from slot 0 (observing pose x = a): blocks a and g
     float A[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
     for (int l = lane; l < L; l += TEAM) {
@@ -1391,6 +1483,7 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
   // --- K. bookkeeping: loop closures to the old slot 0 now live in the prior; new support masks
   for (int k = 1 + lane; k < c; k += TEAM)
     if (w.lct[k] == 0) reci[ly.o_lct + ring_of(k, head, W)] = -1;
+  mk.um &= ~1ull;       // the unary factor of the old slot 0 now lives in the prior
   mk.ps = nps & ~2ull;  // still indexed by the OLD slots; converted with the old head
   mk.ls = nls;
   if (lane == 0) {

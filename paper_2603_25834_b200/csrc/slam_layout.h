@@ -19,7 +19,7 @@ struct Layout {
   int np, pad;         // matrix dimension padded to a multiple of 4 (pad dummy rows before the newest pose)
   // record (32-bit words)
   int rec;             // record stride
-  int o_status, o_pm, o_lm, o_act, o_a, o_e, o_m, o_zodo, o_lct, o_zlc, o_rbm, o_zrb, o_vbar, o_g, o_lam;
+  int o_status, o_pm, o_lm, o_act, o_um, o_a, o_e, o_m, o_zodo, o_lct, o_zlc, o_rbm, o_zrb, o_zun, o_omun, o_vbar, o_g, o_lam;
   // shared memory per warp (32-bit words)
   int s_scr, s_st, s_zodo, s_zlc, s_lct, s_cs, s_rbm, s_first, s_rbase, s_amask, s_ssup, s_sidx, s_sds, s_H;
   int mw;              // 32-bit words of an active-row-pair mask (np/2 + 1 bits)
@@ -46,6 +46,7 @@ static inline Layout make_layout(int N, int W, int L, int cap, int wpc) {
   y.o_pm = o; o += 2;
   y.o_lm = o; o += 2;
   y.o_act = o; o += 2;
+  y.o_um = o; o += 2;   // ring positions that carry a unary absolute-pose factor
   o = pad4(o + 1);
   y.o_a = o; o += 4;
   y.o_e = o; o = pad4(o + 3 * W);
@@ -55,6 +56,8 @@ static inline Layout make_layout(int N, int W, int L, int cap, int wpc) {
   y.o_zlc = o; o = pad4(o + 3 * W);
   y.o_rbm = o; o = pad4(o + W * y.nw);
   y.o_zrb = o; o = pad4(o + W * 2 * L);
+  y.o_zun = o; o = pad4(o + 3 * W);    // unary factors: measured global pose per ring position
+  y.o_omun = o; o = pad4(o + 6 * W);   // ... and its information (xx, xy, yy, xt, yt, tt)
   y.o_vbar = o; o = pad4(o + n);
   y.o_g = o; o = pad4(o + n);
   y.o_lam = o; o = pad4(o + n * (n + 1) / 2);

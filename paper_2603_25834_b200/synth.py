@@ -39,6 +39,7 @@ class Config:
     T: int          # environment steps
     p_lc: float     # loop-closure probability per step
     seed: int = 0
+    p_unary: float = 0.0   # NEXT-1: probability of a scan-match style absolute-pose measurement per step
 
 
 # BASELINE.json `configs`, in order.  Config 4 is a sweep over N; `config4(N)` builds one point.
@@ -60,6 +61,7 @@ PRIOR_SIGMA = (0.01, 0.01, 0.005)
 ODO_SIGMA = (0.05, 0.05, 0.02)
 LC_SIGMA = (0.10, 0.10, 0.03)
 RB_SIGMA = (0.05, 0.01)
+UNARY_SIGMA = (0.03, 0.03, 0.01)   # absolute-pose measurement noise in the robot frame at match score 1
 RB_MIN_RANGE = 0.5
 RB_MAX_RANGE = 8.0
 LM_BOX_HALF = 10.0
@@ -150,6 +152,9 @@ def generate(cfg: Config, *, noise_scale: float = 1.0, dtype=np.float32, env_ids
     rb_meas = np.zeros((T + 1, 2, L, N), dtype)
     gt = np.zeros((T + 1, 3, N), np.float64)
     lm = np.zeros((2, L, N), np.float64)
+    un_valid = np.zeros((T, N), np.int32) if cfg.p_unary > 0 else None
+    un_pose = np.zeros((T, 3, N), dtype) if cfg.p_unary > 0 else None
+    un_info = np.zeros((T, 6, N), dtype) if cfg.p_unary > 0 else None
 
     for l in range(L):
         lm[0, l] = (2.0 * rng.uniform() - 1.0) * LM_BOX_HALF
@@ -190,6 +195,25 @@ def generate(cfg: Config, *, noise_scale: float = 1.0, dtype=np.float32, env_ids
             lc_meas[t - 1] = np.where(has[None, :], z, 0.0)
         if L > 0:
             observe(t, gt[t])
+        if cfg.p_unary > 0:
+            # 5. (only when p_unary > 0, drawn last so that the other streams are unchanged): q ~ U(0,1),
+            #    match score ~ U(0.3,1), three normals; measurement = GT_t + Rot(theta) * noise / sqrt(score);
+            #    information = score * R diag(1/sigma^2) R' in GLOBAL coordinates, packed (xx, xy, yy, xt, yt, tt)
+            q = rng.uniform()
+            score = 0.3 + 0.7 * rng.uniform()
+            nz = [rng.normal() for _ in range(3)]
+            has = q < cfg.p_unary
+            c, s_ = np.cos(gt[t, 2]), np.sin(gt[t, 2])
+            ex = ns * UNARY_SIGMA[0] * nz[0] / np.sqrt(score)
+            ey = ns * UNARY_SIGMA[1] * nz[1] / np.sqrt(score)
+            et = ns * UNARY_SIGMA[2] * nz[2] / np.sqrt(score)
+            zu = np.stack([gt[t, 0] + c * ex - s_ * ey, gt[t, 1] + s_ * ex + c * ey, wrap(gt[t, 2] + et)])
+            wx, wy, wt = score / UNARY_SIGMA[0] ** 2, score / UNARY_SIGMA[1] ** 2, score / UNARY_SIGMA[2] ** 2
+            info = np.stack([c * c * wx + s_ * s_ * wy, c * s_ * (wx - wy), s_ * s_ * wx + c * c * wy,
+                             np.zeros_like(c), np.zeros_like(c), wt])
+            un_valid[t - 1] = has.astype(np.int32)
+            un_pose[t - 1] = np.where(has[None, :], zu, 0.0)
+            un_info[t - 1] = np.where(has[None, :], info, 0.0)
 
-    return dict(odom=odom, lc_back=lc_back, lc_meas=lc_meas, rb_mask=rb_mask, rb_meas=rb_meas,
+    return dict(un_valid=un_valid, un_pose=un_pose, un_info=un_info, odom=odom, lc_back=lc_back, lc_meas=lc_meas, rb_mask=rb_mask, rb_meas=rb_meas,
                 gt=gt, lm=lm, env_ids=env_ids, cfg=cfg, T=T)

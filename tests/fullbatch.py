@@ -68,6 +68,10 @@ class FullBatch:
         if self.L:
             self._observe(t, valid, zrb)
 
+    def add_unary(self, z, Om):
+        """absolute-pose factor on the newest pose, full 3x3 information"""
+        self.fac.append(("un", len(self.x) - 1, np.array(z, float), np.array(Om, float).reshape(3, 3)))
+
     def system(self):
         T = len(self.x)
         lids = sorted(self.lm)
@@ -81,6 +85,13 @@ class FullBatch:
         g[:3] += om0 * r0
         om_rb = 1.0 / self.sig[9:11] ** 2
         for f in self.fac:
+            if f[0] == "un":
+                _, k, z, Om = f
+                r = self.x[k] - z
+                r[2] = wrap(r[2])
+                H[3 * k:3 * k + 3, 3 * k:3 * k + 3] += Om
+                g[3 * k:3 * k + 3] += Om @ r
+                continue
             if f[0] == "b":
                 _, i, j, z, om = f
                 r, Ji, Jj = between_res_jac(self.x[i], self.x[j], z)

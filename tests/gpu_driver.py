@@ -13,6 +13,10 @@ def to_dev(data, device="cuda:0"):
     d["lc_meas"] = torch.from_numpy(np.ascontiguousarray(data["lc_meas"], dtype=np.float32)).to(device)
     d["rb_mask"] = torch.from_numpy(np.ascontiguousarray(data["rb_mask"]).view(np.int32)).to(device)
     d["rb_meas"] = torch.from_numpy(np.ascontiguousarray(data["rb_meas"], dtype=np.float32)).to(device)
+    if data.get("un_valid") is not None:
+        d["un_valid"] = torch.from_numpy(np.ascontiguousarray(data["un_valid"], dtype=np.int32)).to(device)
+        d["un_pose"] = torch.from_numpy(np.ascontiguousarray(data["un_pose"], dtype=np.float32)).to(device)
+        d["un_info"] = torch.from_numpy(np.ascontiguousarray(data["un_info"], dtype=np.float32)).to(device)
     return d
 
 
@@ -33,6 +37,8 @@ def run_gpu(slam, data, iters, fused=True, steps=None, want_poses=True):
     for t in range(1, T + 1):
         args = (dev["odom"][t - 1], dev["lc_back"][t - 1], dev["lc_meas"][t - 1],
                 dev["rb_mask"][t] if L else None, dev["rb_meas"][t] if L else None)
+        if "un_valid" in dev:
+            slam.set_unary(dev["un_pose"][t - 1], dev["un_info"][t - 1], dev["un_valid"][t - 1])
         if fused and not want_poses:
             slam.step(*args, iters=iters, cov=cov[t - 1], logdet=logdet[t - 1])
         else:

@@ -32,6 +32,9 @@ def drive(orc, data, env, iters, on_step=None, steps=None):
     for t in range(1, T + 1):
         odom, back, zlc, valid, zrb = step_inputs(data, t, env)
         orc.push(odom, back, zlc, valid, zrb)
+        un = unary_inputs(data, t, env)
+        if un is not None:
+            orc.add_unary(*un)
         sn = orc.solve(iters)
         S, ld = orc.cov()
         P = orc.poses()
@@ -42,3 +45,13 @@ def drive(orc, data, env, iters, on_step=None, steps=None):
         if orc.count == W:
             orc.marginalize()
     return out
+
+
+def unary_inputs(data, t, env):
+    """(pose3, info3x3) of the unary factor of step t, or None."""
+    if data.get("un_valid") is None or not data["un_valid"][t - 1, env]:
+        return None
+    z = data["un_pose"][t - 1, :, env].astype(np.float64)
+    i6 = data["un_info"][t - 1, :, env].astype(np.float64)
+    Om = np.array([[i6[0], i6[1], i6[3]], [i6[1], i6[2], i6[4]], [i6[3], i6[4], i6[5]]])
+    return z, Om

@@ -403,3 +403,126 @@ def test_run_batch_matches_single_env_driver_and_is_env_independent():
     sub = synth.generate(cfg, env_ids=[1])
     res1 = oracle.run_batch(sub, cfg.iters)
     assert np.array_equal(res1["logdet"][:, 0], res["logdet"][:, 1])
+
+
+# ----------------------------------------------------------------------------- NEXT-1: unary absolute-pose factor
+def _random_spd(rng, scale):
+    A = rng.normal(size=(3, 3))
+    return (A @ A.T + 0.5 * np.eye(3)) * scale
+
+
+def test_unary_factor_jacobians_fd():
+    rng = np.random.default_rng(21)
+    for _ in range(10):
+        a, ek, z = rng.normal(size=3) * [4, 4, 1], rng.normal(size=3), rng.normal(size=3) * [4, 4, 1]
+        r, Ja, Je = oracle.unary_factor(a, ek, z)
+        assert np.allclose(Ja, fd_jac(lambda q: oracle.unary_factor(q, ek, z)[0], a), atol=1e-6)
+        assert np.allclose(Je, fd_jac(lambda q: oracle.unary_factor(a, q, z)[0], ek), atol=1e-6)
+        r0, Ja0, Je0 = oracle.unary_factor(a, ek, z, k_is_frame=True)
+        assert np.allclose(Ja0, np.eye(3)) and np.allclose(Je0, 0)
+    # definition: measuring the pose itself gives r = 0
+    a, e = np.array([1.0, -2.0, 0.4]), np.array([0.3, 0.2, -0.1])
+    x = synth.compose(a[:, None], e[:, None])[:, 0]
+    assert np.allclose(oracle.unary_factor(a, e, x)[0], 0, atol=1e-15)
+
+
+def test_unary_factor_is_the_kalman_update():
+    """One odometry step then an absolute-pose measurement of the predicted pose (zero residual):
+    the posterior covariance is the textbook information-form update (P^-1 + Omega)^-1."""
+    rng = np.random.default_rng(22)
+    P0, Q = SIG[0:3] ** 2, SIG[3:6] ** 2
+    for W in (2, 4):
+        o = Oracle(W, 0)
+        o.reset()
+        Sig = np.diag(P0)
+        for k in range(1, 7):
+            o.push([0.2, 0.0, 0.0])
+            F = np.array([[1, 0, 0], [0, 1, 0.2], [0, 0, 1.0]])
+            Sig = F @ Sig @ F.T + np.diag(Q)
+            Om = _random_spd(rng, 50.0)
+            o.add_unary(o.poses()[o.count - 1], Om)
+            assert o.solve(2) < 1e-12
+            Sig = np.linalg.inv(np.linalg.inv(Sig) + Om)
+            S, ld = o.cov()
+            assert np.allclose(S, Sig, rtol=1e-9, atol=1e-15), (W, k)
+            assert abs(ld - np.log(np.linalg.det(Sig))) < 1e-9
+            if o.count == W:
+                o.marginalize()
+
+
+@pytest.mark.parametrize("W,L,p_lc", [(6, 0, 0.4), (5, 6, 0.3)])
+def test_unary_noise_free_recovery_and_full_batch_equality(W, L, p_lc):
+    cfg = synth.Config("un", N=2, W=W, L=L, iters=2, T=35, p_lc=p_lc, seed=13, p_unary=0.5)
+    data = synth.generate(cfg, noise_scale=0.0, dtype=np.float64)
+    assert data["un_valid"].sum() > 10
+    from tests.helpers import unary_inputs
+    for env in range(cfg.N):
+        fb = fullbatch.FullBatch(SIG, L)
+        o = Oracle(W, L)
+        o.reset()
+        if L:
+            fb.observe_first(*rb_inputs(data, 0, env))
+            o.observe_first(*rb_inputs(data, 0, env))
+        for t in range(1, cfg.T + 1):
+            odom, back, zlc, valid, zrb = step_inputs(data, t, env)
+            fb.push(odom, back, zlc, valid, zrb)
+            o.push(odom, back, zlc, valid, zrb)
+            un = unary_inputs(data, t, env)
+            if un is not None:
+                fb.add_unary(*un)
+                o.add_unary(*un)
+            assert o.solve(2) < 1e-10
+            c = o.count
+            err = o.poses()[:c] - data["gt"][t - c + 1: t + 1, :, env]
+            err[:, 2] = fullbatch.wrap(err[:, 2])
+            assert np.abs(err).max() < 1e-9
+            S, ld = o.cov()
+            ref = fb.last_cov()
+            scale = np.sqrt(np.outer(np.diag(ref), np.diag(ref)))
+            assert np.all(np.abs(S - ref) <= 1e-7 * scale), (t, S, ref)
+            if o.count == W:
+                o.marginalize()
+
+
+def test_unary_linear_gaussian_equals_brute_force():
+    rng = np.random.default_rng(23)
+    W, T = 4, 20
+    P0 = SIG[0:3] ** 2
+    om_odo = 1.0 / SIG[3:6] ** 2
+    x0 = np.array([0.1, 0.2, -0.1])
+    o = Oracle(W, 0, linear=True)
+    o.reset(x0)
+    facs = []       # (A_rows [m x n later], rhs, weight matrix)
+    gt = [x0.copy()]
+    for t in range(1, T + 1):
+        u = rng.normal(size=3) * 0.3
+        gt.append(gt[-1] + u)
+        z = u + rng.normal(size=3) * SIG[3:6]
+        facs.append(("b", t - 1, t, z, np.diag(om_odo)))
+        o.push(z)
+        if rng.uniform() < 0.6:
+            Om = _random_spd(rng, 30.0)
+            zu = gt[t] + rng.normal(size=3) * 0.2
+            facs.append(("u", t, t, zu, Om))
+            o.add_unary(zu, Om)
+        o.solve(1)
+        assert o.solve(1) < 1e-9
+        n = 3 * (t + 1)
+        A = np.zeros((n, n))
+        rv = np.zeros(n)
+        A[:3, :3] += np.diag(1.0 / P0)
+        rv[:3] += x0 / P0
+        for kind, i, j, zz, Om in facs:
+            Jm = np.zeros((3, n))
+            Jm[:, 3 * j:3 * j + 3] = np.eye(3)
+            if kind == "b":
+                Jm[:, 3 * i:3 * i + 3] = -np.eye(3)
+            A += Jm.T @ Om @ Jm
+            rv += Jm.T @ Om @ zz
+        P = np.linalg.inv(A)
+        xhat = P @ rv
+        assert np.allclose(o.poses()[o.count - 1], xhat[-3:], rtol=1e-8, atol=1e-9)
+        assert np.allclose(o.cov()[0], P[-3:, -3:], rtol=1e-7, atol=1e-14)
+        if o.count == W:
+            o.set_state(o.state() + rng.normal(size=o.n) * 0.1)
+            o.marginalize()
