@@ -31,6 +31,9 @@ if ROOT not in sys.path:
 from paper_2603_25834_b200 import replicas, synth, workmodel  # noqa: E402
 
 SM_COUNT, LANES = 148, 128
+# dram__bytes_read.sum + dram__bytes_write.sum of one slam_step_kernel launch from the committed
+# `ncu --set full` capture (profiles/r1_step_kernel_final_full.md), keyed by workload
+NCU_TRAFFIC_BYTES = {"cfg3_landmarks_16384": 152.7e6}
 L2_BYTES = 126 * 2 ** 20
 METRIC = "fixed-lag SLAM env-steps/sec (solve+cov+marginalize)"
 
@@ -272,7 +275,7 @@ def main():
         roof = {"bound": bound, "unit": "TFLOP/s" if bound == "alu" else "GB/s",
                 "achieved": (flops_total / t_meas / 1e12) if bound == "alu" else (bytes_total / t_meas / 1e9),
                 "peak": p_fp32 if bound == "alu" else bw,
-                "frac": max(t_alu, t_hbm) / t_meas, "traffic": None,
+                "frac": max(t_alu, t_hbm) / t_meas, "traffic": NCU_TRAFFIC_BYTES.get(cfg.name),
                 "kernel": "slam_step_kernel", "kernel_ms_avg": ms / K,
                 "alg_flops_per_env_step": flops_total / (N * K), "alg_bytes_per_env_step": bytes_total / (N * K),
                 "alu_frac": t_alu / t_meas, "hbm_frac": t_hbm / t_meas,
