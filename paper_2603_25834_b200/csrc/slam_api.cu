@@ -30,6 +30,9 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head, int c, int flags,
   Team<TEAM> tm;
   tm.bar = 1 + team;
   tm.scr = base + ly.s_scr;
+  Team<32> tm32;
+  tm32.bar = 0;
+  tm32.scr = tm.scr;
   // All teams of a CTA walk through the phases in LOCK-STEP (CTA barriers between phases): the kernel is
   // large (~12 k instructions) and instruction-fetch bound, so warps that execute the same code at the
   // same time share every fetched line.  Teams without an environment in the last round only take part
@@ -44,6 +47,7 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head, int c, int flags,
     const int env = valid ? (mode == 0 ? widx : ovf[1 + widx]) : 0;
     float* rec = state + (size_t)env * ly.rec;
     int cc = c, status = 0, s = 0, total = 0;
+    bool single_warp = false;
     Masks mk;
     Ord od;
     __syncthreads();
@@ -64,6 +68,7 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head, int c, int flags,
       if (valid) {
         total = symbolic<TEAM>(ly, od, w, tm, lane, cc, mk, s);
         need = max(need, total);
+        single_warp = reinterpret_cast<const int*>(tm.scr)[9] <= 32;
         if (stats && lane == 0 && mode == 0) {  // envelope statistics (words per environment): max, sum, count
           atomicMax(stats + 0, (unsigned long long)total);
           atomicAdd(stats + 1, (unsigned long long)total);
@@ -84,11 +89,26 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head, int c, int flags,
         if (LOCK >= 1) __syncthreads();
         if (valid) { assemble<TEAM>(ly, pr, od, rec, w, tm, lane, head, cc, mk, s, total); tm.sync(); }
         if (LOCK >= 2) __syncthreads();
-        if (valid) status |= cholesky<TEAM>(ly, w, tm, lane);
+        if (valid) {
+          // When no column block has more than 32 active row pairs (every pose-only window), one warp
+          // does the factorisation with shuffles and __syncwarp only: no named barriers, no
+          // shared-memory exchange of the diagonal tile.  The other warps of the team wait.
+          if (TEAM > 32 && single_warp) {
+            if (lane < 32) status |= cholesky<32>(ly, w, tm32, lane);
+            tm.sync();
+          } else {
+            status |= cholesky<TEAM>(ly, w, tm, lane);
+          }
+        }
         if (LOCK >= 3) __syncthreads();
         if (valid) {
           if (it < iters) {
-            back_substitute<TEAM>(ly, w, tm, lane);
+            if (TEAM > 32) {  // short rows: one warp, no named barriers
+              if (lane < 32) back_substitute<32>(ly, w, tm32, lane);
+              tm.sync();
+            } else {
+              back_substitute<TEAM>(ly, w, tm, lane);
+            }
             status |= apply_update<TEAM>(ly, od, w, tm, lane, cc, mk);
           } else {
             covariance<TEAM>(ly, w, tm, lane, env, cc, io);

@@ -464,8 +464,9 @@ __device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, const Team
     const int G = np >> 2, NP = (np >> 1) + 1;
     unsigned short* aoff = reinterpret_cast<unsigned short*>(w.amask);
     unsigned char* alist = reinterpret_cast<unsigned char*>(aoff + G + 2);
-    int run = 0;
+    int run = 0, maxcnt = 0;
     for (int J = 0; J < G; ++J) {
+      const int start = run;
       if (lane == 0) aoff[J] = (unsigned short)run;
       for (int base = 2 * J; base < NP; base += 32) {
         const int p = base + lane;
@@ -474,8 +475,9 @@ __device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, const Team
         if (on) alist[run + __popc(bal & ((1u << lane) - 1u))] = (unsigned char)p;
         run += __popc(bal);
       }
+      maxcnt = max(maxcnt, run - start);
     }
-    if (lane == 0) aoff[G] = (unsigned short)run;
+    if (lane == 0) { aoff[G] = (unsigned short)run; reinterpret_cast<int*>(tm.scr)[9] = maxcnt; }
   }
   tm.sync();
   return reinterpret_cast<const int*>(tm.scr)[8];
