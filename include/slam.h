@@ -137,6 +137,24 @@ int slam_get_status(slam_ctx* ctx, int32_t* status);
  * that exceeded the shared-memory capacity and ran from the global-memory fallback. */
 int slam_get_stats(slam_ctx* ctx, unsigned long long* stats8);
 
+/* NEXT-4: the paper's reward, eqs. (7)-(17), elementwise over environments, meant
+ * to be enqueued right after slam_dopt.  The hyper-parameters are on the paper's project page, not in
+ * the paper, so they are inputs; so is the mapping from Sigma_t to the scalar U (e.g. `dopt`).
+ *   R = -lambda_col                                   if collision                              (7)
+ *   R = R*_explore - R_abs + R*_delta                 otherwise
+ *   R_explore = lambda_explore * dcells * I,  I = c + (1-c) iota                                (8),(10)
+ *   c = clip((u_hi - U_prev)/u_hi, 0, 1)^2,  iota = clip(max(U_prev - U, 0)/kappa, 0, 1)        (11),(12)
+ *   R_abs = lambda_abs * exp(U_prev) * U_prev,  R_delta = lambda_delta * exp(U_prev) * (U_prev - U)  (13),(14)
+ *   alpha = clip((d_min - d_crash)/(d_full - d_crash), 0, 1)                                   (15)
+ *   R*_explore = R_explore * alpha;  R*_delta = R_delta * alpha if U_prev - U > 0 else R_delta (16),(17)
+ * u, u_prev, dcells (eq. (9), computed by the simulator side), d_min: [N] float; collision: [N] int32
+ * (non-zero = collision); reward: [N] float out.  All device pointers. */
+typedef struct {
+  float lambda_col, lambda_explore, lambda_abs, lambda_delta, u_hi, kappa, d_crash, d_full;
+} slam_reward_params;
+int slam_reward(slam_ctx* ctx, const slam_reward_params* p, const float* u, const float* u_prev, const float* dcells,
+                const float* d_min, const int32_t* collision, float* reward);
+
 int slam_count(const slam_ctx* ctx);                /* host-side window count c in [1, window] */
 long long slam_launch_count(const slam_ctx* ctx);   /* kernels launched by this context so far */
 const char* slam_last_error(const slam_ctx* ctx);   /* message of the last non-zero return */

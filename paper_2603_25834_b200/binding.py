@@ -23,13 +23,18 @@ SYMBOLS = (
     "slam_default_config", "slam_workspace_bytes", "slam_create", "slam_destroy", "slam_reset",
     "slam_push_step", "slam_set_unary", "slam_observe_first", "slam_solve", "slam_marginal_cov", "slam_dopt",
     "slam_marginalize_oldest", "slam_step", "slam_step_host", "slam_get_poses", "slam_get_landmarks",
-    "slam_get_status", "slam_get_stats", "slam_count", "slam_launch_count", "slam_last_error", "slam_kernel_info",
+    "slam_get_status", "slam_get_stats", "slam_reward", "slam_count", "slam_launch_count", "slam_last_error", "slam_kernel_info",
 )
 
 
 class SlamConfig(C.Structure):
     _fields_ = [("prior_sigma", C.c_float * 3), ("odo_sigma", C.c_float * 3), ("lc_sigma", C.c_float * 3),
                 ("rb_sigma", C.c_float * 2)]
+
+
+class RewardParams(C.Structure):
+    _fields_ = [(n, C.c_float) for n in ("lambda_col", "lambda_explore", "lambda_abs", "lambda_delta", "u_hi", "kappa",
+                                         "d_crash", "d_full")]
 
 
 class SlamError(RuntimeError):
@@ -68,6 +73,7 @@ def _load() -> C.CDLL:
     lib.slam_get_landmarks.argtypes = [vp, fp, ip]
     lib.slam_get_status.argtypes = [vp, ip]
     lib.slam_get_stats.argtypes = [vp, ip]
+    lib.slam_reward.argtypes = [vp, C.POINTER(RewardParams), fp, fp, fp, fp, ip, fp]
     lib.slam_count.argtypes = [vp]
     lib.slam_launch_count.argtypes = [vp]
     lib.slam_launch_count.restype = C.c_longlong
@@ -230,6 +236,13 @@ class FixedLagSlam:
         self._chk(LIB.slam_get_stats(self._h, C.c_void_p(out.data_ptr())))
         v = [int(x) for x in out.cpu()]
         return dict(max_envelope_words=v[0], mean_envelope_words=v[1] / max(v[2], 1), solved=v[2], fallback=v[3])
+
+    def reward(self, params: RewardParams, u, u_prev, dcells, d_min, collision, out=None):
+        out = self._new(self.N) if out is None else out
+        d = lambda x, n, ty=None: self._dev(x, (self.N,), ty or self._F, n)
+        self._chk(LIB.slam_reward(self._h, C.byref(params), d(u, "u"), d(u_prev, "u_prev"), d(dcells, "dcells"),
+                                  d(d_min, "d_min"), d(collision, "collision", self._I), d(out, "reward")))
+        return out
 
     @property
     def count(self) -> int:

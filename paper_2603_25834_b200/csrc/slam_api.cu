@@ -202,6 +202,26 @@ __global__ void slam_copycov_kernel(int N, const float* cache, float* cov, float
   if (dopt) dopt[env] = expf(ld * (1.0f / 3.0f));
 }
 
+// NEXT-4: reward of eqs. (7)-(17), one thread per environment
+__global__ void slam_reward_kernel(int N, slam_reward_params p, const float* u, const float* u_prev, const float* dcells,
+                                   const float* d_min, const int32_t* collision, float* reward) {
+  const int env = blockIdx.x * blockDim.x + threadIdx.x;
+  if (env >= N) return;
+  if (collision[env] != 0) { reward[env] = -p.lambda_col; return; }                       // (7)
+  const float U = u[env], Up = u_prev[env];
+  float cc = fminf(fmaxf((p.u_hi - Up) / p.u_hi, 0.f), 1.f);
+  cc *= cc;                                                                               // (11)
+  const float drop = Up - U;
+  const float iota = fminf(fmaxf(fmaxf(drop, 0.f) / p.kappa, 0.f), 1.f);                  // (12)
+  const float I = cc + (1.f - cc) * iota;                                                 // (10)
+  const float r_explore = p.lambda_explore * dcells[env] * I;                             // (8)
+  const float ex = expf(Up);
+  const float r_abs = p.lambda_abs * ex * Up;                                             // (13)
+  const float r_delta = p.lambda_delta * ex * drop;                                       // (14)
+  const float alpha = fminf(fmaxf((d_min[env] - p.d_crash) / (p.d_full - p.d_crash), 0.f), 1.f);  // (15)
+  reward[env] = r_explore * alpha - r_abs + (drop > 0.f ? r_delta * alpha : r_delta);     // (16), (17), (7)
+}
+
 // ------------------------------------------------------------------ host object
 struct slam_ctx {
   Layout ly;
@@ -587,6 +607,16 @@ int slam_get_stats(slam_ctx* c, unsigned long long* stats8) {
   if (!c || !stats8) return SLAM_EINVAL;
   cudaMemcpyAsync(stats8, c->stats, 64, cudaMemcpyDeviceToDevice, c->stream);
   return check_cuda(c, "slam_get_stats");
+}
+
+int slam_reward(slam_ctx* c, const slam_reward_params* p, const float* u, const float* u_prev, const float* dcells,
+                const float* d_min, const int32_t* collision, float* reward) {
+  if (!c || !p || !u || !u_prev || !dcells || !d_min || !collision || !reward) return c ? fail(c, SLAM_EINVAL, "NULL argument") : SLAM_EINVAL;
+  if (!(p->u_hi > 0.f) || !(p->kappa > 0.f) || !(p->d_full > p->d_crash)) return fail(c, SLAM_EINVAL, "u_hi, kappa > 0 and d_full > d_crash required");
+  const int threads = 256, blocks = (c->ly.N + threads - 1) / threads;
+  slam_reward_kernel<<<blocks, threads, 0, c->stream>>>(c->ly.N, *p, u, u_prev, dcells, d_min, collision, reward);
+  c->launches++;
+  return check_cuda(c, "slam_reward_kernel");
 }
 
 int slam_count(const slam_ctx* c) { return c ? c->count : -1; }
