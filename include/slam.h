@@ -67,6 +67,16 @@ void slam_destroy(slam_ctx* ctx); /* frees the host object only */
  * on it (reading R9); clears landmarks, factors and status. */
 int slam_reset(slam_ctx* ctx, const float* init_pose);
 
+/* NEXT-2: per-environment episode reset (episodes end after 2048 steps or on collision).
+ * Environments with mask[env] != 0 restart with ONE pose at init_pose ([3][N]; NULL -> origin), the
+ * first-pose prior, no landmarks, no factors and a clear status, while the others keep their windows.
+ * The window stays in lock-step on the host (slam_count is the count of the never-reset environments);
+ * a reset environment simply has fewer live poses until its own window is full again: it is not
+ * marginalised before that, its read-outs (slam_get_poses) report only its own poses, and loop closures
+ * that reach behind its reset are ignored like any loop closure that leaves the window.
+ * Call it between steps (after slam_marginalize_oldest / slam_step). */
+int slam_reset_envs(slam_ctx* ctx, const int32_t* mask, const float* init_pose);
+
 /* S0 push (BASELINE.json "initial guess is dead-reckoned"): appends one pose with the
  * dead-reckoned guess e_c = e_{c-1} (+) odom and records this step's factors.
  *   odom    [3][N]  dx, dy, dtheta in the previous pose's frame

@@ -62,6 +62,8 @@ def lib():
         L.orc_unary_factor.argtypes = [_dp, _dp, _dp, C.c_int, _dp, _dp, _dp]
         L.orc_batch_set_unary.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_batch_set_unary.restype = None
+        L.orc_batch_set_resets.argtypes = [C.c_void_p, C.c_void_p]
+        L.orc_batch_set_resets.restype = None
         L.orc_run_batch.restype = C.c_int
         L.orc_run_batch.argtypes = [C.c_int] * 5 + [_dp, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                                     C.c_void_p, _ip, C.c_int, C.c_int, _dp, _dp, _dp, _dp]
@@ -238,11 +240,16 @@ def run_batch(data: dict, iters: int, envs=None, sigmas=DEFAULT_SIGMAS, threads:
     if data.get("un_valid") is not None:
         keep = (np.ascontiguousarray(data["un_valid"], dtype=np.int32), f32(data["un_pose"]), f32(data["un_info"]))
         lib().orc_batch_set_unary(vp(keep[0]), vp(keep[1]), vp(keep[2]))
+    keep2 = None
+    if data.get("reset") is not None:
+        keep2 = (np.ascontiguousarray(data["reset"], dtype=np.int32), f32(data["reset_pose"]))
+        lib().orc_batch_set_resets(vp(keep2[0]), vp(keep2[1]))
     lib().orc_batch_set_f32_storage(int(f32_storage))
     bad = lib().orc_run_batch(N, W, L, T, iters, _p(sig), vp(odom), vp(lc_back), vp(lc_meas), vp(rb_mask),
                               vp(rb_meas), envs.ctypes.data_as(_ip), ne, int(threads),
                               ptr(out["poses"]), ptr(out["cov"]), ptr(out["logdet"]), ptr(out["step"]))
     lib().orc_batch_set_f32_storage(0)
     lib().orc_batch_set_unary(None, None, None)
+    lib().orc_batch_set_resets(None, None)
     out["bad"] = bad
     return out

@@ -768,6 +768,10 @@ static const int* g_un_valid = 0;
 static const float* g_un_pose = 0;
 static const float* g_un_info = 0;
 void orc_batch_set_unary(const int* valid, const float* pose, const float* info) { g_un_valid = valid; g_un_pose = pose; g_un_info = info; }
+/* optional per-environment episode resets (NEXT-2): reset[T][N] (int), reset_pose[T][3][N]; applied before the push of step t */
+static const int* g_reset = 0;
+static const float* g_reset_pose = 0;
+void orc_batch_set_resets(const int* reset, const float* pose) { g_reset = reset; g_reset_pose = pose; }
 void orc_batch_set_f32_storage(int on) { g_batch_f32_storage = on; }
 
 int orc_run_batch(int N, int W, int L, int T, int iters, const double* sig11,
@@ -803,6 +807,11 @@ int orc_run_batch(int N, int W, int L, int T, int iters, const double* sig11,
         zl[k] = lc_meas ? lc_meas[((size_t)(t - 1) * 3 + k) * N + env] : 0.0;
       }
       int back = lc_back ? lc_back[(size_t)(t - 1) * N + env] : 0;
+      if (g_reset && g_reset[(size_t)(t - 1) * N + env]) {
+        double ip[3];
+        for (int k = 0; k < 3; ++k) ip[k] = g_reset_pose[((size_t)(t - 1) * 3 + k) * N + env];
+        orc_reset(o, ip);
+      }
       orc_push(o, od, back, zl, valid, zrb);
       if (g_un_valid && g_un_valid[(size_t)(t - 1) * N + env]) {
         double zp[3], I6[6], I9[9];

@@ -57,6 +57,8 @@ int  orc_add_unary(orc*, const double* pose3, const double* info9);
 void orc_unary_factor(const double* a3, const double* ek3, const double* z3, int k_is_frame,
                       double* r3, double* Ja9, double* Je9);
 void orc_batch_set_unary(const int* valid, const float* pose, const float* info);
+/* NEXT-2: per-environment episode resets for the batch driver: orc_reset(init pose) before the push of step t */
+void orc_batch_set_resets(const int* reset, const float* pose);
 /* returns 0, or -1 if H was singular.  last_step_norm (may be NULL) = max |delta| of the last iteration */
 int  orc_solve(orc*, int iters, double* last_step_norm);
 int  orc_cov(orc*, double* cov9, double* logdet);

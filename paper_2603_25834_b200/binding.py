@@ -21,7 +21,7 @@ _ERR = {1: "SLAM_EINVAL", 2: "SLAM_ESTATE", 3: "SLAM_ENOMEM", 4: "SLAM_ECUDA"}
 # every symbol include/slam.h declares (checked by tests/test_abi.py)
 SYMBOLS = (
     "slam_default_config", "slam_workspace_bytes", "slam_create", "slam_destroy", "slam_reset",
-    "slam_push_step", "slam_set_unary", "slam_observe_first", "slam_solve", "slam_marginal_cov", "slam_dopt",
+    "slam_reset_envs", "slam_push_step", "slam_set_unary", "slam_observe_first", "slam_solve", "slam_marginal_cov", "slam_dopt",
     "slam_marginalize_oldest", "slam_step", "slam_step_host", "slam_get_poses", "slam_get_landmarks",
     "slam_get_status", "slam_get_stats", "slam_reward", "slam_count", "slam_launch_count", "slam_last_error", "slam_kernel_info",
 )
@@ -60,6 +60,7 @@ def _load() -> C.CDLL:
     lib.slam_destroy.argtypes = [vp]
     lib.slam_destroy.restype = None
     lib.slam_reset.argtypes = [vp, fp]
+    lib.slam_reset_envs.argtypes = [vp, ip, fp]
     lib.slam_push_step.argtypes = [vp, fp, ip, fp, ip, fp]
     lib.slam_set_unary.argtypes = [vp, fp, fp, ip]
     lib.slam_observe_first.argtypes = [vp, ip, fp]
@@ -165,6 +166,10 @@ class FixedLagSlam:
     # ---- the C entry points
     def reset(self, init_pose=None):
         self._chk(LIB.slam_reset(self._h, self._dev(init_pose, (3, self.N), self._F, "init_pose")))
+
+    def reset_envs(self, mask, init_pose=None):
+        self._chk(LIB.slam_reset_envs(self._h, self._dev(mask, (self.N,), self._I, "mask"),
+                                      self._dev(init_pose, (3, self.N), self._F, "init_pose")))
 
     def push_step(self, odom, lc_back=None, lc_meas=None, rb_mask=None, rb_meas=None):
         self._chk(LIB.slam_push_step(self._h, *self._push_ptrs(self._dev, odom, lc_back, lc_meas, rb_mask, rb_meas)))

@@ -19,7 +19,7 @@ using namespace slamk;
 // the same device code and are bit-for-bit identical.
 template <int TEAM>
 __global__ void __launch_bounds__(TEAM == 128 ? 896 : (TEAM == 64 ? 512 : 256))
-slam_step_kernel(Layout ly, Params pr, float* state, int head, int c, int flags, int iters, StepIO io,
+slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flags, int iters, StepIO io,
                  unsigned long long* stats, int mode, int* ovf) {
   extern __shared__ float4 smem4[];
   float* smem = reinterpret_cast<float*>(smem4);
@@ -46,7 +46,11 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head, int c, int flags,
     bool valid = widx < nwork;
     const int env = valid ? (mode == 0 ? widx : ovf[1 + widx]) : 0;
     float* rec = state + (size_t)env * ly.rec;
-    int cc = c, status = 0, s = 0, total = 0;
+    // NEXT-2: an environment that was reset mid-run lives in the slots k0.. of the lock-step window:
+    // its own count is c - k0 and its ring head is head + k0 (slam_reset_envs).
+    const int k0 = valid ? reinterpret_cast<const int*>(rec)[ly.o_k0] : 0;
+    const int head = (head_g + k0) % ly.W;
+    int cc = c - k0, status = 0, s = 0, total = 0;
     bool single_warp = false;
     Masks mk;
     Ord od;
@@ -58,8 +62,9 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head, int c, int flags,
       od = make_ord(ly, w.rbm, cc);
       s = build_support<TEAM>(ly, od, w, tm, lane, cc, mk.ps, mk.ls);
     }
+    const bool do_marg = (flags & F_MARG) && k0 == 0;   // a reset environment is not full yet
     int need = 0;
-    if (valid && (flags & F_MARG)) need = marg_need(ly, w, lane, cc, mk);
+    if (valid && do_marg) need = marg_need(ly, w, lane, cc, mk);
     // iters Gauss-Newton iterations, then (F_COV) one more linearisation + factorisation at the final
     // estimate for the covariance: ONE call site per phase keeps the kernel small.
     const int nlin = iters + ((flags & F_COV) ? 1 : 0);
@@ -127,7 +132,8 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head, int c, int flags,
         io.last_pose[(size_t)ly.N + env] = w.st[1] + sn * e[0] + cn * e[1];
         io.last_pose[2 * (size_t)ly.N + env] = wrapf(w.st[2] + e[2]);
       }
-      if (flags & F_MARG) status |= marginalize<TEAM>(ly, pr, rec, w, tm, lane, head, cc, mk, s);
+      if (do_marg) status |= marginalize<TEAM>(ly, pr, rec, w, tm, lane, head, cc, mk, s);
+      else if ((flags & F_MARG) && lane == 0) reinterpret_cast<int*>(rec)[ly.o_k0] = k0 - 1;  // the window slides under it
       store_state<TEAM>(ly, rec, w, tm, lane, head, cc, mk);
       if (status && lane == 0) reinterpret_cast<int*>(rec)[ly.o_status] |= status;
       tm.sync();
@@ -152,12 +158,36 @@ __global__ void slam_reset_kernel(Layout ly, Params pr, float* state, const floa
   }
 }
 
+// NEXT-2: per-environment episode reset (episodes end after 2048 steps or on collision).
+// One warp per environment; only environments with mask != 0 are touched.
+__global__ void slam_reset_envs_kernel(Layout ly, Params pr, float* state, int c, const int32_t* mask, const float* init_pose) {
+  const int env = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (env >= ly.N || mask[env] == 0) return;
+  float* rec = state + (size_t)env * ly.rec;
+  int* reci = reinterpret_cast<int*>(rec);
+  for (int i = lane; i < ly.o_a; i += 32) rec[i] = 0.f;                 // status, support / active / unary masks
+  for (int i = ly.o_vbar + lane; i < ly.o_lam + 8; i += 32) rec[i] = 0.f;
+  for (int i = lane; i < ly.W * ly.nw; i += 32) rec[ly.o_rbm + i] = 0.f;   // the new anchor slot observes nothing
+  for (int k = lane; k < ly.W; k += 32) reci[ly.o_lct + k] = -1;
+  __syncwarp();
+  if (lane == 0) reci[ly.o_k0] = c - 1;                                  // its window restarts with one pose
+  if (lane < 3) {
+    const float a = init_pose ? init_pose[(size_t)lane * ly.N + env] : 0.f;
+    rec[ly.o_a + lane] = a;
+    rec[ly.o_vbar + lane] = a;
+    rec[ly.o_lam + (lane * (lane + 1) / 2) + lane] = pr.om_prior[lane];
+  }
+}
+
 // poses[3][W][N] = a (+) e_k for k < c, else 0
 __global__ void slam_poses_kernel(Layout ly, const float* state, int head, int c, float* poses) {
   const int env = blockIdx.x * blockDim.x + threadIdx.x;
   if (env >= ly.N) return;
   const float* rec = state + (size_t)env * ly.rec;
   const float ax = rec[ly.o_a], ay = rec[ly.o_a + 1], at = rec[ly.o_a + 2];
+  const int k0 = reinterpret_cast<const int*>(rec)[ly.o_k0];
+  c -= k0;
+  head = (head + k0) % ly.W;
   float sn, cn;
   sincos_pi(at, &sn, &cn);
   for (int k = 0; k < ly.W; ++k) {
@@ -476,6 +506,15 @@ int slam_set_unary(slam_ctx* c, const float* pose, const float* info, const int3
   if ((pose == nullptr) != (info == nullptr)) return fail(c, SLAM_EINVAL, "pose and info must both be given (or both NULL to cancel)");
   c->un_pose = pose; c->un_info = info; c->un_valid = pose ? valid : nullptr;
   return SLAM_OK;
+}
+
+int slam_reset_envs(slam_ctx* c, const int32_t* mask, const float* init_pose) {
+  if (!c || !mask) return c ? fail(c, SLAM_EINVAL, "mask is NULL") : SLAM_EINVAL;
+  const int threads = 256, blocks = (int)(((size_t)c->ly.N * 32 + threads - 1) / threads);
+  slam_reset_envs_kernel<<<blocks, threads, 0, c->stream>>>(c->ly, c->pr, c->state, c->count, mask, init_pose);
+  c->launches++;
+  c->cov_valid = false;
+  return check_cuda(c, "slam_reset_envs");
 }
 
 int slam_observe_first(slam_ctx* c, const uint32_t* rb_mask, const float* rb_meas) {

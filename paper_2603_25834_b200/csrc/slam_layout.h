@@ -19,7 +19,7 @@ struct Layout {
   int np, pad;         // matrix dimension padded to a multiple of 4 (pad dummy rows before the newest pose)
   // record (32-bit words)
   int rec;             // record stride
-  int o_status, o_pm, o_lm, o_act, o_um, o_a, o_e, o_m, o_zodo, o_lct, o_zlc, o_rbm, o_zrb, o_zun, o_omun, o_vbar, o_g, o_lam;
+  int o_status, o_k0, o_pm, o_lm, o_act, o_um, o_a, o_e, o_m, o_zodo, o_lct, o_zlc, o_rbm, o_zrb, o_zun, o_omun, o_vbar, o_g, o_lam;
   // shared memory per warp (32-bit words)
   int s_scr, s_st, s_zodo, s_zlc, s_lct, s_cs, s_rbm, s_first, s_rbase, s_amask, s_ssup, s_sidx, s_sds, s_H;
   int mw;              // 32-bit words of an active-row-pair mask (np/2 + 1 bits)
@@ -43,6 +43,7 @@ static inline Layout make_layout(int N, int W, int L, int cap, int wpc) {
   y.np = (y.n + 3) & ~3; y.pad = y.np - y.n;
   int n = y.n, o = 0;
   y.o_status = o; o += 1;
+  y.o_k0 = o; o += 1;   // NEXT-2: first live slot of this environment (0 unless it was reset mid-run)
   y.o_pm = o; o += 2;
   y.o_lm = o; o += 2;
   y.o_act = o; o += 2;

@@ -40,6 +40,7 @@ class Config:
     p_lc: float     # loop-closure probability per step
     seed: int = 0
     p_unary: float = 0.0   # NEXT-1: probability of a scan-match style absolute-pose measurement per step
+    p_reset: float = 0.0   # NEXT-2: probability of an episode reset (SLAM restarts at the true pose) per step
 
 
 # BASELINE.json `configs`, in order.  Config 4 is a sweep over N; `config4(N)` builds one point.
@@ -155,6 +156,8 @@ def generate(cfg: Config, *, noise_scale: float = 1.0, dtype=np.float32, env_ids
     un_valid = np.zeros((T, N), np.int32) if cfg.p_unary > 0 else None
     un_pose = np.zeros((T, 3, N), dtype) if cfg.p_unary > 0 else None
     un_info = np.zeros((T, 6, N), dtype) if cfg.p_unary > 0 else None
+    reset = np.zeros((T, N), np.int32) if cfg.p_reset > 0 else None
+    reset_pose = np.zeros((T, 3, N), dtype) if cfg.p_reset > 0 else None
 
     for l in range(L):
         lm[0, l] = (2.0 * rng.uniform() - 1.0) * LM_BOX_HALF
@@ -215,5 +218,13 @@ def generate(cfg: Config, *, noise_scale: float = 1.0, dtype=np.float32, env_ids
             un_pose[t - 1] = np.where(has[None, :], zu, 0.0)
             un_info[t - 1] = np.where(has[None, :], info, 0.0)
 
-    return dict(un_valid=un_valid, un_pose=un_pose, un_info=un_info, odom=odom, lc_back=lc_back, lc_meas=lc_meas, rb_mask=rb_mask, rb_meas=rb_meas,
+        if cfg.p_reset > 0:
+            # 6. (only when p_reset > 0, drawn last): the estimator of this environment restarts BEFORE the
+            #    push of step t at the true pose GT_{t-1} (a new episode); not on the first two steps
+            q = rng.uniform()
+            has = (q < cfg.p_reset) & (t > 2)
+            reset[t - 1] = has.astype(np.int32)
+            reset_pose[t - 1] = np.where(has[None, :], gt[t - 1], 0.0)
+
+    return dict(reset=reset, reset_pose=reset_pose, un_valid=un_valid, un_pose=un_pose, un_info=un_info, odom=odom, lc_back=lc_back, lc_meas=lc_meas, rb_mask=rb_mask, rb_meas=rb_meas,
                 gt=gt, lm=lm, env_ids=env_ids, cfg=cfg, T=T)

@@ -17,6 +17,9 @@ def to_dev(data, device="cuda:0"):
         d["un_valid"] = torch.from_numpy(np.ascontiguousarray(data["un_valid"], dtype=np.int32)).to(device)
         d["un_pose"] = torch.from_numpy(np.ascontiguousarray(data["un_pose"], dtype=np.float32)).to(device)
         d["un_info"] = torch.from_numpy(np.ascontiguousarray(data["un_info"], dtype=np.float32)).to(device)
+    if data.get("reset") is not None:
+        d["reset"] = torch.from_numpy(np.ascontiguousarray(data["reset"], dtype=np.int32)).to(device)
+        d["reset_pose"] = torch.from_numpy(np.ascontiguousarray(data["reset_pose"], dtype=np.float32)).to(device)
     return d
 
 
@@ -37,6 +40,8 @@ def run_gpu(slam, data, iters, fused=True, steps=None, want_poses=True):
     for t in range(1, T + 1):
         args = (dev["odom"][t - 1], dev["lc_back"][t - 1], dev["lc_meas"][t - 1],
                 dev["rb_mask"][t] if L else None, dev["rb_meas"][t] if L else None)
+        if "reset" in dev:
+            slam.reset_envs(dev["reset"][t - 1], dev["reset_pose"][t - 1])
         if "un_valid" in dev:
             slam.set_unary(dev["un_pose"][t - 1], dev["un_info"][t - 1], dev["un_valid"][t - 1])
         if fused and not want_poses:

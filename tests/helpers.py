@@ -31,6 +31,8 @@ def drive(orc, data, env, iters, on_step=None, steps=None):
     out = []
     for t in range(1, T + 1):
         odom, back, zlc, valid, zrb = step_inputs(data, t, env)
+        if data.get("reset") is not None and data["reset"][t - 1, env]:
+            orc.reset(data["reset_pose"][t - 1, :, env].astype(np.float64))
         orc.push(odom, back, zlc, valid, zrb)
         un = unary_inputs(data, t, env)
         if un is not None:

@@ -278,3 +278,18 @@ def test_unary_pose_factor_next1(W, L, p_lc):
     plain = synth.generate(synth.Config("pl", N=40, W=W, L=L, iters=2, T=50, p_lc=p_lc, seed=17))
     ref_plain = oracle.run_batch(plain, cfg.iters, want=("logdet",))
     assert ref["logdet"][-1].mean() < ref_plain["logdet"][-1].mean() - 1.0
+
+
+@pytest.mark.parametrize("W,L,p_lc", [(7, 0, 0.3), (6, 6, 0.2)])
+def test_per_env_reset_next2(W, L, p_lc):
+    """NEXT-2: slam_reset_envs restarts single environments mid-run while the others keep their windows."""
+    cfg = synth.Config("rs", N=60, W=W, L=L, iters=2, T=70, p_lc=p_lc, seed=23, p_reset=0.05, p_unary=0.1)
+    data = synth.generate(cfg)
+    assert data["reset"].sum() > 50
+    ref = oracle.run_batch(data, cfg.iters)
+    assert ref["bad"] == 0
+    gpu = run_gpu(_slam(cfg.N, W, L), data, cfg.iters, fused=False)
+    assert (gpu["status"] == 0).all()
+    _check(gpu, ref)
+    fused = run_gpu(_slam(cfg.N, W, L), data, cfg.iters, fused=True, want_poses=False)
+    assert np.array_equal(fused["cov"], gpu["cov"]) and np.array_equal(fused["logdet"], gpu["logdet"])

@@ -526,3 +526,40 @@ def test_unary_linear_gaussian_equals_brute_force():
         if o.count == W:
             o.set_state(o.state() + rng.normal(size=o.n) * 0.1)
             o.marginalize()
+
+
+# ----------------------------------------------------------------------------- NEXT-2: per-environment episode reset
+def test_reset_restarts_the_estimator_like_a_fresh_run():
+    """A reset at step t0 at the true pose must give exactly what a fresh estimator started there gives
+    (the batch driver's reset path against single-environment runs), and noise-free recovery must
+    survive resets."""
+    cfg = synth.Config("rs", N=3, W=6, L=4, iters=2, T=40, p_lc=0.3, seed=19, p_reset=0.08)
+    data = synth.generate(cfg)
+    assert data["reset"].sum() >= 3
+    res = oracle.run_batch(data, cfg.iters)
+    for env in range(cfg.N):
+        recs = drive(Oracle(cfg.W, cfg.L), data, env, cfg.iters)
+        for t, rec in enumerate(recs):
+            assert np.allclose(res["cov"][t, env], rec["cov"], rtol=1e-12, atol=0)
+        # after the LAST reset the run equals a fresh estimator initialised at that pose
+        ts = np.where(data["reset"][:, env])[0]
+        if len(ts) == 0:
+            continue
+        t0 = ts[-1]                                   # reset before the push of step t0+1
+        o = Oracle(cfg.W, cfg.L)
+        o.reset(data["reset_pose"][t0, :, env].astype(np.float64))
+        for t in range(t0 + 1, cfg.T + 1):
+            o.push(*step_inputs(data, t, env))
+            o.solve(cfg.iters)
+            S, ld = o.cov()
+            assert np.allclose(S, res["cov"][t - 1, env], rtol=1e-12, atol=0)
+            if o.count == cfg.W:
+                o.marginalize()
+    nf = synth.generate(cfg, noise_scale=0.0, dtype=np.float64)
+    for env in range(cfg.N):
+        for rec in drive(Oracle(cfg.W, cfg.L), nf, env, 2):
+            c = rec["count"]
+            gt = nf["gt"][rec["t"] - c + 1: rec["t"] + 1, :, env]
+            err = rec["poses"][:c] - gt
+            err[:, 2] = fullbatch.wrap(err[:, 2])
+            assert rec["step"] < 1e-10 and np.abs(err).max() < 1e-9
