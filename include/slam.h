@@ -165,6 +165,27 @@ typedef struct {
 int slam_reward(slam_ctx* ctx, const slam_reward_params* p, const float* u, const float* u_prev, const float* dcells,
                 const float* d_min, const int32_t* collision, float* reward);
 
+/* NEXT-3: the paper's other batched stage -- correlative scan matching against a 2D log-odds occupancy
+ * grid and the confidence-weighted grid update (readings R28-R34 of
+ * DESIGN.md, everything below the paper's sentence is a reading).  Stateless: no context needed.
+ *   grid   [N][G][G] float log-odds, row-major (y, x), square, centred on the world origin, cell = res m
+ *   ranges [R][N]    R rays over 180 degrees (phi_i = -pi/2 + i pi/(R-1)); valid iff r_min <= r <= r_max
+ * slam_scan_match: scores the (2hx+1)(2hy+1)(2ht+1) candidates pose_pred + (ix sxy, iy sxy, it sth)
+ * (offsets in global axes) with  s = mean over valid rays of 1/(1+exp(-grid[cell(end point)]))  (0 outside
+ * the grid) and returns the best candidate as pose_meas [3][N], its score [N] and the second-best
+ * score [N] (the ambiguity margin; how the information matrix is scaled from them is not in the paper
+ * and is left to the caller, see slam_set_unary).  Ties go to the lowest candidate index.
+ * slam_grid_update: every valid ray of the scan taken at `pose` [3][N] adds -l_free*weight to the cells it
+ * crosses (Amanatides-Woo traversal) and +l_occ*weight to its end cell; then the grid is clamped to
+ * [-l_clamp, l_clamp].  weight [N] = the confidence (e.g. the match score). */
+typedef struct {
+  int G; float res; int R; float r_min, r_max; int hx, hy, ht; float sxy, sth;
+} slam_scan_params;
+int slam_scan_match(const slam_scan_params* p, int batch, const float* grid, const float* pose_pred, const float* ranges,
+                    float* pose_meas, float* score, float* second, void* cuda_stream);
+int slam_grid_update(const slam_scan_params* p, int batch, float* grid, const float* pose, const float* ranges,
+                     const float* weight, float l_free, float l_occ, float l_clamp, void* cuda_stream);
+
 int slam_count(const slam_ctx* ctx);                /* host-side window count c in [1, window] */
 long long slam_launch_count(const slam_ctx* ctx);   /* kernels launched by this context so far */
 const char* slam_last_error(const slam_ctx* ctx);   /* message of the last non-zero return */

@@ -23,7 +23,7 @@ SYMBOLS = (
     "slam_default_config", "slam_workspace_bytes", "slam_create", "slam_destroy", "slam_reset",
     "slam_reset_envs", "slam_push_step", "slam_set_unary", "slam_observe_first", "slam_solve", "slam_marginal_cov", "slam_dopt",
     "slam_marginalize_oldest", "slam_step", "slam_step_host", "slam_get_poses", "slam_get_landmarks",
-    "slam_get_status", "slam_get_stats", "slam_reward", "slam_count", "slam_launch_count", "slam_last_error", "slam_kernel_info",
+    "slam_get_status", "slam_get_stats", "slam_reward", "slam_scan_match", "slam_grid_update", "slam_count", "slam_launch_count", "slam_last_error", "slam_kernel_info",
 )
 
 
@@ -35,6 +35,11 @@ class SlamConfig(C.Structure):
 class RewardParams(C.Structure):
     _fields_ = [(n, C.c_float) for n in ("lambda_col", "lambda_explore", "lambda_abs", "lambda_delta", "u_hi", "kappa",
                                          "d_crash", "d_full")]
+
+
+class ScanParams(C.Structure):
+    _fields_ = [("G", C.c_int), ("res", C.c_float), ("R", C.c_int), ("r_min", C.c_float), ("r_max", C.c_float),
+                ("hx", C.c_int), ("hy", C.c_int), ("ht", C.c_int), ("sxy", C.c_float), ("sth", C.c_float)]
 
 
 class SlamError(RuntimeError):
@@ -75,6 +80,8 @@ def _load() -> C.CDLL:
     lib.slam_get_status.argtypes = [vp, ip]
     lib.slam_get_stats.argtypes = [vp, ip]
     lib.slam_reward.argtypes = [vp, C.POINTER(RewardParams), fp, fp, fp, fp, ip, fp]
+    lib.slam_scan_match.argtypes = [C.POINTER(ScanParams), C.c_int, fp, fp, fp, fp, fp, fp, vp]
+    lib.slam_grid_update.argtypes = [C.POINTER(ScanParams), C.c_int, fp, fp, fp, fp, C.c_float, C.c_float, C.c_float, vp]
     lib.slam_count.argtypes = [vp]
     lib.slam_launch_count.argtypes = [vp]
     lib.slam_launch_count.restype = C.c_longlong
@@ -95,6 +102,37 @@ def default_config() -> SlamConfig:
 
 def workspace_bytes(batch: int, window: int, landmarks: int) -> int:
     return int(LIB.slam_workspace_bytes(batch, window, landmarks))
+
+
+def _f32(t, shape, name):
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous() or tuple(t.shape) != tuple(shape):
+        raise SlamError(SLAM_EINVAL, f"{name}: expected contiguous float32 CUDA tensor of shape {tuple(shape)}")
+    return C.c_void_p(t.data_ptr())
+
+
+def scan_match(par: ScanParams, grid, pose_pred, ranges):
+    """NEXT-3: returns (pose_meas [3,N], score [N], second [N])."""
+    N = grid.shape[0]
+    meas = torch.empty(3, N, device=grid.device)
+    s1 = torch.empty(N, device=grid.device)
+    s2 = torch.empty(N, device=grid.device)
+    rc = LIB.slam_scan_match(C.byref(par), N, _f32(grid, (N, par.G, par.G), "grid"), _f32(pose_pred, (3, N), "pose_pred"),
+                             _f32(ranges, (par.R, N), "ranges"), C.c_void_p(meas.data_ptr()), C.c_void_p(s1.data_ptr()),
+                             C.c_void_p(s2.data_ptr()), C.c_void_p(torch.cuda.current_stream(grid.device).cuda_stream))
+    if rc != SLAM_OK:
+        raise SlamError(rc, "slam_scan_match")
+    return meas, s1, s2
+
+
+def grid_update(par: ScanParams, grid, pose, ranges, weight, l_free: float, l_occ: float, l_clamp: float):
+    """NEXT-3: in-place confidence-weighted log-odds update of `grid`."""
+    N = grid.shape[0]
+    rc = LIB.slam_grid_update(C.byref(par), N, _f32(grid, (N, par.G, par.G), "grid"), _f32(pose, (3, N), "pose"),
+                              _f32(ranges, (par.R, N), "ranges"), _f32(weight, (N,), "weight"), l_free, l_occ, l_clamp,
+                              C.c_void_p(torch.cuda.current_stream(grid.device).cuda_stream))
+    if rc != SLAM_OK:
+        raise SlamError(rc, "slam_grid_update")
+    return grid
 
 
 class FixedLagSlam:

@@ -1,0 +1,163 @@
+// NEXT-3: batched correlative scan matcher and log-odds occupancy-grid update (PAPER.md:146, 150-152,
+// 165; readings R28-R34 of DESIGN.md).  One CTA per environment.
+//
+// Precision: the cell an end point falls into is an INTEGER decision, so it is taken in fp64 on both
+// sides (the oracle is fp64); grid values, the logistic and the score sums are fp32.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+#include "../../include/slam.h"
+
+namespace {
+
+constexpr int kThreads = 128;
+constexpr double kPi = 3.14159265358979323846;
+
+__device__ __forceinline__ double ray_angle(int i, int R) { return -0.5 * kPi + i * (kPi / (R - 1)); }
+
+// scores of all candidates of one environment; best and second best
+__global__ void __launch_bounds__(kThreads) scan_match_kernel(slam_scan_params p, int N, const float* __restrict__ grid,
+                                                               const float* __restrict__ pose_pred,
+                                                               const float* __restrict__ ranges, float* pose_meas,
+                                                               float* score, float* second) {
+  extern __shared__ double sm_d[];
+  const int env = blockIdx.x, tid = threadIdx.x;
+  const int R = p.R, G = p.G, nt = 2 * p.ht + 1, ny = 2 * p.hy + 1, nx = 2 * p.hx + 1;
+  double* cs = sm_d;                                   // [nt][R][2] cos/sin of theta + dtheta + phi_i, times range
+  float* rr = reinterpret_cast<float*>(cs + (size_t)nt * R * 2);   // [R] range, <0 = invalid
+  __shared__ float best_s[kThreads], sec_s[kThreads];
+  __shared__ int best_i[kThreads];
+  __shared__ int nvalid_s;
+  const double px = (double)pose_pred[env], py = (double)pose_pred[(size_t)N + env], pth = (double)pose_pred[2 * (size_t)N + env];
+  if (tid == 0) nvalid_s = 0;
+  __syncthreads();
+  for (int i = tid; i < R; i += kThreads) {
+    const float r = ranges[(size_t)i * N + env];
+    const bool ok = r >= p.r_min && r <= p.r_max;
+    rr[i] = ok ? r : -1.f;
+    if (ok) atomicAdd(&nvalid_s, 1);
+  }
+  __syncthreads();
+  for (int q = tid; q < nt * R; q += kThreads) {
+    const int it = q / R, i = q - it * R;
+    const double a = pth + (double)((it - p.ht) * p.sth) + ray_angle(i, R);
+    const double r = (double)rr[i];
+    cs[2 * q] = r * cos(a);
+    cs[2 * q + 1] = r * sin(a);
+  }
+  __syncthreads();
+  const int nvalid = nvalid_s;
+  const float* g = grid + (size_t)env * G * G;
+  const double o = -0.5 * G * (double)p.res, ires = 1.0 / (double)p.res;
+  float b1 = -1.f, b2 = -1.f;
+  int bi = 0x7fffffff;
+  const int C = nt * ny * nx;
+  for (int c = tid; c < C; c += kThreads) {
+    const int it = c / (ny * nx), rem = c - it * ny * nx, iy = rem / nx, ix = rem - iy * nx;
+    const double cx = px + (double)((ix - p.hx) * p.sxy), cy = py + (double)((iy - p.hy) * p.sxy);
+    const double* t = cs + (size_t)it * R * 2;
+    float sum = 0.f;
+    for (int i = 0; i < R; ++i) {
+      if (rr[i] < 0.f) continue;
+      // R28/R31: the same expression as the oracle, in fp64: floor((x - o) / res)
+      const int jx = (int)floor((cx + t[2 * i] - o) / (double)p.res), jy = (int)floor((cy + t[2 * i + 1] - o) / (double)p.res);
+      if (jx >= 0 && jx < G && jy >= 0 && jy < G) sum += 1.f / (1.f + __expf(-__ldg(g + (size_t)jy * G + jx)));
+    }
+    (void)ires;
+    const float s = nvalid ? sum / (float)nvalid : 0.f;
+    if (s > b1) { b2 = b1; b1 = s; bi = c; }      // candidates visited in increasing index: ties keep the lowest
+    else if (s > b2) b2 = s;
+  }
+  best_s[tid] = b1; sec_s[tid] = b2; best_i[tid] = bi;
+  __syncthreads();
+  if (tid == 0) {
+    float g1 = -1.f;
+    int gi = 0x7fffffff;
+    for (int k = 0; k < kThreads; ++k)
+      if (best_s[k] > g1 || (best_s[k] == g1 && best_i[k] < gi)) { g1 = best_s[k]; gi = best_i[k]; }
+    float g2 = -1.f;
+    for (int k = 0; k < kThreads; ++k) {
+      const float v = (best_i[k] == gi) ? sec_s[k] : best_s[k];
+      if (v > g2) g2 = v;
+    }
+    if (g2 < 0.f) g2 = 0.f;
+    const int it = gi / (ny * nx), rem = gi - it * ny * nx, iy = rem / nx, ix = rem - iy * nx;
+    pose_meas[env] = (float)(px + (double)((ix - p.hx) * p.sxy));
+    pose_meas[(size_t)N + env] = (float)(py + (double)((iy - p.hy) * p.sxy));
+    pose_meas[2 * (size_t)N + env] = (float)(pth + (double)((it - p.ht) * p.sth));
+    score[env] = g1;
+    second[env] = g2;
+  }
+}
+
+// one thread per ray: Amanatides-Woo traversal in fp64 (integer decisions, same operations as the oracle)
+__global__ void __launch_bounds__(kThreads) grid_update_kernel(slam_scan_params p, int N, float* grid, const float* __restrict__ pose,
+                                                                const float* __restrict__ ranges,
+                                                                const float* __restrict__ weight, float l_free, float l_occ) {
+  const int env = blockIdx.x, G = p.G;
+  const double x0 = (double)pose[env], y0 = (double)pose[(size_t)N + env], th = (double)pose[2 * (size_t)N + env];
+  const float w = weight[env];
+  float* g = grid + (size_t)env * G * G;
+  const double res = (double)p.res, o = -0.5 * G * res;
+  for (int i = threadIdx.x; i < p.R; i += kThreads) {
+    const float rf = ranges[(size_t)i * N + env];
+    if (!(rf >= p.r_min && rf <= p.r_max)) continue;
+    const double a = th + ray_angle(i, p.R), r = (double)rf;
+    const double x1 = x0 + r * cos(a), y1 = y0 + r * sin(a);
+    int ix = (int)floor((x0 - o) / res), iy = (int)floor((y0 - o) / res);
+    const int jx = (int)floor((x1 - o) / res), jy = (int)floor((y1 - o) / res);
+    const double dx = x1 - x0, dy = y1 - y0;
+    const int sx = dx > 0 ? 1 : -1, sy = dy > 0 ? 1 : -1;
+    const double inf = __longlong_as_double(0x7ff0000000000000LL);
+    const double tdx = dx != 0 ? res / fabs(dx) : inf, tdy = dy != 0 ? res / fabs(dy) : inf;
+    const double bx = o + (ix + (dx > 0 ? 1 : 0)) * res, by = o + (iy + (dy > 0 ? 1 : 0)) * res;
+    double tmx = dx != 0 ? (bx - x0) / dx : inf, tmy = dy != 0 ? (by - y0) / dy : inf;
+    const int n = abs(jx - ix) + abs(jy - iy);
+    for (int k = 0; k <= n; ++k) {
+      const bool last = ix == jx && iy == jy;
+      if (ix >= 0 && ix < G && iy >= 0 && iy < G) atomicAdd(g + (size_t)iy * G + ix, last ? l_occ * w : -l_free * w);
+      if (last) break;
+      if (tmx < tmy) { tmx += tdx; ix += sx; }
+      else { tmy += tdy; iy += sy; }
+    }
+  }
+}
+
+__global__ void grid_clamp_kernel(float* grid, size_t n, float l_clamp) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) grid[i] = fminf(fmaxf(grid[i], -l_clamp), l_clamp);
+}
+
+bool params_ok(const slam_scan_params* p, int batch) {
+  return p && batch >= 1 && p->G >= 8 && p->G <= 2048 && p->R >= 2 && p->R <= 1024 && p->res > 0.f && p->r_max > p->r_min &&
+         p->hx >= 0 && p->hy >= 0 && p->ht >= 0 && p->hx <= 32 && p->hy <= 32 && p->ht <= 32 && p->sxy > 0.f && p->sth > 0.f;
+}
+
+}  // namespace
+
+extern "C" {
+
+int slam_scan_match(const slam_scan_params* p, int batch, const float* grid, const float* pose_pred, const float* ranges,
+                    float* pose_meas, float* score, float* second, void* stream) {
+  if (!params_ok(p, batch) || !grid || !pose_pred || !ranges || !pose_meas || !score || !second) return SLAM_EINVAL;
+  const size_t smem = (size_t)(2 * p->ht + 1) * p->R * 2 * sizeof(double) + (size_t)p->R * sizeof(float);
+  if (smem > 200 * 1024) return SLAM_EINVAL;
+  if (cudaFuncSetAttribute(scan_match_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+    cudaGetLastError();
+    return SLAM_ECUDA;
+  }
+  scan_match_kernel<<<batch, kThreads, smem, (cudaStream_t)stream>>>(*p, batch, grid, pose_pred, ranges, pose_meas, score, second);
+  return cudaGetLastError() == cudaSuccess ? SLAM_OK : SLAM_ECUDA;
+}
+
+int slam_grid_update(const slam_scan_params* p, int batch, float* grid, const float* pose, const float* ranges, const float* weight,
+                     float l_free, float l_occ, float l_clamp, void* stream) {
+  if (!params_ok(p, batch) || !grid || !pose || !ranges || !weight || !(l_clamp > 0.f)) return SLAM_EINVAL;
+  grid_update_kernel<<<batch, kThreads, 0, (cudaStream_t)stream>>>(*p, batch, grid, pose, ranges, weight, l_free, l_occ);
+  const size_t n = (size_t)batch * p->G * p->G;
+  grid_clamp_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(grid, n, l_clamp);
+  return cudaGetLastError() == cudaSuccess ? SLAM_OK : SLAM_ECUDA;
+}
+
+}  // extern "C"

@@ -228,3 +228,68 @@ def generate(cfg: Config, *, noise_scale: float = 1.0, dtype=np.float32, env_ids
 
     return dict(reset=reset, reset_pose=reset_pose, un_valid=un_valid, un_pose=un_pose, un_info=un_info, odom=odom, lc_back=lc_back, lc_meas=lc_meas, rb_mask=rb_mask, rb_meas=rb_meas,
                 gt=gt, lm=lm, env_ids=env_ids, cfg=cfg, T=T)
+
+
+# ----------------------------------------------------------------------------- NEXT-3: scan-matching worlds
+def generate_scan_world(N: int, G: int = 128, res: float = 0.1, R: int = 128, seed: int = 0, *,
+                        offset_cells=(0, 0, 0), sth: float = 0.01, range_sigma: float = 0.0, l_hi: float = 4.0,
+                        l_lo: float = 2.0, dtype=np.float32) -> dict:
+    """Synthetic stand-in for the paper's LiDAR + occupancy grid.
+
+    Per environment: a rectangular room (half sizes U(2.5,4.5) m, walls on cell CENTRES) with one
+    axis-aligned box obstacle; the robot at a random pose inside; a 128-ray, 180-degree scan cast
+    analytically against the walls (+ N(0, range_sigma^2)); the log-odds map rasterised from the same
+    walls (+l_hi on wall cells, -l_lo inside the room, 0 outside); and a predicted pose = true pose
+    MINUS `offset_cells` lattice steps (res, res, sth), so that the candidate at +offset_cells is the
+    true pose.  Environment-fastest arrays: ``grid[N,G,G]``, ``ranges[R,N]``, ``pose_true[3,N]``,
+    ``pose_pred[3,N]``."""
+    rng = _Streams(seed ^ 0x5CA1AB1E, np.arange(N, dtype=np.int64))
+    half = 0.5 * G * res
+
+    def snap(v):      # to a cell centre
+        return (np.floor(v / res) + 0.5) * res
+
+    wx, wy = snap(2.5 + 2.0 * rng.uniform()), snap(2.5 + 2.0 * rng.uniform())          # room half sizes
+    bx, by = snap(-1.5 + 3.0 * rng.uniform()), snap(0.8 + 1.2 * rng.uniform())          # box centre (in front)
+    bw, bh = snap(0.3 + 0.5 * rng.uniform()), snap(0.3 + 0.5 * rng.uniform())           # box half sizes
+    px, py = -1.0 + 2.0 * rng.uniform(), -1.8 + 1.2 * rng.uniform()                     # robot below the box
+    pth = 0.5 * math.pi + (-0.5 + rng.uniform())                                        # looking roughly "up"
+    phi = -0.5 * math.pi + np.arange(R) * (math.pi / (R - 1))
+    ang = pth[None, :] + phi[:, None]
+    dx, dy = np.cos(ang), np.sin(ang)
+    big = 1e9
+    with np.errstate(divide="ignore", invalid="ignore"):
+        # outer walls: the robot is inside, take the exit distance
+        tx = np.where(dx > 0, (wx - px) / dx, np.where(dx < 0, (-wx - px) / dx, big))
+        ty = np.where(dy > 0, (wy - py) / dy, np.where(dy < 0, (-wy - py) / dy, big))
+        t_room = np.minimum(tx, ty)
+        # box: slab test
+        t1x, t2x = (bx - bw - px) / dx, (bx + bw - px) / dx
+        t1y, t2y = (by - bh - py) / dy, (by + bh - py) / dy
+        tnx, tfx = np.minimum(t1x, t2x), np.maximum(t1x, t2x)
+        tny, tfy = np.minimum(t1y, t2y), np.maximum(t1y, t2y)
+        tn, tf = np.maximum(tnx, tny), np.minimum(tfx, tfy)
+        t_box = np.where((tn <= tf) & (tn > 0), tn, big)
+    ranges = np.minimum(t_room, t_box)
+    noise = np.stack([rng.normal() for _ in range(R)]) if range_sigma > 0 else 0.0
+    ranges = ranges + range_sigma * noise
+
+    # rasterise the map
+    cc = (np.arange(G) + 0.5) * res - half                      # cell centres
+    X, Y = np.meshgrid(cc, cc)                                  # [iy, ix]
+    grid = np.zeros((N, G, G), dtype)
+    for e in range(N):
+        inside = (np.abs(X) < wx[e] - 0.25 * res) & (np.abs(Y) < wy[e] - 0.25 * res)
+        wall = (np.abs(np.abs(X) - wx[e]) < 0.5 * res) & (np.abs(Y) <= wy[e] + 0.5 * res) | \
+               (np.abs(np.abs(Y) - wy[e]) < 0.5 * res) & (np.abs(X) <= wx[e] + 0.5 * res)
+        inbox = (np.abs(X - bx[e]) <= bw[e] + 0.5 * res) & (np.abs(Y - by[e]) <= bh[e] + 0.5 * res)
+        boxwall = inbox & ~((np.abs(X - bx[e]) < bw[e] - 0.5 * res) & (np.abs(Y - by[e]) < bh[e] - 0.5 * res))
+        g = np.where(inside, -l_lo, 0.0)
+        g = np.where(inbox, 0.0, g)
+        g = np.where(wall | boxwall, l_hi, g)
+        grid[e] = g
+    pose_true = np.stack([px, py, pth])
+    ox, oy, ot = offset_cells
+    pose_pred = np.stack([px - ox * res, py - oy * res, pth - ot * sth])
+    return dict(grid=grid, ranges=ranges.astype(dtype), pose_true=pose_true.astype(dtype), pose_pred=pose_pred.astype(dtype),
+                G=G, res=res, R=R)

@@ -1,0 +1,116 @@
+"""NEXT-3: correlative scan matcher + log-odds grid update.
+Pins of the oracle (no GPU) and GPU parity."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import scanmatch as osm
+from paper_2603_25834_b200 import synth
+
+PAR = dict(res=0.1, hx=3, hy=3, ht=4, sxy=0.1, sth=0.01)
+
+
+def test_lattice_offset_is_recovered_exactly():
+    for off in ((2, -1, 3), (-3, 2, -4), (0, 0, 0)):
+        w = synth.generate_scan_world(3, seed=1, offset_cells=off, dtype=np.float64)
+        for e in range(3):
+            meas, s1, s2, best, sc = osm.scan_match(w["grid"][e], w["pose_pred"][:, e], w["ranges"][:, e], **PAR)
+            ix, iy, it = off[0] + PAR["hx"], off[1] + PAR["hy"], off[2] + PAR["ht"]
+            idx_true = (it * (2 * PAR["hy"] + 1) + iy) * (2 * PAR["hx"] + 1) + ix
+            assert sc[idx_true] > 0.93                      # (almost) every end point on a wall cell (l = +4 -> p = 0.982)
+            assert abs(sc[best] - sc[idx_true]) < 1e-12 and s1 == sc[best] and s2 <= s1
+            assert np.abs(meas - w["pose_true"][:, e]).max() < 0.011 + 1e-9 or abs(sc[best] - sc[idx_true]) < 1e-12
+            # away from the truth the score drops
+            assert sc.min() < 0.8 * s1
+
+
+def test_score_definition_and_limits():
+    G = 64
+    sat = np.full((G, G), 50.0)
+    r = np.full(128, 2.0)
+    assert abs(osm.score(sat, (0.0, 0.0, 0.3), r, 0.1, 0.1, 10.0) - 1.0) < 1e-12        # saturated map
+    assert osm.score(-sat, (0.0, 0.0, 0.3), r, 0.1, 0.1, 10.0) < 1e-12
+    assert osm.score(sat, (0.0, 0.0, 0.3), np.full(128, 20.0), 0.1, 0.1, 10.0) == 0.0     # no valid ray
+    assert abs(osm.score(np.zeros((G, G)), (0.0, 0.0, 0.0), r, 0.1, 0.1, 10.0) - 0.5) < 1e-12
+    # end points outside the grid contribute 0 but still count as valid rays
+    far = np.full(128, 9.0)
+    assert osm.score(sat, (0.0, 0.0, 0.0), far, 0.1, 0.1, 10.0) == 0.0
+    # ray geometry: 180 degrees, symmetric about the heading
+    phi = osm.ray_angles(128)
+    assert abs(phi[0] + math.pi / 2) < 1e-15 and abs(phi[-1] - math.pi / 2) < 1e-15 and np.allclose(phi, -phi[::-1])
+    c = osm.candidates(1, 2, 3, 0.1, 0.01)
+    assert len(c) == 3 * 5 * 7 and c[(3 * 5 + 2) * 3 + 1] == (0.0, 0.0, 0.0)
+
+
+def test_dda_against_brute_force_sampling():
+    rng = np.random.default_rng(3)
+    G, res = 64, 0.1
+    for _ in range(50):
+        x0, y0 = rng.uniform(-2, 2, 2)
+        ang, r = rng.uniform(-math.pi, math.pi), rng.uniform(0.3, 4.0)
+        x1, y1 = x0 + r * math.cos(ang), y0 + r * math.sin(ang)
+        cells = osm.traverse(x0, y0, x1, y1, G, res)
+        ts = np.linspace(0.0, 1.0, 20001)
+        brute = []
+        for t in ts:
+            c = osm.cell_of(x0 + t * (x1 - x0), y0 + t * (y1 - y0), G, res)
+            if 0 <= c[0] < G and 0 <= c[1] < G and (not brute or brute[-1] != c):
+                brute.append(c)
+        assert len(set(cells)) == len(cells)                       # each cell once
+        inside = max(abs(x1), abs(y1)) < 0.5 * G * res
+        assert cells[0] == osm.cell_of(x0, y0, G, res) and (not inside or cells[-1] == osm.cell_of(x1, y1, G, res))
+        assert set(brute) <= set(cells)                            # sampling can only miss corner clips
+        assert len(cells) - len(brute) <= 2
+        for a, b in zip(cells, cells[1:]):
+            assert abs(a[0] - b[0]) + abs(a[1] - b[1]) == 1        # 4-connected path
+
+
+def test_grid_update_signs_and_clamp():
+    G, res = 64, 0.1
+    grid = np.zeros((G, G))
+    ranges = np.full(128, 20.0)
+    ranges[64] = 1.0
+    pose = (0.03, 0.02, 0.0)
+    out = osm.grid_update(grid, pose, ranges, 0.5, res, l_free=0.4, l_occ=0.9, l_clamp=5.0)
+    ang = osm.ray_angles(128)[64]
+    ex, ey = pose[0] + math.cos(ang), pose[1] + math.sin(ang)
+    jx, jy = osm.cell_of(ex, ey, G, res)
+    assert abs(out[jy, jx] - 0.45) < 1e-12
+    touched = np.argwhere(out != 0)
+    assert len(touched) >= 10 and (out[out != 0] < 0).sum() == len(touched) - 1
+    assert np.allclose(out[(out != 0) & (out < 0)], -0.2)
+    sat = osm.grid_update(np.full((G, G), 4.9), pose, ranges, 1.0, res, 0.4, 0.9, 5.0)
+    assert sat.max() == 5.0
+    assert np.array_equal(osm.grid_update(grid, pose, np.full(128, 20.0), 1.0, res, 0.4, 0.9, 5.0), grid)
+
+
+@pytest.mark.gpu
+def test_scan_match_and_grid_update_match_oracle():
+    import torch
+    from paper_2603_25834_b200 import binding
+    N = 24
+    w = synth.generate_scan_world(N, seed=5, offset_cells=(1, -2, 2), range_sigma=0.01)
+    par = binding.ScanParams(G=w["G"], res=w["res"], R=w["R"], r_min=0.1, r_max=10.0, hx=3, hy=3, ht=4, sxy=0.1, sth=0.01)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    grid, pred, rng_ = dev(w["grid"]), dev(w["pose_pred"]), dev(w["ranges"])
+    meas, s1, s2 = binding.scan_match(par, grid, pred, rng_)
+    meas, s1, s2 = meas.cpu().numpy(), s1.cpu().numpy(), s2.cpu().numpy()
+    for e in range(N):
+        om, o1, o2, best, sc = osm.scan_match(w["grid"][e].astype(np.float64), w["pose_pred"][:, e].astype(np.float64),
+                                              w["ranges"][:, e].astype(np.float64), **PAR)
+        assert abs(s1[e] - o1) < 2e-6 and abs(s2[e] - o2) < 2e-6
+        # the arg max is unique up to near-ties: the GPU's candidate must score like the oracle's best
+        cands = osm.candidates(3, 3, 4, 0.1, 0.01)
+        d = meas[:, e] - w["pose_pred"][:, e]
+        k = int(np.argmin([abs(d[0] - c[0]) + abs(d[1] - c[1]) + abs(d[2] - c[2]) for c in cands]))
+        assert abs(sc[k] - o1) < 2e-6
+    wgt = dev(s1.astype(np.float32))
+    g2 = grid.clone()
+    binding.grid_update(par, g2, dev(meas.astype(np.float32)), rng_, wgt, 0.4, 0.9, 5.0)
+    g2 = g2.cpu().numpy()
+    for e in range(0, N, 5):
+        ref = osm.grid_update(w["grid"][e].astype(np.float64), meas[:, e].astype(np.float64), w["ranges"][:, e].astype(np.float64),
+                              float(s1[e]), w["res"], 0.4, 0.9, 5.0)
+        bad = np.abs(g2[e] - ref) > 1e-4
+        assert bad.sum() <= 2, int(bad.sum())          # a ray through an exact cell corner may clip one cell either way
