@@ -69,7 +69,7 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
     // estimate for the covariance: ONE call site per phase keeps the kernel small.
     const int nlin = iters + ((flags & F_COV) ? 1 : 0);
     if (nlin > 0) {
-      __syncthreads();
+      if (LOCK >= 0) __syncthreads();
       if (valid) {
         total = symbolic<TEAM>(ly, od, w, tm, lane, cc, mk, s);
         need = max(need, total);
@@ -122,7 +122,7 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
         }
       }
     }
-    __syncthreads();
+    if (LOCK >= -1) __syncthreads();
     if (valid) {
       if (io.last_pose && lane == 0) {  // newest pose in global coordinates: a (+) e_{c-1}
         float sn, cn;
