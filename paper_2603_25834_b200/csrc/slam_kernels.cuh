@@ -1,21 +1,22 @@
-// Hand-written sm_100a kernels of the batched fixed-lag SE(2) smoother (one WARP per environment).
+// Hand-written sm_100a kernels of the batched fixed-lag SE(2) smoother: device phases of the fused step
+// kernel (slam_api.cu).  A TEAM of 32/64/128 threads owns one environment; everything between loading
+// and storing its record lives in shared memory.
 //
-// Hot path (DESIGN.md "Kernels"): per environment and per step
+// Hot path (DESIGN.md section 7): per environment and per step
 //   S0 push        dead-reckoned guess + factor bookkeeping
 //   S1 linearise   residuals + SE(2) Jacobians of every live factor              (eq. (5))
-//   S2 assemble    H = Lambda + sum J'Omega J, b, in shared memory, envelope (skyline) storage
-//   S3 factor      left-looking envelope Cholesky, lanes over rows; the rhs rides along as an extra
-//                  row (forward solve for free); back substitution; additive update
+//   S2 assemble    H = Lambda + sum J'Omega J, b, in shared memory, envelope (skyline) storage in 4x4 tiles
+//   S3 factor      left-looking envelope Cholesky by 4-column blocks: row pairs per thread, 128-bit loads,
+//                  compact active-pair lists, K-split; the rhs rides along as an extra row (forward solve
+//                  for free); blocked back substitution; additive update
 //   S4 covariance  trailing 6x6 of L -> Sigma_t (global coords), ln det      (eq. (6))
 //   S5 marginalise re-anchor + Schur complement of the oldest pose on the prior's support
 //
-// Elimination order of the window variables (scalar offsets):
+// Elimination order of the window variables (scalar offsets), chosen per environment:
 //   [ passive landmarks | e_1 .. e_{W-2} (chain, 3 each) | observed landmarks | pad | newest pose e_{c-1} (3) | anchor a (3) ]
-// (pad = 0..3 dummy identity rows so that the dimension np is a multiple of 4: the factorisation
-// works on 4-column blocks with 128-bit shared-memory loads)
-// so that the covariance read-out needs only the trailing 6x6 of L, and the weakly determined
-// global anchor `a` (touched by the prior only) is never added into the well determined relative
-// blocks.  Row np of the envelope storage is the right-hand side b (row np+1 is its zero twin).
+// (pad = 0..3 dummy identity rows so that the dimension np is a multiple of 4) so that the covariance
+// read-out needs only the trailing 6x6 of L.  Poses are robot-centric (anchor frame), landmarks global
+// (reading R17b).  Row np of the envelope storage is the right-hand side b (row np+1 is its zero twin).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
