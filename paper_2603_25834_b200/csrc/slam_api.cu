@@ -18,7 +18,7 @@ using namespace slamk;
 // environments.  flags select the phases, so that the separate ABI calls and the fused slam_step share
 // the same device code and are bit-for-bit identical.
 template <int TEAM>
-__global__ void __launch_bounds__(TEAM == 128 ? 896 : (TEAM == 64 ? 512 : 256))
+__global__ void __launch_bounds__(TEAM == 128 ? 896 : 512)
 slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flags, int iters, StepIO io,
                  unsigned long long* stats, int mode, int* ovf) {
   extern __shared__ float4 smem4[];
@@ -318,7 +318,7 @@ static int pick_wpc(int W, int L, int team, int cap) {
   const Layout t = make_layout(1, W, L, cap, 1);
   const size_t wb = (size_t)t.warp_words * 4;
   int wpc = (int)((size_t)227 * 1024 / wb);
-  int maxt = team == 128 ? 7 : 8;   // 896 / 512 / 256 threads per CTA
+  int maxt = team == 128 ? 7 : (team == 64 ? 8 : 15);   // <= 896 / 512 / 480 threads per CTA (15 named barriers)
   const char* e = getenv("SLAM_MAX_WPC");
   if (e && atoi(e) >= 1 && atoi(e) < maxt) maxt = atoi(e);
   if (wpc > maxt) wpc = maxt;
