@@ -92,17 +92,19 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
 #pragma unroll 1
       for (int it = 0; it < nlin; ++it) {
         if (LOCK >= 1) __syncthreads();
-        if (valid) { assemble<TEAM>(ly, pr, od, rec, w, tm, lane, head, cc, mk, s, total); tm.sync(); }
+        // after the first factorisation the column blocks of the passive landmarks keep their factor
+        const int ncb = (valid && it > 0 && ly.lcache) ? od.npas >> 1 : 0;
+        if (valid) { assemble<TEAM>(ly, pr, od, rec, w, tm, lane, head, cc, mk, s, total, 4 * ncb); tm.sync(); }
         if (LOCK >= 2) __syncthreads();
         if (valid) {
           // When no column block has more than 32 active row pairs (every pose-only window), one warp
           // does the factorisation with shuffles and __syncwarp only: no named barriers, no
           // shared-memory exchange of the diagonal tile.  The other warps of the team wait.
           if (TEAM > 32 && single_warp) {
-            if (lane < 32) status |= cholesky<32>(ly, w, tm32, lane);
+            if (lane < 32) status |= cholesky<32>(ly, w, tm32, lane, ncb);
             tm.sync();
           } else {
-            status |= cholesky<TEAM>(ly, w, tm, lane);
+            status |= cholesky<TEAM>(ly, w, tm, lane, ncb);
           }
         }
         if (LOCK >= 3) __syncthreads();
@@ -390,6 +392,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   c->ly = make_layout(batch, window, landmarks, -1, wpc);
   c->ly.team = team;
   { const char* e = getenv("SLAM_LOCK"); if (e) c->ly.lock = atoi(e); }
+  { const char* e = getenv("SLAM_LCACHE"); if (e) c->ly.lcache = atoi(e); }
   const WsPlan p = plan(c->ly);
   if (workspace_bytes < p.total) { delete c; return SLAM_EINVAL; }
   for (int k = 0; k < 3; ++k) {
@@ -438,6 +441,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
     c->ly_small = make_layout(batch, window, landmarks, cap, wpc_s);
     c->ly_small.team = team;
     c->ly_small.lock = c->ly.lock;
+    c->ly_small.lcache = c->ly.lcache;
     c->smem_small = c->ly_small.warp_words * 4 * wpc_s;
     int occ_s = 0;
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_s, kernel_of(team), wpc_s * team, c->smem_small);

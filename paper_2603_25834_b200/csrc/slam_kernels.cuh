@@ -242,6 +242,15 @@ __device__ void load_env(const Layout& ly, const float* rec, const WS& w, const 
   mk.ls = (uint64_t)recu[ly.o_lm] | ((uint64_t)recu[ly.o_lm + 1] << 32);
   mk.act = (uint64_t)recu[ly.o_act] | ((uint64_t)recu[ly.o_act + 1] << 32);
   mk.um = ring_to_slot((uint64_t)recu[ly.o_um] | ((uint64_t)recu[ly.o_um + 1] << 32), head, W) & lowmask(c);
+  {  // the prior (Lambda, g, vbar) is first needed by assemble, thousands of cycles from here: pull it into L2 now
+    const int sp = 3 + 3 * __popcll(pm) + 2 * __popcll(mk.ls);
+    const int nl = ((sp * (sp + 1) >> 1) + 31) >> 5;  // 128-byte lines of the packed triangle
+    for (int i = lane; i < nl; i += TEAM) asm volatile("prefetch.global.L2 [%0];" ::"l"(rec + ly.o_lam + 32 * i));
+    if (lane < ((sp + 31) >> 5)) {
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(rec + ly.o_g + 32 * lane));
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(rec + ly.o_vbar + 32 * lane));
+    }
+  }
   tm.sync();
 }
 
@@ -461,6 +470,11 @@ __device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, const Team
   // active row pairs per 4-column block J: pair p (rows 2p, 2p+1; the rhs pair is p = np/2) takes part
   // in column J iff first <= 4J <= 2p.  Compact lists: aoff[J] (16 bit) offsets into alist (8-bit pair
   // indices, ascending, so the two diagonal pairs 2J and 2J+1 come first).  Built by the first warp.
+  if (lane < 32) {  // loop-closure mask for assemble
+    const uint32_t lo = __ballot_sync(FULLMASK, lane < c && w.lct[lane] >= 0);
+    const uint32_t hi = __ballot_sync(FULLMASK, lane + 32 < c && w.lct[lane + 32] >= 0);
+    if (lane == 0) { w.lct[ly.W] = (int)lo; w.lct[ly.W + 1] = (int)hi; }
+  }
   if (lane < 32) {
     const int G = np >> 2, NP = (np >> 1) + 1;
     unsigned short* aoff = reinterpret_cast<unsigned short*>(w.amask);
@@ -564,9 +578,20 @@ __device__ __forceinline__ void add_i_side(const WS& w, int n, int oi, const flo
 // Builds H and b (row n) at the current state.  `s` = prior support dimension.
 template <int TEAM>
 __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, const float* rec, const WS& w, const Team<TEAM>& tm, int lane, int head,
-                         int c, const Masks& mk, int s, int total) {
+                         int c, const Masks& mk, int s, int total, int cb) {
   const int W = ly.W, L = ly.L, n = ly.np;  // n: row index of the rhs
-  for (int t = lane; t < total; t += TEAM) w.H[t] = 0.f;
+  // cb > 0 (second and later linearisation of one call): the columns [0, cb) -- passive landmarks, which
+  // only the constant prior touches -- still hold their factor L from the previous factorisation; they are
+  // kept (see cholesky) and only the columns >= cb and the rhs rows are rebuilt.
+  if (cb == 0) {
+    for (int t = lane; t < total; t += TEAM) w.H[t] = 0.f;
+  } else {
+    for (int i = lane; i < n + 2; i += TEAM) {
+      const int lo = i < n ? max((int)w.first[i], cb) : 0, hi = (i | 3) + 1;
+      float4* z = reinterpret_cast<float4*>(w.H + w.rbase[i] + lo);
+      for (int t = 0; t < (hi - lo) >> 2; ++t) z[t] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+  }
   // cos/sin of every live pose (slot 0 is the frame itself)
   for (int k = lane; k < c; k += TEAM) {
     float sn = 0.f, cn = 1.f;
@@ -589,7 +614,7 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
   for (int l = lane; l < L; l += TEAM)
     if (!((mk.act >> l) & 1ull)) {
       const int o = off_lm(ly, od, l);
-      w.H[w.rbase[o] + o] = 1.0f; w.H[w.rbase[o + 1] + o + 1] = 1.0f;
+      if (o >= cb) { w.H[w.rbase[o] + o] = 1.0f; w.H[w.rbase[o + 1] + o + 1] = 1.0f; }
     }
   if (lane < ly.pad + (c < 2 ? 3 : 0)) {
     const int o = off_new(ly) - ly.pad + lane;
@@ -601,22 +626,49 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
     // flat over the packed triangle: coalesced, and every iteration is independent (memory-level
     // parallelism: the loads of Lambda come from L2)
     const int ntri = s * (s + 1) >> 1;
-#pragma unroll 4
-    for (int t = lane; t < ntri; t += TEAM) {
-      const int p = tri_row(t), q = t - (p * (p + 1) >> 1);
-      const float v = lam[t];
-      const int ip = w.ssup[p], iq = w.ssup[q];
-      const int hi = max(ip, iq), lo = min(ip, iq);
-      w.H[w.rbase[hi] + lo] += v;
+    // loads first, scatter second: the compiler cannot move a global load above the shared-memory update
+    // of the previous entry, so without the explicit batch every iteration pays a full L2 round trip
+    for (int t0 = lane; t0 < ntri; t0 += 8 * TEAM) {
+      float v[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) { const int t = t0 + u * TEAM; v[u] = t < ntri ? lam[t] : 0.f; }
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        const int t = t0 + u * TEAM;
+        if (t < ntri) {
+          const int p = tri_row(t), q = t - (p * (p + 1) >> 1);
+          const int ip = w.ssup[p], iq = w.ssup[q];
+          const int hi = max(ip, iq), lo = min(ip, iq);
+          if (lo >= cb) w.H[w.rbase[hi] + lo] += v[u];
+        }
+      }
     }
-    // b -= Lambda d + g
+    // b -= Lambda d + g (row p: the packed row, then the column below the diagonal; 8 loads in flight)
     float* rhs = w.H + w.rbase[n];
     for (int p = lane; p < s; p += TEAM) {
-      float acc = rec[ly.o_g + p];
+      float acc0 = rec[ly.o_g + p], acc1 = 0.f;
       const float* lrow = lam + (p * (p + 1) >> 1);
-      for (int q = 0; q <= p; ++q) acc = fmaf(lrow[q], w.sds[q], acc);
-      for (int q = p + 1; q < s; ++q) acc = fmaf(lam[(q * (q + 1) >> 1) + p], w.sds[q], acc);
-      rhs[w.ssup[p]] -= acc;
+      for (int q0 = 0; q0 <= p; q0 += 8) {
+        float v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) v[u] = q0 + u <= p ? lrow[q0 + u] : 0.f;
+#pragma unroll
+        for (int u = 0; u < 8; u += 2) {
+          acc0 = fmaf(v[u], q0 + u <= p ? w.sds[q0 + u] : 0.f, acc0);
+          acc1 = fmaf(v[u + 1], q0 + u + 1 <= p ? w.sds[q0 + u + 1] : 0.f, acc1);
+        }
+      }
+      for (int q0 = p + 1; q0 < s; q0 += 8) {
+        float v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) { const int q = q0 + u; v[u] = q < s ? lam[(q * (q + 1) >> 1) + p] : 0.f; }
+#pragma unroll
+        for (int u = 0; u < 8; u += 2) {
+          acc0 = fmaf(v[u], q0 + u < s ? w.sds[q0 + u] : 0.f, acc0);
+          acc1 = fmaf(v[u + 1], q0 + u + 1 < s ? w.sds[q0 + u + 1] : 0.f, acc1);
+        }
+      }
+      rhs[w.ssup[p]] -= acc0 + acc1;
     }
   }
   tm.sync();
@@ -638,30 +690,38 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
     }
     tm.sync();
   }
-  // loop closures t -> k: phase C (j side: at most one per k), phase D (i side: lane per target)
-  for (int k = 1 + lane; k < c; k += TEAM) {
-    const int t = w.lct[k];
-    if (t < 0) continue;
-    const Between b = between_eval(w.st + st_pose(t), w.cs[2 * t], w.cs[2 * t + 1], w.st + st_pose(k), w.zlc + 3 * k);
-    float Ji[3][3], Jj[3][3];
-    between_jac(b, Ji, Jj);
-    add_j_side(w, n, off_slot(ly, od, k, c), t >= 1 ? off_slot(ly, od, t, c) : 0, Ji, Jj, pr.om_lc, b.r, t >= 1);
-  }
-  tm.sync();
-  for (int t = 1 + lane; t < c - 1; t += TEAM) {
-    float Hii[6] = {0, 0, 0, 0, 0, 0}, gi[3] = {0, 0, 0};
-    bool any = false;
-    for (int k = t + 1; k < c; ++k) {
-      if (w.lct[k] != t) continue;
+  // loop closures t -> k: phase C (j side: at most one per k), phase D (i side: lane per target).
+  // lcm (bit k: slot k closes a loop; from the symbolic phase) skips both when there is none and
+  // bounds the search of phase D.
+  const uint64_t lcm = (uint64_t)(uint32_t)w.lct[W] | ((uint64_t)(uint32_t)w.lct[W + 1] << 32);
+  if (lcm) {
+    for (int k = 1 + lane; k < c; k += TEAM) {
+      const int t = w.lct[k];
+      if (t < 0) continue;
       const Between b = between_eval(w.st + st_pose(t), w.cs[2 * t], w.cs[2 * t + 1], w.st + st_pose(k), w.zlc + 3 * k);
       float Ji[3][3], Jj[3][3];
       between_jac(b, Ji, Jj);
-      acc_i_side(Ji, pr.om_lc, b.r, Hii, gi);
-      any = true;
+      add_j_side(w, n, off_slot(ly, od, k, c), t >= 1 ? off_slot(ly, od, t, c) : 0, Ji, Jj, pr.om_lc, b.r, t >= 1);
     }
-    if (any) add_i_side(w, n, off_slot(ly, od, t, c), Hii, gi);
+    tm.sync();
+    for (int t = 1 + lane; t < c - 1; t += TEAM) {
+      float Hii[6] = {0, 0, 0, 0, 0, 0}, gi[3] = {0, 0, 0};
+      bool any = false;
+      uint64_t km = lcm & ~((2ull << t) - 1ull);
+      while (km) {
+        const int k = __ffsll((long long)km) - 1;
+        km &= km - 1;
+        if (w.lct[k] != t) continue;
+        const Between b = between_eval(w.st + st_pose(t), w.cs[2 * t], w.cs[2 * t + 1], w.st + st_pose(k), w.zlc + 3 * k);
+        float Ji[3][3], Jj[3][3];
+        between_jac(b, Ji, Jj);
+        acc_i_side(Ji, pr.om_lc, b.r, Hii, gi);
+        any = true;
+      }
+      if (any) add_i_side(w, n, off_slot(ly, od, t, c), Hii, gi);
+    }
+    tm.sync();
   }
-  tm.sync();
   // unary absolute-pose factors (NEXT-1): r = (a (+) e_k) - z, full 3x3 information,
   // J_a = [[1,0,-dy],[0,1,dx],[0,0,1]] (d = Rot(a_th) t_k), J_e = blockdiag(Rot(a_th), 1); slot 0: x = a.
   if (mk.um) {
@@ -813,22 +873,30 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
       }
     }
     if (TEAM == 32) tm.sync();
-    // ---- pass B: lane = landmark
+    // ---- pass B: one landmark per group of 2^g lanes, which split its observing poses round-robin and
+    // combine by shuffles (g > 0 when few landmarks are in view, else one lane would walk the whole window)
     float A[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};  // gg(3), <a2,g0>, <a2,g1>, <a2,a2>, <g0,r>, <g1,r>, <a2,r>
-    for (int l = doB ? laneB : L; l < L; l += halfA) {
-      const bool inl = (od.obs >> l) & 1ull;
+    const int nobs = __popcll(od.obs);
+    int g = 0;
+    while (g < 3 && (nobs << (g + 1)) <= 32) ++g;
+    const int sub = laneB & ((1 << g) - 1), per = halfA >> g;
+    for (int i0 = doB ? 0 : nobs; i0 < nobs; i0 += per) {
+      const int idx = i0 + (laneB >> g);
+      const bool inl = idx < nobs;
+      const int l = inl ? nth_set_bit(od.obs, idx) : 0;
       const float mx = inl ? mloc[2 * l] : 0.f, my = inl ? mloc[2 * l + 1] : 0.f;
       float Lxx = 0.f, Lxy = 0.f, Lyy = 0.f, bgx = 0.f, bgy = 0.f, ag0 = 0.f, ag1 = 0.f, a22 = 0.f, a2r = 0.f;
       uint64_t km = 0ull;  // slots that observe this landmark
       if (inl)
         for (int k = 0; k < c; ++k) km |= (uint64_t)((w.rbm[k * ly.nw + (l >> 5)] >> (l & 31)) & 1u) << k;
+      for (int j = 0; j < sub && km; ++j) km &= km - 1;  // this lane takes the bits sub, sub + 2^g, ...
       int knext = km ? __ffsll((long long)km) - 1 : 0;  // measurements prefetched one slot ahead (L2)
       int rn = ring_of(knext, head, W);
       float zr_n = km ? rec[ly.o_zrb + (rn * 2 + 0) * L + l] : 0.f, zb_n = km ? rec[ly.o_zrb + (rn * 2 + 1) * L + l] : 0.f;
       while (km) {
         const int k = knext;
         const float zr = zr_n, zb = zb_n;
-        km &= km - 1;
+        for (int j = 0; j < (1 << g) && km; ++j) km &= km - 1;
         if (km) {
           knext = __ffsll((long long)km) - 1;
           rn = ring_of(knext, head, W);
@@ -846,7 +914,12 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
         ag0 += wa2a * Ux + wa2b * Vx; ag1 += wa2a * Uy + wa2b * Vy; a22 += wa2a * j0 + wa2b * j1;
         bgx += wg0a * r0 + wg0b * r1; bgy += wg1a * r0 + wg1b * r1; a2r += wa2a * r0 + wa2b * r1;
       }
-      if (inl) {
+      for (int o = (1 << g) >> 1; o > 0; o >>= 1) {  // (uniform trip count: every lane of the warp is here)
+        Lxx += __shfl_xor_sync(FULLMASK, Lxx, o); Lxy += __shfl_xor_sync(FULLMASK, Lxy, o); Lyy += __shfl_xor_sync(FULLMASK, Lyy, o);
+        ag0 += __shfl_xor_sync(FULLMASK, ag0, o); ag1 += __shfl_xor_sync(FULLMASK, ag1, o); a22 += __shfl_xor_sync(FULLMASK, a22, o);
+        bgx += __shfl_xor_sync(FULLMASK, bgx, o); bgy += __shfl_xor_sync(FULLMASK, bgy, o); a2r += __shfl_xor_sync(FULLMASK, a2r, o);
+      }
+      if (inl && sub == 0) {
         const int ol = off_lm(ly, od, l);
         float* r0p = w.H + w.rbase[ol];
         float* r1p = w.H + w.rbase[ol + 1];
@@ -891,7 +964,10 @@ __device__ __forceinline__ void st4(float* p, float4 v) { *reinterpret_cast<floa
   ACC = fmaf(-XV.w, BV.w, ACC);
 
 template <int TEAM>
-__device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int lane) {
+__device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int lane, int ncb) {
+  // ncb: number of leading column blocks whose factor is still valid from the previous factorisation of
+  // this call (see assemble): there only the rhs pair -- the last entry of the column's list -- is
+  // processed, on the lanes and with the K-split it has in a full pass, so y is bit-identical.
   const int np = ly.np, G = np >> 2;
   int flag = 0;
   for (int J = 0; J < G; ++J) {
@@ -913,10 +989,15 @@ __device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int
     const int per_pass = TEAM >> lg;
     const int t = lane & (ch - 1);
     float d0 = 1.f, d1 = 1.f, d2 = 1.f, d3 = 1.f, l10 = 0.f, l20 = 0.f, l21 = 0.f, l30 = 0.f, l31 = 0.f, l32 = 0.f;
-    for (int q0 = 0; q0 < cnt; q0 += per_pass) {
-      const bool first_pass = q0 == 0;
+    const bool cached = J < ncb;
+    if (cached) {
+      const float4 t0 = ld4(rJ0 + c0), t1 = ld4(rJ1 + c0), t2 = ld4(rJ2 + c0), t3 = ld4(rJ3 + c0);
+      d0 = t0.x; l10 = t1.x; d1 = t1.y; l20 = t2.x; l21 = t2.y; d2 = t2.z; l30 = t3.x; l31 = t3.y; l32 = t3.z; d3 = t3.w;
+    }
+    for (int q0 = cached ? ((cnt - 1) & ~(per_pass - 1)) : 0; q0 < cnt; q0 += per_pass) {
+      const bool first_pass = !cached && q0 == 0;
       const int q = q0 + (lane >> lg);
-      const bool act = q < cnt;
+      const bool act = cached ? q == cnt - 1 : q < cnt;
       // a warp without any pair in this pass only takes part in the barriers
       const bool warp_idle = TEAM > 32 && q0 + ((lane & ~31) >> lg) >= cnt;
       if (warp_idle) {

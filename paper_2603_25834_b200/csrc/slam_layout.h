@@ -27,6 +27,7 @@ struct Layout {
   int warp_words;      // total shared words per warp
   int wpc;             // teams (environments in flight) per CTA
   int team;            // threads per environment: 32, 64 or 128
+  int lcache;          // 1: keep the factor columns of passive landmarks across the linearisations of one call
   int lock;            // lock-step level: CTA barriers before assemble (1), + before Cholesky (2), + before the solve (3)
 };
 
@@ -69,7 +70,7 @@ static inline Layout make_layout(int N, int W, int L, int cap, int wpc) {
   y.s_st = s; s = pad4(s + n + 3);
   y.s_zodo = s; s = pad4(s + 3 * W);
   y.s_zlc = s; s = pad4(s + 3 * W);
-  y.s_lct = s; s = pad4(s + W);
+  y.s_lct = s; s = pad4(s + W + 2);  // + the loop-closure mask (two words)
   y.s_cs = s; s = pad4(s + 2 * W);
   y.s_rbm = s; s = pad4(s + W * y.nw);
   y.s_first = s; s = pad4(s + y.np + 2);
@@ -95,6 +96,7 @@ static inline Layout make_layout(int N, int W, int L, int cap, int wpc) {
   y.wpc = wpc;
   y.team = 32;
   y.lock = 0;
+  y.lcache = 1;
   return y;
 }
 
