@@ -18,7 +18,10 @@ using namespace slamk;
 // environments.  flags select the phases, so that the separate ABI calls and the fused slam_step share
 // the same device code and are bit-for-bit identical.
 template <int TEAM>
-__global__ void __launch_bounds__(TEAM == 128 ? 896 : 512)
+#ifndef SLAM_MAXTHREADS
+#define SLAM_MAXTHREADS 512
+#endif
+__global__ void __launch_bounds__(TEAM == 128 ? 896 : SLAM_MAXTHREADS)
 slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flags, int iters, StepIO io,
                  unsigned long long* stats, int mode, int* ovf) {
   extern __shared__ float4 smem4[];
@@ -276,6 +279,13 @@ struct slam_ctx {
   int grid_small, smem_small, ctas_small;
   bool two_pass;
   int* ovf;                               // [0] count, [1..N] environments that did not fit
+  // Feedback for the two-pass launch: the overflow count of a recent first pass, copied to pinned host
+  // memory asynchronously and read without blocking.  While most environments overflow, the first pass
+  // is skipped (dense launch only) except for a probe every 8th launch.  Results do not depend on it.
+  int* h_ovf;
+  cudaEvent_t ovf_ev;
+  bool ovf_pending, adaptive;
+  int ovf_last, dense_streak;
   char err[256];
 };
 
@@ -306,27 +316,38 @@ static int pick_team(int W, int L) {
 }
 // Shared-memory capacity (words) of the first launch.  Environments whose envelope does not fit are
 // re-run by a second launch with the dense capacity.  SLAM_CAP_FRAC (0..1] overrides.  Landmark windows
-// are nearly dense while the robot is among the landmarks, so they use the dense capacity directly.
-static int pick_cap(int W, int L) {
+// are nearly dense while the robot is among the landmarks and sparse after it has left: 0.6 there, with
+// the first pass skipped adaptively while most environments overflow (launch_step; SLAM_ADAPTIVE=0 disables).
+static int max_teams(int team) {  // <= 896 / 512 / 480 threads per CTA (register file, 15 named barriers)
+  int maxt = team == 128 ? 7 : (team == 64 ? SLAM_MAXTHREADS / 64 : 15);
+  const char* e = getenv("SLAM_MAX_WPC");
+  if (e && atoi(e) >= 1 && atoi(e) < maxt) maxt = atoi(e);
+  return maxt;
+}
+static int pick_cap(int W, int L, int team) {
   const Layout d = make_layout(1, W, L, -1, 1);
-  double frac = L > 0 ? 1.0 : 0.45;
+  // the largest capacity with which as many teams as the register file allows still share one SM ...
+  const int fixed = d.warp_words - d.cap;
+  int cap = (((226 * 1024 / 4) / max_teams(team)) & ~3) - fixed;  // (226 KB: room for two CTAs per SM)
+  // ... unless that is a small part of the dense size (large windows): then a fixed fraction
+  if (cap < (int)(0.45 * d.cap)) cap = (int)(0.45 * d.cap);
+  (void)L;
   const char* e = getenv("SLAM_CAP_FRAC");
-  if (e) { const double f = atof(e); if (f > 0.0 && f <= 1.0) frac = f; }
-  int cap = (int)(frac * d.cap);
+  if (e) { const double f = atof(e); if (f > 0.0 && f <= 1.0) cap = (int)(f * d.cap); }
   if (cap < 256) cap = 256;
+  cap &= ~3;
   return cap >= d.cap ? -1 : cap;
 }
 static int pick_wpc(int W, int L, int team, int cap) {
   const Layout t = make_layout(1, W, L, cap, 1);
   const size_t wb = (size_t)t.warp_words * 4;
   int wpc = (int)((size_t)227 * 1024 / wb);
-  int maxt = team == 128 ? 7 : (team == 64 ? 8 : 15);   // <= 896 / 512 / 480 threads per CTA (15 named barriers)
-  const char* e = getenv("SLAM_MAX_WPC");
-  if (e && atoi(e) >= 1 && atoi(e) < maxt) maxt = atoi(e);
+  const int maxt = max_teams(team);
   if (wpc > maxt) wpc = maxt;
   // Two smaller CTAs per SM when that loses no team: their lock-step phases drift apart, which spreads
   // the load on the shared-memory and FMA pipes, and the tail of the last wave is finer grained
-  // (measured, config 2: 0.684 -> 0.587 ms per step).  SLAM_SPLIT_CTA=0 disables.
+  // (measured, config 2: 0.697 -> 0.585 ms per step, config 3: 2.89 -> 2.64; four CTAs are slower
+  // again: 0.611 / 3.51).  SLAM_SPLIT_CTA=0 disables.
   const char* sp = getenv("SLAM_SPLIT_CTA");
   if (!(sp && sp[0] == '0') && wpc >= 4 && wpc % 2 == 0 && (size_t)wpc * wb + 2048 <= (size_t)228 * 1024) wpc /= 2;
   return wpc;  // 0 if one environment does not fit
@@ -435,7 +456,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   c->grid = need < sms * occ ? need : sms * occ;
   // optional first launch with a smaller capacity (more environments in flight per SM)
   c->two_pass = false;
-  const int cap = pick_cap(window, landmarks);
+  const int cap = pick_cap(window, landmarks, team);
   if (cap > 0) {
     const int wpc_s = pick_wpc(window, landmarks, team, cap);
     c->ly_small = make_layout(batch, window, landmarks, cap, wpc_s);
@@ -452,13 +473,26 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
       c->grid_small = need_s < sms * occ_s ? need_s : sms * occ_s;
     }
   }
+  c->h_ovf = nullptr; c->ovf_ev = nullptr; c->ovf_pending = false; c->ovf_last = 0; c->dense_streak = 0;
+  c->adaptive = c->two_pass;
+  { const char* e = getenv("SLAM_ADAPTIVE"); if (e && e[0] == '0') c->adaptive = false; }
+  if (c->adaptive && (cudaHostAlloc((void**)&c->h_ovf, sizeof(int), cudaHostAllocDefault) != cudaSuccess ||
+                      cudaEventCreateWithFlags(&c->ovf_ev, cudaEventDisableTiming) != cudaSuccess)) {
+    cudaGetLastError();
+    c->adaptive = false;  // no feedback channel: always run both passes
+  }
   *out = c;
   const int rc = slam_reset(c, nullptr);
-  if (rc != SLAM_OK) { *out = nullptr; delete c; }
+  if (rc != SLAM_OK) { *out = nullptr; slam_destroy(c); }
   return rc;
 }
 
-void slam_destroy(slam_ctx* ctx) { delete ctx; }
+void slam_destroy(slam_ctx* ctx) {
+  if (!ctx) return;
+  if (ctx->ovf_ev) { cudaEventSynchronize(ctx->ovf_ev); cudaEventDestroy(ctx->ovf_ev); }
+  if (ctx->h_ovf) cudaFreeHost(ctx->h_ovf);
+  delete ctx;
+}
 
 int slam_reset(slam_ctx* c, const float* init_pose) {
   if (!c) return SLAM_EINVAL;
@@ -467,15 +501,31 @@ int slam_reset(slam_ctx* c, const float* init_pose) {
   slam_reset_kernel<<<blocks, threads, 0, c->stream>>>(c->ly, c->pr, c->state, init_pose);
   c->launches++;
   c->head = 0; c->count = 1; c->cov_valid = false;
+  c->ovf_last = 0; c->dense_streak = 0;
   return check_cuda(c, "slam_reset");
 }
 
 static int launch_step(slam_ctx* c, int flags, int iters, const StepIO& io) {
   const step_fn fn = kernel_of(c->ly.team);
-  if (c->two_pass) {
+  bool two = c->two_pass;
+  const bool solves = iters > 0 || (flags & (F_COV | F_MARG));
+  if (two && c->adaptive && solves) {
+    if (c->ovf_pending && cudaEventQuery(c->ovf_ev) == cudaSuccess) { c->ovf_last = *c->h_ovf; c->ovf_pending = false; }
+    if (2 * (long long)c->ovf_last > c->ly.N) {
+      if (++c->dense_streak % 8 != 0) two = false;
+    } else {
+      c->dense_streak = 0;
+    }
+  }
+  if (two) {
     cudaMemsetAsync(c->ovf, 0, 4, c->stream);
     fn<<<c->grid_small, c->ly_small.wpc * c->ly.team, c->smem_small, c->stream>>>(c->ly_small, c->pr, c->state, c->head, c->count,
                                                                                    flags, iters, io, c->stats, 0, c->ovf);
+    if (c->adaptive && solves && !c->ovf_pending) {
+      cudaMemcpyAsync(c->h_ovf, c->ovf, 4, cudaMemcpyDeviceToHost, c->stream);
+      cudaEventRecord(c->ovf_ev, c->stream);
+      c->ovf_pending = true;
+    }
     fn<<<c->grid, c->ly.wpc * c->ly.team, c->smem_bytes, c->stream>>>(c->ly, c->pr, c->state, c->head, c->count, flags, iters,
                                                                         io, c->stats, 1, c->ovf);
     c->launches += 2;

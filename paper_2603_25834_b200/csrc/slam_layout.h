@@ -95,7 +95,7 @@ static inline Layout make_layout(int N, int W, int L, int cap, int wpc) {
   y.warp_words = pad4(s);
   y.wpc = wpc;
   y.team = 32;
-  y.lock = 0;
+  y.lock = 1;
   y.lcache = 1;
   return y;
 }

@@ -254,6 +254,22 @@ def test_results_do_not_depend_on_capacity_or_team(monkeypatch):
     assert st["fallback"] > 0, st                       # the overflow path really ran
     assert np.array_equal(a["cov"], b["cov"]) and np.array_equal(a["logdet"], b["logdet"])
     assert (b["status"] == 0).all()
+    # a capacity that nearly every environment overflows: the host skips the first pass (feedback from the
+    # overflow count, probe every 8th launch) -- fewer launches, the same bits
+    monkeypatch.setenv("SLAM_CAP_FRAC", "0.08")
+    slam = _slam(cfg.N, cfg.W, cfg.L)
+    dev = to_dev(data)
+    slam.reset()
+    cov = torch.zeros(cfg.T, 9, cfg.N, device="cuda:0")
+    ld = torch.zeros(cfg.T, cfg.N, device="cuda:0")
+    n0 = slam.launch_count
+    for t in range(1, cfg.T + 1):
+        slam.step(dev["odom"][t - 1], dev["lc_back"][t - 1], dev["lc_meas"][t - 1], None, None, iters=cfg.iters,
+                  cov=cov[t - 1], logdet=ld[t - 1])
+        torch.cuda.synchronize()
+    assert slam.launch_count - n0 < 2 * cfg.T - 20, (slam.launch_count - n0, slam.get_stats())
+    assert np.array_equal(ld.cpu().numpy().astype(np.float64), a["logdet"])
+    assert np.array_equal(cov.cpu().numpy().reshape(cfg.T, 3, 3, cfg.N).transpose(0, 3, 1, 2).astype(np.float64), a["cov"])
     monkeypatch.delenv("SLAM_CAP_FRAC")
     ref = oracle.run_batch(data, cfg.iters, envs=np.arange(0, cfg.N, 25, dtype=np.int32))
     for team in ("32", "128"):
