@@ -36,6 +36,11 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
   Team<32> tm32;
   tm32.bar = 0;
   tm32.scr = tm.scr;
+  // The warp of a team that works alone in the single-warp phases.  Warps are spread over the four
+  // sub-partitions of the SM by warp index mod 4: with two warps per team and always the first one working,
+  // only sub-partitions 0 and 2 would issue (measured: "not selected" stalls 19 % while two sub-partitions
+  // idle), so teams alternate.
+  const int solo = TEAM == 64 ? ((team >> 1) & 1) : 0;
   // All teams of a CTA walk through the phases in LOCK-STEP (CTA barriers between phases): the kernel is
   // large (~12 k instructions) and instruction-fetch bound, so warps that execute the same code at the
   // same time share every fetched line.  Teams without an environment in the last round only take part
@@ -104,7 +109,7 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
           // does the factorisation with shuffles and __syncwarp only: no named barriers, no
           // shared-memory exchange of the diagonal tile.  The other warps of the team wait.
           if (TEAM > 32 && single_warp) {
-            if (lane < 32) status |= cholesky<32>(ly, w, tm32, lane, ncb);
+            if ((lane >> 5) == solo) status |= cholesky<32>(ly, w, tm32, lane & 31, ncb);
             tm.sync();
           } else {
             status |= cholesky<TEAM>(ly, w, tm, lane, ncb);
@@ -114,7 +119,7 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
         if (valid) {
           if (it < iters) {
             if (TEAM > 32) {  // short rows: one warp, no named barriers
-              if (lane < 32) back_substitute<32>(ly, w, tm32, lane);
+              if ((lane >> 5) == solo) back_substitute<32>(ly, w, tm32, lane & 31);
               tm.sync();
             } else {
               back_substitute<TEAM>(ly, w, tm, lane);
@@ -140,7 +145,7 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
       if (do_marg) status |= marginalize<TEAM>(ly, pr, rec, w, tm, lane, head, cc, mk, s);
       else if ((flags & F_MARG) && lane == 0) reinterpret_cast<int*>(rec)[ly.o_k0] = k0 - 1;  // the window slides under it
       store_state<TEAM>(ly, rec, w, tm, lane, head, cc, mk);
-      if (status && lane == 0) reinterpret_cast<int*>(rec)[ly.o_status] |= status;
+      if (status && (lane & 31) == 0) atomicOr(reinterpret_cast<int*>(rec) + ly.o_status, status);  // (any warp may hold a flag)
       tm.sync();
     }
   }
