@@ -350,7 +350,8 @@ def main():
                        "l2": ("flushed between steps (untimed)" if flush else
                               f"not flushed: {touched_per_step / 2 ** 20:.0f} MiB algorithmic working set per step > L2")},
             "roofline": roof, "clocks": clocks, "gpu_launches": launches,
-            "status_flagged_envs": status_bad, "outputs_finite": finite, "kernel_info": slam.kernel_info(),
+            "status_flagged_envs": status_bad, "outputs_finite": finite,
+            "kernel_info": dict(slam.kernel_info(), pool_waits=slam.get_stats()["waited"]),
         }
         if e2e:
             out["e2e"] = {"value": replicas.whole_job_rate(N * K, world, e2e_s_max), "unit": "env-steps/s",

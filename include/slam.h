@@ -143,8 +143,9 @@ int slam_get_landmarks(slam_ctx* ctx, float* lm, uint32_t* active);
 int slam_get_status(slam_ctx* ctx, int32_t* status);
 
 /* Device counters since the last reset, copied to stats8 ([8] uint64, device): [0] max and [1] sum of the
- * envelope words (shared-memory footprint of H) over [2] solved environment-instances, [3] instances
- * that exceeded the shared-memory capacity and ran from the global-memory fallback. */
+ * envelope words (shared-memory footprint of H) over [2] solved environment-instances, [3] rounds an
+ * environment waited for space in the shared-memory pool of its CTA (it is solved one round later; the
+ * result does not depend on it). */
 int slam_get_stats(slam_ctx* ctx, unsigned long long* stats8);
 
 /* NEXT-4: the paper's reward, eqs. (7)-(17), elementwise over environments, meant

@@ -278,7 +278,7 @@ class FixedLagSlam:
         out = self._new(8, dtype=torch.int64)
         self._chk(LIB.slam_get_stats(self._h, C.c_void_p(out.data_ptr())))
         v = [int(x) for x in out.cpu()]
-        return dict(max_envelope_words=v[0], mean_envelope_words=v[1] / max(v[2], 1), solved=v[2], fallback=v[3])
+        return dict(max_envelope_words=v[0], mean_envelope_words=v[1] / max(v[2], 1), solved=v[2], waited=v[3])
 
     def reward(self, params: RewardParams, u, u_prev, dcells, d_min, collision, out=None):
         out = self._new(self.N) if out is None else out

@@ -14,22 +14,33 @@
 using namespace slamk;
 
 // ------------------------------------------------------------------ kernels
-// One TEAM of 32/64/128 threads per environment, `wpc` teams per CTA, persistent grid-stride loop over
-// environments.  flags select the phases, so that the separate ABI calls and the fused slam_step share
-// the same device code and are bit-for-bit identical.
-template <int TEAM>
+// One TEAM of 32/64/128 threads per environment, `wpc` teams per CTA, persistent loop over the
+// environments blockIdx.x, blockIdx.x + gridDim.x, ... in ROUNDS.  flags select the phases, so that the
+// separate ABI calls and the fused slam_step share the same device code and are bit-for-bit identical.
+//
+// Shared memory = a fixed part per team (state, factor data, row tables) + ONE POOL per CTA.  The
+// envelope of H is data dependent (a third to all of the dense size), so a fixed dense slot per team
+// would leave most of the shared memory unused.  Instead, in every round each team loads its
+// environment, runs the symbolic phase to learn how many words it NEEDS (envelope + rhs rows +
+// active-pair lists, or the marginalisation scratch), and the pool is handed out first-fit in team
+// order; a team that does not fit keeps its environment (loaded, untouched in memory) and goes FIRST in
+// the next round.  The pool is at least the dense need, so a waiting team always gets in.  Which round
+// solves an environment does not change a single bit of its result.
 #ifndef SLAM_MAXTHREADS
 #define SLAM_MAXTHREADS 512
 #endif
+template <int TEAM>
 __global__ void __launch_bounds__(TEAM == 128 ? 896 : SLAM_MAXTHREADS)
 slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flags, int iters, StepIO io,
-                 unsigned long long* stats, int mode, int* ovf) {
+                 unsigned long long* stats) {
   extern __shared__ float4 smem4[];
+  __shared__ int s_env[16], s_need[16], s_off[16], s_new[16], s_ctl[2];
   float* smem = reinterpret_cast<float*>(smem4);
   const int team = threadIdx.x / TEAM, lane = threadIdx.x % TEAM;
   const int LOCK = ly.lock;
-  float* base = smem + (size_t)team * ly.warp_words;
-  const WS w = make_ws(ly, base);
+  float* base = smem + (size_t)team * ly.team_words;
+  float* pool = smem + (size_t)ly.wpc * ly.team_words;
+  WS w = make_ws(ly, base);
   Team<TEAM> tm;
   tm.bar = 1 + team;
   tm.scr = base + ly.s_scr;
@@ -41,60 +52,97 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
   // only sub-partitions 0 and 2 would issue (measured: "not selected" stalls 19 % while two sub-partitions
   // idle), so teams alternate.
   const int solo = TEAM == 64 ? ((team >> 1) & 1) : 0;
+  // iters Gauss-Newton iterations, then (F_COV) one more linearisation + factorisation at the final
+  // estimate for the covariance: ONE call site per phase keeps the kernel small.
+  const int nlin = iters + ((flags & F_COV) ? 1 : 0);
+  // the environment this team has in hand (kept across rounds while it waits for pool space)
+  int env = -1, k0 = 0, head = 0, cc = 0, s = 0, total = 0, need = 0;
+  bool waiting = false, do_marg = false;
+  Masks mk;
+  Ord od;
+  if (threadIdx.x < 16) { s_env[threadIdx.x] = -1; s_off[threadIdx.x] = 0; }
+  if (threadIdx.x == 0) s_ctl[0] = 0;
   // All teams of a CTA walk through the phases in LOCK-STEP (CTA barriers between phases): the kernel is
   // large (~12 k instructions) and instruction-fetch bound, so warps that execute the same code at the
-  // same time share every fetched line.  Teams without an environment in the last round only take part
-  // in the barriers.
-  // mode 0: every environment; one whose envelope (or marginalisation scratch) exceeds this launch's
-  // shared-memory capacity is appended to the overflow list ovf[1..] (count in ovf[0]) and left untouched.
-  // mode 1: the environments of that list (launched with the dense capacity).
-  const int nwork = mode == 0 ? ly.N : ovf[0];
-  for (int env0 = blockIdx.x * ly.wpc; env0 < nwork; env0 += gridDim.x * ly.wpc) {
-    const int widx = env0 + team;
-    bool valid = widx < nwork;
-    const int env = valid ? (mode == 0 ? widx : ovf[1 + widx]) : 0;
-    float* rec = state + (size_t)env * ly.rec;
-    // NEXT-2: an environment that was reset mid-run lives in the slots k0.. of the lock-step window:
-    // its own count is c - k0 and its ring head is head + k0 (slam_reset_envs).
-    const int k0 = valid ? reinterpret_cast<const int*>(rec)[ly.o_k0] : 0;
-    const int head = (head_g + k0) % ly.W;
-    int cc = c - k0, status = 0, s = 0, total = 0;
-    bool single_warp = false;
-    Masks mk;
-    Ord od;
+  // same time share every fetched line.  Teams without an environment only take part in the barriers.
+  for (;;) {
     __syncthreads();
-    if (valid) {
-      load_env<TEAM>(ly, rec, w, tm, lane, head, cc, mk);
-      if (flags & F_OBS0) record_rb<TEAM>(ly, rec, w, tm, lane, env, head, 0, 0.f, 0.f, 0.f, io, mk);
-      if (flags & F_PUSH) cc = push_env<TEAM>(ly, rec, w, tm, lane, env, head, cc, io, mk);
-      od = make_ord(ly, w.rbm, cc);
-      s = build_support<TEAM>(ly, od, w, tm, lane, cc, mk.ps, mk.ls);
-    }
-    const bool do_marg = (flags & F_MARG) && k0 == 0;   // a reset environment is not full yet
-    int need = 0;
-    if (valid && do_marg) need = marg_need(ly, w, lane, cc, mk);
-    // iters Gauss-Newton iterations, then (F_COV) one more linearisation + factorisation at the final
-    // estimate for the covariance: ONE call site per phase keeps the kernel small.
-    const int nlin = iters + ((flags & F_COV) ? 1 : 0);
-    if (nlin > 0) {
-      if (LOCK >= 0) __syncthreads();
-      if (valid) {
-        total = symbolic<TEAM>(ly, od, w, tm, lane, cc, mk, s);
-        need = max(need, total);
-        single_warp = reinterpret_cast<const int*>(tm.scr)[9] <= 32;
-        if (stats && lane == 0 && mode == 0) {  // envelope statistics (words per environment): max, sum, count
-          atomicMax(stats + 0, (unsigned long long)total);
-          atomicAdd(stats + 1, (unsigned long long)total);
-          atomicAdd(stats + 2, 1ull);
+    if (threadIdx.x == 0) {  // teams that are not waiting take the next environments of this CTA, in team order
+      int nk = s_ctl[0], live = 0;
+      for (int t = 0; t < ly.wpc; ++t) {
+        if (s_off[t] != -1) {
+          const long long e = (long long)blockIdx.x + (long long)nk * gridDim.x;
+          if (e < ly.N) { s_env[t] = (int)e; ++nk; } else s_env[t] = -1;
         }
+        live += s_env[t] >= 0;
+      }
+      s_ctl[0] = nk; s_ctl[1] = live;
+    }
+    __syncthreads();
+    if (s_ctl[1] == 0) break;
+    if (!waiting) {
+      env = s_env[team];
+      if (env >= 0) {
+        float* rec = state + (size_t)env * ly.rec;
+        // NEXT-2: an environment that was reset mid-run lives in the slots k0.. of the lock-step window:
+        // its own count is c - k0 and its ring head is head + k0 (slam_reset_envs).
+        k0 = reinterpret_cast<const int*>(rec)[ly.o_k0];
+        head = (head_g + k0) % ly.W;
+        cc = c - k0;
+        load_env<TEAM>(ly, rec, w, tm, lane, head, cc, mk);
+        if (flags & F_OBS0) record_rb<TEAM>(ly, rec, w, tm, lane, env, head, 0, 0.f, 0.f, 0.f, io, mk);
+        if (flags & F_PUSH) cc = push_env<TEAM>(ly, rec, w, tm, lane, env, head, cc, io, mk);
+        od = make_ord(ly, w.rbm, cc);
+        s = build_support<TEAM>(ly, od, w, tm, lane, cc, mk.ps, mk.ls);
+        do_marg = (flags & F_MARG) && k0 == 0;   // a reset environment is not full yet
+        need = do_marg ? marg_need(ly, w, lane, cc, mk) : 0;
+        total = 0;
+        if (nlin > 0) {
+          total = symbolic<TEAM>(ly, od, w, tm, lane, cc, mk, s);
+          need = max(need, total + reinterpret_cast<const int*>(tm.scr)[10]);
+          if (flags & F_COV) need = max(need, 272);  // fp64 scratch of the covariance tail
+          if (stats && lane == 0) {  // envelope statistics (words per environment): max, sum, count
+            atomicMax(stats + 0, (unsigned long long)total);
+            atomicAdd(stats + 1, (unsigned long long)total);
+            atomicAdd(stats + 2, 1ull);
+          }
+        }
+        need = (need + 3) & ~3;
       }
     }
-    if (valid && need > ly.cap) {  // does not fit this launch: hand over to the dense-capacity launch
-      if (lane == 0) {
-        if (mode == 0) { const int slot = atomicAdd(ovf, 1); ovf[1 + slot] = env; atomicAdd(stats + 3, 1ull); }
-        else reinterpret_cast<int*>(rec)[ly.o_status] |= 4;
+    if (lane == 0) s_need[team] = env >= 0 ? need : 0;
+    __syncthreads();
+    if (threadIdx.x == 0) {  // first fit in team order, the teams that waited first
+      int off = 0;
+      for (int pass = 0; pass < 2; ++pass)
+        for (int t = 0; t < ly.wpc; ++t) {
+          if (s_env[t] < 0) { s_new[t] = 0; continue; }
+          if ((s_off[t] == -1) != (pass == 0)) continue;
+          const int nd = s_need[t];
+          if (nd > ly.pool) s_new[t] = -2;
+          else if (off + nd <= ly.pool) { s_new[t] = off; off += nd; }
+          else s_new[t] = -1;
+        }
+      for (int t = 0; t < ly.wpc; ++t) s_off[t] = s_new[t];
+    }
+    __syncthreads();
+    const int off = env >= 0 ? s_off[team] : -3;
+    const bool valid = off >= 0;
+    waiting = off == -1;
+    float* rec = state + (size_t)(env >= 0 ? env : 0) * ly.rec;
+    if (lane == 0) {
+      if (off == -2) reinterpret_cast<int*>(rec)[ly.o_status] |= 4;  // (cannot happen: the pool holds a dense window)
+      if (waiting && stats) atomicAdd(stats + 3, 1ull);
+    }
+    int status = 0;
+    bool single_warp = false;
+    if (valid) {
+      w.H = pool + off;
+      w.amask = reinterpret_cast<uint32_t*>(w.H + total);
+      if (nlin > 0) {
+        build_lists<TEAM>(ly, w, tm, lane);
+        single_warp = reinterpret_cast<const int*>(tm.scr)[9] <= 32;
       }
-      valid = false;
     }
     if (nlin > 0) {
 #pragma unroll 1
@@ -279,18 +327,7 @@ struct slam_ctx {
   const float *un_pose, *un_info;   // pending unary factor for the next pushed pose (NEXT-1)
   const int32_t* un_valid;
   long long launches;
-  int grid, smem_bytes, ctas_per_sm;      // dense-capacity launch (the only one if !two_pass)
-  Layout ly_small;                        // first launch with a smaller shared-memory capacity
-  int grid_small, smem_small, ctas_small;
-  bool two_pass;
-  int* ovf;                               // [0] count, [1..N] environments that did not fit
-  // Feedback for the two-pass launch: the overflow count of a recent first pass, copied to pinned host
-  // memory asynchronously and read without blocking.  While most environments overflow, the first pass
-  // is skipped (dense launch only) except for a probe every 8th launch.  Results do not depend on it.
-  int* h_ovf;
-  cudaEvent_t ovf_ev;
-  bool ovf_pending, adaptive;
-  int ovf_last, dense_streak;
+  int grid, smem_bytes, ctas_per_sm;
   char err[256];
 };
 
@@ -310,65 +347,68 @@ static bool sizes_ok(int batch, int window, int landmarks) {
   return batch >= 1 && window >= 2 && window <= SLAM_MAX_WINDOW && landmarks >= 0 && landmarks <= SLAM_MAX_LANDMARKS;
 }
 
-// Threads per environment: SLAM_TEAM={32,64,128} overrides; default by state dimension (a dense-ish
-// window of ~100 variables has enough rows and factors for four warps; small windows for one).
-static int pick_team(int W, int L) {
+// Threads per environment: SLAM_TEAM={32,64,128} overrides.  One warp per environment keeps the most
+// environments in flight (the register file holds 15 one-warp teams per SM but only 8 two-warp teams) and
+// wins whenever the batch fills the SMs (measured with the pooled shared memory, ms per step, 32 vs 64
+// threads: config 2 0.39 / 0.61, config 3 2.36 / 2.70, config 4 3.44 / 3.51); a small batch (config 1:
+// 750 environments = 5 per SM) is latency bound and prefers two warps per environment (0.135 / 0.108).
+static int pick_team(int W, int L, int batch) {
   const char* e = getenv("SLAM_TEAM");
   if (e) { const int t = atoi(e); if (t == 32 || t == 64 || t == 128) return t; }
   const int n = 3 * W + 2 * L;
-  if (n >= 48) return 64;
+  if (n >= 48 && batch < 148 * 8) return 64;
   return 32;
 }
-// Shared-memory capacity (words) of the first launch.  Environments whose envelope does not fit are
-// re-run by a second launch with the dense capacity.  SLAM_CAP_FRAC (0..1] overrides.  Landmark windows
-// are nearly dense while the robot is among the landmarks and sparse after it has left: 0.6 there, with
-// the first pass skipped adaptively while most environments overflow (launch_step; SLAM_ADAPTIVE=0 disables).
-static int max_teams(int team) {  // <= 896 / 512 / 480 threads per CTA (register file, 15 named barriers)
+static int max_teams(int team) {  // threads per CTA: register file (launch bounds), 15 named barriers, 16 table slots
   int maxt = team == 128 ? 7 : (team == 64 ? SLAM_MAXTHREADS / 64 : 15);
+  if (maxt > 15) maxt = 15;
   const char* e = getenv("SLAM_MAX_WPC");
   if (e && atoi(e) >= 1 && atoi(e) < maxt) maxt = atoi(e);
   return maxt;
 }
-static int pick_cap(int W, int L, int team) {
-  const Layout d = make_layout(1, W, L, -1, 1);
-  // the largest capacity with which as many teams as the register file allows still share one SM ...
-  const int fixed = d.warp_words - d.cap;
-  int cap = (((226 * 1024 / 4) / max_teams(team)) & ~3) - fixed;  // (226 KB: room for two CTAs per SM)
-  // ... unless that is a small part of the dense size (large windows): then a fixed fraction
-  if (cap < (int)(0.45 * d.cap)) cap = (int)(0.45 * d.cap);
-  (void)L;
-  const char* e = getenv("SLAM_CAP_FRAC");
-  if (e) { const double f = atof(e); if (f > 0.0 && f <= 1.0) cap = (int)(f * d.cap); }
-  if (cap < 256) cap = 256;
-  cap &= ~3;
-  return cap >= d.cap ? -1 : cap;
-}
-static int pick_wpc(int W, int L, int team, int cap) {
-  const Layout t = make_layout(1, W, L, cap, 1);
-  const size_t wb = (size_t)t.warp_words * 4;
-  int wpc = (int)((size_t)227 * 1024 / wb);
-  const int maxt = max_teams(team);
-  if (wpc > maxt) wpc = maxt;
-  // Two smaller CTAs per SM when that loses no team: their lock-step phases drift apart, which spreads
-  // the load on the shared-memory and FMA pipes, and the tail of the last wave is finer grained
-  // (measured, config 2: 0.697 -> 0.585 ms per step, config 3: 2.89 -> 2.64; four CTAs are slower
-  // again: 0.611 / 3.51).  SLAM_SPLIT_CTA=0 disables.
+// Teams per CTA and words of the CTA pool.  More teams = more environments in flight but a smaller pool
+// (each team has a fixed part); the expected number in flight is min(teams, pool / typical need) with the
+// typical need a fraction of the dense size (measured envelopes: about a third of dense for pose-only
+// windows, a half with landmarks).  SLAM_POOL_FRAC (0..1] shrinks the pool (tests: forces waiting).
+static const int SMEM_BUDGET = 227 * 1024 - 512;  // dynamic shared memory per CTA (static tables: < 512 B)
+static int pick_launch(int W, int L, int team, int* pool_words) {
+  const Layout d = make_layout(1, W, L, 0, 1);
+  const double typical = (L > 0 ? 0.5 : 0.34) * d.dense;
+  int best = 0, best_pool = 0;
+  double best_est = 0.0;
+  // ctas = 2: two smaller CTAs per SM (each with its own pool) when that loses no team: their lock-step
+  // phases drift apart, which spreads the load on the shared-memory and FMA pipes, and the tail of the
+  // last wave is finer grained (measured with fixed slots, config 2: 0.697 -> 0.585 ms per step,
+  // config 3: 2.89 -> 2.64).  SLAM_SPLIT_CTA=0 disables.
   const char* sp = getenv("SLAM_SPLIT_CTA");
-  if (!(sp && sp[0] == '0') && wpc >= 4 && wpc % 2 == 0 && (size_t)wpc * wb + 2048 <= (size_t)228 * 1024) wpc /= 2;
-  return wpc;  // 0 if one environment does not fit
+  const int max_ctas = (sp && sp[0] == '0') ? 1 : 2;
+  for (int ctas = 1; ctas <= max_ctas; ++ctas) {
+    const int budget = ctas == 1 ? SMEM_BUDGET : (228 * 1024 / 2 - 1024 - 512);
+    for (int wpc = 1; wpc * ctas <= max_teams(team); ++wpc) {
+      const int pool = (budget / 4 - wpc * d.team_words) & ~3;
+      if (pool < d.dense) break;
+      const double fit = pool / typical;
+      double est = ctas * (fit < wpc ? fit : wpc);
+      if (ctas == 2) est += 0.25;  // at equal expected occupancy prefer two CTAs
+      if (est > best_est + 1e-9) { best_est = est; best = wpc; best_pool = pool; }
+    }
+  }
+  const char* e = getenv("SLAM_POOL_FRAC");
+  if (best && e) { const double f = atof(e); if (f > 0.0 && f <= 1.0) { best_pool = (int)(f * best_pool) & ~3; if (best_pool < d.dense) best_pool = d.dense; } }
+  *pool_words = best_pool;
+  return best;  // 0 if one environment does not fit
 }
-typedef void (*step_fn)(Layout, Params, float*, int, int, int, int, StepIO, unsigned long long*, int, int*);
+typedef void (*step_fn)(Layout, Params, float*, int, int, int, int, StepIO, unsigned long long*);
 static step_fn kernel_of(int team) {
   return team == 128 ? slam_step_kernel<128> : (team == 64 ? slam_step_kernel<64> : slam_step_kernel<32>);
 }
 
-struct WsPlan { size_t stats, ovf, state, cache, odom, lcb, lcm, rbk, rbm, cov, ld, pose, total; };
+struct WsPlan { size_t stats, state, cache, odom, lcb, lcm, rbk, rbm, cov, ld, pose, total; };
 static WsPlan plan(const Layout& ly) {
   WsPlan p;
   size_t o = 0;
   const size_t N = (size_t)ly.N;
   p.stats = o; o = al256(o + 64);
-  p.ovf = o; o = al256(o + (N + 1) * 4);
   p.state = o; o = al256(o + N * ly.rec * 4);
   p.cache = o; o = al256(o + N * 10 * 4);
   p.odom = o; o = al256(o + N * 3 * 4);
@@ -394,9 +434,10 @@ void slam_default_config(slam_config* cfg) {
 
 size_t slam_workspace_bytes(int batch, int window, int landmarks) {
   if (!sizes_ok(batch, window, landmarks)) return 0;
-  const int wpc = pick_wpc(window, landmarks, pick_team(window, landmarks), -1);
+  int pool = 0;
+  const int wpc = pick_launch(window, landmarks, pick_team(window, landmarks, batch), &pool);
   if (wpc < 1) return 0;
-  return plan(make_layout(batch, window, landmarks, -1, wpc)).total;
+  return plan(make_layout(batch, window, landmarks, pool, wpc)).total;
 }
 
 int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam_config* cfg, void* workspace,
@@ -404,8 +445,9 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   if (!out) return SLAM_EINVAL;
   *out = nullptr;
   if (!sizes_ok(batch, window, landmarks) || !workspace || ((uintptr_t)workspace & 255)) return SLAM_EINVAL;
-  const int team = pick_team(window, landmarks);
-  const int wpc = pick_wpc(window, landmarks, team, -1);
+  const int team = pick_team(window, landmarks, batch);
+  int pool = 0;
+  const int wpc = pick_launch(window, landmarks, team, &pool);
   if (wpc < 1) return SLAM_EINVAL;
   slam_config dc;
   slam_default_config(&dc);
@@ -415,7 +457,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   if (!(cfg->rb_sigma[0] > 0.f) || !(cfg->rb_sigma[1] > 0.f)) return SLAM_EINVAL;
   slam_ctx* c = new (std::nothrow) slam_ctx();
   if (!c) return SLAM_ENOMEM;
-  c->ly = make_layout(batch, window, landmarks, -1, wpc);
+  c->ly = make_layout(batch, window, landmarks, pool, wpc);
   c->ly.team = team;
   { const char* e = getenv("SLAM_LOCK"); if (e) c->ly.lock = atoi(e); }
   { const char* e = getenv("SLAM_LCACHE"); if (e) c->ly.lcache = atoi(e); }
@@ -431,7 +473,6 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   c->stream = (cudaStream_t)cuda_stream;
   char* base = (char*)workspace;
   c->stats = (unsigned long long*)(base + p.stats);
-  c->ovf = (int*)(base + p.ovf);
   c->state = (float*)(base + p.state);
   c->cov_cache = (float*)(base + p.cache);
   c->st_odom = (float*)(base + p.odom);
@@ -445,8 +486,8 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   c->launches = 0;
   c->err[0] = 0;
   c->un_pose = nullptr; c->un_info = nullptr; c->un_valid = nullptr;
-  c->smem_bytes = c->ly.warp_words * 4 * wpc;
-  if (cudaFuncSetAttribute(kernel_of(team), cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) {
+  c->smem_bytes = (c->ly.team_words * wpc + c->ly.pool) * 4;
+  if (cudaFuncSetAttribute(kernel_of(team), cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET) != cudaSuccess) {
     cudaGetLastError();
     delete c;
     return SLAM_ECUDA;
@@ -459,33 +500,6 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   c->ctas_per_sm = occ;
   const int need = (batch + wpc - 1) / wpc;
   c->grid = need < sms * occ ? need : sms * occ;
-  // optional first launch with a smaller capacity (more environments in flight per SM)
-  c->two_pass = false;
-  const int cap = pick_cap(window, landmarks, team);
-  if (cap > 0) {
-    const int wpc_s = pick_wpc(window, landmarks, team, cap);
-    c->ly_small = make_layout(batch, window, landmarks, cap, wpc_s);
-    c->ly_small.team = team;
-    c->ly_small.lock = c->ly.lock;
-    c->ly_small.lcache = c->ly.lcache;
-    c->smem_small = c->ly_small.warp_words * 4 * wpc_s;
-    int occ_s = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_s, kernel_of(team), wpc_s * team, c->smem_small);
-    if (occ_s >= 1 && occ_s * wpc_s > occ * wpc) {
-      c->two_pass = true;
-      c->ctas_small = occ_s;
-      const int need_s = (batch + wpc_s - 1) / wpc_s;
-      c->grid_small = need_s < sms * occ_s ? need_s : sms * occ_s;
-    }
-  }
-  c->h_ovf = nullptr; c->ovf_ev = nullptr; c->ovf_pending = false; c->ovf_last = 0; c->dense_streak = 0;
-  c->adaptive = c->two_pass;
-  { const char* e = getenv("SLAM_ADAPTIVE"); if (e && e[0] == '0') c->adaptive = false; }
-  if (c->adaptive && (cudaHostAlloc((void**)&c->h_ovf, sizeof(int), cudaHostAllocDefault) != cudaSuccess ||
-                      cudaEventCreateWithFlags(&c->ovf_ev, cudaEventDisableTiming) != cudaSuccess)) {
-    cudaGetLastError();
-    c->adaptive = false;  // no feedback channel: always run both passes
-  }
   *out = c;
   const int rc = slam_reset(c, nullptr);
   if (rc != SLAM_OK) { *out = nullptr; slam_destroy(c); }
@@ -494,8 +508,6 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
 
 void slam_destroy(slam_ctx* ctx) {
   if (!ctx) return;
-  if (ctx->ovf_ev) { cudaEventSynchronize(ctx->ovf_ev); cudaEventDestroy(ctx->ovf_ev); }
-  if (ctx->h_ovf) cudaFreeHost(ctx->h_ovf);
   delete ctx;
 }
 
@@ -506,39 +518,14 @@ int slam_reset(slam_ctx* c, const float* init_pose) {
   slam_reset_kernel<<<blocks, threads, 0, c->stream>>>(c->ly, c->pr, c->state, init_pose);
   c->launches++;
   c->head = 0; c->count = 1; c->cov_valid = false;
-  c->ovf_last = 0; c->dense_streak = 0;
   return check_cuda(c, "slam_reset");
 }
 
 static int launch_step(slam_ctx* c, int flags, int iters, const StepIO& io) {
   const step_fn fn = kernel_of(c->ly.team);
-  bool two = c->two_pass;
-  const bool solves = iters > 0 || (flags & (F_COV | F_MARG));
-  if (two && c->adaptive && solves) {
-    if (c->ovf_pending && cudaEventQuery(c->ovf_ev) == cudaSuccess) { c->ovf_last = *c->h_ovf; c->ovf_pending = false; }
-    if (2 * (long long)c->ovf_last > c->ly.N) {
-      if (++c->dense_streak % 8 != 0) two = false;
-    } else {
-      c->dense_streak = 0;
-    }
-  }
-  if (two) {
-    cudaMemsetAsync(c->ovf, 0, 4, c->stream);
-    fn<<<c->grid_small, c->ly_small.wpc * c->ly.team, c->smem_small, c->stream>>>(c->ly_small, c->pr, c->state, c->head, c->count,
-                                                                                   flags, iters, io, c->stats, 0, c->ovf);
-    if (c->adaptive && solves && !c->ovf_pending) {
-      cudaMemcpyAsync(c->h_ovf, c->ovf, 4, cudaMemcpyDeviceToHost, c->stream);
-      cudaEventRecord(c->ovf_ev, c->stream);
-      c->ovf_pending = true;
-    }
-    fn<<<c->grid, c->ly.wpc * c->ly.team, c->smem_bytes, c->stream>>>(c->ly, c->pr, c->state, c->head, c->count, flags, iters,
-                                                                        io, c->stats, 1, c->ovf);
-    c->launches += 2;
-  } else {
-    fn<<<c->grid, c->ly.wpc * c->ly.team, c->smem_bytes, c->stream>>>(c->ly, c->pr, c->state, c->head, c->count, flags, iters,
-                                                                        io, c->stats, 0, c->ovf);
-    c->launches++;
-  }
+  fn<<<c->grid, c->ly.wpc * c->ly.team, c->smem_bytes, c->stream>>>(c->ly, c->pr, c->state, c->head, c->count, flags, iters, io,
+                                                                      c->stats);
+  c->launches++;
   return check_cuda(c, "slam_step_kernel");
 }
 
@@ -728,9 +715,9 @@ const char* slam_last_error(const slam_ctx* c) { return c ? c->err : "null conte
 
 int slam_kernel_info(const slam_ctx* c, int* smem_bytes_per_cta, int* warps_per_cta, int* ctas_per_sm) {
   if (!c) return SLAM_EINVAL;
-  if (smem_bytes_per_cta) *smem_bytes_per_cta = c->two_pass ? c->smem_small : c->smem_bytes;
-  if (warps_per_cta) *warps_per_cta = (c->two_pass ? c->ly_small.wpc : c->ly.wpc) * c->ly.team / 32;
-  if (ctas_per_sm) *ctas_per_sm = c->two_pass ? c->ctas_small : c->ctas_per_sm;
+  if (smem_bytes_per_cta) *smem_bytes_per_cta = c->smem_bytes;
+  if (warps_per_cta) *warps_per_cta = c->ly.wpc * c->ly.team / 32;
+  if (ctas_per_sm) *ctas_per_sm = c->ctas_per_sm;
   return SLAM_OK;
 }
 

@@ -45,9 +45,9 @@ __device__ __forceinline__ WS make_ws(const Layout& ly, float* base) {
   WS w;
   w.st = base + ly.s_st; w.zodo = base + ly.s_zodo; w.zlc = base + ly.s_zlc;
   w.lct = (int*)(base + ly.s_lct); w.cs = base + ly.s_cs; w.rbm = (uint32_t*)(base + ly.s_rbm);
-  w.first = (int*)(base + ly.s_first); w.rbase = (int*)(base + ly.s_rbase); w.amask = (uint32_t*)(base + ly.s_amask);
+  w.first = (int*)(base + ly.s_first); w.rbase = (int*)(base + ly.s_rbase);
   w.ssup = (int*)(base + ly.s_ssup); w.sidx = (int*)(base + ly.s_sidx); w.sds = base + ly.s_sds;
-  w.H = base + ly.s_H;
+  w.amask = nullptr; w.H = nullptr;  // set once the environment has its share of the CTA pool (slam_step_kernel)
   return w;
 }
 
@@ -122,7 +122,7 @@ __device__ __forceinline__ float warp_sum(float v) {
 template <int TEAM>
 struct Team {
   int bar;     // named barrier id (1..15)
-  float* scr;  // shared scratch, 384 floats: [0,64) reductions / diagonal tile, [64,384) fp64 covariance tail
+  float* scr;  // shared scratch, 64 floats: reductions, diagonal tile, counters of the symbolic phase
   static constexpr int NW = TEAM / 32;
   __device__ __forceinline__ void sync() const {
     if (TEAM == 32) __syncwarp();
@@ -467,14 +467,32 @@ __device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, const Team
     if (lane == 0) reinterpret_cast<int*>(tm.scr)[8] = run;
   }
   tm.sync();
-  // active row pairs per 4-column block J: pair p (rows 2p, 2p+1; the rhs pair is p = np/2) takes part
-  // in column J iff first <= 4J <= 2p.  Compact lists: aoff[J] (16 bit) offsets into alist (8-bit pair
-  // indices, ascending, so the two diagonal pairs 2J and 2J+1 come first).  Built by the first warp.
   if (lane < 32) {  // loop-closure mask for assemble
     const uint32_t lo = __ballot_sync(FULLMASK, lane < c && w.lct[lane] >= 0);
     const uint32_t hi = __ballot_sync(FULLMASK, lane + 32 < c && w.lct[lane + 32] >= 0);
     if (lane == 0) { w.lct[ly.W] = (int)lo; w.lct[ly.W + 1] = (int)hi; }
   }
+  // words of the active-pair lists (build_lists): pair p (rows 2p, 2p+1; the rhs pair is p = np/2) is
+  // active in the column blocks J with first <= 4J <= 2p, so the list sizes follow from first[] alone
+  if (lane < 32) {
+    const int G = np >> 2, NP = (np >> 1) + 1;
+    int cntp = 0;
+    for (int p = lane; p < NP; p += 32) cntp += min(p >> 1, G - 1) - (w.first[2 * p] >> 2) + 1;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) cntp += __shfl_xor_sync(FULLMASK, cntp, o);
+    if (lane == 0) reinterpret_cast<int*>(tm.scr)[10] = ((2 * (G + 2) + cntp + 3) >> 2) + 3 & ~3;
+  }
+  tm.sync();
+  return reinterpret_cast<const int*>(tm.scr)[8];
+}
+
+// Second part of the symbolic phase, after the environment got its share of the pool (w.amask is set):
+// active row pairs per 4-column block J: pair p (rows 2p, 2p+1; the rhs pair is p = np/2) takes part
+// in column J iff first <= 4J <= 2p.  Compact lists: aoff[J] (16 bit) offsets into alist (8-bit pair
+// indices, ascending, so the two diagonal pairs 2J and 2J+1 come first).  Built by the first warp.
+template <int TEAM>
+__device__ void build_lists(const Layout& ly, const WS& w, const Team<TEAM>& tm, int lane) {
+  const int np = ly.np;
   if (lane < 32) {
     const int G = np >> 2, NP = (np >> 1) + 1;
     unsigned short* aoff = reinterpret_cast<unsigned short*>(w.amask);
@@ -495,8 +513,8 @@ __device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, const Team
     if (lane == 0) { aoff[G] = (unsigned short)run; reinterpret_cast<int*>(tm.scr)[9] = maxcnt; }
   }
   tm.sync();
-  return reinterpret_cast<const int*>(tm.scr)[8];
 }
+
 
 // ------------------------------------------------------------------ S1 + S2: linearise and assemble
 struct Between {  // residual and the pieces of J_i, J_j of a between factor (A.2)
@@ -587,7 +605,7 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
     for (int t = lane; t < total; t += TEAM) w.H[t] = 0.f;
   } else {
     for (int i = lane; i < n + 2; i += TEAM) {
-      const int lo = i < n ? max((int)w.first[i], cb) : 0, hi = (i | 3) + 1;
+      const int lo = i < n ? max((int)w.first[i], cb) : 0, hi = i < n ? (i | 3) + 1 : n;  // (the rhs rows span [0, n))
       float4* z = reinterpret_cast<float4*>(w.H + w.rbase[i] + lo);
       for (int t = 0; t < (hi - lo) >> 2; ++t) z[t] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
@@ -1156,7 +1174,9 @@ template <int TEAM>
 __device__ void covariance(const Layout& ly, const WS& w, const Team<TEAM>& tm, int lane, int env, int c, const StepIO& io) {
   if (lane >= 32) return;  // first warp of the team; stages separated by __syncwarp, fp64 scratch in shared memory
   const int n = ly.np, N = ly.N;
-  double* Lm = reinterpret_cast<double*>(tm.scr + 64);  // [6][6] trailing block of L (diagonal = 1/L_jj)
+  // fp64 scratch (135 doubles) at the start of this environment's pool share: the factor is dead after
+  // this call, and the trailing block is read into registers before the first scratch word is written
+  double* Lm = reinterpret_cast<double*>(w.H);          // [6][6] trailing block of L (diagonal = 1/L_jj)
   double* Li = Lm + 36;                                 // [6][6] its inverse
   double* S6 = Li + 36;                                 // [6][6] Sigma_6 = Li' Li
   double* T = S6 + 36;                                  // [6][3] Sigma_6 J'
@@ -1169,16 +1189,22 @@ __device__ void covariance(const Layout& ly, const WS& w, const Team<TEAM>& tm, 
   const float* e = w.st + st_pose(c >= 2 ? c - 1 : 0);
   const double dx = ca * e[0] - sa * e[1], dy = sa * e[0] + ca * e[1];
   const double J[3][6] = {{je * ca, -je * sa, 0, 1, 0, -dy}, {je * sa, je * ca, 0, 0, 1, dx}, {0, 0, je, 0, 0, 1}};
+  float lrow[6];
   if (lane < 6) {  // row `lane` of the trailing block
     const int i = n - 6 + lane, fi = w.first[i];
+#pragma unroll
     for (int y = 0; y < 6; ++y) {
       const int j = n - 6 + y;
-      double v = 0.0;
-      if (y == lane) v = (double)w.H[w.rbase[i] + i];
-      else if (y < lane && j >= fi) v = (double)w.H[w.rbase[i] + j];
-      Lm[lane * 6 + y] = v;
-      Li[lane * 6 + y] = 0.0;
+      float v = 0.f;
+      if (y == lane) v = w.H[w.rbase[i] + i];
+      else if (y < lane && j >= fi) v = w.H[w.rbase[i] + j];
+      lrow[y] = v;
     }
+  }
+  __syncwarp();
+  if (lane < 6) {
+#pragma unroll
+    for (int y = 0; y < 6; ++y) { Lm[lane * 6 + y] = (double)lrow[y]; Li[lane * 6 + y] = 0.0; }
   }
   __syncwarp();
   if (lane < 6) {  // column `lane` of L^{-1} by forward substitution

@@ -20,11 +20,14 @@ struct Layout {
   // record (32-bit words)
   int rec;             // record stride
   int o_status, o_k0, o_pm, o_lm, o_act, o_um, o_a, o_e, o_m, o_zodo, o_lct, o_zlc, o_rbm, o_zrb, o_zun, o_omun, o_vbar, o_g, o_lam;
-  // shared memory per warp (32-bit words)
-  int s_scr, s_st, s_zodo, s_zlc, s_lct, s_cs, s_rbm, s_first, s_rbase, s_amask, s_ssup, s_sidx, s_sds, s_H;
-  int mw;              // 32-bit words of an active-row-pair mask (np/2 + 1 bits)
-  int cap;             // words available for H (envelope + rhs row) / marginalisation scratch
-  int warp_words;      // total shared words per warp
+  // shared memory: a FIXED part per team (32-bit words) ...
+  int s_scr, s_st, s_zodo, s_zlc, s_lct, s_cs, s_rbm, s_first, s_rbase, s_ssup, s_sidx, s_sds;
+  int team_words;      // fixed shared words per team
+  // ... and one POOL per CTA from which every environment of a round takes what its envelope needs
+  // (H + rhs rows + active-pair lists, or the marginalisation scratch): slam_step_kernel
+  int pool;            // words of the pool (>= dense: one environment always fits)
+  int cap;             // = pool: the most one environment can get
+  int dense;           // words that suffice for ANY environment of this size
   int wpc;             // teams (environments in flight) per CTA
   int team;            // threads per environment: 32, 64 or 128
   int lcache;          // 1: keep the factor columns of passive landmarks across the linearisations of one call
@@ -37,8 +40,8 @@ struct Params {
 
 static inline int pad4(int x) { return (x + 3) & ~3; }
 
-// Fills every offset.  `cap` < 0 selects the dense capacity (always sufficient).
-static inline Layout make_layout(int N, int W, int L, int cap, int wpc) {
+// Fills every offset.  `pool` = words of the CTA pool (raised to the dense need of one environment).
+static inline Layout make_layout(int N, int W, int L, int pool, int wpc) {
   Layout y;
   y.N = N; y.W = W; y.L = L; y.n = 3 * W + 2 * L; y.nw = (L + 31) / 32;
   y.np = (y.n + 3) & ~3; y.pad = y.np - y.n;
@@ -66,7 +69,7 @@ static inline Layout make_layout(int N, int W, int L, int cap, int wpc) {
   y.rec = (o + 31) & ~31;  // 128-byte multiple
 
   int s = 0;
-  y.s_scr = s; s += 384;  // team scratch (reductions, diagonal tile, fp64 covariance tail)
+  y.s_scr = s; s += 64;   // team scratch (reductions, diagonal tile, counters)
   y.s_st = s; s = pad4(s + n + 3);
   y.s_zodo = s; s = pad4(s + 3 * W);
   y.s_zlc = s; s = pad4(s + 3 * W);
@@ -75,24 +78,22 @@ static inline Layout make_layout(int N, int W, int L, int cap, int wpc) {
   y.s_rbm = s; s = pad4(s + W * y.nw);
   y.s_first = s; s = pad4(s + y.np + 2);
   y.s_rbase = s; s = pad4(s + y.np + 2);
-  y.mw = (y.np / 2 + 1 + 31) / 32;
-  {  // active-pair lists: G+1 offsets (16 bit) then at most sum_J (NP - 2J) pair indices (8 bit)
-    const int G4 = y.np / 4, NPp = y.np / 2 + 1;
-    const int bytes = 2 * (G4 + 2) + G4 * NPp - G4 * (G4 - 1);
-    y.s_amask = s; s = pad4(s + (bytes + 3) / 4);
-  }
   y.s_ssup = s; s = pad4(s + n);
   y.s_sidx = s; s = pad4(s + n);
   y.s_sds = s; s = pad4(s + n + 2 * L);  // prior displacement (<= n) + anchor-frame landmarks (2L)
-  y.s_H = s;
-  // dense capacity: full 4x4 tiles of the lower triangle + two rhs rows; or the marginalisation scratch
-  const int G = y.np / 4;
-  int dense = 8 * G * (G + 1) + 2 * y.np;
+  y.team_words = pad4(s);
+  // dense need of one environment: full 4x4 tiles of the lower triangle + two rhs rows + the longest
+  // active-pair lists (G+2 offsets of 16 bit, then at most sum_J (NP - 2J) pair indices of 8 bit);
+  // or the marginalisation scratch; or the fp64 scratch of the covariance tail
+  const int G = y.np / 4, NPp = y.np / 2 + 1;
+  const int list_bytes = 2 * (G + 2) + G * NPp - G * (G - 1);
+  int dense = 8 * G * (G + 1) + 2 * y.np + pad4((list_bytes + 3) / 4);
   const int marg = n * (n + 1) / 2 + 8 * n + 16;
   if (marg > dense) dense = marg;
-  y.cap = pad4(cap < 0 ? dense : cap);
-  s += y.cap;
-  y.warp_words = pad4(s);
+  if (dense < 272) dense = 272;
+  y.dense = pad4(dense);
+  y.pool = pool < y.dense ? y.dense : (pool & ~3);
+  y.cap = y.pool;
   y.wpc = wpc;
   y.team = 32;
   y.lock = 1;
