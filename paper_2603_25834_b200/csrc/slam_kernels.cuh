@@ -480,27 +480,45 @@ __device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, const Team
     for (int p = lane; p < NP; p += 32) cntp += min(p >> 1, G - 1) - (w.first[2 * p] >> 2) + 1;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) cntp += __shfl_xor_sync(FULLMASK, cntp, o);
-    if (lane == 0) reinterpret_cast<int*>(tm.scr)[10] = ((2 * (G + 2) + cntp + 3) >> 2) + 3 & ~3;
+    if (lane == 0) reinterpret_cast<int*>(tm.scr)[10] = (G + 1) + NP + ((cntp + 3) >> 2) + 3 & ~3;
   }
   tm.sync();
   return reinterpret_cast<const int*>(tm.scr)[8];
 }
 
 // Second part of the symbolic phase, after the environment got its share of the pool (w.amask is set):
-// active row pairs per 4-column block J: pair p (rows 2p, 2p+1; the rhs pair is p = np/2) takes part
-// in column J iff first <= 4J <= 2p.  Compact lists: aoff[J] (16 bit) offsets into alist (8-bit pair
-// indices, ascending, so the two diagonal pairs 2J and 2J+1 come first).  Built by the first warp.
+// the tables the factorisation walks, so that one shared-memory load per column block and one per lane
+// replace the chains of dependent index look-ups (measured: ~280 instructions of fixed cost per block).
+//   hdr[J]   (G+1 words)  offset of the block's list (14 bit) | pairs in it (8 bit) | K-split log2 for
+//                         teams of 32 / 64 / 128 threads (2 bit each)
+//   ptab[p]  (NP words)   row pair p (rows 2p, 2p+1 of one 4-row group; p = np/2 is the rhs pair):
+//                         start of row 2p in H / 4 (14 bit) | first / 4 (7 bit) | row length / 4 (7 bit)
+//   alist    (bytes)      active pairs per 4-column block J: pair p takes part in column J iff
+//                         first <= 4J <= 2p; ascending, so the two diagonal pairs 2J, 2J+1 come first
+// Built by the first warp.
+struct Tables { const uint32_t* hdr; const uint32_t* ptab; const unsigned char* alist; };
+__device__ __forceinline__ Tables tables_of(const Layout& ly, const WS& w) {
+  Tables t;
+  t.hdr = w.amask;
+  t.ptab = w.amask + (ly.np >> 2) + 1;
+  t.alist = reinterpret_cast<const unsigned char*>(t.ptab + (ly.np >> 1) + 1);
+  return t;
+}
 template <int TEAM>
 __device__ void build_lists(const Layout& ly, const WS& w, const Team<TEAM>& tm, int lane) {
   const int np = ly.np;
   if (lane < 32) {
     const int G = np >> 2, NP = (np >> 1) + 1;
-    unsigned short* aoff = reinterpret_cast<unsigned short*>(w.amask);
-    unsigned char* alist = reinterpret_cast<unsigned char*>(aoff + G + 2);
+    uint32_t* hdr = w.amask;
+    uint32_t* ptab = hdr + G + 1;
+    unsigned char* alist = reinterpret_cast<unsigned char*>(ptab + NP);
+    for (int p = lane; p < NP; p += 32) {
+      const int i = 2 * p, f = w.first[i], len = i < np ? (i | 3) + 1 - f : np;
+      ptab[p] = (uint32_t)((w.rbase[i] + f) >> 2) | ((uint32_t)(f >> 2) << 14) | ((uint32_t)(len >> 2) << 21);
+    }
     int run = 0, maxcnt = 0;
     for (int J = 0; J < G; ++J) {
       const int start = run;
-      if (lane == 0) aoff[J] = (unsigned short)run;
       for (int base = 2 * J; base < NP; base += 32) {
         const int p = base + lane;
         const bool on = p < NP && w.first[2 * p] <= 4 * J;
@@ -508,13 +526,32 @@ __device__ void build_lists(const Layout& ly, const WS& w, const Team<TEAM>& tm,
         if (on) alist[run + __popc(bal & ((1u << lane) - 1u))] = (unsigned char)p;
         run += __popc(bal);
       }
-      maxcnt = max(maxcnt, run - start);
+      const int cnt = run - start;
+      maxcnt = max(maxcnt, cnt);
+      if (lane == 0) {
+        // K-split: when a column has fewer pairs than threads, 2^lg adjacent lanes share one pair and split
+        // its dot-product range; only worth it when the dot products are long
+        uint32_t lgs = 0;
+        if (4 * J - w.first[4 * J] >= 32) {
+#pragma unroll
+          for (int q = 0; q < 3; ++q) {
+            int lg = 0;
+            while (lg < 3 && (cnt << (lg + 1)) <= (32 << q)) ++lg;
+            lgs |= (uint32_t)lg << (2 * q);
+          }
+        }
+        hdr[J] = (uint32_t)start | ((uint32_t)cnt << 14) | (lgs << 22);
+      }
     }
-    if (lane == 0) { aoff[G] = (unsigned short)run; reinterpret_cast<int*>(tm.scr)[9] = maxcnt; }
+    if (lane == 0) { hdr[G] = (uint32_t)run; reinterpret_cast<int*>(tm.scr)[9] = maxcnt; }
   }
   tm.sync();
 }
-
+__device__ __forceinline__ float rsqrt_fast(float x) {  // MUFU.RSQ; the operands here are normal numbers
+  float y;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
 
 // ------------------------------------------------------------------ S1 + S2: linearise and assemble
 struct Between {  // residual and the pieces of J_i, J_j of a between factor (A.2)
@@ -987,22 +1024,22 @@ __device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int
   // this call (see assemble): there only the rhs pair -- the last entry of the column's list -- is
   // processed, on the lanes and with the K-split it has in a full pass, so y is bit-identical.
   const int np = ly.np, G = np >> 2;
+  const Tables tb = tables_of(ly, w);
   int flag = 0;
   for (int J = 0; J < G; ++J) {
     const int c0 = 4 * J;
-    const int fJ = w.first[c0];
-    const float* rJ0 = w.H + w.rbase[c0];
-    const float* rJ1 = w.H + w.rbase[c0 + 1];
-    const float* rJ2 = w.H + w.rbase[c0 + 2];
-    const float* rJ3 = w.H + w.rbase[c0 + 3];
+    const uint32_t hd = tb.hdr[J], eJ = tb.ptab[2 * J];
+    const int fJ = (int)((eJ >> 14) & 0x7fu) << 2, lenJ = (int)(eJ >> 21) << 2;
+    const float* rJ0 = w.H + ((int)(eJ & 0x3fffu) << 2) - fJ;  // the four rows of the block share first and length
+    const float* rJ1 = rJ0 + lenJ;
+    const float* rJ2 = rJ1 + lenJ;
+    const float* rJ3 = rJ2 + lenJ;
     // The ACTIVE row pairs of this column (compact list from the symbolic phase) sit on the lowest
     // threads.  K-split: when fewer pairs than threads, `ch` adjacent lanes share one pair and
     // split the dot-product range; partial sums are combined by shuffles.
-    const unsigned short* aoff = reinterpret_cast<const unsigned short*>(w.amask);
-    const unsigned char* alist = reinterpret_cast<const unsigned char*>(aoff + G + 2) + aoff[J];
-    const int cnt = aoff[J + 1] - aoff[J];
-    int lg = 0;  // ch = 1 << lg; only worth it when the dot products are long
-    if (c0 - fJ >= 32) while (lg < 3 && (cnt << (lg + 1)) <= TEAM) ++lg;
+    const unsigned char* alist = tb.alist + (hd & 0x3fffu);
+    const int cnt = (int)((hd >> 14) & 0xffu);
+    const int lg = (int)((hd >> (TEAM == 32 ? 22 : (TEAM == 64 ? 24 : 26))) & 3u);
     const int ch = 1 << lg;
     const int per_pass = TEAM >> lg;
     const int t = lane & (ch - 1);
@@ -1022,15 +1059,16 @@ __device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int
         if (first_pass) tm.sync();
         continue;
       }
-      const int i0 = act ? 2 * (int)alist[q] : c0;
       float4 a0 = make_float4(0.f, 0.f, 0.f, 0.f), a1 = a0;
       float* p0 = nullptr;
       float* p1 = nullptr;
       if (act) {
-        p0 = w.H + w.rbase[i0];
-        p1 = w.H + w.rbase[i0 + 1];
+        const uint32_t e = tb.ptab[alist[q]];
+        const int fi = (int)((e >> 14) & 0x7fu) << 2;
+        p0 = w.H + ((int)(e & 0x3fffu) << 2) - fi;
+        p1 = p0 + ((int)(e >> 21) << 2);
         if (t == 0) { a0 = ld4(p0 + c0); a1 = ld4(p1 + c0); }  // (rows np, np+1 are the rhs pair)
-        const int ks = max(w.first[i0], fJ);
+        const int ks = max(fi, fJ);
         const int nblk = (c0 - ks) >> 2;
         const int kb = ks + 4 * ((t * nblk) >> lg), ke = ks + 4 * (((t + 1) * nblk) >> lg);
         for (int k = kb; k < ke; k += 4) {
@@ -1063,19 +1101,19 @@ __device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int
           s30 = dg[6]; s31 = dg[7]; s32 = dg[8]; s33 = dg[9];
         }
         bool bad = !(s00 > 0.f);
-        d0 = rsqrtf(s00);
+        d0 = rsqrt_fast(s00);
         l10 = s10 * d0; l20 = s20 * d0; l30 = s30 * d0;
         const float t11 = fmaf(-l10, l10, s11);
         bad |= !(t11 > 0.f);
-        d1 = rsqrtf(t11);
+        d1 = rsqrt_fast(t11);
         l21 = fmaf(-l20, l10, s21) * d1; l31 = fmaf(-l30, l10, s31) * d1;
         const float t22 = fmaf(-l21, l21, fmaf(-l20, l20, s22));
         bad |= !(t22 > 0.f);
-        d2 = rsqrtf(t22);
+        d2 = rsqrt_fast(t22);
         l32 = fmaf(-l31, l21, fmaf(-l30, l20, s32)) * d2;
         const float t33 = fmaf(-l32, l32, fmaf(-l31, l31, fmaf(-l30, l30, s33)));
         bad |= !(t33 > 0.f);
-        d3 = rsqrtf(t33);
+        d3 = rsqrt_fast(t33);
         if (bad) {
           flag |= ENV_NOT_PD;
           if (!(s00 > 0.f)) d0 = 1.f;
@@ -1110,13 +1148,16 @@ __device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int
 template <int TEAM>
 __device__ void back_substitute(const Layout& ly, const WS& w, const Team<TEAM>& tm, int lane) {
   const int np = ly.np, G = np >> 2;
+  const Tables tb = tables_of(ly, w);
   float* y = w.H + w.rbase[np];
   for (int I = G - 1; I >= 0; --I) {
     const int c0 = 4 * I;
-    const float* r0 = w.H + w.rbase[c0];
-    const float* r1 = w.H + w.rbase[c0 + 1];
-    const float* r2 = w.H + w.rbase[c0 + 2];
-    const float* r3 = w.H + w.rbase[c0 + 3];
+    const uint32_t eI = tb.ptab[2 * I];
+    const int fI = (int)((eI >> 14) & 0x7fu) << 2, lenI = (int)(eI >> 21) << 2;
+    const float* r0 = w.H + ((int)(eI & 0x3fffu) << 2) - fI;
+    const float* r1 = r0 + lenI;
+    const float* r2 = r1 + lenI;
+    const float* r3 = r2 + lenI;
     const float4 yy = ld4(y + c0), t0 = ld4(r0 + c0), t1 = ld4(r1 + c0), t2 = ld4(r2 + c0), t3 = ld4(r3 + c0);
     const float e3 = yy.w * t3.w;
     const float e2 = fmaf(-t3.z, e3, yy.z) * t2.z;
@@ -1124,7 +1165,7 @@ __device__ void back_substitute(const Layout& ly, const WS& w, const Team<TEAM>&
     const float e0 = fmaf(-t3.x, e3, fmaf(-t2.x, e2, fmaf(-t1.x, e1, yy.x))) * t0.x;
     tm.sync();
     if (lane == 0) st4(y + c0, make_float4(e0, e1, e2, e3));
-    for (int k = w.first[c0] + 4 * lane; k < c0; k += 4 * TEAM) {
+    for (int k = fI + 4 * lane; k < c0; k += 4 * TEAM) {
       const float4 x0 = ld4(r0 + k), x1 = ld4(r1 + k), x2 = ld4(r2 + k), x3 = ld4(r3 + k);
       float4 v = ld4(y + k);
       v.x = fmaf(-x3.x, e3, fmaf(-x2.x, e2, fmaf(-x1.x, e1, fmaf(-x0.x, e0, v.x))));
