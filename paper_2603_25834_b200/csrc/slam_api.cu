@@ -32,7 +32,7 @@ using namespace slamk;
 template <int TEAM>
 __global__ void __launch_bounds__(TEAM == 128 ? 896 : SLAM_MAXTHREADS)
 slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flags, int iters, StepIO io,
-                 unsigned long long* stats) {
+                 unsigned long long* stats, const int* __restrict__ perm, int* __restrict__ keys) {
   extern __shared__ float4 smem4[];
   __shared__ int s_env[16], s_need[16], s_off[16], s_new[16], s_ctl[2];
   float* smem = reinterpret_cast<float*>(smem4);
@@ -71,8 +71,11 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
       int nk = s_ctl[0], live = 0;
       for (int t = 0; t < ly.wpc; ++t) {
         if (s_off[t] != -1) {
-          const long long e = (long long)blockIdx.x + (long long)nk * gridDim.x;
-          if (e < ly.N) { s_env[t] = (int)e; ++nk; } else s_env[t] = -1;
+          // the k-th environment of this CTA: chunks of wpc consecutive entries of the cost-ordered list
+          // (slam_order_kernel), dealt round-robin to the CTAs -- the environments of one round cost about
+          // the same, so the lock-step barriers wait for little, and every CTA gets the same mix
+          const long long idx = ((long long)(nk / ly.wpc) * gridDim.x + blockIdx.x) * ly.wpc + nk % ly.wpc;
+          if (idx < ly.N) { s_env[t] = perm[idx]; ++nk; } else s_env[t] = -1;
         }
         live += s_env[t] >= 0;
       }
@@ -101,6 +104,7 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
           total = symbolic<TEAM>(ly, od, w, tm, lane, cc, mk, s);
           need = max(need, total + reinterpret_cast<const int*>(tm.scr)[10]);
           if (flags & F_COV) need = max(need, 272);  // fp64 scratch of the covariance tail
+          if (lane == 0) keys[env] = total;  // cost key for the order of the next launches
           if (stats && lane == 0) {  // envelope statistics (words per environment): max, sum, count
             atomicMax(stats + 0, (unsigned long long)total);
             atomicAdd(stats + 1, (unsigned long long)total);
@@ -199,10 +203,60 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
   }
 }
 
+// Cost order of the environments for the next launches: counting sort of keys[] (envelope words of the
+// last solve, a good predictor of this step's cost: the window slides by one pose) into perm[], most
+// expensive first.  One CTA.  Keys cluster (many environments share an envelope size), so lanes with the
+// same bucket are combined by __match_any_sync before the shared-memory atomic.  The order inside a
+// bucket is arbitrary -- scheduling only, the results do not depend on it.
+#define ORDER_BUCKETS 1024
+__global__ void __launch_bounds__(1024) slam_order_kernel(int N, int key_max, const int* __restrict__ keys, int* __restrict__ perm) {
+  __shared__ int cnt[ORDER_BUCKETS];
+  __shared__ int wsum[32];
+  const int tid = threadIdx.x, lane = tid & 31;
+  cnt[tid] = 0;
+  __syncthreads();
+  const float scale = (float)(ORDER_BUCKETS - 1) / (float)(key_max > 0 ? key_max : 1);
+  const int rounds = (N + 1023) >> 10;
+  for (int r = 0; r < rounds; ++r) {
+    const int i = r * 1024 + tid;
+    const int b = i < N ? ORDER_BUCKETS - 1 - (int)((float)min(max(keys[i], 0), key_max) * scale) : -1;
+    const unsigned m = __match_any_sync(0xffffffffu, b);
+    if (b >= 0 && lane == __ffs(m) - 1) atomicAdd(&cnt[b], __popc(m));
+  }
+  __syncthreads();
+  // exclusive scan of the 1024 counters
+  const int v = cnt[tid];
+  int x = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+  if (lane == 31) wsum[tid >> 5] = x;
+  __syncthreads();
+  if (tid < 32) {
+    int w = wsum[tid];
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, w, o); if (tid >= o) w += y; }
+    wsum[tid] = w;
+  }
+  __syncthreads();
+  cnt[tid] = x - v + (tid >= 32 ? wsum[(tid >> 5) - 1] : 0);
+  __syncthreads();
+  for (int r = 0; r < rounds; ++r) {
+    const int i = r * 1024 + tid;
+    const int b = i < N ? ORDER_BUCKETS - 1 - (int)((float)min(max(keys[i], 0), key_max) * scale) : -1;
+    const unsigned m = __match_any_sync(0xffffffffu, b);
+    const int leader = __ffs(m) - 1;
+    int base = 0;
+    if (b >= 0 && lane == leader) base = atomicAdd(&cnt[b], __popc(m));
+    base = __shfl_sync(0xffffffffu, base, leader);
+    if (b >= 0) perm[base + __popc(m & ((1u << lane) - 1u))] = i;
+  }
+}
+
 // reset: one warp per environment
-__global__ void slam_reset_kernel(Layout ly, Params pr, float* state, const float* init_pose) {
+__global__ void slam_reset_kernel(Layout ly, Params pr, float* state, const float* init_pose, int* perm, int* keys) {
   const int env = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (env >= ly.N) return;
+  if (lane == 0) { perm[env] = env; keys[env] = 0; }
   float* rec = state + (size_t)env * ly.rec;
   int* reci = reinterpret_cast<int*>(rec);
   for (int i = lane; i < ly.o_lam + 8; i += 32) rec[i] = 0.f;
@@ -318,6 +372,8 @@ struct slam_ctx {
   float* state;
   float* cov_cache;
   unsigned long long* stats;  // [8] device counters: max / sum / count of envelope words, ...
+  int *perm, *keys;           // [N] cost order of the environments and the keys it is sorted by
+  bool order;                 // re-sort after every solve (SLAM_ORDER=0 disables)
   // device staging for slam_step_host
   float *st_odom, *st_lc_meas, *st_rb_meas, *st_cov, *st_logdet, *st_pose;
   int32_t* st_lc_back;
@@ -376,12 +432,11 @@ static int pick_launch(int W, int L, int team, int* pool_words) {
   const double typical = (L > 0 ? 0.5 : 0.34) * d.dense;
   int best = 0, best_pool = 0;
   double best_est = 0.0;
-  // ctas = 2: two smaller CTAs per SM (each with its own pool) when that loses no team: their lock-step
-  // phases drift apart, which spreads the load on the shared-memory and FMA pipes, and the tail of the
-  // last wave is finer grained (measured with fixed slots, config 2: 0.697 -> 0.585 ms per step,
-  // config 3: 2.89 -> 2.64).  SLAM_SPLIT_CTA=0 disables.
+  // ctas = 2 (SLAM_SPLIT_CTA=1): two smaller CTAs per SM, each with its own pool.  It paid with fixed
+  // slots per team (the phases of the two CTAs drift apart); with the pool one large CTA packs better
+  // (measured, ms per step, one / two CTAs: config 3 2.34 / 2.46, config 4 3.31 / 3.42).
   const char* sp = getenv("SLAM_SPLIT_CTA");
-  const int max_ctas = (sp && sp[0] == '0') ? 1 : 2;
+  const int max_ctas = (sp && sp[0] == '1') ? 2 : 1;
   for (int ctas = 1; ctas <= max_ctas; ++ctas) {
     const int budget = ctas == 1 ? SMEM_BUDGET : (228 * 1024 / 2 - 1024 - 512);
     for (int wpc = 1; wpc * ctas <= max_teams(team); ++wpc) {
@@ -398,17 +453,19 @@ static int pick_launch(int W, int L, int team, int* pool_words) {
   *pool_words = best_pool;
   return best;  // 0 if one environment does not fit
 }
-typedef void (*step_fn)(Layout, Params, float*, int, int, int, int, StepIO, unsigned long long*);
+typedef void (*step_fn)(Layout, Params, float*, int, int, int, int, StepIO, unsigned long long*, const int*, int*);
 static step_fn kernel_of(int team) {
   return team == 128 ? slam_step_kernel<128> : (team == 64 ? slam_step_kernel<64> : slam_step_kernel<32>);
 }
 
-struct WsPlan { size_t stats, state, cache, odom, lcb, lcm, rbk, rbm, cov, ld, pose, total; };
+struct WsPlan { size_t stats, perm, keys, state, cache, odom, lcb, lcm, rbk, rbm, cov, ld, pose, total; };
 static WsPlan plan(const Layout& ly) {
   WsPlan p;
   size_t o = 0;
   const size_t N = (size_t)ly.N;
   p.stats = o; o = al256(o + 64);
+  p.perm = o; o = al256(o + N * 4);
+  p.keys = o; o = al256(o + N * 4);
   p.state = o; o = al256(o + N * ly.rec * 4);
   p.cache = o; o = al256(o + N * 10 * 4);
   p.odom = o; o = al256(o + N * 3 * 4);
@@ -473,6 +530,9 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   c->stream = (cudaStream_t)cuda_stream;
   char* base = (char*)workspace;
   c->stats = (unsigned long long*)(base + p.stats);
+  c->perm = (int*)(base + p.perm);
+  c->keys = (int*)(base + p.keys);
+  { const char* e = getenv("SLAM_ORDER"); c->order = !(e && e[0] == '0'); }
   c->state = (float*)(base + p.state);
   c->cov_cache = (float*)(base + p.cache);
   c->st_odom = (float*)(base + p.odom);
@@ -515,7 +575,7 @@ int slam_reset(slam_ctx* c, const float* init_pose) {
   if (!c) return SLAM_EINVAL;
   const int threads = 256, blocks = (int)(((size_t)c->ly.N * 32 + threads - 1) / threads);
   cudaMemsetAsync(c->stats, 0, 64, c->stream);
-  slam_reset_kernel<<<blocks, threads, 0, c->stream>>>(c->ly, c->pr, c->state, init_pose);
+  slam_reset_kernel<<<blocks, threads, 0, c->stream>>>(c->ly, c->pr, c->state, init_pose, c->perm, c->keys);
   c->launches++;
   c->head = 0; c->count = 1; c->cov_valid = false;
   return check_cuda(c, "slam_reset");
@@ -524,8 +584,14 @@ int slam_reset(slam_ctx* c, const float* init_pose) {
 static int launch_step(slam_ctx* c, int flags, int iters, const StepIO& io) {
   const step_fn fn = kernel_of(c->ly.team);
   fn<<<c->grid, c->ly.wpc * c->ly.team, c->smem_bytes, c->stream>>>(c->ly, c->pr, c->state, c->head, c->count, flags, iters, io,
-                                                                      c->stats);
+                                                                      c->stats, c->perm, c->keys);
   c->launches++;
+  // the solve left fresh cost keys: order the next launches by them (pointless unless every CTA runs
+  // several rounds, and a small batch is latency bound: one more kernel boundary per step would show)
+  if (c->order && iters > 0 && (long long)c->ly.N >= 4ll * c->grid * c->ly.wpc) {
+    slam_order_kernel<<<1, 1024, 0, c->stream>>>(c->ly.N, c->ly.dense, c->keys, c->perm);
+    c->launches++;
+  }
   return check_cuda(c, "slam_step_kernel");
 }
 

@@ -53,6 +53,12 @@ __device__ __forceinline__ WS make_ws(const Layout& ly, float* base) {
 
 // ------------------------------------------------------------------ small helpers
 #define FULLMASK 0xffffffffu
+#ifndef SLAM_KUNROLL
+#define SLAM_KUNROLL 1   // unroll factor of the factorisation's dot-product loop
+#endif
+#ifndef SLAM_KSPLIT_MIN
+#define SLAM_KSPLIT_MIN 32  // shortest dot product (columns) for which lanes split the range
+#endif
 
 __device__ __forceinline__ float wrapf(float x) {  // to [-pi, pi], 2*pi split hi/lo
   const float k = rintf(x * 0.15915494309189535f);
@@ -532,7 +538,7 @@ __device__ void build_lists(const Layout& ly, const WS& w, const Team<TEAM>& tm,
         // K-split: when a column has fewer pairs than threads, 2^lg adjacent lanes share one pair and split
         // its dot-product range; only worth it when the dot products are long
         uint32_t lgs = 0;
-        if (4 * J - w.first[4 * J] >= 32) {
+        if (4 * J - w.first[4 * J] >= SLAM_KSPLIT_MIN) {
 #pragma unroll
           for (int q = 0; q < 3; ++q) {
             int lg = 0;
@@ -1025,6 +1031,7 @@ __device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int
   // processed, on the lanes and with the K-split it has in a full pass, so y is bit-identical.
   const int np = ly.np, G = np >> 2;
   const Tables tb = tables_of(ly, w);
+  constexpr int KUNROLL = SLAM_KUNROLL;
   int flag = 0;
   for (int J = 0; J < G; ++J) {
     const int c0 = 4 * J;
@@ -1071,6 +1078,7 @@ __device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int
         const int ks = max(fi, fJ);
         const int nblk = (c0 - ks) >> 2;
         const int kb = ks + 4 * ((t * nblk) >> lg), ke = ks + 4 * (((t + 1) * nblk) >> lg);
+#pragma unroll KUNROLL
         for (int k = kb; k < ke; k += 4) {
           const float4 x0 = ld4(p0 + k), x1 = ld4(p1 + k);
           const float4 b0 = ld4(rJ0 + k), b1 = ld4(rJ1 + k), b2 = ld4(rJ2 + k), b3 = ld4(rJ3 + k);
