@@ -416,8 +416,8 @@ static int pick_team(int W, int L, int batch) {
   return 32;
 }
 static int max_teams(int team) {  // threads per CTA: register file (launch bounds), 15 named barriers, 16 table slots
-  int maxt = team == 128 ? 7 : (team == 64 ? SLAM_MAXTHREADS / 64 : 15);
-  if (maxt > 15) maxt = 15;
+  int maxt = team == 128 ? 7 : SLAM_MAXTHREADS / team;   // (32 threads: 16 teams = the whole register file)
+  if (maxt > (team == 32 ? 16 : 15)) maxt = team == 32 ? 16 : 15;
   const char* e = getenv("SLAM_MAX_WPC");
   if (e && atoi(e) >= 1 && atoi(e) < maxt) maxt = atoi(e);
   return maxt;
@@ -587,8 +587,10 @@ static int launch_step(slam_ctx* c, int flags, int iters, const StepIO& io) {
                                                                       c->stats, c->perm, c->keys);
   c->launches++;
   // the solve left fresh cost keys: order the next launches by them (pointless unless every CTA runs
-  // several rounds, and a small batch is latency bound: one more kernel boundary per step would show)
-  if (c->order && iters > 0 && (long long)c->ly.N >= 4ll * c->grid * c->ly.wpc) {
+  // several rounds; a small batch is latency bound: one more kernel boundary per step would show; and
+  // measured only landmark windows gain -- their cost varies most: config 3 2.40 -> 2.31 ms per step,
+  // config 4 3.49 -> 3.53)
+  if (c->order && iters > 0 && c->ly.L > 0 && (long long)c->ly.N >= 4ll * c->grid * c->ly.wpc) {
     slam_order_kernel<<<1, 1024, 0, c->stream>>>(c->ly.N, c->ly.dense, c->keys, c->perm);
     c->launches++;
   }
