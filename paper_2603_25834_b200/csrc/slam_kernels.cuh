@@ -36,20 +36,28 @@ struct StepIO {
   const float* un_pose; const float* un_info; const int32_t* un_valid;
 };
 
-struct WS {  // per-warp views into shared memory
-  float* st; float* zodo; float* zlc; int* lct; float* cs; uint32_t* rbm;
-  int* first; int* rbase; uint32_t* amask;  /* amask: active-pair lists per column block */ int* ssup; int* sidx; float* sds; float* H;
+struct WS {  // per-team views into shared memory
+  float* st; int* lct; float* cs; uint32_t* rbm;
+  uint32_t* rbf;   // per matrix row: offset such that H(i,j) = H[rbase + j] (16 bit) | first column / 4 (bits 16..)
+  uint32_t* sup;   // per prior-support scalar: elimination offset (9 bit) | state index (9 bit) | angle flag (bit 18)
+  float* sds;      // prior displacement, anchor-frame landmarks; scratch of the symbolic phase
+  uint32_t* amask; // tables of the factorisation (pool)
+  float* H;        // envelope of H + rhs rows (pool)
 };
 
 __device__ __forceinline__ WS make_ws(const Layout& ly, float* base) {
   WS w;
-  w.st = base + ly.s_st; w.zodo = base + ly.s_zodo; w.zlc = base + ly.s_zlc;
+  w.st = base + ly.s_st;
   w.lct = (int*)(base + ly.s_lct); w.cs = base + ly.s_cs; w.rbm = (uint32_t*)(base + ly.s_rbm);
-  w.first = (int*)(base + ly.s_first); w.rbase = (int*)(base + ly.s_rbase);
-  w.ssup = (int*)(base + ly.s_ssup); w.sidx = (int*)(base + ly.s_sidx); w.sds = base + ly.s_sds;
+  w.rbf = (uint32_t*)(base + ly.s_rbf); w.sup = (uint32_t*)(base + ly.s_sup); w.sds = base + ly.s_sds;
   w.amask = nullptr; w.H = nullptr;  // set once the environment has its share of the CTA pool (slam_step_kernel)
   return w;
 }
+__device__ __forceinline__ int rb_of(const WS& w, int i) { return (int)(w.rbf[i] & 0xffffu); }
+__device__ __forceinline__ int first_of(const WS& w, int i) { return (int)(w.rbf[i] >> 16) << 2; }
+__device__ __forceinline__ int sup_off(uint32_t e) { return (int)(e & 0x1ffu); }
+__device__ __forceinline__ int sup_idx(uint32_t e) { return (int)((e >> 9) & 0x1ffu); }
+__device__ __forceinline__ bool sup_angle(uint32_t e) { return (e >> 18) & 1u; }
 
 // ------------------------------------------------------------------ small helpers
 #define FULLMASK 0xffffffffu
@@ -231,8 +239,6 @@ __device__ void load_env(const Layout& ly, const float* rec, const WS& w, const 
     const int k = i / 3, j = i - 3 * k, r = ring_of(k, head, W);
     const bool live = k < c;
     w.st[3 + i] = (live && k > 0) ? rec[ly.o_e + 3 * r + j] : 0.0f;
-    w.zodo[i] = live ? rec[ly.o_zodo + 3 * r + j] : 0.0f;
-    w.zlc[i] = live ? rec[ly.o_zlc + 3 * r + j] : 0.0f;
   }
   for (int k = lane; k < W; k += TEAM) {
     const int r = ring_of(k, head, W);
@@ -335,10 +341,8 @@ __device__ int push_env(const Layout& ly, float* rec, const WS& w, const Team<TE
   }
   if (lane < 3) {
     const float z = lane == 0 ? zx : (lane == 1 ? zy : zt);
-    w.zodo[3 * c + lane] = z;
-    rec[ly.o_zodo + 3 * r + lane] = z;
+    rec[ly.o_zodo + 3 * r + lane] = z;   // (measurements stay in the record: read from L2 once per linearisation)
     const float zl = io.lc_meas ? io.lc_meas[(size_t)lane * N + env] : 0.0f;
-    w.zlc[3 * c + lane] = zl;
     rec[ly.o_zlc + 3 * r + lane] = zl;
   }
   mk.um &= ~(1ull << c);
@@ -369,7 +373,7 @@ __device__ int build_support(const Layout& ly, const Ord& od, const WS& w, const
       const int q = p - 3 - 3 * npo, b = q >> 1, j = q & 1, l = nth_set_bit(ls, b);
       off = off_lm(ly, od, l) + j; idx = st_lm(ly, l) + j;
     }
-    w.ssup[p] = off; w.sidx[p] = idx;
+    w.sup[p] = (uint32_t)off | ((uint32_t)(idx & 0xffff) << 9) | ((idx & 0x10000) ? (1u << 18) : 0u);
   }
   tm.sync();
   return s;
@@ -384,6 +388,7 @@ template <int TEAM>
 __device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, const Team<TEAM>& tm, int lane, int c, const Masks& mk, int s) {
   const int L = ly.L, np = ly.np;
   const int oC = 2 * od.npas, oL = oC + 3 * (ly.W - 2), oP = 3 * (ly.W - 2) + 2 * L, oN = off_new(ly), oA = off_a(ly);
+  int* tfirst = reinterpret_cast<int*>(w.sds);  // first column per row while it is being built (sds is free until assemble)
   // own block offsets
   for (int i = lane; i < np + 2; i += TEAM) {
     int f;
@@ -394,7 +399,7 @@ __device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, const Team
     else if (i < oA) f = oN;
     else if (i < np) f = oA;
     else f = 0;
-    w.first[i] = f;
+    tfirst[i] = f;
   }
   tm.sync();
   // pose rows
@@ -409,7 +414,7 @@ __device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, const Team
       if (ly.nw > 1) m |= (uint64_t)w.rbm[k * ly.nw + 1] << 32;
       if (m) f = min(f, off_lm(ly, od, __ffsll((long long)m) - 1));
     }
-    w.first[o] = f; w.first[o + 1] = f; w.first[o + 2] = f;
+    tfirst[o] = f; tfirst[o + 1] = f; tfirst[o + 2] = f;
   }
   // landmark rows: first chain pose (slots 1..c-2) that observes them
   for (int l = lane; l < L; l += TEAM) {
@@ -417,15 +422,15 @@ __device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, const Team
     int f = o;
     for (int k = 1; k <= c - 2; ++k)
       if ((w.rbm[k * ly.nw + (l >> 5)] >> (l & 31)) & 1u) { f = oC + 3 * (k - 1); break; }
-    w.first[o] = f; w.first[o + 1] = f;
+    tfirst[o] = f; tfirst[o + 1] = f;
   }
   tm.sync();
   // prior: all support blocks are mutually coupled
   if (s > 3) {
     int fs = np;
-    for (int p = 3 + lane; p < s; p += TEAM) fs = min(fs, w.ssup[p]);
+    for (int p = 3 + lane; p < s; p += TEAM) fs = min(fs, sup_off(w.sup[p]));
     fs = tm.min_int(fs, lane);
-    for (int p = lane; p < s; p += TEAM) { const int i = w.ssup[p]; w.first[i] = min(w.first[i], fs); }
+    for (int p = lane; p < s; p += TEAM) { const int i = sup_off(w.sup[p]); tfirst[i] = min(tfirst[i], fs); }
   }
   tm.sync();
   // landmarks are global: every range-bearing factor also touches the anchor, whose rows therefore
@@ -441,12 +446,12 @@ __device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, const Team
       }
     }
     fa = tm.min_int(fa, lane);
-    if (lane < 3) w.first[oA + lane] = min(w.first[oA + lane], fa);
+    if (lane < 3) tfirst[oA + lane] = min(tfirst[oA + lane], fa);
   }
   tm.sync();
   if (mk.um >> 1) {  // unary factors couple the anchor to their pose (x_k = a (+) e_k)
     const int kmin = __ffsll((long long)(mk.um >> 1));  // lowest slot >= 1
-    if (lane < 3) w.first[oA + lane] = min(w.first[oA + lane], off_slot(ly, od, kmin, c));
+    if (lane < 3) tfirst[oA + lane] = min(tfirst[oA + lane], off_slot(ly, od, kmin, c));
     tm.sync();
   }
   // group rows in fours (shared first, aligned down to 4); prefix sum of the row lengths -> rbase
@@ -458,7 +463,7 @@ __device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, const Team
       int f = 0, len = 0;
       if (i < np) {
         const int g4 = i & ~3;
-        f = min(min(w.first[g4], w.first[g4 + 1]), min(w.first[g4 + 2], w.first[g4 + 3])) & ~3;
+        f = min(min(tfirst[g4], tfirst[g4 + 1]), min(tfirst[g4 + 2], tfirst[g4 + 3])) & ~3;
         len = g4 + 4 - f;
       } else if (i < np + 2) {
         len = np;
@@ -467,7 +472,7 @@ __device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, const Team
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(FULLMASK, x, o); if (lane >= o) x += y; }
       __syncwarp();
-      if (i < np + 2) { w.first[i] = f; w.rbase[i] = run + x - len - f; }
+      if (i < np + 2) w.rbf[i] = (uint32_t)(run + x - len - f) | ((uint32_t)(f >> 2) << 16);
       run += __shfl_sync(FULLMASK, x, 31);
     }
     if (lane == 0) reinterpret_cast<int*>(tm.scr)[8] = run;
@@ -483,7 +488,7 @@ __device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, const Team
   if (lane < 32) {
     const int G = np >> 2, NP = (np >> 1) + 1;
     int cntp = 0;
-    for (int p = lane; p < NP; p += 32) cntp += min(p >> 1, G - 1) - (w.first[2 * p] >> 2) + 1;
+    for (int p = lane; p < NP; p += 32) cntp += min(p >> 1, G - 1) - (first_of(w, 2 * p) >> 2) + 1;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) cntp += __shfl_xor_sync(FULLMASK, cntp, o);
     if (lane == 0) reinterpret_cast<int*>(tm.scr)[10] = (G + 1) + NP + ((cntp + 3) >> 2) + 3 & ~3;
@@ -519,15 +524,15 @@ __device__ void build_lists(const Layout& ly, const WS& w, const Team<TEAM>& tm,
     uint32_t* ptab = hdr + G + 1;
     unsigned char* alist = reinterpret_cast<unsigned char*>(ptab + NP);
     for (int p = lane; p < NP; p += 32) {
-      const int i = 2 * p, f = w.first[i], len = i < np ? (i | 3) + 1 - f : np;
-      ptab[p] = (uint32_t)((w.rbase[i] + f) >> 2) | ((uint32_t)(f >> 2) << 14) | ((uint32_t)(len >> 2) << 21);
+      const int i = 2 * p, f = first_of(w, i), len = i < np ? (i | 3) + 1 - f : np;
+      ptab[p] = (uint32_t)((rb_of(w, i) + f) >> 2) | ((uint32_t)(f >> 2) << 14) | ((uint32_t)(len >> 2) << 21);
     }
     int run = 0, maxcnt = 0;
     for (int J = 0; J < G; ++J) {
       const int start = run;
       for (int base = 2 * J; base < NP; base += 32) {
         const int p = base + lane;
-        const bool on = p < NP && w.first[2 * p] <= 4 * J;
+        const bool on = p < NP && first_of(w, 2 * p) <= 4 * J;
         const uint32_t bal = __ballot_sync(FULLMASK, on);
         if (on) alist[run + __popc(bal & ((1u << lane) - 1u))] = (unsigned char)p;
         run += __popc(bal);
@@ -538,7 +543,7 @@ __device__ void build_lists(const Layout& ly, const WS& w, const Team<TEAM>& tm,
         // K-split: when a column has fewer pairs than threads, 2^lg adjacent lanes share one pair and split
         // its dot-product range; only worth it when the dot products are long
         uint32_t lgs = 0;
-        if (4 * J - w.first[4 * J] >= SLAM_KSPLIT_MIN) {
+        if (4 * J - first_of(w, 4 * J) >= SLAM_KSPLIT_MIN) {
 #pragma unroll
           for (int q = 0; q < 3; ++q) {
             int lg = 0;
@@ -584,10 +589,10 @@ __device__ __forceinline__ void between_jac(const Between& b, float Ji[3][3], fl
 // H(rowblock oj, colblock oi) += Jj' Om Ji (full 3x3), H(oj,oj) += Jj' Om Jj (lower), b(oj) -= Jj' Om r
 __device__ __forceinline__ void add_j_side(const WS& w, int n, int oj, int oi, const float Ji[3][3], const float Jj[3][3],
                                            const float* om, const float* r, bool has_i) {
-  float* rhs = w.H + w.rbase[n];
+  float* rhs = w.H + rb_of(w, n);
 #pragma unroll
   for (int x = 0; x < 3; ++x) {
-    float* row = w.H + w.rbase[oj + x];
+    float* row = w.H + rb_of(w, oj + x);
     float g = 0.f;
 #pragma unroll
     for (int k = 0; k < 3; ++k) g = fmaf(Jj[k][x] * om[k], r[k], g);
@@ -625,11 +630,11 @@ __device__ __forceinline__ void acc_i_side(const float Ji[3][3], const float* om
   }
 }
 __device__ __forceinline__ void add_i_side(const WS& w, int n, int oi, const float Hii[6], const float gi[3]) {
-  float* rhs = w.H + w.rbase[n];
+  float* rhs = w.H + rb_of(w, n);
   int t = 0;
 #pragma unroll
   for (int x = 0; x < 3; ++x) {
-    float* row = w.H + w.rbase[oi + x];
+    float* row = w.H + rb_of(w, oi + x);
     rhs[oi + x] -= gi[x];
 #pragma unroll
     for (int y = 0; y <= x; ++y) row[oi + y] += Hii[t++];
@@ -648,8 +653,8 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
     for (int t = lane; t < total; t += TEAM) w.H[t] = 0.f;
   } else {
     for (int i = lane; i < n + 2; i += TEAM) {
-      const int lo = i < n ? max((int)w.first[i], cb) : 0, hi = i < n ? (i | 3) + 1 : n;  // (the rhs rows span [0, n))
-      float4* z = reinterpret_cast<float4*>(w.H + w.rbase[i] + lo);
+      const int lo = i < n ? max(first_of(w, i), cb) : 0, hi = i < n ? (i | 3) + 1 : n;  // (the rhs rows span [0, n))
+      float4* z = reinterpret_cast<float4*>(w.H + rb_of(w, i) + lo);
       for (int t = 0; t < (hi - lo) >> 2; ++t) z[t] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
   }
@@ -660,26 +665,29 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
     w.cs[2 * k] = cn; w.cs[2 * k + 1] = sn;
   }
   // prior displacement d = v - vbar on the support (angles wrapped)
+  bool dnz = false;  // any non-zero displacement?  (none at the first linearisation after a marginalisation)
   for (int p = lane; p < s; p += TEAM) {
-    const int id = w.sidx[p];
-    float d = w.st[id & 0xffff] - rec[ly.o_vbar + p];
-    if (id & 0x10000) d = wrapf(d);
+    const uint32_t e = w.sup[p];
+    float d = w.st[sup_idx(e)] - rec[ly.o_vbar + p];
+    if (sup_angle(e)) d = wrapf(d);
     w.sds[p] = d;
+    dnz |= d != 0.0f;
   }
+  dnz = tm.any(dnz, lane);
   tm.sync();
   // identity rows for unused chain slots, the unused newest slot (c == 1), inactive landmarks, padding
   for (int k = max(c - 1, 1) + lane; k <= W - 2; k += TEAM) {
     const int o = 2 * od.npas + 3 * (k - 1);
-    w.H[w.rbase[o] + o] = 1.0f; w.H[w.rbase[o + 1] + o + 1] = 1.0f; w.H[w.rbase[o + 2] + o + 2] = 1.0f;
+    w.H[rb_of(w, o) + o] = 1.0f; w.H[rb_of(w, o + 1) + o + 1] = 1.0f; w.H[rb_of(w, o + 2) + o + 2] = 1.0f;
   }
   for (int l = lane; l < L; l += TEAM)
     if (!((mk.act >> l) & 1ull)) {
       const int o = off_lm(ly, od, l);
-      if (o >= cb) { w.H[w.rbase[o] + o] = 1.0f; w.H[w.rbase[o + 1] + o + 1] = 1.0f; }
+      if (o >= cb) { w.H[rb_of(w, o) + o] = 1.0f; w.H[rb_of(w, o + 1) + o + 1] = 1.0f; }
     }
   if (lane < ly.pad + (c < 2 ? 3 : 0)) {
     const int o = off_new(ly) - ly.pad + lane;
-    w.H[w.rbase[o] + o] = 1.0f;
+    w.H[rb_of(w, o) + o] = 1.0f;
   }
   // prior: H += Lambda (row by row, coalesced over the packed lower triangle)
   {
@@ -698,17 +706,18 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
         const int t = t0 + u * TEAM;
         if (t < ntri) {
           const int p = tri_row(t), q = t - (p * (p + 1) >> 1);
-          const int ip = w.ssup[p], iq = w.ssup[q];
+          const int ip = sup_off(w.sup[p]), iq = sup_off(w.sup[q]);
           const int hi = max(ip, iq), lo = min(ip, iq);
-          if (lo >= cb) w.H[w.rbase[hi] + lo] += v[u];
+          if (lo >= cb) w.H[rb_of(w, hi) + lo] += v[u];
         }
       }
     }
     // b -= Lambda d + g (row p: the packed row, then the column below the diagonal; 8 loads in flight)
-    float* rhs = w.H + w.rbase[n];
+    float* rhs = w.H + rb_of(w, n);
     for (int p = lane; p < s; p += TEAM) {
       float acc0 = rec[ly.o_g + p], acc1 = 0.f;
       const float* lrow = lam + (p * (p + 1) >> 1);
+      if (!dnz) { rhs[sup_off(w.sup[p])] -= acc0; continue; }  // Lambda d = 0: the same value without the products
       for (int q0 = 0; q0 <= p; q0 += 8) {
         float v[8];
 #pragma unroll
@@ -729,7 +738,7 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
           acc1 = fmaf(v[u + 1], q0 + u + 1 < s ? w.sds[q0 + u + 1] : 0.f, acc1);
         }
       }
-      rhs[w.ssup[p]] -= acc0 + acc1;
+      rhs[sup_off(w.sup[p])] -= acc0 + acc1;
     }
   }
   tm.sync();
@@ -738,7 +747,7 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
     for (int k = 1 + lane; k < c; k += TEAM) {
       const float* pi = w.st + st_pose(k - 1);
       const float* pj = w.st + st_pose(k);
-      const Between b = between_eval(pi, w.cs[2 * (k - 1)], w.cs[2 * (k - 1) + 1], pj, w.zodo + 3 * k);
+      const Between b = between_eval(pi, w.cs[2 * (k - 1)], w.cs[2 * (k - 1) + 1], pj, rec + ly.o_zodo + 3 * ring_of(k, head, W));
       float Ji[3][3], Jj[3][3];
       between_jac(b, Ji, Jj);
       if (pass == 0) {
@@ -759,7 +768,7 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
     for (int k = 1 + lane; k < c; k += TEAM) {
       const int t = w.lct[k];
       if (t < 0) continue;
-      const Between b = between_eval(w.st + st_pose(t), w.cs[2 * t], w.cs[2 * t + 1], w.st + st_pose(k), w.zlc + 3 * k);
+      const Between b = between_eval(w.st + st_pose(t), w.cs[2 * t], w.cs[2 * t + 1], w.st + st_pose(k), rec + ly.o_zlc + 3 * ring_of(k, head, W));
       float Ji[3][3], Jj[3][3];
       between_jac(b, Ji, Jj);
       add_j_side(w, n, off_slot(ly, od, k, c), t >= 1 ? off_slot(ly, od, t, c) : 0, Ji, Jj, pr.om_lc, b.r, t >= 1);
@@ -773,7 +782,7 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
         const int k = __ffsll((long long)km) - 1;
         km &= km - 1;
         if (w.lct[k] != t) continue;
-        const Between b = between_eval(w.st + st_pose(t), w.cs[2 * t], w.cs[2 * t + 1], w.st + st_pose(k), w.zlc + 3 * k);
+        const Between b = between_eval(w.st + st_pose(t), w.cs[2 * t], w.cs[2 * t + 1], w.st + st_pose(k), rec + ly.o_zlc + 3 * ring_of(k, head, W));
         float Ji[3][3], Jj[3][3];
         between_jac(b, Ji, Jj);
         acc_i_side(Ji, pr.om_lc, b.r, Hii, gi);
@@ -786,7 +795,7 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
   // unary absolute-pose factors (NEXT-1): r = (a (+) e_k) - z, full 3x3 information,
   // J_a = [[1,0,-dy],[0,1,dx],[0,0,1]] (d = Rot(a_th) t_k), J_e = blockdiag(Rot(a_th), 1); slot 0: x = a.
   if (mk.um) {
-    float* rhs = w.H + w.rbase[n];
+    float* rhs = w.H + rb_of(w, n);
     const int oA = off_a(ly);
     float sa, ca;
     sincos_pi(w.st[2], &sa, &ca);
@@ -823,8 +832,8 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
         const int op = off_slot(ly, od, k, c);
 #pragma unroll
         for (int x = 0; x < 3; ++x) {
-          float* row = w.H + w.rbase[op + x];
-          float* arow = w.H + w.rbase[oA + x];
+          float* row = w.H + rb_of(w, op + x);
+          float* arow = w.H + rb_of(w, oA + x);
 #pragma unroll
           for (int y = 0; y <= x; ++y) row[op + y] += Je[0][x] * OJe[0][y] + Je[1][x] * OJe[1][y] + Je[2][x] * OJe[2][y];
 #pragma unroll
@@ -836,9 +845,9 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
     tm.sync();
     tm.sum_n(A, lane);
     if (lane == 0) {
-      float* qa0 = w.H + w.rbase[oA];
-      float* qa1 = w.H + w.rbase[oA + 1];
-      float* qa2 = w.H + w.rbase[oA + 2];
+      float* qa0 = w.H + rb_of(w, oA);
+      float* qa1 = w.H + rb_of(w, oA + 1);
+      float* qa2 = w.H + rb_of(w, oA + 2);
       qa0[oA] += A[0]; qa1[oA] += A[1]; qa1[oA + 1] += A[2];
       qa2[oA] += A[3]; qa2[oA + 1] += A[4]; qa2[oA + 2] += A[5];
       rhs[oA] -= A[6]; rhs[oA + 1] -= A[7]; rhs[oA + 2] -= A[8];
@@ -852,7 +861,7 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
   // landmarks stay in registers: pose diagonal, gradient, anchor x pose block); pass B one lane per
   // LANDMARK (landmark diagonal, gradient, anchor x landmark block, anchor diagonal partial sums).
   if (L > 0 && od.obs) {
-    float* rhs = w.H + w.rbase[n];
+    float* rhs = w.H + rb_of(w, n);
     const float w0 = pr.om_rb[0], w1 = pr.om_rb[1];
     const int oA = off_a(ly);
     float sa, ca;
@@ -904,14 +913,14 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
         const float ge10 = -(wg1a * ux + wg1b * vx), ge11 = -(wg1a * uy + wg1b * vy), ge12 = -wg1b;
         const int ol = off_lm(ly, od, l);
         if (op < ol) {  // chain pose: landmark rows, pose columns
-          float* r0p = w.H + w.rbase[ol];
-          float* r1p = w.H + w.rbase[ol + 1];
+          float* r0p = w.H + rb_of(w, ol);
+          float* r1p = w.H + rb_of(w, ol + 1);
           r0p[op] += ge00; r0p[op + 1] += ge01; r0p[op + 2] += ge02;
           r1p[op] += ge10; r1p[op + 1] += ge11; r1p[op + 2] += ge12;
         } else {        // newest pose: pose rows, landmark columns
-          w.H[w.rbase[op] + ol] += ge00; w.H[w.rbase[op] + ol + 1] += ge10;
-          w.H[w.rbase[op + 1] + ol] += ge01; w.H[w.rbase[op + 1] + ol + 1] += ge11;
-          w.H[w.rbase[op + 2] + ol] += ge02; w.H[w.rbase[op + 2] + ol + 1] += ge12;
+          w.H[rb_of(w, op) + ol] += ge00; w.H[rb_of(w, op) + ol + 1] += ge10;
+          w.H[rb_of(w, op + 1) + ol] += ge01; w.H[rb_of(w, op + 1) + ol + 1] += ge11;
+          w.H[rb_of(w, op + 2) + ol] += ge02; w.H[rb_of(w, op + 2) + ol + 1] += ge12;
         }
         const float e0a = w0 * ux, e0b = w1 * vx, e1a = w0 * uy, e1b = w1 * vy;
         R[0] += e0a * ux + e0b * vx; R[1] += e1a * ux + e1b * vx; R[2] += e1a * uy + e1b * vy;
@@ -921,15 +930,15 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
         R[12] -= ge10; R[13] -= ge11; R[14] -= ge12;
         R[15] -= wa2a * ux + wa2b * vx; R[16] -= wa2a * uy + wa2b * vy; R[17] -= wa2b;
       }
-      float* q0 = w.H + w.rbase[op];
-      float* q1 = w.H + w.rbase[op + 1];
-      float* q2 = w.H + w.rbase[op + 2];
+      float* q0 = w.H + rb_of(w, op);
+      float* q1 = w.H + rb_of(w, op + 1);
+      float* q2 = w.H + rb_of(w, op + 2);
       q0[op] += R[0]; q1[op] += R[1]; q1[op + 1] += R[2];
       q2[op] += R[3]; q2[op + 1] += R[4]; q2[op + 2] += R[5];
       rhs[op] -= R[6]; rhs[op + 1] -= R[7]; rhs[op + 2] -= R[8];
 #pragma unroll
       for (int i = 0; i < 3; ++i) {
-        float* qa = w.H + w.rbase[oA + i];
+        float* qa = w.H + rb_of(w, oA + i);
         qa[op] += R[9 + 3 * i]; qa[op + 1] += R[10 + 3 * i]; qa[op + 2] += R[11 + 3 * i];
       }
     }
@@ -982,14 +991,14 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
       }
       if (inl && sub == 0) {
         const int ol = off_lm(ly, od, l);
-        float* r0p = w.H + w.rbase[ol];
-        float* r1p = w.H + w.rbase[ol + 1];
+        float* r0p = w.H + rb_of(w, ol);
+        float* r1p = w.H + rb_of(w, ol + 1);
         r0p[ol] += Lxx; r1p[ol] += Lxy; r1p[ol + 1] += Lyy;
         rhs[ol] -= bgx; rhs[ol + 1] -= bgy;
         // anchor rows x landmark columns: a0 = -g0, a1 = -g1, a2
-        float* qa0 = w.H + w.rbase[oA];
-        float* qa1 = w.H + w.rbase[oA + 1];
-        float* qa2 = w.H + w.rbase[oA + 2];
+        float* qa0 = w.H + rb_of(w, oA);
+        float* qa1 = w.H + rb_of(w, oA + 1);
+        float* qa2 = w.H + rb_of(w, oA + 2);
         qa0[ol] -= Lxx; qa0[ol + 1] -= Lxy;
         qa1[ol] -= Lxy; qa1[ol + 1] -= Lyy;
         qa2[ol] += ag0; qa2[ol + 1] += ag1;
@@ -1000,9 +1009,9 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
     tm.sync();
     tm.sum_n(A, lane);
     if (lane == 0) {  // anchor diagonal block and gradient
-      float* qa0 = w.H + w.rbase[oA];
-      float* qa1 = w.H + w.rbase[oA + 1];
-      float* qa2 = w.H + w.rbase[oA + 2];
+      float* qa0 = w.H + rb_of(w, oA);
+      float* qa1 = w.H + rb_of(w, oA + 1);
+      float* qa2 = w.H + rb_of(w, oA + 2);
       qa0[oA] += A[0]; qa1[oA] += A[1]; qa1[oA + 1] += A[2];
       qa2[oA] -= A[3]; qa2[oA + 1] -= A[4]; qa2[oA + 2] += A[5];
       rhs[oA] += A[6]; rhs[oA + 1] += A[7]; rhs[oA + 2] -= A[8];
@@ -1157,7 +1166,7 @@ template <int TEAM>
 __device__ void back_substitute(const Layout& ly, const WS& w, const Team<TEAM>& tm, int lane) {
   const int np = ly.np, G = np >> 2;
   const Tables tb = tables_of(ly, w);
-  float* y = w.H + w.rbase[np];
+  float* y = w.H + rb_of(w, np);
   for (int I = G - 1; I >= 0; --I) {
     const int c0 = 4 * I;
     const uint32_t eI = tb.ptab[2 * I];
@@ -1190,7 +1199,7 @@ __device__ void back_substitute(const Layout& ly, const WS& w, const Team<TEAM>&
 template <int TEAM>
 __device__ int apply_update(const Layout& ly, const Ord& od, const WS& w, const Team<TEAM>& tm, int lane, int c, const Masks& mk) {
   const int W = ly.W, L = ly.L;
-  const float* dl = w.H + w.rbase[ly.np];
+  const float* dl = w.H + rb_of(w, ly.np);
   int bad = 0;
   if (lane < 3) {
     const float d = dl[off_a(ly) + lane];
@@ -1240,13 +1249,13 @@ __device__ void covariance(const Layout& ly, const WS& w, const Team<TEAM>& tm, 
   const double J[3][6] = {{je * ca, -je * sa, 0, 1, 0, -dy}, {je * sa, je * ca, 0, 0, 1, dx}, {0, 0, je, 0, 0, 1}};
   float lrow[6];
   if (lane < 6) {  // row `lane` of the trailing block
-    const int i = n - 6 + lane, fi = w.first[i];
+    const int i = n - 6 + lane, fi = first_of(w, i);
 #pragma unroll
     for (int y = 0; y < 6; ++y) {
       const int j = n - 6 + y;
       float v = 0.f;
-      if (y == lane) v = w.H[w.rbase[i] + i];
-      else if (y < lane && j >= fi) v = w.H[w.rbase[i] + j];
+      if (y == lane) v = w.H[rb_of(w, i) + i];
+      else if (y < lane && j >= fi) v = w.H[rb_of(w, i) + j];
       lrow[y] = v;
     }
   }
@@ -1354,13 +1363,13 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
   float* X = gam + s;
   float* Q = X + 3 * s;
   int* omap = (int*)(Q + 3 * s);
-  int* nidx = w.ssup;  // elimination offsets are dead from here on
+  int* nidx = reinterpret_cast<int*>(w.sup);  // the old table is dead once step B has read it
 
   // --- B. old displacement d, old -> new scalar map, new state-index table
   for (int p = lane; p < s_old; p += TEAM) {
-    const int id = w.sidx[p];
-    float d = w.st[id & 0xffff] - rec[ly.o_vbar + p];
-    if (id & 0x10000) d = wrapf(d);
+    const uint32_t e = w.sup[p];
+    float d = w.st[sup_idx(e)] - rec[ly.o_vbar + p];
+    if (sup_angle(e)) d = wrapf(d);
     w.sds[p] = d;
     int P;
     if (p < 3) P = p;
@@ -1429,7 +1438,7 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
   tm.sync();
   // --- D. factors touching slot 0 (the frame): J_j = I for between factors
   if (lane < 3) {
-    float r = w.st[st_pose(1) + lane] - w.zodo[3 + lane];
+    float r = w.st[st_pose(1) + lane] - rec[ly.o_zodo + 3 * ring_of(1, head, W) + lane];
     if (lane == 2) r = wrapf(r);
     Hs[tri(3 + lane, 3 + lane)] += pr.om_odo[lane];
     gam[3 + lane] += pr.om_odo[lane] * r;
@@ -1439,7 +1448,7 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
     if (w.lct[k] == 0) {
       const int P = 3 + 3 * __popcll(nps & lowmask(k));
       for (int x = 0; x < 3; ++x) {
-        float r = w.st[st_pose(k) + x] - w.zlc[3 * k + x];
+        float r = w.st[st_pose(k) + x] - rec[ly.o_zlc + 3 * ring_of(k, head, W) + x];
         if (x == 2) r = wrapf(r);
         Hs[tri(P + x, P + x)] += pr.om_lc[x];
         gam[P + x] += pr.om_lc[x] * r;

@@ -21,7 +21,7 @@ struct Layout {
   int rec;             // record stride
   int o_status, o_k0, o_pm, o_lm, o_act, o_um, o_a, o_e, o_m, o_zodo, o_lct, o_zlc, o_rbm, o_zrb, o_zun, o_omun, o_vbar, o_g, o_lam;
   // shared memory: a FIXED part per team (32-bit words) ...
-  int s_scr, s_st, s_zodo, s_zlc, s_lct, s_cs, s_rbm, s_first, s_rbase, s_ssup, s_sidx, s_sds;
+  int s_scr, s_st, s_lct, s_cs, s_rbm, s_rbf, s_sup, s_sds;
   int team_words;      // fixed shared words per team
   // ... and one POOL per CTA from which every environment of a round takes what its envelope needs
   // (H + rhs rows + active-pair lists, or the marginalisation scratch): slam_step_kernel
@@ -71,16 +71,13 @@ static inline Layout make_layout(int N, int W, int L, int pool, int wpc) {
   int s = 0;
   y.s_scr = s; s += 64;   // team scratch (reductions, diagonal tile, counters)
   y.s_st = s; s = pad4(s + n + 3);
-  y.s_zodo = s; s = pad4(s + 3 * W);
-  y.s_zlc = s; s = pad4(s + 3 * W);
   y.s_lct = s; s = pad4(s + W + 2);  // + the loop-closure mask (two words)
   y.s_cs = s; s = pad4(s + 2 * W);
   y.s_rbm = s; s = pad4(s + W * y.nw);
-  y.s_first = s; s = pad4(s + y.np + 2);
-  y.s_rbase = s; s = pad4(s + y.np + 2);
-  y.s_ssup = s; s = pad4(s + n);
-  y.s_sidx = s; s = pad4(s + n);
-  y.s_sds = s; s = pad4(s + n + 2 * L);  // prior displacement (<= n) + anchor-frame landmarks (2L)
+  y.s_rbf = s; s = pad4(s + y.np + 2);   // row pointer | first column, packed
+  y.s_sup = s; s = pad4(s + n);          // prior support: elimination offset | state index, packed
+  // prior displacement (<= n) + anchor-frame landmarks (2L); scratch of the symbolic phase (np + 2)
+  y.s_sds = s; s = pad4(s + (n + 2 * L > y.np + 2 ? n + 2 * L : y.np + 2));
   y.team_words = pad4(s);
   // dense need of one environment: full 4x4 tiles of the lower triangle + two rhs rows + the tables of
   // the factorisation (G+1 column headers, NP row-pair entries, at most sum_J (NP - 2J) pair indices of 8 bit);
