@@ -5,7 +5,7 @@
 
 One "step" = one pass of the whole hot path (push -> Gauss-Newton solve -> last-pose covariance and
 log-det -> marginalisation) over the whole batch of environments = ONE fused kernel launch
-(slam_step).  Default workload: BASELINE.json configs[3] (N=16384 envs, W=20 poses, L=24 landmarks,
+(slam_step; landmark windows add a tiny second launch that orders the environments for the next step).  Default workload: BASELINE.json configs[3] (N=16384 envs, W=20 poses, L=24 landmarks,
 2 GN iterations, 300 steps), the configuration the north_star's roofline target is quoted on.
 Inputs are seeded synthetic trajectories (paper_2603_25834_b200/synth.py), resident in HBM before
 the timed region.  Rank 0 prints ONE JSON line.  Multi-GPU: environments are independent, so N ranks
@@ -32,8 +32,8 @@ from paper_2603_25834_b200 import replicas, synth, workmodel  # noqa: E402
 
 SM_COUNT, LANES = 148, 128
 # dram__bytes_read.sum + dram__bytes_write.sum of one slam_step_kernel launch from the committed
-# `ncu --set full` capture (profiles/r1_step_kernel_final_full.md), keyed by workload
-NCU_TRAFFIC_BYTES = {"cfg3_landmarks_16384": 152.7e6}
+# `ncu --set full` capture (profiles/r1b_step_kernel_full.md), keyed by workload
+NCU_TRAFFIC_BYTES = {"cfg3_landmarks_16384": 167.3e6}
 L2_BYTES = 126 * 2 ** 20
 METRIC = "fixed-lag SLAM env-steps/sec (solve+cov+marginalize)"
 

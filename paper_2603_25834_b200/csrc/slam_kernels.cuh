@@ -16,7 +16,7 @@
 //   [ passive landmarks | e_1 .. e_{W-2} (chain, 3 each) | observed landmarks | pad | newest pose e_{c-1} (3) | anchor a (3) ]
 // (pad = 0..3 dummy identity rows so that the dimension np is a multiple of 4) so that the covariance
 // read-out needs only the trailing 6x6 of L.  Poses are robot-centric (anchor frame), landmarks global
-// (reading R17b).  Row np of the envelope storage is the right-hand side b (row np+1 is its zero twin).
+// (reading R17b).  Row np of the envelope storage is the right-hand side b (row index np+1 aliases it).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -382,7 +382,7 @@ __device__ int build_support(const Layout& ly, const Ord& od, const WS& w, const
 // ------------------------------------------------------------------ symbolic phase: envelope of H
 // Rows are grouped in fours; all rows of group g store the columns [first, 4g+3] (whole 4x4 tiles,
 // first a multiple of 4), so every tile row is one aligned 128-bit word.  first[i] = first column
-// of row i; rbase[i] + j addresses H(i,j).  Rows np (rhs) and np+1 (zero twin) span [0, np).
+// of row i; rbase[i] + j addresses H(i,j).  Row np (the rhs; index np+1 is an alias of it) spans [0, np).
 // Returns the total words used.
 template <int TEAM>
 __device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, const Team<TEAM>& tm, int lane, int c, const Masks& mk, int s) {
@@ -465,14 +465,14 @@ __device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, const Team
         const int g4 = i & ~3;
         f = min(min(tfirst[g4], tfirst[g4 + 1]), min(tfirst[g4 + 2], tfirst[g4 + 3])) & ~3;
         len = g4 + 4 - f;
-      } else if (i < np + 2) {
+      } else if (i == np) {   // the rhs row; its pair twin (row np + 1) is the SAME storage, see build_lists
         len = np;
       }
       int x = len;
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(FULLMASK, x, o); if (lane >= o) x += y; }
       __syncwarp();
-      if (i < np + 2) w.rbf[i] = (uint32_t)(run + x - len - f) | ((uint32_t)(f >> 2) << 16);
+      if (i < np + 2) w.rbf[i] = (uint32_t)(run + x - (i == np + 1 ? np : len) - f) | ((uint32_t)(f >> 2) << 16);
       run += __shfl_sync(FULLMASK, x, 31);
     }
     if (lane == 0) reinterpret_cast<int*>(tm.scr)[8] = run;
@@ -524,7 +524,9 @@ __device__ void build_lists(const Layout& ly, const WS& w, const Team<TEAM>& tm,
     uint32_t* ptab = hdr + G + 1;
     unsigned char* alist = reinterpret_cast<unsigned char*>(ptab + NP);
     for (int p = lane; p < NP; p += 32) {
-      const int i = 2 * p, f = first_of(w, i), len = i < np ? (i | 3) + 1 - f : np;
+      // the rhs "pair" is the rhs row twice (length 0 between its rows): both lanes' results are the same
+      // bits written to the same words, and no zero twin row has to be stored
+      const int i = 2 * p, f = first_of(w, i), len = i < np ? (i | 3) + 1 - f : 0;
       ptab[p] = (uint32_t)((rb_of(w, i) + f) >> 2) | ((uint32_t)(f >> 2) << 14) | ((uint32_t)(len >> 2) << 21);
     }
     int run = 0, maxcnt = 0;
@@ -1026,7 +1028,7 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
 // 128-bit shared-memory loads (own rows: 2 loads, the four rows of block J: 4 broadcast loads, 32 FMA).
 // The 4x4 diagonal tile (lanes 0 and 1 of pass 0) is shuffled to every lane, factorised redundantly in
 // registers, and each lane finishes its rows by a 4-term forward substitution.  Diagonal slots store
-// 1/L_jj.  Rows np (rhs b) and np+1 ride along, so on exit row np holds y = L^{-1} b.
+// 1/L_jj.  Row np (rhs b; its pair twin np+1 is the same storage) rides along, so on exit it holds y = L^{-1} b.
 __device__ __forceinline__ float4 ld4(const float* p) { return *reinterpret_cast<const float4*>(p); }
 __device__ __forceinline__ void st4(float* p, float4 v) { *reinterpret_cast<float4*>(p) = v; }
 #define FMA4(ACC, XV, BV)                                                                    \

@@ -79,12 +79,12 @@ static inline Layout make_layout(int N, int W, int L, int pool, int wpc) {
   // prior displacement (<= n) + anchor-frame landmarks (2L); scratch of the symbolic phase (np + 2)
   y.s_sds = s; s = pad4(s + (n + 2 * L > y.np + 2 ? n + 2 * L : y.np + 2));
   y.team_words = pad4(s);
-  // dense need of one environment: full 4x4 tiles of the lower triangle + two rhs rows + the tables of
+  // dense need of one environment: full 4x4 tiles of the lower triangle + the rhs row + the tables of
   // the factorisation (G+1 column headers, NP row-pair entries, at most sum_J (NP - 2J) pair indices of 8 bit);
   // or the marginalisation scratch; or the fp64 scratch of the covariance tail
   const int G = y.np / 4, NPp = y.np / 2 + 1;
   const int list_bytes = G * NPp - G * (G - 1);
-  int dense = 8 * G * (G + 1) + 2 * y.np + pad4((G + 1) + NPp + (list_bytes + 3) / 4);
+  int dense = 8 * G * (G + 1) + y.np + pad4((G + 1) + NPp + (list_bytes + 3) / 4);
   const int marg = n * (n + 1) / 2 + 8 * n + 16;
   if (marg > dense) dense = marg;
   if (dense < 272) dense = 272;

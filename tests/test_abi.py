@@ -48,6 +48,8 @@ def test_workspace_bytes_and_size_validation(lib):
     n = 3 * 20 + 2 * 24
     assert big >= 16384 * (n * (n + 1) // 2) * 4
     assert big < 16384 * 64 * 1024
+    # the largest supported window (W = 64, L = 64: n = 320) still fits the shared memory of one SM
+    assert lib.slam_workspace_bytes(1, 64, 64) > 0
     # the largest BASELINE configuration fits the 180 GB of one B200 many times over
     assert lib.slam_workspace_bytes(65536, 50, 0) < 8 * 2 ** 30
 

@@ -84,6 +84,7 @@ def test_config0_all_envs_all_steps():
     (12, 1, 0.5, 1, 40, 3),      # single env, single landmark
     (64, 0, 0.2, 3, 100, 2),     # maximum window
     (4, 64, 0.0, 3, 30, 2),      # maximum landmarks
+    (64, 64, 0.1, 2, 68, 2),     # maximum window AND landmarks: one team per CTA, the pool holds exactly one window
 ])
 def test_small_cases_every_env(W, L, p_lc, N, T, iters):
     cfg = synth.Config("t", N=N, W=W, L=L, iters=iters, T=T, p_lc=p_lc, seed=3)
