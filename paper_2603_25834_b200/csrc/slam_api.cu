@@ -424,12 +424,16 @@ static int max_teams(int team) {  // threads per CTA: register file (launch boun
 }
 // Teams per CTA and words of the CTA pool.  More teams = more environments in flight but a smaller pool
 // (each team has a fixed part); the expected number in flight is min(teams, pool / typical need) with the
-// typical need a fraction of the dense size (measured envelopes: about a third of dense for pose-only
-// windows, a half with landmarks).  SLAM_POOL_FRAC (0..1] shrinks the pool (tests: forces waiting).
+// typical need a fraction of the dense size.  Measured (ms per step by teams per SM): config 3: 14 2.19,
+// 15 2.25, 16 2.13; config 4: 12 3.20, 13 3.23, 14 3.18, 15 3.37, 16 3.20 -- rather a full pool with some
+// teams waiting than idle shared memory, hence fractions below the measured mean envelopes (0.5 / 0.33).
+// SLAM_TYPICAL_FRAC overrides; SLAM_POOL_FRAC (0..1] shrinks the pool (tests: forces waiting).
 static const int SMEM_BUDGET = 227 * 1024 - 512;  // dynamic shared memory per CTA (static tables: < 512 B)
 static int pick_launch(int W, int L, int team, int* pool_words) {
   const Layout d = make_layout(1, W, L, 0, 1);
-  const double typical = (L > 0 ? 0.5 : 0.34) * d.dense;
+  double tf = L > 0 ? 0.4 : 0.28;
+  { const char* e = getenv("SLAM_TYPICAL_FRAC"); if (e && atof(e) > 0.0 && atof(e) <= 1.0) tf = atof(e); }
+  const double typical = tf * d.dense;
   int best = 0, best_pool = 0;
   double best_est = 0.0;
   // ctas = 2 (SLAM_SPLIT_CTA=1): two smaller CTAs per SM, each with its own pool.  It paid with fixed
@@ -442,6 +446,7 @@ static int pick_launch(int W, int L, int team, int* pool_words) {
     for (int wpc = 1; wpc * ctas <= max_teams(team); ++wpc) {
       const int pool = (budget / 4 - wpc * d.team_words) & ~3;
       if (pool < d.dense) break;
+      if (wpc > 4 && (wpc & 1)) continue;  // even team counts load the four sub-partitions evenly (measured: 15 teams slower than 14 and 16)
       const double fit = pool / typical;
       double est = ctas * (fit < wpc ? fit : wpc);
       if (ctas == 2) est += 0.25;  // at equal expected occupancy prefer two CTAs
