@@ -90,6 +90,28 @@ __device__ __forceinline__ void sincos_pi(float x, float* sn, float* cn) {
   *sn = (q & 2) ? -s0 : s0;
   *cn = ((q + 1) & 2) ? -c0 : c0;
 }
+__device__ __forceinline__ float rsqrt_fast(float x) {  // MUFU.RSQ; the operands here are normal numbers
+  float y;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+// atan2 for the bearing residual: octant reduction to |t| <= tan(pi/8) with ONE approximate division
+// (t = min/max, or (min - max)/(min + max) shifted by pi/4) and the single-precision minimax kernel of
+// Cephes atanf; ~2e-7 rad absolute, a third of the instructions of atan2f (57 per call with the wrap,
+// measured: the largest single line of the assembly).  atan2(0, 0) = 0.
+__device__ __forceinline__ float atan2_fast(float y, float x) {
+  const float ax = fabsf(x), ay = fabsf(y);
+  const float mx = fmaxf(ax, ay), mn = fminf(ax, ay);
+  const bool big = mn > 0.41421356237f * mx;
+  const float num = big ? mn - mx : mn, den = fmaxf(big ? mn + mx : mx, 1e-30f);
+  const float t = __fdividef(num, den);
+  const float z = t * t;
+  float r = fmaf(fmaf(fmaf(fmaf(8.05374449538e-2f, z, -1.38776856032e-1f), z, 1.99777106478e-1f), z, -3.33329491539e-1f) * z, t, t);
+  if (big) r += 0.78539816339744831f;
+  if (ay > ax) r = 1.5707963267948966f - r;
+  if (x < 0.f) r = 3.1415926535897932f - r;
+  return copysignf(r, y);
+}
 __device__ __forceinline__ uint64_t lowmask(int k) { return k >= 64 ? ~0ull : ((1ull << k) - 1ull); }
 __device__ __forceinline__ uint64_t ring_to_slot(uint64_t ring, int head, int W) {
   const uint64_t mW = lowmask(W);
@@ -560,11 +582,6 @@ __device__ void build_lists(const Layout& ly, const WS& w, const Team<TEAM>& tm,
   }
   tm.sync();
 }
-__device__ __forceinline__ float rsqrt_fast(float x) {  // MUFU.RSQ; the operands here are normal numbers
-  float y;
-  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-}
 
 // ------------------------------------------------------------------ S1 + S2: linearise and assemble
 struct Between {  // residual and the pieces of J_i, J_j of a between factor (A.2)
@@ -903,8 +920,8 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
         }
         const float mx = mloc[2 * l], my = mloc[2 * l + 1];
         const float dx = mx - px, dy = my - py;
-        const float q = dx * dx + dy * dy, irho = rsqrtf(q), rho = q * irho, iq = irho * irho;
-        const float r0 = rho - zr, r1 = wrapf(atan2f(dy, dx) - pt - zb);
+        const float q = dx * dx + dy * dy, irho = rsqrt_fast(q), rho = q * irho, iq = irho * irho;
+        const float r0 = rho - zr, r1 = wrapf(atan2_fast(dy, dx) - pt - zb);
         const float ux = dx * irho, uy = dy * irho, vx = -dy * iq, vy = dx * iq;     // J_l rows
         const float Ux = ca * ux - sa * uy, Uy = sa * ux + ca * uy;                  // J_g rows
         const float Vx = ca * vx - sa * vy, Vy = sa * vx + ca * vy;
@@ -976,8 +993,8 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
         }
         const float* p = w.st + st_pose(k);
         const float dx = mx - p[0], dy = my - p[1];
-        const float q = dx * dx + dy * dy, irho = rsqrtf(q), rho = q * irho, iq = irho * irho;
-        const float r0 = rho - zr, r1 = wrapf(atan2f(dy, dx) - p[2] - zb);
+        const float q = dx * dx + dy * dy, irho = rsqrt_fast(q), rho = q * irho, iq = irho * irho;
+        const float r0 = rho - zr, r1 = wrapf(atan2_fast(dy, dx) - p[2] - zb);
         const float ux = dx * irho, uy = dy * irho, vx = -dy * iq, vy = dx * iq;
         const float Ux = ca * ux - sa * uy, Uy = sa * ux + ca * uy, Vx = ca * vx - sa * vy, Vy = sa * vx + ca * vy;
         const float j0 = ux * my - uy * mx, j1 = vx * my - vy * mx;
@@ -1475,8 +1492,8 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
         const float zr = rec[ly.o_zrb + (head * 2 + 0) * L + l], zb = rec[ly.o_zrb + (head * 2 + 1) * L + l];
         const float gxl = w.st[st_lm(ly, l)] - w.st[0], gyl = w.st[st_lm(ly, l) + 1] - w.st[1];
         const float dx = ca * gxl + sa * gyl, dy = -sa * gxl + ca * gyl;  // m = Rot(a_th)'(g - a_t)
-        const float q = dx * dx + dy * dy, irho = rsqrtf(q), rho = q * irho, iq = irho * irho;
-        const float r0 = rho - zr, r1 = wrapf(atan2f(dy, dx) - zb);
+        const float q = dx * dx + dy * dy, irho = rsqrt_fast(q), rho = q * irho, iq = irho * irho;
+        const float r0 = rho - zr, r1 = wrapf(atan2_fast(dy, dx) - zb);
         const float ux = dx * irho, uy = dy * irho, vx = -dy * iq, vy = dx * iq;
         const float Ux = ca * ux - sa * uy, Uy = sa * ux + ca * uy, Vx = ca * vx - sa * vy, Vy = sa * vx + ca * vy;
         const float j0 = ux * dy - uy * dx, j1 = vx * dy - vy * dx;       // = 0, -1 (kept in the general form)
