@@ -1376,7 +1376,7 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
   const int npn = __popcll(nps), nln = __popcll(nls);
   const int s = 3 + 3 * npn + 2 * nln, nbk = 1 + npn + nln;
   const int npo = __popcll(mk.ps);
-  if ((s * (s + 1) >> 1) + 8 * s > ly.cap) return 4;  // cannot happen with the dense capacity
+  if ((s * (s + 1) >> 1) + 8 * s > ly.cap) return 4;  // cannot happen: the pool holds a dense window
   float* Hs = w.H;
   float* gam = Hs + (s * (s + 1) >> 1);
   float* X = gam + s;
