@@ -29,7 +29,7 @@ using namespace slamk;
 #ifndef SLAM_MAXTHREADS
 #define SLAM_MAXTHREADS 512
 #endif
-template <int TEAM>
+template <int TEAM, bool PAIRS>
 __global__ void __launch_bounds__(TEAM == 128 ? 896 : SLAM_MAXTHREADS)
 slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flags, int iters, StepIO io,
                  unsigned long long* stats, const int* __restrict__ perm, int* __restrict__ keys) {
@@ -161,20 +161,20 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
           // does the factorisation with shuffles and __syncwarp only: no named barriers, no
           // shared-memory exchange of the diagonal tile.  The other warps of the team wait.
           if (TEAM > 32 && single_warp) {
-            if ((lane >> 5) == solo) status |= cholesky<32>(ly, w, tm32, lane & 31, ncb);
+            if ((lane >> 5) == solo) status |= cholesky<32, PAIRS>(ly, w, tm32, lane & 31, ncb);
             tm.sync();
           } else {
-            status |= cholesky<TEAM>(ly, w, tm, lane, ncb);
+            status |= cholesky<TEAM, PAIRS>(ly, w, tm, lane, ncb);
           }
         }
         if (LOCK >= 3) __syncthreads();
         if (valid) {
           if (it < iters) {
             if (TEAM > 32) {  // short rows: one warp, no named barriers
-              if ((lane >> 5) == solo) back_substitute<32>(ly, w, tm32, lane & 31);
+              if ((lane >> 5) == solo) back_substitute<32, PAIRS>(ly, w, tm32, lane & 31);
               tm.sync();
             } else {
-              back_substitute<TEAM>(ly, w, tm, lane);
+              back_substitute<TEAM, PAIRS>(ly, w, tm, lane);
             }
             status |= apply_update<TEAM>(ly, od, w, tm, lane, cc, mk);
           } else {
@@ -459,8 +459,19 @@ static int pick_launch(int W, int L, int team, int* pool_words) {
   return best;  // 0 if one environment does not fit
 }
 typedef void (*step_fn)(Layout, Params, float*, int, int, int, int, StepIO, unsigned long long*, const int*, int*);
-static step_fn kernel_of(int team) {
-  return team == 128 ? slam_step_kernel<128> : (team == 64 ? slam_step_kernel<64> : slam_step_kernel<32>);
+static step_fn kernel_of(int team, int pairs) {
+  if (pairs) return team == 128 ? slam_step_kernel<128, true> : (team == 64 ? slam_step_kernel<64, true> : slam_step_kernel<32, true>);
+  return team == 128 ? slam_step_kernel<128, false> : (team == 64 ? slam_step_kernel<64, false> : slam_step_kernel<32, false>);
+}
+// Envelope rows in pairs instead of fours: 12-18 % fewer shared-memory words per environment, ~5 % more
+// instructions.  Pays where the pool bounds the environments in flight even at a third of the dense
+// size per environment (large pose-only windows; measured, ms per step, fours / pairs: config 4 3.18 /
+// 2.90, config 2 0.399 / 0.417, config 3 2.08 / 2.10).  SLAM_PAIRS=0/1 overrides.
+static int pick_pairs(int W, int L, int team) {
+  const char* e = getenv("SLAM_PAIRS");
+  if (e && (e[0] == '0' || e[0] == '1')) return e[0] == '1';
+  const Layout d = make_layout(1, W, L, 0, 1);
+  return L == 0 && team == 32 && 16.0 * (d.team_words + 0.3 * d.dense) > SMEM_BUDGET / 4;
 }
 
 struct WsPlan { size_t stats, perm, keys, state, cache, odom, lcb, lcm, rbk, rbm, cov, ld, pose, total; };
@@ -521,6 +532,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   if (!c) return SLAM_ENOMEM;
   c->ly = make_layout(batch, window, landmarks, pool, wpc);
   c->ly.team = team;
+  c->ly.pairs = pick_pairs(window, landmarks, team);
   { const char* e = getenv("SLAM_LOCK"); if (e) c->ly.lock = atoi(e); }
   { const char* e = getenv("SLAM_LCACHE"); if (e) c->ly.lcache = atoi(e); }
   const WsPlan p = plan(c->ly);
@@ -552,7 +564,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   c->err[0] = 0;
   c->un_pose = nullptr; c->un_info = nullptr; c->un_valid = nullptr;
   c->smem_bytes = (c->ly.team_words * wpc + c->ly.pool) * 4;
-  if (cudaFuncSetAttribute(kernel_of(team), cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET) != cudaSuccess) {
+  if (cudaFuncSetAttribute(kernel_of(team, c->ly.pairs), cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET) != cudaSuccess) {
     cudaGetLastError();
     delete c;
     return SLAM_ECUDA;
@@ -560,7 +572,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   int dev = 0, sms = 0, occ = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel_of(team), wpc * team, c->smem_bytes);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel_of(team, c->ly.pairs), wpc * team, c->smem_bytes);
   if (occ < 1 || sms < 1) { cudaGetLastError(); delete c; return SLAM_ECUDA; }
   c->ctas_per_sm = occ;
   const int need = (batch + wpc - 1) / wpc;
@@ -587,7 +599,7 @@ int slam_reset(slam_ctx* c, const float* init_pose) {
 }
 
 static int launch_step(slam_ctx* c, int flags, int iters, const StepIO& io) {
-  const step_fn fn = kernel_of(c->ly.team);
+  const step_fn fn = kernel_of(c->ly.team, c->ly.pairs);
   fn<<<c->grid, c->ly.wpc * c->ly.team, c->smem_bytes, c->stream>>>(c->ly, c->pr, c->state, c->head, c->count, flags, iters, io,
                                                                       c->stats, c->perm, c->keys);
   c->launches++;

@@ -402,7 +402,7 @@ __device__ int build_support(const Layout& ly, const Ord& od, const WS& w, const
 }
 
 // ------------------------------------------------------------------ symbolic phase: envelope of H
-// Rows are grouped in fours; all rows of group g store the columns [first, 4g+3] (whole 4x4 tiles,
+// Rows are grouped in pairs; both rows of a pair store the columns [first, 4g+3] of their tile row g (whole 4x4 tiles,
 // first a multiple of 4), so every tile row is one aligned 128-bit word.  first[i] = first column
 // of row i; rbase[i] + j addresses H(i,j).  Row np (the rhs; index np+1 is an alias of it) spans [0, np).
 // Returns the total words used.
@@ -476,17 +476,26 @@ __device__ int symbolic(const Layout& ly, const Ord& od, const WS& w, const Team
     if (lane < 3) tfirst[oA + lane] = min(tfirst[oA + lane], off_slot(ly, od, kmin, c));
     tm.sync();
   }
-  // group rows in fours (shared first, aligned down to 4); prefix sum of the row lengths -> rbase
-  // (done by the first warp of the team)
+  // group rows in fours, or (ly.pairs) in PAIRS (shared first, aligned down to 4: whole 4x4 tile rows);
+  // prefix sum of the row lengths -> rbase (done by the first warp of the team).  A pair is what one
+  // lane of the factorisation owns; with pairs the two pairs of a 4-column block may start at different
+  // columns (cholesky<.., true> splits its dot products there), which stores 12-18 % fewer words than a
+  // common start for all four rows at ~30 more instructions per column block: worth it where shared
+  // memory bounds the environments in flight (slam_api.cu: pick_pairs).
   if (lane < 32) {
     int run = 0;
     for (int base = 0; base < np + 2; base += 32) {
       const int i = base + lane;
       int f = 0, len = 0;
       if (i < np) {
-        const int g4 = i & ~3;
-        f = min(min(tfirst[g4], tfirst[g4 + 1]), min(tfirst[g4 + 2], tfirst[g4 + 3])) & ~3;
-        len = g4 + 4 - f;
+        if (ly.pairs) {
+          const int g2 = i & ~1;
+          f = min(tfirst[g2], tfirst[g2 + 1]) & ~3;
+        } else {
+          const int g4 = i & ~3;
+          f = min(min(tfirst[g4], tfirst[g4 + 1]), min(tfirst[g4 + 2], tfirst[g4 + 3])) & ~3;
+        }
+        len = (i | 3) + 1 - f;
       } else if (i == np) {   // the rhs row; its pair twin (row np + 1) is the SAME storage, see build_lists
         len = np;
       }
@@ -567,7 +576,7 @@ __device__ void build_lists(const Layout& ly, const WS& w, const Team<TEAM>& tm,
         // K-split: when a column has fewer pairs than threads, 2^lg adjacent lanes share one pair and split
         // its dot-product range; only worth it when the dot products are long
         uint32_t lgs = 0;
-        if (4 * J - first_of(w, 4 * J) >= SLAM_KSPLIT_MIN) {
+        if (4 * J - min(first_of(w, 4 * J), first_of(w, 4 * J + 2)) >= SLAM_KSPLIT_MIN) {
 #pragma unroll
           for (int q = 0; q < 3; ++q) {
             int lg = 0;
@@ -1052,7 +1061,7 @@ __device__ __forceinline__ void st4(float* p, float4 v) { *reinterpret_cast<floa
   ACC = fmaf(-XV.x, BV.x, ACC); ACC = fmaf(-XV.y, BV.y, ACC); ACC = fmaf(-XV.z, BV.z, ACC); \
   ACC = fmaf(-XV.w, BV.w, ACC);
 
-template <int TEAM>
+template <int TEAM, bool PAIRS>
 __device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int lane, int ncb) {
   // ncb: number of leading column blocks whose factor is still valid from the previous factorisation of
   // this call (see assemble): there only the rhs pair -- the last entry of the column's list -- is
@@ -1063,12 +1072,16 @@ __device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int
   int flag = 0;
   for (int J = 0; J < G; ++J) {
     const int c0 = 4 * J;
-    const uint32_t hd = tb.hdr[J], eJ = tb.ptab[2 * J];
-    const int fJ = (int)((eJ >> 14) & 0x7fu) << 2, lenJ = (int)(eJ >> 21) << 2;
-    const float* rJ0 = w.H + ((int)(eJ & 0x3fffu) << 2) - fJ;  // the four rows of the block share first and length
-    const float* rJ1 = rJ0 + lenJ;
-    const float* rJ2 = rJ1 + lenJ;
-    const float* rJ3 = rJ2 + lenJ;
+    // the block's rows: pair A = rows c0, c0+1 (columns from fA), pair B = rows c0+2, c0+3 (from fB)
+    // (!PAIRS: the four rows share first and length, one table entry describes them)
+    const uint32_t hd = tb.hdr[J], eA = tb.ptab[2 * J], eB = PAIRS ? tb.ptab[2 * J + 1] : 0u;
+    const int fA = (int)((eA >> 14) & 0x7fu) << 2, lenA = (int)(eA >> 21) << 2;
+    const int fB = PAIRS ? (int)((eB >> 14) & 0x7fu) << 2 : fA;
+    const float* rJ0 = w.H + ((int)(eA & 0x3fffu) << 2) - fA;
+    const float* rJ1 = rJ0 + lenA;
+    const float* rJ2 = PAIRS ? w.H + ((int)(eB & 0x3fffu) << 2) - fB : rJ1 + lenA;
+    const float* rJ3 = rJ2 + (PAIRS ? (int)(eB >> 21) << 2 : lenA);
+    const int fJ = min(fA, fB), fH = max(fA, fB);    // both pairs have entries from fH on, one of them from fJ
     // The ACTIVE row pairs of this column (compact list from the symbolic phase) sit on the lowest
     // threads.  K-split: when fewer pairs than threads, `ch` adjacent lanes share one pair and
     // split the dot-product range; partial sums are combined by shuffles.
@@ -1106,8 +1119,21 @@ __device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int
         const int ks = max(fi, fJ);
         const int nblk = (c0 - ks) >> 2;
         const int kb = ks + 4 * ((t * nblk) >> lg), ke = ks + 4 * (((t + 1) * nblk) >> lg);
+        if (PAIRS && fA != fB) {  // (block-uniform) columns [kb, fH): only the earlier pair of the block has entries
+          const float* rL0 = fA < fB ? rJ0 : rJ2;
+          const float* rL1 = fA < fB ? rJ1 : rJ3;
+          float u00 = 0.f, u01 = 0.f, u10 = 0.f, u11 = 0.f;
+          const int km = min(ke, fH);
+          for (int k = kb; k < km; k += 4) {
+            const float4 x0 = ld4(p0 + k), x1 = ld4(p1 + k);
+            const float4 b0 = ld4(rL0 + k), b1 = ld4(rL1 + k);
+            FMA4(u00, x0, b0) FMA4(u01, x0, b1) FMA4(u10, x1, b0) FMA4(u11, x1, b1)
+          }
+          if (fA < fB) { a0.x += u00; a0.y += u01; a1.x += u10; a1.y += u11; }
+          else { a0.z += u00; a0.w += u01; a1.z += u10; a1.w += u11; }
+        }
 #pragma unroll KUNROLL
-        for (int k = kb; k < ke; k += 4) {
+        for (int k = max(kb, fH); k < ke; k += 4) {
           const float4 x0 = ld4(p0 + k), x1 = ld4(p1 + k);
           const float4 b0 = ld4(rJ0 + k), b1 = ld4(rJ1 + k), b2 = ld4(rJ2 + k), b3 = ld4(rJ3 + k);
           FMA4(a0.x, x0, b0) FMA4(a0.y, x0, b1) FMA4(a0.z, x0, b2) FMA4(a0.w, x0, b3)
@@ -1181,19 +1207,20 @@ __device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int
 
 // Solves L' delta = y in place in row np, by 4-row blocks from the bottom: delta_I from the diagonal
 // tile (every lane redundantly), then y_K -= L(I,K)' delta_I with lanes over the column blocks K.
-template <int TEAM>
+template <int TEAM, bool PAIRS>
 __device__ void back_substitute(const Layout& ly, const WS& w, const Team<TEAM>& tm, int lane) {
   const int np = ly.np, G = np >> 2;
   const Tables tb = tables_of(ly, w);
   float* y = w.H + rb_of(w, np);
   for (int I = G - 1; I >= 0; --I) {
     const int c0 = 4 * I;
-    const uint32_t eI = tb.ptab[2 * I];
-    const int fI = (int)((eI >> 14) & 0x7fu) << 2, lenI = (int)(eI >> 21) << 2;
-    const float* r0 = w.H + ((int)(eI & 0x3fffu) << 2) - fI;
-    const float* r1 = r0 + lenI;
-    const float* r2 = r1 + lenI;
-    const float* r3 = r2 + lenI;
+    const uint32_t eA = tb.ptab[2 * I], eB = PAIRS ? tb.ptab[2 * I + 1] : 0u;
+    const int fA = (int)((eA >> 14) & 0x7fu) << 2, lenA = (int)(eA >> 21) << 2;
+    const int fB = PAIRS ? (int)((eB >> 14) & 0x7fu) << 2 : fA, fI = min(fA, fB);
+    const float* r0 = w.H + ((int)(eA & 0x3fffu) << 2) - fA;
+    const float* r1 = r0 + lenA;
+    const float* r2 = PAIRS ? w.H + ((int)(eB & 0x3fffu) << 2) - fB : r1 + lenA;
+    const float* r3 = r2 + (PAIRS ? (int)(eB >> 21) << 2 : lenA);
     const float4 yy = ld4(y + c0), t0 = ld4(r0 + c0), t1 = ld4(r1 + c0), t2 = ld4(r2 + c0), t3 = ld4(r3 + c0);
     const float e3 = yy.w * t3.w;
     const float e2 = fmaf(-t3.z, e3, yy.z) * t2.z;
@@ -1202,12 +1229,17 @@ __device__ void back_substitute(const Layout& ly, const WS& w, const Team<TEAM>&
     tm.sync();
     if (lane == 0) st4(y + c0, make_float4(e0, e1, e2, e3));
     for (int k = fI + 4 * lane; k < c0; k += 4 * TEAM) {
-      const float4 x0 = ld4(r0 + k), x1 = ld4(r1 + k), x2 = ld4(r2 + k), x3 = ld4(r3 + k);
       float4 v = ld4(y + k);
-      v.x = fmaf(-x3.x, e3, fmaf(-x2.x, e2, fmaf(-x1.x, e1, fmaf(-x0.x, e0, v.x))));
-      v.y = fmaf(-x3.y, e3, fmaf(-x2.y, e2, fmaf(-x1.y, e1, fmaf(-x0.y, e0, v.y))));
-      v.z = fmaf(-x3.z, e3, fmaf(-x2.z, e2, fmaf(-x1.z, e1, fmaf(-x0.z, e0, v.z))));
-      v.w = fmaf(-x3.w, e3, fmaf(-x2.w, e2, fmaf(-x1.w, e1, fmaf(-x0.w, e0, v.w))));
+      if (!PAIRS || k >= fA) {   // (a pair has no entries left of its first column)
+        const float4 x0 = ld4(r0 + k), x1 = ld4(r1 + k);
+        v.x = fmaf(-x1.x, e1, fmaf(-x0.x, e0, v.x)); v.y = fmaf(-x1.y, e1, fmaf(-x0.y, e0, v.y));
+        v.z = fmaf(-x1.z, e1, fmaf(-x0.z, e0, v.z)); v.w = fmaf(-x1.w, e1, fmaf(-x0.w, e0, v.w));
+      }
+      if (!PAIRS || k >= fB) {
+        const float4 x2 = ld4(r2 + k), x3 = ld4(r3 + k);
+        v.x = fmaf(-x3.x, e3, fmaf(-x2.x, e2, v.x)); v.y = fmaf(-x3.y, e3, fmaf(-x2.y, e2, v.y));
+        v.z = fmaf(-x3.z, e3, fmaf(-x2.z, e2, v.z)); v.w = fmaf(-x3.w, e3, fmaf(-x2.w, e2, v.w));
+      }
       st4(y + k, v);
     }
     tm.sync();

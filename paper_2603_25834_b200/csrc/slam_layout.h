@@ -30,6 +30,7 @@ struct Layout {
   int dense;           // words that suffice for ANY environment of this size
   int wpc;             // teams (environments in flight) per CTA
   int team;            // threads per environment: 32, 64 or 128
+  int pairs;           // 1: envelope rows grouped in pairs instead of fours (less shared memory, more instructions)
   int lcache;          // 1: keep the factor columns of passive landmarks across the linearisations of one call
   int lock;            // lock-step level: CTA barriers before assemble (1), + before Cholesky (2), + before the solve (3)
 };
@@ -95,6 +96,7 @@ static inline Layout make_layout(int N, int W, int L, int pool, int wpc) {
   y.team = 32;
   y.lock = 1;
   y.lcache = 1;
+  y.pairs = 0;
   return y;
 }
 

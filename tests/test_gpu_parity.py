@@ -264,6 +264,22 @@ def test_results_do_not_depend_on_capacity_or_team(monkeypatch):
         monkeypatch.setenv("SLAM_TEAM", team)
         c = run_gpu(_slam(cfg.N, cfg.W, cfg.L), data, cfg.iters, fused=True, want_poses=False)
         _check(_sub(c, np.arange(0, cfg.N, 25)), ref, what=("cov", "logdet"))
+    monkeypatch.delenv("SLAM_TEAM")
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("W,L,p_lc,pairs", [(40, 0, 0.3, "1"), (40, 0, 0.3, "0"), (7, 9, 0.3, "1"), (64, 64, 0.1, "1")])
+def test_envelope_rows_in_pairs_or_fours(monkeypatch, W, L, p_lc, pairs):
+    """SLAM_PAIRS selects how the envelope rows are grouped (storage and the split dot products of the
+    factorisation); both groupings hold the stated tolerances, with and without landmarks."""
+    monkeypatch.setenv("SLAM_PAIRS", pairs)
+    N, T = (3, 68) if W == 64 else (60, 60)
+    cfg = synth.Config("pairs", N=N, W=W, L=L, iters=2, T=T, p_lc=p_lc, seed=13)
+    data = synth.generate(cfg)
+    ref = oracle.run_batch(data, cfg.iters)
+    gpu = run_gpu(_slam(cfg.N, cfg.W, cfg.L), data, cfg.iters, fused=True, want_poses=False)
+    assert (gpu["status"] == 0).all()
+    _check(gpu, ref, what=("cov", "logdet"))
 
 
 @pytest.mark.parametrize("W,L,p_lc", [(8, 0, 0.3), (6, 7, 0.2)])
