@@ -425,13 +425,14 @@ static int max_teams(int team) {  // threads per CTA: register file (launch boun
 // Teams per CTA and words of the CTA pool.  More teams = more environments in flight but a smaller pool
 // (each team has a fixed part); the expected number in flight is min(teams, pool / typical need) with the
 // typical need a fraction of the dense size.  Measured (ms per step by teams per SM): config 3: 14 2.19,
-// 15 2.25, 16 2.13; config 4: 12 3.20, 13 3.23, 14 3.18, 15 3.37, 16 3.20 -- rather a full pool with some
+// 15 2.25, 16 2.13; config 4: 12 3.20, 13 3.23, 14 3.18, 15 3.37, 16 3.20 (rows in pairs: 14 2.95, 16 2.91)
+// -- rather a full pool with some
 // teams waiting than idle shared memory, hence fractions below the measured mean envelopes (0.5 / 0.33).
 // SLAM_TYPICAL_FRAC overrides; SLAM_POOL_FRAC (0..1] shrinks the pool (tests: forces waiting).
 static const int SMEM_BUDGET = 227 * 1024 - 512;  // dynamic shared memory per CTA (static tables: < 512 B)
 static int pick_launch(int W, int L, int team, int* pool_words) {
   const Layout d = make_layout(1, W, L, 0, 1);
-  double tf = L > 0 ? 0.4 : 0.28;
+  double tf = L > 0 ? 0.4 : 0.24;
   { const char* e = getenv("SLAM_TYPICAL_FRAC"); if (e && atof(e) > 0.0 && atof(e) <= 1.0) tf = atof(e); }
   const double typical = tf * d.dense;
   int best = 0, best_pool = 0;
