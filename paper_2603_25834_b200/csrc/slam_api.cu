@@ -373,7 +373,7 @@ struct slam_ctx {
   float* cov_cache;
   unsigned long long* stats;  // [8] device counters: max / sum / count of envelope words, ...
   int *perm, *keys;           // [N] cost order of the environments and the keys it is sorted by
-  bool order;                 // re-sort after every solve (SLAM_ORDER=0 disables)
+  bool order, order_all;      // re-sort after every solve (SLAM_ORDER=0 disables, 2: pose-only windows too)
   // device staging for slam_step_host
   float *st_odom, *st_lc_meas, *st_rb_meas, *st_cov, *st_logdet, *st_pose;
   int32_t* st_lc_back;
@@ -550,7 +550,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   c->stats = (unsigned long long*)(base + p.stats);
   c->perm = (int*)(base + p.perm);
   c->keys = (int*)(base + p.keys);
-  { const char* e = getenv("SLAM_ORDER"); c->order = !(e && e[0] == '0'); }
+  { const char* e = getenv("SLAM_ORDER"); c->order = !(e && e[0] == '0'); c->order_all = e && e[0] == '2'; }
   c->state = (float*)(base + p.state);
   c->cov_cache = (float*)(base + p.cache);
   c->st_odom = (float*)(base + p.odom);
@@ -608,7 +608,7 @@ static int launch_step(slam_ctx* c, int flags, int iters, const StepIO& io) {
   // several rounds; a small batch is latency bound: one more kernel boundary per step would show; and
   // measured only landmark windows gain -- their cost varies most: config 3 2.40 -> 2.31 ms per step,
   // config 4 3.49 -> 3.53)
-  if (c->order && iters > 0 && c->ly.L > 0 && (long long)c->ly.N >= 4ll * c->grid * c->ly.wpc) {
+  if (c->order && iters > 0 && (c->ly.L > 0 || c->order_all) && (long long)c->ly.N >= 4ll * c->grid * c->ly.wpc) {
     slam_order_kernel<<<1, 1024, 0, c->stream>>>(c->ly.N, c->ly.dense, c->keys, c->perm);
     c->launches++;
   }
