@@ -29,7 +29,7 @@ using namespace slamk;
 #ifndef SLAM_MAXTHREADS
 #define SLAM_MAXTHREADS 512
 #endif
-template <int TEAM, bool PAIRS>
+template <int TEAM, bool PAIRS, bool LM>
 __global__ void __launch_bounds__(TEAM == 128 ? 896 : SLAM_MAXTHREADS)
 slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flags, int iters, StepIO io,
                  unsigned long long* stats, const int* __restrict__ perm, int* __restrict__ keys) {
@@ -153,7 +153,7 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
       for (int it = 0; it < nlin; ++it) {
         if (LOCK >= 1) __syncthreads();
         // after the first factorisation the column blocks of the passive landmarks keep their factor
-        const int ncb = (valid && it > 0 && ly.lcache) ? od.npas >> 1 : 0;
+        const int ncb = (LM && valid && it > 0 && ly.lcache) ? od.npas >> 1 : 0;
         if (valid) { assemble<TEAM>(ly, pr, od, rec, w, tm, lane, head, cc, mk, s, total, 4 * ncb); tm.sync(); }
         if (LOCK >= 2) __syncthreads();
         if (valid) {
@@ -161,10 +161,10 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
           // does the factorisation with shuffles and __syncwarp only: no named barriers, no
           // shared-memory exchange of the diagonal tile.  The other warps of the team wait.
           if (TEAM > 32 && single_warp) {
-            if ((lane >> 5) == solo) status |= cholesky<32, PAIRS>(ly, w, tm32, lane & 31, ncb);
+            if ((lane >> 5) == solo) status |= cholesky<32, PAIRS, LM>(ly, w, tm32, lane & 31, ncb);
             tm.sync();
           } else {
-            status |= cholesky<TEAM, PAIRS>(ly, w, tm, lane, ncb);
+            status |= cholesky<TEAM, PAIRS, LM>(ly, w, tm, lane, ncb);
           }
         }
         if (LOCK >= 3) __syncthreads();
@@ -460,9 +460,15 @@ static int pick_launch(int W, int L, int team, int* pool_words) {
   return best;  // 0 if one environment does not fit
 }
 typedef void (*step_fn)(Layout, Params, float*, int, int, int, int, StepIO, unsigned long long*, const int*, int*);
-static step_fn kernel_of(int team, int pairs) {
-  if (pairs) return team == 128 ? slam_step_kernel<128, true> : (team == 64 ? slam_step_kernel<64, true> : slam_step_kernel<32, true>);
-  return team == 128 ? slam_step_kernel<128, false> : (team == 64 ? slam_step_kernel<64, false> : slam_step_kernel<32, false>);
+template <bool PAIRS, bool LM>
+static step_fn kernel_pick(int team) {
+  return team == 128 ? slam_step_kernel<128, PAIRS, LM> : (team == 64 ? slam_step_kernel<64, PAIRS, LM> : slam_step_kernel<32, PAIRS, LM>);
+}
+// One instantiation per (team size, envelope rows in pairs, window has landmarks): the pose-only kernels
+// carry no code for cached landmark columns, the fours kernels none for split dot products.
+static step_fn kernel_of(int team, int pairs, int landmarks) {
+  if (pairs) return landmarks ? kernel_pick<true, true>(team) : kernel_pick<true, false>(team);
+  return landmarks ? kernel_pick<false, true>(team) : kernel_pick<false, false>(team);
 }
 // Envelope rows in pairs instead of fours: 12-18 % fewer shared-memory words per environment, ~5 % more
 // instructions.  Pays where the pool bounds the environments in flight even at a third of the dense
@@ -565,7 +571,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   c->err[0] = 0;
   c->un_pose = nullptr; c->un_info = nullptr; c->un_valid = nullptr;
   c->smem_bytes = (c->ly.team_words * wpc + c->ly.pool) * 4;
-  if (cudaFuncSetAttribute(kernel_of(team, c->ly.pairs), cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET) != cudaSuccess) {
+  if (cudaFuncSetAttribute(kernel_of(team, c->ly.pairs, c->ly.L), cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET) != cudaSuccess) {
     cudaGetLastError();
     delete c;
     return SLAM_ECUDA;
@@ -573,7 +579,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   int dev = 0, sms = 0, occ = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel_of(team, c->ly.pairs), wpc * team, c->smem_bytes);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel_of(team, c->ly.pairs, c->ly.L), wpc * team, c->smem_bytes);
   if (occ < 1 || sms < 1) { cudaGetLastError(); delete c; return SLAM_ECUDA; }
   c->ctas_per_sm = occ;
   const int need = (batch + wpc - 1) / wpc;
@@ -600,7 +606,7 @@ int slam_reset(slam_ctx* c, const float* init_pose) {
 }
 
 static int launch_step(slam_ctx* c, int flags, int iters, const StepIO& io) {
-  const step_fn fn = kernel_of(c->ly.team, c->ly.pairs);
+  const step_fn fn = kernel_of(c->ly.team, c->ly.pairs, c->ly.L);
   fn<<<c->grid, c->ly.wpc * c->ly.team, c->smem_bytes, c->stream>>>(c->ly, c->pr, c->state, c->head, c->count, flags, iters, io,
                                                                       c->stats, c->perm, c->keys);
   c->launches++;

@@ -579,6 +579,7 @@ __device__ void build_lists(const Layout& ly, const WS& w, const Team<TEAM>& tm,
         if (4 * J - min(first_of(w, 4 * J), first_of(w, 4 * J + 2)) >= SLAM_KSPLIT_MIN) {
 #pragma unroll
           for (int q = 0; q < 3; ++q) {
+            if (q != 0 && (32 << q) != TEAM) continue;   // only the team sizes this kernel factorises with
             int lg = 0;
             while (lg < 3 && (cnt << (lg + 1)) <= (32 << q)) ++lg;
             lgs |= (uint32_t)lg << (2 * q);
@@ -1061,7 +1062,7 @@ __device__ __forceinline__ void st4(float* p, float4 v) { *reinterpret_cast<floa
   ACC = fmaf(-XV.x, BV.x, ACC); ACC = fmaf(-XV.y, BV.y, ACC); ACC = fmaf(-XV.z, BV.z, ACC); \
   ACC = fmaf(-XV.w, BV.w, ACC);
 
-template <int TEAM, bool PAIRS>
+template <int TEAM, bool PAIRS, bool CACHE>
 __device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int lane, int ncb) {
   // ncb: number of leading column blocks whose factor is still valid from the previous factorisation of
   // this call (see assemble): there only the rhs pair -- the last entry of the column's list -- is
@@ -1092,7 +1093,7 @@ __device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int
     const int per_pass = TEAM >> lg;
     const int t = lane & (ch - 1);
     float d0 = 1.f, d1 = 1.f, d2 = 1.f, d3 = 1.f, l10 = 0.f, l20 = 0.f, l21 = 0.f, l30 = 0.f, l31 = 0.f, l32 = 0.f;
-    const bool cached = J < ncb;
+    const bool cached = CACHE && J < ncb;   // (CACHE = windows with landmarks: pose-only kernels drop the path)
     if (cached) {
       const float4 t0 = ld4(rJ0 + c0), t1 = ld4(rJ1 + c0), t2 = ld4(rJ2 + c0), t3 = ld4(rJ3 + c0);
       d0 = t0.x; l10 = t1.x; d1 = t1.y; l20 = t2.x; l21 = t2.y; d2 = t2.z; l30 = t3.x; l31 = t3.y; l32 = t3.z; d3 = t3.w;
