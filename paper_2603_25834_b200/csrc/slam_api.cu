@@ -430,18 +430,20 @@ static int max_teams(int team) {  // threads per CTA: register file (launch boun
 // teams waiting than idle shared memory, hence fractions below the measured mean envelopes (0.5 / 0.33).
 // SLAM_TYPICAL_FRAC overrides; SLAM_POOL_FRAC (0..1] shrinks the pool (tests: forces waiting).
 static const int SMEM_BUDGET = 227 * 1024 - 512;  // dynamic shared memory per CTA (static tables: < 512 B)
-static int pick_launch(int W, int L, int team, int* pool_words) {
+static int pick_launch(int W, int L, int team, int pairs, int* pool_words) {
   const Layout d = make_layout(1, W, L, 0, 1);
   double tf = L > 0 ? 0.4 : 0.24;
   { const char* e = getenv("SLAM_TYPICAL_FRAC"); if (e && atof(e) > 0.0 && atof(e) <= 1.0) tf = atof(e); }
   const double typical = tf * d.dense;
   int best = 0, best_pool = 0;
   double best_est = 0.0;
-  // ctas = 2 (SLAM_SPLIT_CTA=1): two smaller CTAs per SM, each with its own pool.  It paid with fixed
-  // slots per team (the phases of the two CTAs drift apart); with the pool one large CTA packs better
-  // (measured, ms per step, one / two CTAs: config 3 2.34 / 2.46, config 4 3.31 / 3.42).
+  // ctas = 2: two smaller CTAs per SM, each with its own pool, when the estimate loses no environment in
+  // flight: the lock-step rounds of the two CTAs drift apart, so one CTA's work fills the tail of the
+  // other's round (measured, ms per step, one / two CTAs: config 1 0.107 / 0.102, config 2 0.393 / 0.384,
+  // config 3 2.076 / 2.043; config 4, whose windows need half a pool of 8 teams and more, 2.845 / 3.004:
+  // the estimate keeps it on one CTA).  SLAM_SPLIT_CTA=0 disables.
   const char* sp = getenv("SLAM_SPLIT_CTA");
-  const int max_ctas = (sp && sp[0] == '1') ? 2 : 1;
+  const int max_ctas = ((sp && sp[0] == '0') || pairs) ? 1 : 2;   // (rows in pairs = shared memory binds: one pool)
   for (int ctas = 1; ctas <= max_ctas; ++ctas) {
     const int budget = ctas == 1 ? SMEM_BUDGET : (228 * 1024 / 2 - 1024 - 512);
     for (int wpc = 1; wpc * ctas <= max_teams(team); ++wpc) {
@@ -515,7 +517,7 @@ void slam_default_config(slam_config* cfg) {
 size_t slam_workspace_bytes(int batch, int window, int landmarks) {
   if (!sizes_ok(batch, window, landmarks)) return 0;
   int pool = 0;
-  const int wpc = pick_launch(window, landmarks, pick_team(window, landmarks, batch), &pool);
+  const int wpc = pick_launch(window, landmarks, pick_team(window, landmarks, batch), 0, &pool);
   if (wpc < 1) return 0;
   return plan(make_layout(batch, window, landmarks, pool, wpc)).total;
 }
@@ -527,7 +529,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   if (!sizes_ok(batch, window, landmarks) || !workspace || ((uintptr_t)workspace & 255)) return SLAM_EINVAL;
   const int team = pick_team(window, landmarks, batch);
   int pool = 0;
-  const int wpc = pick_launch(window, landmarks, team, &pool);
+  const int wpc = pick_launch(window, landmarks, team, pick_pairs(window, landmarks, team), &pool);
   if (wpc < 1) return SLAM_EINVAL;
   slam_config dc;
   slam_default_config(&dc);
