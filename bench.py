@@ -32,8 +32,8 @@ from paper_2603_25834_b200 import replicas, synth, workmodel  # noqa: E402
 
 SM_COUNT, LANES = 148, 128
 # dram__bytes_read.sum + dram__bytes_write.sum of one slam_step_kernel launch from the committed
-# `ncu --set full` capture (profiles/r1c_step_kernel_full.md), keyed by workload
-NCU_TRAFFIC_BYTES = {"cfg3_landmarks_16384": 168.5e6}
+# `ncu --set full` capture (profiles/r1e_step_kernel_full.md), keyed by workload
+NCU_TRAFFIC_BYTES = {"cfg3_landmarks_16384": 169.1e6}
 L2_BYTES = 126 * 2 ** 20
 METRIC = "fixed-lag SLAM env-steps/sec (solve+cov+marginalize)"
 
