@@ -15,7 +15,7 @@ using namespace slamk;
 
 // ------------------------------------------------------------------ kernels
 // One TEAM of 32/64/128 threads per environment, `wpc` teams per CTA, persistent loop over the
-// environments blockIdx.x, blockIdx.x + gridDim.x, ... in ROUNDS.  flags select the phases, so that the
+// environments of its CTA (chunks of the cost-ordered list, see the assignment below) in ROUNDS.  flags select the phases, so that the
 // separate ABI calls and the fused slam_step share the same device code and are bit-for-bit identical.
 //
 // Shared memory = a fixed part per team (state, factor data, row tables) + ONE POOL per CTA.  The
