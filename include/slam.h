@@ -19,7 +19,8 @@
  *    trouble is per environment and asynchronous: a sticky status word (slam_get_status).
  *  - All environments move in lock-step: one host-side window count (slam_count).
  *  - Not re-entrant: one context per stream, one host thread per context.
- *  - Arithmetic: fp32, except the final 6x6 -> 3x3 covariance/log-det tail (fp64, O(1) per env).
+ *  - Arithmetic: fp32, except the final 6x6 -> 3x3 covariance/log-det tail (fp64, O(1) per env) and the
+ *    windows the conditioning watch hands to the fp64 path (slam_set_precision).
  */
 #ifndef SLAM_H
 #define SLAM_H
@@ -145,7 +146,7 @@ int slam_get_status(slam_ctx* ctx, int32_t* status);
 /* Device counters since the last reset, copied to stats8 ([8] uint64, device): [0] max and [1] sum of the
  * envelope words (shared-memory footprint of H) over [2] solved environment-instances, [3] rounds an
  * environment waited for space in the shared-memory pool of its CTA (it is solved one round later; the
- * result does not depend on it). */
+ * result does not depend on it), [4] environment-calls that ran on the fp64 path. */
 int slam_get_stats(slam_ctx* ctx, unsigned long long* stats8);
 
 /* NEXT-4: the paper's reward, eqs. (7)-(17), elementwise over environments, meant
@@ -186,6 +187,19 @@ int slam_scan_match(const slam_scan_params* p, int batch, const float* grid, con
                     float* pose_meas, float* score, float* second, void* cuda_stream);
 int slam_grid_update(const slam_scan_params* p, int batch, float* grid, const float* pose, const float* ranges,
                      const float* weight, float l_free, float l_occ, float l_clamp, void* cuda_stream);
+
+/* Precision of the solve (eq. (6), is the quantity at stake).  A robot
+ * that dead-reckoned for a while and re-observes a landmark has information on its anchor pose spanning six
+ * decades: no fp32 information-form factorisation keeps Sigma_t to 1e-3 there.  The fp32 kernel therefore watches
+ * the cancellation in the anchor's pivots, r = max_i H_ii / L_ii^2 over the three anchor rows, in every
+ * factorisation.  mode 1: an environment with r > ratio_hi (or a failed factorisation) is not committed by the
+ * fp32 kernel; the same call is redone for it by the fp64 kernel, which keeps the environment's state and prior in
+ * an fp64 shadow record until r < ratio_lo again.  mode 0: fp32 only, no watch.  mode 2: every environment on the
+ * fp64 kernel (an independent second implementation: the device reference of the tests).  mode -1: the default
+ * rule -- 1 for windows with landmarks or once slam_set_unary was used, else 0 (pose-only windows keep the anchor
+ * out of every factor).  ratio_hi / ratio_lo: 0 keeps the current value (defaults 300 / 150).
+ * Bit-for-bit equality of slam_step with the separate calls holds for environments that stay in one mode. */
+int slam_set_precision(slam_ctx* ctx, int mode, float ratio_hi, float ratio_lo);
 
 int slam_count(const slam_ctx* ctx);                /* host-side window count c in [1, window] */
 long long slam_launch_count(const slam_ctx* ctx);   /* kernels launched by this context so far */

@@ -23,7 +23,7 @@ SYMBOLS = (
     "slam_default_config", "slam_workspace_bytes", "slam_create", "slam_destroy", "slam_reset",
     "slam_reset_envs", "slam_push_step", "slam_set_unary", "slam_observe_first", "slam_solve", "slam_marginal_cov", "slam_dopt",
     "slam_marginalize_oldest", "slam_step", "slam_step_host", "slam_get_poses", "slam_get_landmarks",
-    "slam_get_status", "slam_get_stats", "slam_reward", "slam_scan_match", "slam_grid_update", "slam_count", "slam_launch_count", "slam_last_error", "slam_kernel_info",
+    "slam_get_status", "slam_get_stats", "slam_set_precision", "slam_reward", "slam_scan_match", "slam_grid_update", "slam_count", "slam_launch_count", "slam_last_error", "slam_kernel_info",
 )
 
 
@@ -82,6 +82,7 @@ def _load() -> C.CDLL:
     lib.slam_reward.argtypes = [vp, C.POINTER(RewardParams), fp, fp, fp, fp, ip, fp]
     lib.slam_scan_match.argtypes = [C.POINTER(ScanParams), C.c_int, fp, fp, fp, fp, fp, fp, vp]
     lib.slam_grid_update.argtypes = [C.POINTER(ScanParams), C.c_int, fp, fp, fp, fp, C.c_float, C.c_float, C.c_float, vp]
+    lib.slam_set_precision.argtypes = [vp, C.c_int, C.c_float, C.c_float]
     lib.slam_count.argtypes = [vp]
     lib.slam_launch_count.argtypes = [vp]
     lib.slam_launch_count.restype = C.c_longlong
@@ -278,7 +279,11 @@ class FixedLagSlam:
         out = self._new(8, dtype=torch.int64)
         self._chk(LIB.slam_get_stats(self._h, C.c_void_p(out.data_ptr())))
         v = [int(x) for x in out.cpu()]
-        return dict(max_envelope_words=v[0], mean_envelope_words=v[1] / max(v[2], 1), solved=v[2], waited=v[3])
+        return dict(max_envelope_words=v[0], mean_envelope_words=v[1] / max(v[2], 1), solved=v[2], waited=v[3], fp64_calls=v[4])
+
+    def set_precision(self, mode: int, ratio_hi: float = 0.0, ratio_lo: float = 0.0):
+        """-1 default rule, 0 fp32 only, 1 fp32 + fp64 fallback on ill-conditioned windows, 2 fp64 everywhere."""
+        self._chk(LIB.slam_set_precision(self._h, int(mode), float(ratio_hi), float(ratio_lo)))
 
     def reward(self, params: RewardParams, u, u_prev, dcells, d_min, collision, out=None):
         out = self._new(self.N) if out is None else out

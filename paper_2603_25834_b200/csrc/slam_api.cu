@@ -10,6 +10,7 @@
 
 #include "../../include/slam.h"
 #include "slam_kernels.cuh"
+#include "slam_ref64.cuh"
 
 using namespace slamk;
 
@@ -32,7 +33,8 @@ using namespace slamk;
 template <int TEAM, bool PAIRS, bool LM>
 __global__ void __launch_bounds__(TEAM == 128 ? 896 : SLAM_MAXTHREADS)
 slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flags, int iters, StepIO io,
-                 unsigned long long* stats, const int* __restrict__ perm, int* __restrict__ keys) {
+                 unsigned long long* stats, const int* __restrict__ perm, int* __restrict__ keys,
+                 int* __restrict__ fb_list, int* __restrict__ fb_cnt) {
   extern __shared__ float4 smem4[];
   __shared__ int s_env[16], s_need[16], s_off[16], s_new[16], s_ctl[2];
   float* smem = reinterpret_cast<float*>(smem4);
@@ -85,6 +87,12 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
     if (s_ctl[1] == 0) break;
     if (!waiting) {
       env = s_env[team];
+      // an environment whose state and prior live in the fp64 shadow record belongs to the fp64 path
+      // (slam_ref64.cuh): queue it there and leave this team idle for the round
+      if (env >= 0 && fb_list && reinterpret_cast<const int*>(state + (size_t)env * ly.rec)[ly.o_mode] != 0) {
+        if (lane == 0) { fb_list[atomicAdd(fb_cnt, 1)] = env; s_env[team] = -1; }
+        env = -1;
+      }
       if (env >= 0) {
         float* rec = state + (size_t)env * ly.rec;
         // NEXT-2: an environment that was reset mid-run lives in the slots k0.. of the lock-step window:
@@ -185,7 +193,16 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
       }
     }
     if (LOCK >= -1) __syncthreads();
-    if (valid) {
+    // Conditioning: the anchor pivots cancelled beyond what fp32 can carry (or the
+    // factorisation failed outright).  Nothing of this call is committed for the environment -- the record still
+    // holds its state before the call -- and the fp64 path redoes the call.
+    bool redo = false;
+    if (valid && fb_list && nlin > 0) {
+      redo = tm.any(status != 0, lane);
+      if (redo && lane == 0) fb_list[atomicAdd(fb_cnt, 1)] = env;
+    }
+    if (valid && !redo) {
+      status &= ~ENV_ILLCOND;
       if (io.last_pose && lane == 0) {  // newest pose in global coordinates: a (+) e_{c-1}
         float sn, cn;
         sincos_pi(w.st[2], &sn, &cn);
@@ -252,6 +269,13 @@ __global__ void __launch_bounds__(1024) slam_order_kernel(int N, int key_max, co
   }
 }
 
+// precision mode 2 (device reference): every environment goes to the fp64 path
+__global__ void slam_fill_list_kernel(int N, int* list, int* cnt) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < N) list[i] = i;
+  if (i == 0) cnt[0] = N;
+}
+
 // reset: one warp per environment
 __global__ void slam_reset_kernel(Layout ly, Params pr, float* state, const float* init_pose, int* perm, int* keys) {
   const int env = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
@@ -292,14 +316,30 @@ __global__ void slam_reset_envs_kernel(Layout ly, Params pr, float* state, int c
 }
 
 // poses[3][W][N] = a (+) e_k for k < c, else 0
-__global__ void slam_poses_kernel(Layout ly, const float* state, int head, int c, float* poses) {
+__global__ void slam_poses_kernel(Layout ly, const float* state, const double* state64, int head, int c, float* poses) {
   const int env = blockIdx.x * blockDim.x + threadIdx.x;
   if (env >= ly.N) return;
   const float* rec = state + (size_t)env * ly.rec;
-  const float ax = rec[ly.o_a], ay = rec[ly.o_a + 1], at = rec[ly.o_a + 2];
   const int k0 = reinterpret_cast<const int*>(rec)[ly.o_k0];
   c -= k0;
   head = (head + k0) % ly.W;
+  if (reinterpret_cast<const int*>(rec)[ly.o_mode] != 0) {   // the state lives in the fp64 shadow record
+    const double* r64 = state64 + (size_t)env * ly.rec;
+    const double ax = r64[ly.o_a], ay = r64[ly.o_a + 1], at = r64[ly.o_a + 2], sn = sin(at), cn = cos(at);
+    for (int k = 0; k < ly.W; ++k) {
+      double x = 0.0, y = 0.0, t = 0.0;
+      if (k < c) {
+        const int r = ring_of(k, head, ly.W);
+        const double ex = k ? r64[ly.o_e + 3 * r] : 0.0, ey = k ? r64[ly.o_e + 3 * r + 1] : 0.0, et = k ? r64[ly.o_e + 3 * r + 2] : 0.0;
+        x = ax + cn * ex - sn * ey; y = ay + sn * ex + cn * ey; t = slamr::wrapr(at + et);
+      }
+      poses[((size_t)0 * ly.W + k) * ly.N + env] = (float)x;
+      poses[((size_t)1 * ly.W + k) * ly.N + env] = (float)y;
+      poses[((size_t)2 * ly.W + k) * ly.N + env] = (float)t;
+    }
+    return;
+  }
+  const float ax = rec[ly.o_a], ay = rec[ly.o_a + 1], at = rec[ly.o_a + 2];
   float sn, cn;
   sincos_pi(at, &sn, &cn);
   for (int k = 0; k < ly.W; ++k) {
@@ -315,15 +355,17 @@ __global__ void slam_poses_kernel(Layout ly, const float* state, int head, int c
   }
 }
 
-__global__ void slam_landmarks_kernel(Layout ly, const float* state, float* lm, uint32_t* active) {
+__global__ void slam_landmarks_kernel(Layout ly, const float* state, const double* state64, float* lm, uint32_t* active) {
   const int env = blockIdx.x * blockDim.x + threadIdx.x;
   if (env >= ly.N) return;
   const float* rec = state + (size_t)env * ly.rec;
+  const double* r64 = state64 + (size_t)env * ly.rec;
   const uint32_t* recu = reinterpret_cast<const uint32_t*>(rec);
+  const bool m64 = recu[ly.o_mode] != 0;
   for (int q = 0; q < ly.nw; ++q) active[(size_t)q * ly.N + env] = recu[ly.o_act + q];
   for (int l = 0; l < ly.L; ++l) {
     const bool act = (recu[ly.o_act + (l >> 5)] >> (l & 31)) & 1u;
-    const float mx = rec[ly.o_m + 2 * l], my = rec[ly.o_m + 2 * l + 1];
+    const float mx = m64 ? (float)r64[ly.o_m + 2 * l] : rec[ly.o_m + 2 * l], my = m64 ? (float)r64[ly.o_m + 2 * l + 1] : rec[ly.o_m + 2 * l + 1];
     lm[((size_t)0 * ly.L + l) * ly.N + env] = act ? mx : 0.f;  // landmarks are stored in global coordinates
     lm[((size_t)1 * ly.L + l) * ly.N + env] = act ? my : 0.f;
   }
@@ -373,6 +415,14 @@ struct slam_ctx {
   float* cov_cache;
   unsigned long long* stats;  // [8] device counters: max / sum / count of envelope words, ...
   int *perm, *keys;           // [N] cost order of the environments and the keys it is sorted by
+  // fp64 path (slam_ref64.cuh): shadow records, the list of environments it has to process, launch shape
+  double* state64;
+  int *fb_list, *fb_cnt;
+  double* hglob;
+  int precision;              // 0: fp32 only, 1: fp32 with fp64 fallback on ill-conditioned windows, 2: fp64 everywhere
+  bool precision_auto;        // the default rule decides (landmarks or unary factors -> 1, else 0)
+  float ratio_hi, ratio_lo;
+  int ref_grid, ref_smem;
   bool order, order_all;      // re-sort after every solve (SLAM_ORDER=0 disables, 2: pose-only windows too)
   // device staging for slam_step_host
   float *st_odom, *st_lc_meas, *st_rb_meas, *st_cov, *st_logdet, *st_pose;
@@ -461,7 +511,7 @@ static int pick_launch(int W, int L, int team, int pairs, int* pool_words) {
   *pool_words = best_pool;
   return best;  // 0 if one environment does not fit
 }
-typedef void (*step_fn)(Layout, Params, float*, int, int, int, int, StepIO, unsigned long long*, const int*, int*);
+typedef void (*step_fn)(Layout, Params, float*, int, int, int, int, StepIO, unsigned long long*, const int*, int*, int*, int*);
 template <bool PAIRS, bool LM>
 static step_fn kernel_pick(int team) {
   return team == 128 ? slam_step_kernel<128, PAIRS, LM> : (team == 64 ? slam_step_kernel<64, PAIRS, LM> : slam_step_kernel<32, PAIRS, LM>);
@@ -483,7 +533,13 @@ static int pick_pairs(int W, int L, int team) {
   return L == 0 && team == 32 && 16.0 * (d.team_words + 0.3 * d.dense) > SMEM_BUDGET / 4;
 }
 
-struct WsPlan { size_t stats, perm, keys, state, cache, odom, lcb, lcm, rbk, rbm, cov, ld, pose, total; };
+// fp64 path: dynamic shared memory of one CTA (everything but H, plus H when it fits) and the global scratch
+// for H when it does not (one packed triangle per resident CTA; grid = 2 CTAs per SM then)
+static const int REF_MAX_GRID_GLOBAL = 2 * 160;
+static size_t ref_small_bytes(const Layout& ly) { return slamr::ref_smem_doubles(ly) * 8 + slamr::ref_smem_ints(ly) * 4 + 32; }
+static bool ref_h_in_smem(const Layout& ly) { return ref_small_bytes(ly) + slamr::ref_tri(ly) * 8 <= (size_t)SMEM_BUDGET; }
+static size_t ref_hglob_bytes(const Layout& ly) { return ref_h_in_smem(ly) ? 0 : (size_t)REF_MAX_GRID_GLOBAL * slamr::ref_tri(ly) * 8; }
+struct WsPlan { size_t stats, perm, keys, state, cache, odom, lcb, lcm, rbk, rbm, cov, ld, pose, fbl, fbc, s64, hg, total; };
 static WsPlan plan(const Layout& ly) {
   WsPlan p;
   size_t o = 0;
@@ -501,6 +557,10 @@ static WsPlan plan(const Layout& ly) {
   p.cov = o; o = al256(o + N * 9 * 4);
   p.ld = o; o = al256(o + N * 4);
   p.pose = o; o = al256(o + N * 3 * 4);
+  p.fbl = o; o = al256(o + N * 4);
+  p.fbc = o; o = al256(o + 64);
+  p.s64 = o; o = al256(o + N * ly.rec * 8);
+  p.hg = o; o = al256(o + ref_hglob_bytes(ly));
   p.total = o;
   return p;
 }
@@ -572,6 +632,23 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   c->launches = 0;
   c->err[0] = 0;
   c->un_pose = nullptr; c->un_info = nullptr; c->un_valid = nullptr;
+  c->fb_list = (int*)(base + p.fbl);
+  c->fb_cnt = (int*)(base + p.fbc);
+  c->state64 = (double*)(base + p.s64);
+  c->hglob = ref_h_in_smem(c->ly) ? nullptr : (double*)(base + p.hg);
+  // Precision.  Pose-only windows without absolute measurements keep the anchor out of
+  // every factor: fp32 holds the tolerances with a wide margin and the watch is off.  Landmarks (global, so every
+  // range-bearing factor touches the anchor) and unary factors switch it on: slam_set_precision overrides.
+  c->precision_auto = true;
+  c->precision = landmarks > 0 ? 1 : 0;
+  c->ratio_hi = 300.f; c->ratio_lo = 150.f;
+  { const char* e = getenv("SLAM_PRECISION"); if (e && e[0] >= '0' && e[0] <= '2') { c->precision = e[0] - '0'; c->precision_auto = false; } }
+  c->ref_smem = (int)(ref_small_bytes(c->ly) + (c->hglob ? 0 : slamr::ref_tri(c->ly) * 8));
+  if (cudaFuncSetAttribute(slamr::slam_ref64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET) != cudaSuccess) {
+    cudaGetLastError();
+    delete c;
+    return SLAM_ECUDA;
+  }
   c->smem_bytes = (c->ly.team_words * wpc + c->ly.pool) * 4;
   if (cudaFuncSetAttribute(kernel_of(team, c->ly.pairs, c->ly.L), cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET) != cudaSuccess) {
     cudaGetLastError();
@@ -586,6 +663,14 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   c->ctas_per_sm = occ;
   const int need = (batch + wpc - 1) / wpc;
   c->grid = need < sms * occ ? need : sms * occ;
+  {
+    int rocc = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&rocc, slamr::slam_ref64_kernel, slamr::NT, c->ref_smem);
+    if (rocc < 1) { cudaGetLastError(); delete c; return SLAM_ECUDA; }
+    long long g = (long long)sms * rocc;
+    if (c->hglob && g > REF_MAX_GRID_GLOBAL) g = REF_MAX_GRID_GLOBAL;
+    c->ref_grid = (int)(g < batch ? g : batch);
+  }
   *out = c;
   const int rc = slam_reset(c, nullptr);
   if (rc != SLAM_OK) { *out = nullptr; slam_destroy(c); }
@@ -601,6 +686,7 @@ int slam_reset(slam_ctx* c, const float* init_pose) {
   if (!c) return SLAM_EINVAL;
   const int threads = 256, blocks = (int)(((size_t)c->ly.N * 32 + threads - 1) / threads);
   cudaMemsetAsync(c->stats, 0, 64, c->stream);
+  cudaMemsetAsync(c->fb_cnt, 0, 64, c->stream);
   slam_reset_kernel<<<blocks, threads, 0, c->stream>>>(c->ly, c->pr, c->state, init_pose, c->perm, c->keys);
   c->launches++;
   c->head = 0; c->count = 1; c->cov_valid = false;
@@ -609,9 +695,24 @@ int slam_reset(slam_ctx* c, const float* init_pose) {
 
 static int launch_step(slam_ctx* c, int flags, int iters, const StepIO& io) {
   const step_fn fn = kernel_of(c->ly.team, c->ly.pairs, c->ly.L);
-  fn<<<c->grid, c->ly.wpc * c->ly.team, c->smem_bytes, c->stream>>>(c->ly, c->pr, c->state, c->head, c->count, flags, iters, io,
-                                                                      c->stats, c->perm, c->keys);
-  c->launches++;
+  if (c->precision == 2) {   // device reference: every environment through the fp64 path
+    const int threads = 256, blocks = (c->ly.N + threads - 1) / threads;
+    slam_fill_list_kernel<<<blocks, threads, 0, c->stream>>>(c->ly.N, c->fb_list, c->fb_cnt);
+    c->launches++;
+  } else {
+    Layout ly = c->ly;
+    ly.ratio_hi = c->precision == 1 ? c->ratio_hi : 0.f;
+    fn<<<c->grid, c->ly.wpc * c->ly.team, c->smem_bytes, c->stream>>>(ly, c->pr, c->state, c->head, c->count, flags, iters, io,
+                                                                        c->stats, c->perm, c->keys,
+                                                                        c->precision == 1 ? c->fb_list : nullptr, c->fb_cnt);
+    c->launches++;
+  }
+  if (c->precision >= 1) {   // the environments the fp32 kernel queued: fp64 records, and the windows it refused to commit
+    slamr::RefArgs ra = {c->state, c->state64, c->head, c->count, flags, iters, c->fb_list, c->fb_cnt, c->stats, c->hglob,
+                         (double)c->ratio_lo, c->precision == 2 ? 1 : 0};
+    slamr::slam_ref64_kernel<<<c->ref_grid, slamr::NT, c->ref_smem, c->stream>>>(c->ly, c->pr, ra, io);
+    c->launches++;
+  }
   // the solve left fresh cost keys: order the next launches by them (pointless unless every CTA runs
   // several rounds; a small batch is latency bound: one more kernel boundary per step would show; and
   // measured only landmark windows gain -- their cost varies most: config 3 2.40 -> 2.31 ms per step,
@@ -650,6 +751,7 @@ int slam_set_unary(slam_ctx* c, const float* pose, const float* info, const int3
   if (!c) return SLAM_EINVAL;
   if ((pose == nullptr) != (info == nullptr)) return fail(c, SLAM_EINVAL, "pose and info must both be given (or both NULL to cancel)");
   c->un_pose = pose; c->un_info = info; c->un_valid = pose ? valid : nullptr;
+  if (pose && c->precision_auto && c->precision == 0) c->precision = 1;   // absolute measurements couple the anchor to the window
   return SLAM_OK;
 }
 
@@ -764,7 +866,7 @@ int slam_step_host(slam_ctx* c, const float* odom, const int32_t* lc_back, const
 int slam_get_poses(slam_ctx* c, float* poses) {
   if (!c || !poses) return SLAM_EINVAL;
   const int threads = 128, blocks = (c->ly.N + threads - 1) / threads;
-  slam_poses_kernel<<<blocks, threads, 0, c->stream>>>(c->ly, c->state, c->head, c->count, poses);
+  slam_poses_kernel<<<blocks, threads, 0, c->stream>>>(c->ly, c->state, c->state64, c->head, c->count, poses);
   c->launches++;
   return check_cuda(c, "slam_poses_kernel");
 }
@@ -774,7 +876,7 @@ int slam_get_landmarks(slam_ctx* c, float* lm, uint32_t* active) {
   if (c->ly.L == 0) return SLAM_OK;
   if (!lm || !active) return fail(c, SLAM_EINVAL, "lm/active are NULL");
   const int threads = 128, blocks = (c->ly.N + threads - 1) / threads;
-  slam_landmarks_kernel<<<blocks, threads, 0, c->stream>>>(c->ly, c->state, lm, active);
+  slam_landmarks_kernel<<<blocks, threads, 0, c->stream>>>(c->ly, c->state, c->state64, lm, active);
   c->launches++;
   return check_cuda(c, "slam_landmarks_kernel");
 }
@@ -801,6 +903,19 @@ int slam_reward(slam_ctx* c, const slam_reward_params* p, const float* u, const 
   slam_reward_kernel<<<blocks, threads, 0, c->stream>>>(c->ly.N, *p, u, u_prev, dcells, d_min, collision, reward);
   c->launches++;
   return check_cuda(c, "slam_reward_kernel");
+}
+
+int slam_set_precision(slam_ctx* c, int mode, float ratio_hi, float ratio_lo) {
+  if (!c) return SLAM_EINVAL;
+  if (mode < -1 || mode > 2) return fail(c, SLAM_EINVAL, "precision mode must be -1 (default rule), 0, 1 or 2");
+  if (ratio_hi < 0.f || ratio_lo < 0.f || (ratio_hi > 0.f && ratio_lo > ratio_hi)) return fail(c, SLAM_EINVAL, "need 0 < ratio_lo <= ratio_hi (0 keeps the current value)");
+  if (mode == -1) { c->precision_auto = true; c->precision = c->ly.L > 0 ? 1 : 0; }
+  else { c->precision_auto = false; c->precision = mode; }
+  if (ratio_hi > 0.f) c->ratio_hi = ratio_hi;
+  if (ratio_lo > 0.f) c->ratio_lo = ratio_lo;
+  if (c->ratio_lo > c->ratio_hi) c->ratio_lo = c->ratio_hi;
+  c->cov_valid = false;
+  return SLAM_OK;
 }
 
 int slam_count(const slam_ctx* c) { return c ? c->count : -1; }

@@ -26,7 +26,7 @@
 namespace slamk {
 
 enum { F_PUSH = 1, F_OBS0 = 2, F_COV = 4, F_MARG = 8, F_COPYCOV = 16 };
-enum { ENV_NOT_PD = 1, ENV_NONFINITE = 2 };
+enum { ENV_NOT_PD = 1, ENV_NONFINITE = 2, ENV_ILLCOND = 8 };  // ILLCOND is internal: never stored in the status word
 
 struct StepIO {
   const float* odom; const int32_t* lc_back; const float* lc_meas; const uint32_t* rb_mask; const float* rb_meas;
@@ -1071,6 +1071,14 @@ __device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int
   const Tables tb = tables_of(ly, w);
   constexpr int KUNROLL = SLAM_KUNROLL;
   int flag = 0;
+  // Conditioning watch: the anchor's pivots are what fp32 loses first -- a robot that
+  // dead-reckoned and re-observes a landmark has information on `a` spanning six decades.  Keep the assembled
+  // diagonal of the three anchor rows; after the last column block compare it with the pivots.
+  float ha0 = 0.f, ha1 = 0.f, ha2 = 0.f;
+  if (ly.ratio_hi > 0.f) {
+    const int oA = np - 3;
+    ha0 = w.H[rb_of(w, oA) + oA]; ha1 = w.H[rb_of(w, oA + 1) + oA + 1]; ha2 = w.H[rb_of(w, oA + 2) + oA + 2];
+  }
   for (int J = 0; J < G; ++J) {
     const int c0 = 4 * J;
     // the block's rows: pair A = rows c0, c0+1 (columns from fA), pair B = rows c0+2, c0+3 (from fB)
@@ -1184,6 +1192,8 @@ __device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int
           if (!(t22 > 0.f)) d2 = 1.f;
           if (!(t33 > 0.f)) d3 = 1.f;
         }
+        // rows np-3 .. np-1 of the last block are the anchor: H_ii / L_ii^2 = H_ii d_i^2
+        if (J == G - 1 && fmaxf(fmaxf(ha0 * d1 * d1, ha1 * d2 * d2), ha2 * d3 * d3) > ly.ratio_hi && ly.ratio_hi > 0.f) flag |= ENV_ILLCOND;
       }
       if (act && t == 0) {
         if (first_pass && q < 2) {

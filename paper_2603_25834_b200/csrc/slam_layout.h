@@ -19,7 +19,7 @@ struct Layout {
   int np, pad;         // matrix dimension padded to a multiple of 4 (pad dummy rows before the newest pose)
   // record (32-bit words)
   int rec;             // record stride
-  int o_status, o_k0, o_pm, o_lm, o_act, o_um, o_a, o_e, o_m, o_zodo, o_lct, o_zlc, o_rbm, o_zrb, o_zun, o_omun, o_vbar, o_g, o_lam;
+  int o_status, o_k0, o_pm, o_lm, o_act, o_um, o_mode, o_a, o_e, o_m, o_zodo, o_lct, o_zlc, o_rbm, o_zrb, o_zun, o_omun, o_vbar, o_g, o_lam;
   // shared memory: a FIXED part per team (32-bit words) ...
   int s_scr, s_st, s_lct, s_cs, s_rbm, s_rbf, s_sup, s_sds;
   int team_words;      // fixed shared words per team
@@ -33,6 +33,7 @@ struct Layout {
   int pairs;           // 1: envelope rows grouped in pairs instead of fours (less shared memory, more instructions)
   int lcache;          // 1: keep the factor columns of passive landmarks across the linearisations of one call
   int lock;            // lock-step level: CTA barriers before assemble (1), + before Cholesky (2), + before the solve (3)
+  float ratio_hi;      // anchor pivot ratio H_aa / L_aa^2 above which the fp32 kernel hands the environment to the fp64 path (0: never)
 };
 
 struct Params {
@@ -53,6 +54,7 @@ static inline Layout make_layout(int N, int W, int L, int pool, int wpc) {
   y.o_lm = o; o += 2;
   y.o_act = o; o += 2;
   y.o_um = o; o += 2;   // ring positions that carry a unary absolute-pose factor
+  y.o_mode = o; o += 1; // 0: state and prior live in this fp32 record; 1: in the fp64 shadow record (slam_ref64.cuh)
   o = pad4(o + 1);
   y.o_a = o; o += 4;
   y.o_e = o; o = pad4(o + 3 * W);
@@ -95,6 +97,7 @@ static inline Layout make_layout(int N, int W, int L, int pool, int wpc) {
   y.wpc = wpc;
   y.team = 32;
   y.lock = 1;
+  y.ratio_hi = 0.f;
   y.lcache = 1;
   y.pairs = 0;
   return y;
