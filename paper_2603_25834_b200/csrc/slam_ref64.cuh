@@ -64,7 +64,7 @@ struct Sm {
 
 __host__ __device__ inline size_t ref_smem_doubles(const Layout& ly) {  // everything but H
   const int n = ly.n, m = ly.W > ly.L ? ly.W : ly.L;
-  return (size_t)4 * n + 2 * ly.W + 9 * m + 6 * n + 16;
+  return (size_t)4 * n + 2 * ly.W + ((9 * m + 1) & ~1) + 6 * n + 16;
 }
 __host__ __device__ inline size_t ref_smem_ints(const Layout& ly) { return (size_t)4 * ly.n + ly.W + ly.W * (ly.nw ? ly.nw : 1) + 8; }
 __host__ __device__ inline size_t ref_tri(const Layout& ly) { return (size_t)ly.n * (ly.n + 1) / 2; }
@@ -152,7 +152,7 @@ __device__ inline Sm carve(const Layout& ly, double* base, double* hglob) {
   const int n = ly.n, m = ly.W > ly.L ? ly.W : ly.L;
   double* p = base;
   s.v = p; p += n; s.b = p; p += n; s.d = p; p += n; s.col = p; p += n;
-  s.cs = p; p += 2 * ly.W; s.part = p; p += 9 * m; s.X = p; p += 3 * n; s.Q = p; p += 3 * n; p += 16;
+  s.cs = p; p += 2 * ly.W; s.part = p; p += (9 * m + 1) & ~1; s.X = p; p += 3 * n; s.Q = p; p += 3 * n; p += 16;
   int* q = reinterpret_cast<int*>(p);
   s.pos = q; q += n; s.first = q; q += n; s.sidx = q; q += n; s.omap = q; q += n; s.lct = q; q += ly.W;
   s.rbm = reinterpret_cast<uint32_t*>(q); q += ly.W * (ly.nw ? ly.nw : 1); q += 8;
@@ -308,12 +308,7 @@ __device__ void ref_assemble(const Layout& ly, const Params& pr, const Ctx& e, c
     s.d[p] = d;
   }
   __syncthreads();
-  // identity rows: unused pose slots, inactive landmarks
-  for (int i = 3 + tid; i < n; i += NT) {
-    const bool unused = i < 3 * W ? (i / 3) >= c : !((e.act >> ((i - 3 * W) >> 1)) & 1ull);
-    if (unused) H[tri(s.pos[i], s.pos[i])] = 1.0;
-  }
-  // prior: H += Lambda, b -= Lambda d + g
+  // prior: H = Lambda on the support; b = -(Lambda d + g) read back from shared memory (no second pass over HBM)
   {
     const int st = e.s * (e.s + 1) / 2;
     for (int t = tid; t < st; t += NT) {
@@ -321,13 +316,20 @@ __device__ void ref_assemble(const Layout& ly, const Params& pr, const Ctx& e, c
       while ((p + 1) * (p + 2) / 2 <= t) ++p;
       while (p * (p + 1) / 2 > t) --p;
       const int q = t - p * (p + 1) / 2;
-      Hat(H, s.pos[s.sidx[p]], s.pos[s.sidx[q]]) += ldr(e, ly.o_lam + t);
+      Hat(H, s.pos[s.sidx[p]], s.pos[s.sidx[q]]) = ldr(e, ly.o_lam + t);
     }
+    __syncthreads();
     for (int p = tid; p < e.s; p += NT) {
+      const int pp = s.pos[s.sidx[p]];
       real acc = ldr(e, ly.o_g + p);
-      for (int q = 0; q < e.s; ++q) acc += ldr(e, ly.o_lam + (q <= p ? tri(p, q) : tri(q, p))) * s.d[q];
-      s.b[s.pos[s.sidx[p]]] -= acc;
+      for (int q = 0; q < e.s; ++q) acc += Hat(H, pp, s.pos[s.sidx[q]]) * s.d[q];
+      s.b[pp] = -acc;
     }
+  }
+  // identity rows: unused pose slots, inactive landmarks
+  for (int i = 3 + tid; i < n; i += NT) {
+    const bool unused = i < 3 * W ? (i / 3) >= c : !((e.act >> ((i - 3 * W) >> 1)) & 1ull);
+    if (unused) H[tri(s.pos[i], s.pos[i])] = 1.0;
   }
   __syncthreads();
   // odometry k-1 -> k: j side, then i side
@@ -494,69 +496,166 @@ __device__ void ref_assemble(const Layout& ly, const Params& pr, const Ctx& e, c
   }
 }
 
-// ------------------------------------------------------------------ Cholesky (right-looking, column by column)
-// On exit H holds L (diagonal = L_jj), b holds y = L^{-1} b.  Returns status bits; *ratio = max over the
-// anchor rows of H_ii / L_ii^2 (the cancellation the fp32 kernel cannot afford).
+// ------------------------------------------------------------------ Cholesky (right-looking, blocks of 4 columns)
+// Per block: the first warp factorises the 4x4 diagonal tile (and the rhs entries of the block) in registers and
+// publishes it; the rows with entries in the block scale their four entries (kept in col4 for the others) and are
+// gathered in a compact list; the rank-4 update of the trailing envelope runs flat over the pairs of that list.
+// Two barriers per block.  On exit H holds L (diagonal = L_jj), b holds y = L^{-1} b, s.d holds 1 / L_jj.
+// Returns status bits; *ratio = max over the anchor rows of H_ii / L_ii^2 (the cancellation the fp32 kernel
+// cannot afford).
 __device__ int ref_cholesky(const Layout& ly, const Sm& s, int tid, real* ratio) {
   const int n = ly.n;
   real* H = s.H;
-  __shared__ real sh_d, sh_y, sh_ha[3];
-  __shared__ int sh_flag;
+  real* col4 = s.X;   // [n][4] (X and Q are contiguous: 6n doubles; only the marginalisation uses them as X, Q)
+  real* dinv = s.d;   // 1 / L_jj for the back substitution (the prior displacement is dead by now)
+  int* act = s.omap;  // compact list of the rows that take part in the current block
   for (int p = tid; p < n; p += NT) {  // envelope: first non-zero of each row (fill stays inside it)
     int f = 0;
     while (f < p && H[tri(p, f)] == 0.0) ++f;
     s.first[p] = f;
   }
-  if (tid < 3) sh_ha[tid] = H[tri(n - 3 + tid, n - 3 + tid)];
-  if (tid == 0) sh_flag = 0;
+  real ha[3];
+#pragma unroll
+  for (int x = 0; x < 3; ++x) ha[x] = H[tri(n - 3 + x, n - 3 + x)];
+  int flag = 0;
+  __shared__ int sh_cnt[3][NT / 32];   // active rows per (chunk of NT rows, warp)
+  __shared__ real sh_t[4][4], sh_ti[4], sh_y[4];
+  __shared__ int sh_flag;
+  const int lane = tid & 31, wid = tid >> 5;
   __syncthreads();
-  for (int j = 0; j < n; ++j) {
-    if (tid == 0) {
-      real piv = H[tri(j, j)];
-      if (!(piv > 0.0)) { sh_flag |= slamk::ENV_NOT_PD; piv = 1.0; }
-      const real dj = sqrt(piv);
-      H[tri(j, j)] = dj;
-      sh_d = dj;
-      sh_y = s.b[j] / dj;
-      s.b[j] = sh_y;
+  for (int j = 0; j < n; j += 4) {
+    const int nb = n - j < 4 ? n - j : 4, r0 = j + nb;
+    // rows below the block that have entries in it (first < r0): ballots now, list after the barrier
+    unsigned bal[3];
+#pragma unroll
+    for (int ch = 0; ch < 3; ++ch) {
+      const int i = r0 + ch * NT + tid;
+      bal[ch] = __ballot_sync(0xffffffffu, i < n && s.first[i] < r0);
+      if (lane == 0) sh_cnt[ch][wid] = __popc(bal[ch]);
+    }
+    if (wid == 0) {   // diagonal tile, identity-padded when nb < 4 (every lane the same arithmetic)
+      real t[4][4], y[4], ti[4];
+#pragma unroll
+      for (int x = 0; x < 4; ++x) {
+#pragma unroll
+        for (int c = 0; c < 4; ++c) t[x][c] = (x < nb && c <= x) ? H[tri(j + x, j + c)] : (x == c ? 1.0 : 0.0);
+        y[x] = x < nb ? s.b[j + x] : 0.0;
+      }
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        real piv = t[c][c];
+#pragma unroll
+        for (int k = 0; k < c; ++k) piv -= t[c][k] * t[c][k];
+        if (!(piv > 0.0)) { flag |= slamk::ENV_NOT_PD; piv = 1.0; }
+        const real dj = sqrt(piv), inv = 1.0 / dj;
+        t[c][c] = dj; ti[c] = inv;
+#pragma unroll
+        for (int x = c + 1; x < 4; ++x) {
+          real v = t[x][c];
+#pragma unroll
+          for (int k = 0; k < c; ++k) v -= t[x][k] * t[c][k];
+          t[x][c] = v * inv;
+        }
+        real yy = y[c];
+#pragma unroll
+        for (int k = 0; k < c; ++k) yy -= t[c][k] * y[k];
+        y[c] = yy * inv;
+      }
+      __syncwarp();   // every lane has read the tile before lane 0 overwrites it
+      if (lane == 0) {
+#pragma unroll
+        for (int x = 0; x < 4; ++x) {
+#pragma unroll
+          for (int c = 0; c < 4; ++c) sh_t[x][c] = t[x][c];
+          sh_ti[x] = ti[x]; sh_y[x] = y[x];
+          if (x < nb) {
+#pragma unroll
+            for (int c = 0; c <= x; ++c) H[tri(j + x, j + c)] = t[x][c];
+            s.b[j + x] = y[x];
+            dinv[j + x] = ti[x];
+          }
+        }
+      }
     }
     __syncthreads();
-    const real inv = 1.0 / sh_d;
-    for (int i = j + 1 + tid; i < n; i += NT) {
-      real l = 0.0;
-      if (s.first[i] <= j) { l = H[tri(i, j)] * inv; H[tri(i, j)] = l; }
-      s.col[i] = l;
+    // active rows: L(i, j..j+3) by forward substitution with the tile; the rhs rides along
+    int m = 0;
+#pragma unroll
+    for (int ch = 0; ch < 3; ++ch) {
+      int base = m;
+#pragma unroll
+      for (int w2 = 0; w2 < NT / 32; ++w2) { const int cw = sh_cnt[ch][w2]; if (w2 < wid) base += cw; m += cw; }
+      if ((bal[ch] >> lane) & 1u) {
+        const int i = r0 + ch * NT + tid;
+        real* hp = H + tri(i, j);
+        const real l0 = hp[0] * sh_ti[0];
+        real l1 = 0.0, l2 = 0.0, l3 = 0.0;
+        if (nb > 1) l1 = (hp[1] - l0 * sh_t[1][0]) * sh_ti[1];
+        if (nb > 2) l2 = (hp[2] - l0 * sh_t[2][0] - l1 * sh_t[2][1]) * sh_ti[2];
+        if (nb > 3) l3 = (hp[3] - l0 * sh_t[3][0] - l1 * sh_t[3][1] - l2 * sh_t[3][2]) * sh_ti[3];
+        hp[0] = l0;
+        if (nb > 1) hp[1] = l1;
+        if (nb > 2) hp[2] = l2;
+        if (nb > 3) hp[3] = l3;
+        reinterpret_cast<double2*>(col4 + 4 * i)[0] = make_double2(l0, l1);
+        reinterpret_cast<double2*>(col4 + 4 * i)[1] = make_double2(l2, l3);
+        s.b[i] -= l0 * sh_y[0] + l1 * sh_y[1] + l2 * sh_y[2] + l3 * sh_y[3];
+        act[base + __popc(bal[ch] & ((1u << lane) - 1u))] = i;
+      }
     }
     __syncthreads();
-    const real yj = sh_y;
-    for (int i = j + 1 + tid; i < n; i += NT) {
-      const real li = s.col[i];
-      if (li == 0.0) continue;
-      real* row = H + tri(i, 0);
-      for (int k = j + 1; k <= i; ++k) row[k] -= li * s.col[k];
-      s.b[i] -= li * yj;
+    // rank-4 update of the trailing envelope, flat over the pairs (a >= b) of active rows
+    const int npair = m * (m + 1) >> 1;
+    for (int p = tid; p < npair; p += NT) {
+      int a = (int)((sqrtf(8.0f * (float)p + 1.0f) - 1.0f) * 0.5f);
+      if ((a + 1) * (a + 2) / 2 <= p) ++a;
+      if (a * (a + 1) / 2 > p) --a;
+      const int bq = p - (a * (a + 1) >> 1);
+      const int i = act[a], k = act[bq];
+      const double2 a01 = reinterpret_cast<const double2*>(col4 + 4 * i)[0], a23 = reinterpret_cast<const double2*>(col4 + 4 * i)[1];
+      const double2 b01 = reinterpret_cast<const double2*>(col4 + 4 * k)[0], b23 = reinterpret_cast<const double2*>(col4 + 4 * k)[1];
+      H[tri(i, k)] -= a01.x * b01.x + a01.y * b01.y + a23.x * b23.x + a23.y * b23.y;
     }
     __syncthreads();
   }
-  if (tid == 0) {
-    real r = 0.0;
-    for (int x = 0; x < 3; ++x) { const real l = H[tri(n - 3 + x, n - 3 + x)]; r = fmax(r, sh_ha[x] / (l * l)); }
-    *ratio = fmax(*ratio, r);
-  }
+  real r = 0.0;
+#pragma unroll
+  for (int x = 0; x < 3; ++x) { const real l = H[tri(n - 3 + x, n - 3 + x)]; r = fmax(r, ha[x] / (l * l)); }
+  if (tid == 0) { *ratio = fmax(*ratio, r); sh_flag = flag; }   // (thread 0 is in the warp that factorised the tiles)
   __syncthreads();
   return sh_flag;
 }
 
-// L' delta = y, in place in b
+// L' delta = y, in place in b: blocks of 4 rows from the bottom; the 4x4 tile solve is done by every thread
 __device__ void ref_backsub(const Layout& ly, const Sm& s, int tid) {
   const int n = ly.n;
-  __shared__ real sh_x;
-  for (int j = n - 1; j >= 0; --j) {
-    if (tid == 0) { sh_x = s.b[j] / s.H[tri(j, j)]; s.b[j] = sh_x; }
+  const int jlast = ((n - 1) >> 2) << 2;
+  for (int j = jlast; j >= 0; j -= 4) {
+    const int nb = n - j < 4 ? n - j : 4;
+    real t[4][4], x[4];
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+#pragma unroll
+      for (int c = 0; c < 4; ++c) t[r][c] = (r < nb && c < r) ? s.H[tri(j + r, j + c)] : 0.0;
+      x[r] = r < nb ? s.b[j + r] : 0.0;
+    }
+#pragma unroll
+    for (int r = 3; r >= 0; --r) {
+      real v = x[r];
+#pragma unroll
+      for (int k = r + 1; k < 4; ++k) v -= t[k][r] * x[k];
+      x[r] = v * (r < nb ? s.d[j + r] : 1.0);   // s.d holds 1 / L_jj (ref_cholesky)
+    }
     __syncthreads();
-    const real x = sh_x;
-    const real* row = s.H + tri(j, 0);
-    for (int k = s.first[j] + tid; k < j; k += NT) s.b[k] -= row[k] * x;
+#pragma unroll
+    for (int r = 0; r < 4; ++r) if (tid == r && r < nb) s.b[j + r] = x[r];
+    for (int k = tid; k < j; k += NT) {
+      real acc = 0.0;
+#pragma unroll
+      for (int r = 0; r < 4; ++r)
+        if (r < nb && s.first[j + r] <= k) acc += s.H[tri(j + r, k)] * x[r];
+      s.b[k] -= acc;
+    }
     __syncthreads();
   }
 }
@@ -667,9 +766,10 @@ __device__ void ref_marginalize(const Layout& ly, const Params& pr, Ctx& e, cons
     const int q = t - p * (p + 1) / 2;
     Hat(Hs, s.omap[p], s.omap[q]) = ldr(e, ly.o_lam + t);
   }
+  __syncthreads();
   for (int p = tid; p < so; p += NT) {
     real acc = ldr(e, ly.o_g + p);
-    for (int q = 0; q < so; ++q) acc += ldr(e, ly.o_lam + (q <= p ? tri(p, q) : tri(q, p))) * s.d[q];
+    for (int q = 0; q < so; ++q) acc += Hat(Hs, s.omap[p], s.omap[q]) * s.d[q];
     gam[s.omap[p]] = acc;
   }
   __syncthreads();
@@ -915,7 +1015,7 @@ __device__ void ref_store(const Layout& ly, const Ctx& e, const Sm& s, int tid, 
 }
 
 // ------------------------------------------------------------------ the kernel: persistent CTAs pull environments from the list
-__global__ void __launch_bounds__(NT) slam_ref64_kernel(Layout ly, Params pr, RefArgs ra, StepIO io) {
+__global__ void __launch_bounds__(NT, 3) slam_ref64_kernel(Layout ly, Params pr, RefArgs ra, StepIO io) {
   extern __shared__ double ref_smem[];
   __shared__ int sh_i;
   const int tid = threadIdx.x;
