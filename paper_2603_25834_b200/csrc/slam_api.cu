@@ -544,7 +544,7 @@ static WsPlan plan(const Layout& ly) {
   WsPlan p;
   size_t o = 0;
   const size_t N = (size_t)ly.N;
-  p.stats = o; o = al256(o + 64);
+  p.stats = o; o = al256(o + 256);
   p.perm = o; o = al256(o + N * 4);
   p.keys = o; o = al256(o + N * 4);
   p.state = o; o = al256(o + N * ly.rec * 4);
@@ -685,7 +685,7 @@ void slam_destroy(slam_ctx* ctx) {
 int slam_reset(slam_ctx* c, const float* init_pose) {
   if (!c) return SLAM_EINVAL;
   const int threads = 256, blocks = (int)(((size_t)c->ly.N * 32 + threads - 1) / threads);
-  cudaMemsetAsync(c->stats, 0, 64, c->stream);
+  cudaMemsetAsync(c->stats, 0, 256, c->stream);
   cudaMemsetAsync(c->fb_cnt, 0, 64, c->stream);
   slam_reset_kernel<<<blocks, threads, 0, c->stream>>>(c->ly, c->pr, c->state, init_pose, c->perm, c->keys);
   c->launches++;
@@ -710,6 +710,9 @@ static int launch_step(slam_ctx* c, int flags, int iters, const StepIO& io) {
   if (c->precision >= 1) {   // the environments the fp32 kernel queued: fp64 records, and the windows it refused to commit
     slamr::RefArgs ra = {c->state, c->state64, c->head, c->count, flags, iters, c->fb_list, c->fb_cnt, c->stats, c->hglob,
                          (double)c->ratio_lo, c->precision == 2 ? 1 : 0};
+#ifdef SLAM_REF_PROFILE
+    cudaMemcpyToSymbolAsync(slamr::g_ref_prof, &c->stats, sizeof(c->stats), 0, cudaMemcpyHostToDevice, c->stream);
+#endif
     slamr::slam_ref64_kernel<<<c->ref_grid, slamr::NT, c->ref_smem, c->stream>>>(c->ly, c->pr, ra, io);
     c->launches++;
   }
@@ -891,7 +894,11 @@ int slam_get_status(slam_ctx* c, int32_t* status) {
 
 int slam_get_stats(slam_ctx* c, unsigned long long* stats8) {
   if (!c || !stats8) return SLAM_EINVAL;
+#ifdef SLAM_REF_PROFILE
+  cudaMemcpyAsync(stats8, c->stats + 8, 64, cudaMemcpyDeviceToDevice, c->stream);
+#else
   cudaMemcpyAsync(stats8, c->stats, 64, cudaMemcpyDeviceToDevice, c->stream);
+#endif
   return check_cuda(c, "slam_get_stats");
 }
 

@@ -31,6 +31,15 @@ using slamk::slot_to_ring;
 typedef double real;
 constexpr int NT = 128;  // threads per environment (one CTA)
 
+#ifdef SLAM_REF_PROFILE   // developer build: cycles per phase into stats[8 + slot] (read with slam_get_stats)
+__device__ unsigned long long* g_ref_prof;
+#define REF_TICK(slot) { __syncthreads(); if (threadIdx.x == 0) { const long long tk1 = clock64(); atomicAdd(g_ref_prof + 8 + (slot), (unsigned long long)(tk1 - ref_tk0)); ref_tk0 = clock64(); } }
+#define REF_TICK_DECL long long ref_tk0 = clock64();
+#else
+#define REF_TICK(slot)
+#define REF_TICK_DECL
+#endif
+
 struct RefArgs {
   float* state32;
   double* state64;
@@ -134,11 +143,14 @@ __device__ __forceinline__ Rb rangebearing(const real* a, real ca, real sa, cons
   const real ddx = ca * ex - sa * ey, ddy = sa * ex + ca * ey;      // d = Rot(a_th) t_k
   const real xx = a[0] + ddx, xy = a[1] + ddy, xt = a[2] + et;
   const real dx = g[0] - xx, dy = g[1] - xy;
-  const real q = dx * dx + dy * dy, rho = sqrt(q);
+  // one reciprocal square root instead of a square root and four divisions (fp64 division and sqrt are long
+  // software sequences: the factor evaluation is the latency chain of the assembly)
+  const real q = dx * dx + dy * dy, irho = rsqrt(q), rho = q * irho, iq = irho * irho;
   f.r[0] = rho - zr;
   f.r[1] = wrapr(atan2(dy, dx) - xt - zb);
-  const real Jx[2][3] = {{-dx / rho, -dy / rho, 0.0}, {dy / q, -dx / q, -1.0}};
-  f.Jg[0][0] = dx / rho; f.Jg[0][1] = dy / rho; f.Jg[1][0] = -dy / q; f.Jg[1][1] = dx / q;
+  const real ux = dx * irho, uy = dy * irho, vx = dy * iq, vy = dx * iq;
+  const real Jx[2][3] = {{-ux, -uy, 0.0}, {vx, -vy, -1.0}};
+  f.Jg[0][0] = ux; f.Jg[0][1] = uy; f.Jg[1][0] = -vx; f.Jg[1][1] = vy;
 #pragma unroll
   for (int i = 0; i < 2; ++i) {
     f.Ja[i][0] = Jx[i][0]; f.Ja[i][1] = Jx[i][1]; f.Ja[i][2] = -Jx[i][0] * ddy + Jx[i][1] * ddx + Jx[i][2];
@@ -293,6 +305,7 @@ __device__ void ref_order(const Layout& ly, Ctx& e, const Sm& s, int tid) {
 // ------------------------------------------------------------------ assemble H, b at the current state
 __device__ void ref_assemble(const Layout& ly, const Params& pr, const Ctx& e, const Sm& s, int tid) {
   const int W = ly.W, L = ly.L, n = ly.n, c = e.c;
+  REF_TICK_DECL
   real* H = s.H;
   const int ntri = n * (n + 1) / 2;
   for (int t = tid; t < ntri; t += NT) H[t] = 0.0;
@@ -308,6 +321,7 @@ __device__ void ref_assemble(const Layout& ly, const Params& pr, const Ctx& e, c
     s.d[p] = d;
   }
   __syncthreads();
+  REF_TICK(0)
   // prior: H = Lambda on the support; b = -(Lambda d + g) read back from shared memory (no second pass over HBM)
   {
     const int st = e.s * (e.s + 1) / 2;
@@ -332,6 +346,7 @@ __device__ void ref_assemble(const Layout& ly, const Params& pr, const Ctx& e, c
     if (unused) H[tri(s.pos[i], s.pos[i])] = 1.0;
   }
   __syncthreads();
+  REF_TICK(1)
   // odometry k-1 -> k: j side, then i side
   const real om_odo[3] = {pr.om_odo[0], pr.om_odo[1], pr.om_odo[2]}, om_lc[3] = {pr.om_lc[0], pr.om_lc[1], pr.om_lc[2]};
   for (int pass = 0; pass < 2; ++pass) {
@@ -355,6 +370,7 @@ __device__ void ref_assemble(const Layout& ly, const Params& pr, const Ctx& e, c
     }
     __syncthreads();
   }
+  REF_TICK(2)
   // loop closures t -> k: j side (one per k), i side (thread per target, serial over its sources)
   for (int k = 1 + tid; k < c; k += NT) {
     const int t = s.lct[k];
@@ -382,6 +398,7 @@ __device__ void ref_assemble(const Layout& ly, const Params& pr, const Ctx& e, c
   __syncthreads();
   const int oA = n - 3;
   const real sa = sin(s.v[2]), ca = cos(s.v[2]);
+  REF_TICK(3)
   // unary absolute-pose factors: r = (a (+) e_k) - z, full 3x3 information
   if (e.um) {
     for (int k = tid; k < W; k += NT) {
@@ -432,14 +449,19 @@ __device__ void ref_assemble(const Layout& ly, const Params& pr, const Ctx& e, c
   // pass B: thread per landmark (landmark block, anchor x landmark, partial sums of the anchor block)
   if (L > 0 && e.obs) {
     const real om_rb[3] = {pr.om_rb[0], pr.om_rb[1], 0.0};
-    for (int k = 1 + tid; k < c; k += NT) {
-      uint64_t m = vis_of(ly, s, k);
-      if (!m) continue;
-      const int r = ring_of(k, e.head, W), pe = s.pos[vpose(k)];
+    // four adjacent lanes share one pose (pass A) / one landmark (pass B): each takes every fourth factor, the
+    // partial sums are combined by shuffles in a fixed order (deterministic)
+    const int grp = tid >> 2, sub = tid & 3;
+    for (int k0 = 1; k0 < c; k0 += NT / 4) {
+      const int k = k0 + grp;
+      uint64_t m = k < c ? vis_of(ly, s, k) : 0ull;
+      const bool any = m != 0ull;
+      const int r = ring_of(k < c ? k : 0, e.head, W), pe = k < c ? s.pos[vpose(k)] : 0;
       real E[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}}, AE[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}}, be[3] = {0, 0, 0};
-      while (m) {
+      for (int cnt = 0; m; ++cnt) {
         const int l = __ffsll((long long)m) - 1;
         m &= m - 1;
+        if ((cnt & 3) != sub) continue;
         const Rb f = rangebearing(s.v, ca, sa, s.v + vpose(k), false, s.v + vlm(ly, l), (real)e.r32[ly.o_zrb + (r * 2 + 0) * L + l],
                                   (real)e.r32[ly.o_zrb + (r * 2 + 1) * L + l]);
         real GE[2][3];
@@ -454,36 +476,76 @@ __device__ void ref_assemble(const Layout& ly, const Params& pr, const Ctx& e, c
           for (int y = 0; y < 3; ++y) GE[x][y] = f.Jg[0][x] * om_rb[0] * f.Je[0][y] + f.Jg[1][x] * om_rb[1] * f.Je[1][y];
         add_block(H, s.pos[vlm(ly, l)], pe, GE, false);
       }
-      add_block(H, pe, pe, E, true);
-      add_block(H, oA, pe, AE, false);
-      for (int x = 0; x < 3; ++x) s.b[pe + x] -= be[x];
-    }
-    __syncthreads();
-    for (int l = tid; l < L; l += NT) {
-      real* P = s.part + 9 * l;
-      for (int x = 0; x < 9; ++x) P[x] = 0.0;
-      if (!((e.obs >> l) & 1ull)) continue;
-      const int pg = s.pos[vlm(ly, l)];
-      real GG[2][2] = {{0, 0}, {0, 0}}, AG[3][2] = {{0, 0}, {0, 0}, {0, 0}}, bg[2] = {0, 0};
-      for (int k = 0; k < c; ++k) {
-        if (!((s.rbm[k * ly.nw + (l >> 5)] >> (l & 31)) & 1u)) continue;
-        const int r = ring_of(k, e.head, W);
-        const Rb f = rangebearing(s.v, ca, sa, s.v + vpose(k), k == 0, s.v + vlm(ly, l), (real)e.r32[ly.o_zrb + (r * 2 + 0) * L + l],
-                                  (real)e.r32[ly.o_zrb + (r * 2 + 1) * L + l]);
-        for (int x = 0; x < 2; ++x) {
-          for (int y = 0; y < 2; ++y) GG[x][y] += f.Jg[0][x] * om_rb[0] * f.Jg[0][y] + f.Jg[1][x] * om_rb[1] * f.Jg[1][y];
-          bg[x] += f.Jg[0][x] * om_rb[0] * f.r[0] + f.Jg[1][x] * om_rb[1] * f.r[1];
-        }
-        int t = 0;
+#pragma unroll
+      for (int o = 1; o < 4; o <<= 1) {
+#pragma unroll
         for (int x = 0; x < 3; ++x) {
-          for (int y = 0; y < 2; ++y) AG[x][y] += f.Ja[0][x] * om_rb[0] * f.Jg[0][y] + f.Ja[1][x] * om_rb[1] * f.Jg[1][y];
-          for (int y = 0; y <= x; ++y) P[t++] += f.Ja[0][x] * om_rb[0] * f.Ja[0][y] + f.Ja[1][x] * om_rb[1] * f.Ja[1][y];
-          P[6 + x] += f.Ja[0][x] * om_rb[0] * f.r[0] + f.Ja[1][x] * om_rb[1] * f.r[1];
+#pragma unroll
+          for (int y = 0; y < 3; ++y) {
+            E[x][y] += __shfl_xor_sync(0xffffffffu, E[x][y], o);
+            AE[x][y] += __shfl_xor_sync(0xffffffffu, AE[x][y], o);
+          }
+          be[x] += __shfl_xor_sync(0xffffffffu, be[x], o);
         }
       }
-      add_block(H, pg, pg, GG, true);
-      add_block(H, oA, pg, AG, false);
-      s.b[pg] -= bg[0]; s.b[pg + 1] -= bg[1];
+      if (any && sub == 0) {
+        add_block(H, pe, pe, E, true);
+        add_block(H, oA, pe, AE, false);
+        for (int x = 0; x < 3; ++x) s.b[pe + x] -= be[x];
+      }
+    }
+    __syncthreads();
+    REF_TICK(4)
+    for (int l0 = 0; l0 < L; l0 += NT / 4) {
+      const int l = l0 + grp;
+      const bool on = l < L && ((e.obs >> l) & 1ull);
+      real P9[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+      real GG[2][2] = {{0, 0}, {0, 0}}, AG[3][2] = {{0, 0}, {0, 0}, {0, 0}}, bg[2] = {0, 0};
+      if (on) {
+        int cnt = 0;
+        for (int k = 0; k < c; ++k) {
+          if (!((s.rbm[k * ly.nw + (l >> 5)] >> (l & 31)) & 1u)) continue;
+          if (((cnt++) & 3) != sub) continue;
+          const int r = ring_of(k, e.head, W);
+          const Rb f = rangebearing(s.v, ca, sa, s.v + vpose(k), k == 0, s.v + vlm(ly, l), (real)e.r32[ly.o_zrb + (r * 2 + 0) * L + l],
+                                    (real)e.r32[ly.o_zrb + (r * 2 + 1) * L + l]);
+          for (int x = 0; x < 2; ++x) {
+            for (int y = 0; y < 2; ++y) GG[x][y] += f.Jg[0][x] * om_rb[0] * f.Jg[0][y] + f.Jg[1][x] * om_rb[1] * f.Jg[1][y];
+            bg[x] += f.Jg[0][x] * om_rb[0] * f.r[0] + f.Jg[1][x] * om_rb[1] * f.r[1];
+          }
+          int t = 0;
+          for (int x = 0; x < 3; ++x) {
+            for (int y = 0; y < 2; ++y) AG[x][y] += f.Ja[0][x] * om_rb[0] * f.Jg[0][y] + f.Ja[1][x] * om_rb[1] * f.Jg[1][y];
+            for (int y = 0; y <= x; ++y) P9[t++] += f.Ja[0][x] * om_rb[0] * f.Ja[0][y] + f.Ja[1][x] * om_rb[1] * f.Ja[1][y];
+            P9[6 + x] += f.Ja[0][x] * om_rb[0] * f.r[0] + f.Ja[1][x] * om_rb[1] * f.r[1];
+          }
+        }
+      }
+#pragma unroll
+      for (int o = 1; o < 4; o <<= 1) {
+#pragma unroll
+        for (int x = 0; x < 9; ++x) P9[x] += __shfl_xor_sync(0xffffffffu, P9[x], o);
+#pragma unroll
+        for (int x = 0; x < 2; ++x) {
+#pragma unroll
+          for (int y = 0; y < 2; ++y) GG[x][y] += __shfl_xor_sync(0xffffffffu, GG[x][y], o);
+          bg[x] += __shfl_xor_sync(0xffffffffu, bg[x], o);
+        }
+#pragma unroll
+        for (int x = 0; x < 3; ++x)
+#pragma unroll
+          for (int y = 0; y < 2; ++y) AG[x][y] += __shfl_xor_sync(0xffffffffu, AG[x][y], o);
+      }
+      if (l < L && sub == 0) {
+        real* P = s.part + 9 * l;
+        for (int x = 0; x < 9; ++x) P[x] = P9[x];
+        if (on) {
+          const int pg = s.pos[vlm(ly, l)];
+          add_block(H, pg, pg, GG, true);
+          add_block(H, oA, pg, AG, false);
+          s.b[pg] -= bg[0]; s.b[pg + 1] -= bg[1];
+        }
+      }
     }
     __syncthreads();
     if (tid < 9) {
@@ -494,6 +556,7 @@ __device__ void ref_assemble(const Layout& ly, const Params& pr, const Ctx& e, c
     }
     __syncthreads();
   }
+  REF_TICK(5)
 }
 
 // ------------------------------------------------------------------ Cholesky (right-looking, blocks of 4 columns)
@@ -547,8 +610,8 @@ __device__ int ref_cholesky(const Layout& ly, const Sm& s, int tid, real* ratio)
 #pragma unroll
         for (int k = 0; k < c; ++k) piv -= t[c][k] * t[c][k];
         if (!(piv > 0.0)) { flag |= slamk::ENV_NOT_PD; piv = 1.0; }
-        const real dj = sqrt(piv), inv = 1.0 / dj;
-        t[c][c] = dj; ti[c] = inv;
+        const real inv = rsqrt(piv);
+        t[c][c] = piv * inv; ti[c] = inv;
 #pragma unroll
         for (int x = c + 1; x < 4; ++x) {
           real v = t[x][c];
@@ -1048,7 +1111,7 @@ __global__ void __launch_bounds__(NT, 3) slam_ref64_kernel(Layout ly, Params pr,
     __syncthreads();
     for (int it = 0; it < nlin; ++it) {
       ref_assemble(ly, pr, e, s, tid);
-      status |= ref_cholesky(ly, s, tid, &sh_ratio);
+      { REF_TICK_DECL status |= ref_cholesky(ly, s, tid, &sh_ratio); REF_TICK(6) }
       if (it < ra.iters) {
         ref_backsub(ly, s, tid);
         status |= ref_update(ly, e, s, tid);
