@@ -26,7 +26,8 @@ def to_dev(data, device="cuda:0"):
 def run_gpu(slam, data, iters, fused=True, steps=None, want_poses=True):
     """reset -> (observe_first) -> T x [push, solve, cov, dopt, (marginalize iff full)] through the C ABI.
 
-    Returns numpy arrays poses[T,N,W,3] (global), cov[T,N,3,3], logdet[T,N], status[N]."""
+    Returns numpy arrays poses[T,N,W,3] (global), cov[T,N,3,3], logdet[T,N], status[N]; the fused path
+    (one slam_step per step) returns last_pose[T,N,3] (newest pose, global) instead of the whole window."""
     cfg = data["cfg"]
     T = data["T"] if steps is None else steps
     N, W, L = slam.N, slam.W, slam.L
@@ -37,6 +38,7 @@ def run_gpu(slam, data, iters, fused=True, steps=None, want_poses=True):
     cov = torch.zeros(T, 9, N, device=slam.device)
     logdet = torch.zeros(T, N, device=slam.device)
     poses = torch.zeros(T, 3, W, N, device=slam.device) if want_poses else None
+    last = torch.zeros(T, 3, N, device=slam.device) if (fused and not want_poses) else None
     for t in range(1, T + 1):
         args = (dev["odom"][t - 1], dev["lc_back"][t - 1], dev["lc_meas"][t - 1],
                 dev["rb_mask"][t] if L else None, dev["rb_meas"][t] if L else None)
@@ -45,7 +47,7 @@ def run_gpu(slam, data, iters, fused=True, steps=None, want_poses=True):
         if "un_valid" in dev:
             slam.set_unary(dev["un_pose"][t - 1], dev["un_info"][t - 1], dev["un_valid"][t - 1])
         if fused and not want_poses:
-            slam.step(*args, iters=iters, cov=cov[t - 1], logdet=logdet[t - 1])
+            slam.step(*args, iters=iters, cov=cov[t - 1], logdet=logdet[t - 1], last_pose=last[t - 1])
         else:
             slam.push_step(*args)
             slam.solve(iters)
@@ -60,6 +62,8 @@ def run_gpu(slam, data, iters, fused=True, steps=None, want_poses=True):
                logdet=logdet.cpu().numpy().astype(np.float64), status=slam.get_status().cpu().numpy())
     if want_poses:
         out["poses"] = poses.cpu().numpy().transpose(0, 3, 2, 1).astype(np.float64)
+    if last is not None:
+        out["last_pose"] = last.cpu().numpy().transpose(0, 2, 1).astype(np.float64)
     return out
 
 
@@ -72,6 +76,15 @@ def parity_errors(gpu, ref, counts=None):
     poses: max_k |dx_k|_inf / (1e-4 max(1, max_k |x_k|_inf)), angles wrapped;
     cov:   max_ij |dS_ij| / (1e-3 sqrt(S_ii S_jj)) with the oracle's S;  logdet: |d| / 1e-3."""
     out = {}
+    if gpu.get("last_pose") is not None and ref.get("poses") is not None:
+        # newest pose of the window after the solve of step t: slot min(t + 1, W) - 1 (or `counts` - 1 per env)
+        T, ne, W, _ = ref["poses"].shape
+        c = np.minimum(np.arange(T) + 2, W)[:, None] * np.ones((1, ne), int) if counts is None else counts
+        newest = np.take_along_axis(ref["poses"], (c - 1)[:, :, None, None].repeat(3, axis=3), axis=2)[:, :, 0]
+        d = gpu["last_pose"] - newest
+        d[..., 2] = wrap(d[..., 2])
+        scale = np.maximum(1.0, np.abs(ref["poses"]).max(axis=(2, 3)))
+        out["last_pose"] = np.abs(d).max(axis=2) / (1e-4 * scale)
     if "poses" in gpu and gpu["poses"] is not None and ref.get("poses") is not None:
         d = gpu["poses"] - ref["poses"]
         d[..., 2] = wrap(d[..., 2])

@@ -10,59 +10,83 @@ import torch
 import oracle
 from paper_2603_25834_b200 import synth
 from tests.gpu_driver import parity_errors, run_gpu, to_dev
+from tests.helpers import determined, drive
 
 pytestmark = pytest.mark.gpu
 
 
-def _slam(N, W, L):
+def _slam(N, W, L, precision=None):
     from paper_2603_25834_b200.binding import FixedLagSlam
-    return FixedLagSlam(N, W, L)
+    slam = FixedLagSlam(N, W, L)
+    if precision is not None:
+        slam.set_precision(precision)
+    return slam
 
 
-PROBE_FORK = 1.0 / 12.0        # an environment "forks" when fp32 STORAGE alone costs 1/12 of a tolerance
-FORKED_FACTOR = 100.0          # after the fork (loose sanity bound): error <= 100 x max(1, probe's running maximum)
-MAX_EXCEED_FRACTION = 0.01     # at most 1 % of all env-steps may exceed the stated tolerance at all
-MIN_STRICT_COVERAGE = 0.80
+def _fused_equals_separate(cfg, data, ref=None):
+    """slam_step against the composition of the separate calls.  Bit for bit while an environment stays in one
+    precision mode (0: the fp32 kernel, 2: the fp64 kernel); with the conditioning watch on (mode 1) the fused call
+    sees all its factorisations at once and the separate calls one at a time, so an environment near the threshold
+    may change hands at a different call: both then hold the stated tolerances, not the same bits."""
+    for mode in (0, 2):
+        a = run_gpu(_slam(cfg.N, cfg.W, cfg.L, mode), data, cfg.iters, fused=False, want_poses=False)
+        b = run_gpu(_slam(cfg.N, cfg.W, cfg.L, mode), data, cfg.iters, fused=True, want_poses=False)
+        assert np.array_equal(a["cov"], b["cov"]) and np.array_equal(a["logdet"], b["logdet"]), mode
+        c = run_gpu(_slam(cfg.N, cfg.W, cfg.L, mode), data, cfg.iters, fused=True, want_poses=False)   # and launch to launch
+        assert np.array_equal(b["cov"], c["cov"]) and np.array_equal(b["last_pose"], c["last_pose"]), mode
+    if ref is not None:
+        b = run_gpu(_slam(cfg.N, cfg.W, cfg.L), data, cfg.iters, fused=True, want_poses=False)
+        _check(b, ref, what=("cov", "logdet"))
 
 
-def _check(gpu, ref, what=("poses", "cov", "logdet"), probe=None, min_coverage=MIN_STRICT_COVERAGE):
-    """Every (step, env) must be within the stated tolerances R23 (error <= 1.0 in tolerance units).
+def _check(gpu, ref, what=("poses", "last_pose", "cov", "logdet"), det=None):
+    """Every (step, env) must be within the stated tolerances R23 (error <= 1.0 in tolerance units).  `det` (config 3
+    only): the env-steps the ORACLE itself determines (tests/helpers.determined: its outputs do not move when one
+    input changes by one float32 ulp); at least 99.9 % must be, the others are not compared.
 
-    Conditioning: in config 3, late in the run, the information matrix of some
-    environments is so ill-conditioned that the ORACLE's own outputs move by a tolerance or more when H,
-    b, the prior and the state are merely rounded to fp32 (`probe` = that run of the same fp64 algorithm).
-    No fp32 implementation can follow the oracle there, and the two trajectories stay apart afterwards
-    (the prior is linearised at different points).  So: an environment is held to the STATED tolerance
-    on every step before the first one where the probe's error reaches 1/12 of a tolerance (its "fork");
-    after the fork the two runs are different trajectories (chaotic sensitivity), so only a loose sanity
-    bound applies (100 x max(1, the probe's running maximum)); and over everything at most 1 % of env-steps
-    may exceed the stated tolerance.  Pose-only configs never fork."""
+    Windows whose information matrix fp32 cannot carry (config 3 after the robot left the landmark box and
+    re-observes a landmark) are recognised by the library's own conditioning watch and solved by its fp64 kernel
+    (slam_set_precision): the test does not know about them."""
     err = parity_errors(gpu, ref)
     keys = [k for k in what if k in err]
     assert keys
     G = np.max([err[k] for k in keys], axis=0)
     assert np.isfinite(G).all()
-    if probe is None:
-        worst = float(G.max())
-        assert worst <= 1.0, f"{worst:.3g} x tolerance at {np.unravel_index(G.argmax(), G.shape)}"
-        return err
-    perr = parity_errors(probe, ref)
-    P = np.max([perr[k] for k in keys], axis=0)
-    T = G.shape[0]
-    forked = np.maximum.accumulate(P > PROBE_FORK, axis=0)
-    strict = ~forked
-    assert strict.mean() >= min_coverage, f"strict coverage {strict.mean():.3f}"
-    if strict.any():
-        worst = float(G[strict].max())
-        assert worst <= 1.0, f"{worst:.3g} x tolerance on a well-conditioned env-step"
-    bound = FORKED_FACTOR * np.maximum(1.0, np.maximum.accumulate(P, axis=0))
-    assert (G <= bound).all(), f"forked env-step beyond {FORKED_FACTOR} x probe: {float((G / bound).max()):.3g}"
-    assert (G > 1.0).mean() <= MAX_EXCEED_FRACTION, f"{(G > 1.0).mean():.3%} of env-steps exceed the stated tolerance"
+    if det is not None:
+        assert det.mean() >= 0.999, f"only {det.mean():.5f} of the env-steps are determined by the oracle"
+        G = np.where(det, G, 0.0)
+    worst = float(G.max())
+    assert worst <= 1.0, f"{worst:.3g} x tolerance at (step, env) {np.unravel_index(G.argmax(), G.shape)}: " + \
+        ", ".join(f"{k} {float(err[k].max()):.3g}" for k in keys)
     return err
 
 
 def _sub(gpu, envs):
     return {k: (v[:, envs] if k != "status" else v[envs]) for k, v in gpu.items()}
+
+
+def _window_after_step(slam, ref, t, envs=None, det=None):
+    """slam_get_poses after the fused step t (1-based) against the oracle's window of that step: marginalisation
+    only re-expresses the window in the next anchor's frame, so the global poses of the slots that stay are
+    unchanged (oracle slots 1.. of step t = library slots 0.. after the step, once the window is full)."""
+    W = slam.W
+    P = slam.get_poses().cpu().numpy().transpose(2, 1, 0).astype(np.float64)     # [N, W, 3]
+    if envs is not None:
+        P = P[envs]
+    R = ref["poses"][t - 1]                                                        # [ne, W, 3] after the solve of step t
+    c = min(t + 1, W)
+    if c == W:
+        got, exp = P[:, : W - 1], R[:, 1:W]
+    else:
+        got, exp = P[:, :c], R[:, :c]
+    d = got - exp
+    d[..., 2] = np.arctan2(np.sin(d[..., 2]), np.cos(d[..., 2]))
+    scale = np.maximum(1.0, np.abs(R).max(axis=(1, 2)))
+    e = np.abs(d).max(axis=(1, 2)) / (1e-4 * scale)
+    if det is not None:
+        e = np.where(det[t - 1], e, 0.0)
+    worst = float(e.max())
+    assert worst <= 1.0, f"window poses after step {t}: {worst:.3g} x tolerance (env index {int(e.argmax())})"
 
 
 def test_config0_all_envs_all_steps():
@@ -73,7 +97,7 @@ def test_config0_all_envs_all_steps():
     assert (gpu["status"] == 0).all()
     _check(gpu, ref)
     fused = run_gpu(_slam(cfg.N, cfg.W, cfg.L), data, cfg.iters, fused=True, want_poses=False)
-    _check(fused, ref, what=("cov", "logdet"))
+    _check(fused, ref, what=("last_pose", "cov", "logdet"))
 
 
 @pytest.mark.parametrize("W,L,p_lc,N,T,iters", [
@@ -100,13 +124,7 @@ def test_small_cases_every_env(W, L, p_lc, N, T, iters):
 def test_fused_step_is_bitwise_the_composition(W, L, p_lc):
     cfg = synth.Config("f", N=70, W=W, L=L, iters=2, T=40, p_lc=p_lc, seed=8)
     data = synth.generate(cfg)
-    a = run_gpu(_slam(cfg.N, W, L), data, cfg.iters, fused=False, want_poses=False)
-    b = run_gpu(_slam(cfg.N, W, L), data, cfg.iters, fused=True, want_poses=False)
-    assert np.array_equal(a["cov"], b["cov"])
-    assert np.array_equal(a["logdet"], b["logdet"])
-    # and the run is reproducible launch to launch
-    c = run_gpu(_slam(cfg.N, W, L), data, cfg.iters, fused=True, want_poses=False)
-    assert np.array_equal(b["cov"], c["cov"])
+    _fused_equals_separate(cfg, data, oracle.run_batch(data, cfg.iters))
 
 
 def test_noise_free_recovers_ground_truth():
@@ -121,47 +139,127 @@ def test_noise_free_recovers_ground_truth():
         assert np.abs(err).max() < 2e-4 * max(1.0, np.abs(gt).max())
 
 
-def _full_config(cfg, n_sample, steps=None):
+def _full_config(cfg, n_sample, steps=None, check_determined=False):
+    """The FULL batch in the launch configuration bench.py times (fused slam_step, default precision), compared on
+    `n_sample` environments spread over the batch: newest pose (`last_pose`), covariance and ln det at every
+    step, the whole window (slam_get_poses) after the last step; and, on EVERY environment, properties that hold at
+    any size."""
     data = synth.generate(cfg, steps=steps)
+    T = data["T"]
     envs = np.unique(np.linspace(0, cfg.N - 1, n_sample).astype(np.int32))
     ref = oracle.run_batch(data, cfg.iters, envs=envs)
-    probe = oracle.run_batch(data, cfg.iters, envs=envs, f32_storage=True)
     assert ref["bad"] == 0
+    det = determined(oracle, data, cfg.iters, envs, ref) if check_determined else None
     slam = _slam(cfg.N, cfg.W, cfg.L)
-    gpu = run_gpu(slam, data, cfg.iters, fused=True, want_poses=False)   # the launch configuration bench.py times
+    gpu = run_gpu(slam, data, cfg.iters, fused=True, want_poses=False)
     assert (gpu["status"] == 0).all()
-    assert np.isfinite(gpu["cov"]).all() and np.isfinite(gpu["logdet"]).all()
-    _check(_sub(gpu, envs), ref, what=("cov", "logdet"), probe=probe)
-    # properties that hold at any size: symmetric positive-definite covariances on EVERY env and step
+    assert np.isfinite(gpu["cov"]).all() and np.isfinite(gpu["logdet"]).all() and np.isfinite(gpu["last_pose"]).all()
+    _check(_sub(gpu, envs), ref, what=("last_pose", "cov", "logdet"), det=det)
+    _window_after_step(slam, ref, T, envs, det)
     S = gpu["cov"]
     assert np.array_equal(S, S.transpose(0, 1, 3, 2))
     assert (np.linalg.eigvalsh(S.reshape(-1, 3, 3)).min(axis=1) > 0).all()
-    return data, envs, ref, probe
+    return slam, data, envs, ref, gpu
 
 
-def test_config1_full_size_sampled_envs():
-    cfg = synth.CONFIGS[1]
-    data, envs, ref, probe = _full_config(cfg, 24)
-    # poses through the separate calls on the same sampled environments
-    sub = synth.generate(cfg, env_ids=envs)
-    gpu = run_gpu(_slam(len(envs), cfg.W, cfg.L), sub, cfg.iters, fused=False)
-    _check(gpu, ref, probe=probe, min_coverage=1.0)      # pose-only: no environment forks
+def test_config1_full_size_every_env():
+    _full_config(synth.CONFIGS[1], synth.CONFIGS[1].N)      # all 750 environments x 500 steps
 
 
 def test_config2_full_size_sampled_envs():
-    _full_config(synth.CONFIGS[2], 10)
+    _full_config(synth.CONFIGS[2], 256)
 
 
 def test_config3_full_size_sampled_envs():
+    """The headline configuration: 256 environments x all 300 steps at the stated tolerances on every env-step the
+    oracle determines (all but ~1e-4 of them, tests/helpers.determined); the windows fp32 cannot carry go through
+    the fp64 kernel, and that really happened."""
     cfg = synth.CONFIGS[3]
-    data, envs, ref, probe = _full_config(cfg, 48)
-    sub = synth.generate(cfg, env_ids=envs)
-    gpu = run_gpu(_slam(len(envs), cfg.W, cfg.L), sub, cfg.iters, fused=False)
-    _check(gpu, ref, probe=probe)
+    slam, data, envs, ref, gpu = _full_config(cfg, 256, check_determined=True)
+    st = slam.get_stats()
+    assert 0 < st["fp64_calls"] < 0.10 * cfg.N * cfg.T, st     # a few percent of the env-steps (measured: 4.4 %)
+    # landmarks: the read-out against the oracle's (single environments driven step by step)
+    lm, act = slam.get_landmarks()
+    lm, act = lm.cpu().numpy(), act.cpu().numpy().view(np.uint32)
+    for q in (0, 100, 255):
+        env = int(envs[q])
+        one = synth.generate(cfg, env_ids=np.array([env], np.int32))
+        o = oracle.Oracle(cfg.W, cfg.L)
+        drive(o, one, 0, cfg.iters)
+        olm, oact = o.landmarks()
+        gact = np.array([(int(act[l // 32, env]) >> (l % 32)) & 1 for l in range(cfg.L)])
+        assert np.array_equal(gact, oact)
+        d = np.abs(lm[:, :, env].T - olm)
+        assert d.max() <= 1e-4 * max(1.0, np.abs(olm).max()), (env, d.max())
 
 
-def test_config4_n16384_sampled_envs():
-    _full_config(synth.config4(16384), 6)
+@pytest.mark.parametrize("N,n_sample,steps", [(256, 64, 70), (16384, 128, None), (65536, 64, 70)])
+def test_config4_sweep_sampled_envs(N, n_sample, steps):
+    _full_config(synth.config4(N), n_sample, steps=steps)
+
+
+def test_device_reference_agrees_at_full_batch_config3():
+    """at full batch the oracle covers a sample; EVERY environment is
+    diffed against the device reference (precision mode 2: the fp64 kernel, an independent second implementation
+    of the same mathematics: dense packed storage, right-looking factorisation, CTA per environment).  While the
+    robot is among the landmarks (steps 1..60 here) both must agree within the stated tolerances on all 16384."""
+    cfg = synth.CONFIGS[3]
+    data = synth.generate(cfg, steps=60)
+    a = run_gpu(_slam(cfg.N, cfg.W, cfg.L), data, cfg.iters, fused=True, want_poses=False)
+    slam = _slam(cfg.N, cfg.W, cfg.L)
+    slam.set_precision(2)
+    b = run_gpu(slam, data, cfg.iters, fused=True, want_poses=False)
+    assert slam.get_stats()["fp64_calls"] == cfg.N * 61       # observe_first + 60 steps, every environment
+    dg = np.sqrt(np.einsum("tnii->tni", b["cov"]))
+    ec = (np.abs(a["cov"] - b["cov"]) / (1e-3 * dg[..., :, None] * dg[..., None, :])).max()
+    el = (np.abs(a["logdet"] - b["logdet"]) / 1e-3).max()
+    d = a["last_pose"] - b["last_pose"]
+    d[..., 2] = np.arctan2(np.sin(d[..., 2]), np.cos(d[..., 2]))
+    ep = (np.abs(d).max(axis=2) / (1e-4 * np.maximum(1.0, np.abs(b["last_pose"]).max(axis=2)))).max()
+    assert max(ec, el, ep) <= 1.0, (ec, el, ep)
+
+
+def test_outputs_permute_with_the_environments():
+    """Environments are independent: permuting the columns of every input permutes the
+    outputs bit for bit, whichever CTA, team, round or cost-order position an environment lands on."""
+    cfg = synth.Config("perm", N=1500, W=12, L=6, iters=2, T=40, p_lc=0.2, seed=21)
+    data = synth.generate(cfg)
+    rng = np.random.default_rng(5)
+    perm = rng.permutation(cfg.N)
+    pd = dict(data)
+    for k in ("odom", "lc_back", "lc_meas", "rb_mask", "rb_meas"):
+        pd[k] = np.ascontiguousarray(data[k][..., perm])
+    a = run_gpu(_slam(cfg.N, cfg.W, cfg.L), data, cfg.iters, fused=True, want_poses=False)
+    b = run_gpu(_slam(cfg.N, cfg.W, cfg.L), pd, cfg.iters, fused=True, want_poses=False)
+    for k in ("cov", "logdet", "last_pose"):
+        assert np.array_equal(a[k][:, perm], b[k]), k
+
+
+def test_step_time_does_not_depend_on_the_step_index():
+    """PAPER.md:144 "constant-time updates independent of trajectory length": once the window is full the
+    per-step device time of a pose-only configuration (whose structure is stationary) stays flat: the mean over
+    steps 150..249 and over steps 400..499 of config 2 agree within 5 %."""
+    cfg = synth.CONFIGS[2]
+    data = synth.generate(cfg)
+    dev = to_dev(data)
+    slam = _slam(cfg.N, cfg.W, cfg.L)
+    cov = torch.zeros(9, cfg.N, device="cuda")
+    ld = torch.zeros(cfg.N, device="cuda")
+    best = None
+    for rep in range(3):
+        slam.reset()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(cfg.T + 1)]
+        torch.cuda.synchronize()
+        ev[0].record()
+        for t in range(1, cfg.T + 1):
+            slam.step(dev["odom"][t - 1], dev["lc_back"][t - 1], dev["lc_meas"][t - 1], iters=cfg.iters, cov=cov, logdet=ld)
+            ev[t].record()
+        torch.cuda.synchronize()
+        ms = np.array([ev[t].elapsed_time(ev[t + 1]) for t in range(cfg.T)])
+        best = ms if best is None else np.minimum(best, ms)
+    early, late = best[150:250].mean(), best[400:500].mean()
+    assert abs(late / early - 1.0) <= 0.05, (early, late)
+    assert best[:cfg.W - 2].mean() < early        # the window-fill phase is cheaper, never dearer
 
 
 def test_state_errors_and_ignored_inputs():
@@ -292,8 +390,7 @@ def test_unary_pose_factor_next1(W, L, p_lc):
     gpu = run_gpu(_slam(cfg.N, W, L), data, cfg.iters, fused=False)
     assert (gpu["status"] == 0).all()
     _check(gpu, ref)
-    fused = run_gpu(_slam(cfg.N, W, L), data, cfg.iters, fused=True, want_poses=False)
-    assert np.array_equal(fused["cov"], gpu["cov"]) and np.array_equal(fused["logdet"], gpu["logdet"])
+    _fused_equals_separate(cfg, data, ref)
     # the absolute measurements really bound the uncertainty: without them log-det keeps growing
     plain = synth.generate(synth.Config("pl", N=40, W=W, L=L, iters=2, T=50, p_lc=p_lc, seed=17))
     ref_plain = oracle.run_batch(plain, cfg.iters, want=("logdet",))
@@ -311,5 +408,4 @@ def test_per_env_reset_next2(W, L, p_lc):
     gpu = run_gpu(_slam(cfg.N, W, L), data, cfg.iters, fused=False)
     assert (gpu["status"] == 0).all()
     _check(gpu, ref)
-    fused = run_gpu(_slam(cfg.N, W, L), data, cfg.iters, fused=True, want_poses=False)
-    assert np.array_equal(fused["cov"], gpu["cov"]) and np.array_equal(fused["logdet"], gpu["logdet"])
+    _fused_equals_separate(cfg, data, ref)
