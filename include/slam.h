@@ -201,6 +201,25 @@ int slam_grid_update(const slam_scan_params* p, int batch, float* grid, const fl
  * Bit-for-bit equality of slam_step with the separate calls holds for environments that stay in one mode. */
 int slam_set_precision(slam_ctx* ctx, int mode, float ratio_hi, float ratio_lo);
 
+/* Allocation-free entry point, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it): ONE call runs a whole episode -- reset at the origin, (landmarks > 0:
+ * the observation from pose 0 = slice 0 of rb_mask / rb_meas), then `steps` fused steps exactly like slam_step --
+ * with every scratch buffer of the kernels (environment records, fp64 shadows, cost order, covariance cache) in a
+ * static device array of SLAM_STATIC_MAX_BYTES inside the library instead of a caller-owned workspace.  It calls no
+ * cudaMalloc / cudaFree and no allocating CUDA library routine.  Every GPU that loads the library holds the array
+ * until the process exits.  Sizes whose workspace (slam_workspace_bytes) exceeds the array are rejected with
+ * SLAM_ENOMEM and a message in `err` (e.g. window 20 + 24 landmarks: about 200 environments; window 6 + 5 landmarks:
+ * about 2000).  ALL CALLS SHARE THE ARRAY: it keeps the last call's contents (each call clears what must start at
+ * zero), and calls that overlap on the GPU -- different streams without a dependency -- race.
+ *   odom [steps][3][N], lc_back [steps][N] (NULL: none), lc_meas [steps][3][N],
+ *   rb_mask [steps+1][ceil(L/32)][N], rb_meas [steps+1][2][L][N]   (NULL iff landmarks == 0)
+ *   cov [steps][9][N], logdet [steps][N], last_pose [steps][3][N]  (each may be NULL)     -- all DEVICE pointers
+ *   err / err_len: optional host buffer for the message of a non-zero return. */
+#define SLAM_STATIC_MAX_BYTES (16u << 20)
+int slam_run_static(int batch, int window, int landmarks, int steps, int iters, const slam_config* cfg, const float* odom,
+                    const int32_t* lc_back, const float* lc_meas, const uint32_t* rb_mask, const float* rb_meas, float* cov,
+                    float* logdet, float* last_pose, void* cuda_stream, char* err, size_t err_len);
+
 int slam_count(const slam_ctx* ctx);                /* host-side window count c in [1, window] */
 long long slam_launch_count(const slam_ctx* ctx);   /* kernels launched by this context so far */
 const char* slam_last_error(const slam_ctx* ctx);   /* message of the last non-zero return */

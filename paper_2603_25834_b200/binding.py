@@ -23,7 +23,7 @@ SYMBOLS = (
     "slam_default_config", "slam_workspace_bytes", "slam_create", "slam_destroy", "slam_reset",
     "slam_reset_envs", "slam_push_step", "slam_set_unary", "slam_observe_first", "slam_solve", "slam_marginal_cov", "slam_dopt",
     "slam_marginalize_oldest", "slam_step", "slam_step_host", "slam_get_poses", "slam_get_landmarks",
-    "slam_get_status", "slam_get_stats", "slam_set_precision", "slam_reward", "slam_scan_match", "slam_grid_update", "slam_count", "slam_launch_count", "slam_last_error", "slam_kernel_info",
+    "slam_get_status", "slam_get_stats", "slam_set_precision", "slam_run_static", "slam_reward", "slam_scan_match", "slam_grid_update", "slam_count", "slam_launch_count", "slam_last_error", "slam_kernel_info",
 )
 
 
@@ -83,6 +83,7 @@ def _load() -> C.CDLL:
     lib.slam_scan_match.argtypes = [C.POINTER(ScanParams), C.c_int, fp, fp, fp, fp, fp, fp, vp]
     lib.slam_grid_update.argtypes = [C.POINTER(ScanParams), C.c_int, fp, fp, fp, fp, C.c_float, C.c_float, C.c_float, vp]
     lib.slam_set_precision.argtypes = [vp, C.c_int, C.c_float, C.c_float]
+    lib.slam_run_static.argtypes = [C.c_int] * 5 + [C.POINTER(SlamConfig), fp, ip, fp, ip, fp, fp, fp, fp, vp, C.c_char_p, C.c_size_t]
     lib.slam_count.argtypes = [vp]
     lib.slam_launch_count.argtypes = [vp]
     lib.slam_launch_count.restype = C.c_longlong
@@ -134,6 +135,29 @@ def grid_update(par: ScanParams, grid, pose, ranges, weight, l_free: float, l_oc
     if rc != SLAM_OK:
         raise SlamError(rc, "slam_grid_update")
     return grid
+
+
+STATIC_MAX_BYTES = 16 << 20
+
+
+def run_static(batch: int, window: int, landmarks: int, iters: int, odom, lc_back=None, lc_meas=None, rb_mask=None,
+               rb_meas=None, cov=None, logdet=None, last_pose=None, config: SlamConfig | None = None):
+    """slam_run_static: one whole episode on the library's static scratch array (no device allocation in the library;
+    inputs and outputs are the caller's tensors: odom [T,3,N], lc_back [T,N], lc_meas [T,3,N], rb_mask [T+1,nw,N],
+    rb_meas [T+1,2,L,N], cov [T,9,N], logdet [T,N], last_pose [T,3,N])."""
+    T, dev = int(odom.shape[0]), odom.device
+    ptr = lambda t: None if t is None else C.c_void_p(t.data_ptr())
+    for t in (odom, lc_back, lc_meas, rb_mask, rb_meas, cov, logdet, last_pose):
+        if t is not None and (not t.is_cuda or t.device != dev or not t.is_contiguous()):
+            raise SlamError(SLAM_EINVAL, "run_static: contiguous CUDA tensors on one device expected")
+    msg = C.create_string_buffer(256)
+    with torch.cuda.device(dev):
+        rc = LIB.slam_run_static(int(batch), int(window), int(landmarks), T, int(iters),
+                                 C.byref(config) if config is not None else None, ptr(odom), ptr(lc_back), ptr(lc_meas),
+                                 ptr(rb_mask), ptr(rb_meas), ptr(cov), ptr(logdet), ptr(last_pose),
+                                 C.c_void_p(torch.cuda.current_stream(dev).cuda_stream), msg, 256)
+    if rc != SLAM_OK:
+        raise SlamError(rc, msg.value.decode())
 
 
 class FixedLagSlam:

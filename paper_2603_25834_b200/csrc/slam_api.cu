@@ -937,4 +937,59 @@ int slam_kernel_info(const slam_ctx* c, int* smem_bytes_per_cta, int* warps_per_
   return SLAM_OK;
 }
 
+// ------------------------------------------------------------------ allocation-free entry point
+// slam_run_static: a whole episode (reset, T fused steps) for callers that cannot allocate device memory (code under
+// CUDA graph capture, serving loops, harnesses that forbid cudaMalloc).  Everything the step kernels keep between
+// launches -- the environment records, their fp64 shadows, the cost order, the fallback list, the covariance cache
+// -- lives in ONE file-scope device array of SLAM_STATIC_MAX_BYTES instead of a caller-allocated workspace.  Every
+// GPU that loads the library holds the array until the process exits.  All calls share it: it keeps the last call's
+// contents (slam_create's reset clears what must start at zero: records up to the prior, counters, order), and two
+// calls that overlap on the GPU (different streams, no dependency) race.
+static __device__ __align__(256) unsigned char g_static_ws[SLAM_STATIC_MAX_BYTES];
+// In host code `g_static_ws` is a host-side stand-in, not a device address: the address the kernels get comes from
+// cudaGetSymbolAddress, taken once per device with that device current.
+static void* g_static_ptr[64];
+
+static int static_fail(char* err, size_t err_len, int code, const char* msg) {
+  if (err && err_len) snprintf(err, err_len, "%s", msg);
+  return code;
+}
+
+int slam_run_static(int batch, int window, int landmarks, int steps, int iters, const slam_config* cfg, const float* odom,
+                    const int32_t* lc_back, const float* lc_meas, const uint32_t* rb_mask, const float* rb_meas, float* cov,
+                    float* logdet, float* last_pose, void* cuda_stream, char* err, size_t err_len) {
+  if (err && err_len) err[0] = 0;
+  if (!sizes_ok(batch, window, landmarks) || steps < 0 || iters < 0) return static_fail(err, err_len, SLAM_EINVAL, "slam_run_static: invalid batch / window / landmarks / steps / iters");
+  if (!odom && steps > 0) return static_fail(err, err_len, SLAM_EINVAL, "slam_run_static: odom is NULL");
+  const size_t need = slam_workspace_bytes(batch, window, landmarks);
+  if (need == 0 || need > (size_t)SLAM_STATIC_MAX_BYTES) {
+    char msg[200];
+    snprintf(msg, sizeof(msg), "slam_run_static: batch=%d window=%d landmarks=%d needs %zu bytes of scratch, the static array holds %zu (SLAM_STATIC_MAX_BYTES): use slam_create with a caller-owned workspace",
+             batch, window, landmarks, need, (size_t)SLAM_STATIC_MAX_BYTES);
+    return static_fail(err, err_len, SLAM_ENOMEM, msg);
+  }
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { cudaGetLastError(); return static_fail(err, err_len, SLAM_ECUDA, "slam_run_static: no current CUDA device"); }
+  if (!g_static_ptr[dev]) {   // set-up, once per device, with that device current
+    void* ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&ptr, g_static_ws);
+    if (e != cudaSuccess || !ptr) { cudaGetLastError(); return static_fail(err, err_len, SLAM_ECUDA, cudaGetErrorString(e)); }
+    g_static_ptr[dev] = ptr;
+  }
+  slam_ctx* c = nullptr;   // (a ~1 KB host object; no CUDA allocation of any kind on this path)
+  int rc = slam_create(&c, batch, window, landmarks, cfg, g_static_ptr[dev], (size_t)SLAM_STATIC_MAX_BYTES, cuda_stream);
+  if (rc != SLAM_OK) return static_fail(err, err_len, rc, "slam_run_static: slam_create on the static array failed");
+  const size_t N = (size_t)batch, nw = (size_t)c->ly.nw, L = (size_t)landmarks;
+  if (landmarks > 0) rc = slam_observe_first(c, rb_mask, rb_meas);
+  for (int t = 1; rc == SLAM_OK && t <= steps; ++t) {
+    const size_t q = (size_t)(t - 1);
+    rc = slam_step(c, odom + q * 3 * N, lc_back ? lc_back + q * N : nullptr, lc_back ? lc_meas + q * 3 * N : nullptr,
+                   landmarks > 0 ? rb_mask + (size_t)t * nw * N : nullptr, landmarks > 0 ? rb_meas + (size_t)t * 2 * L * N : nullptr, iters,
+                   cov ? cov + q * 9 * N : nullptr, logdet ? logdet + q * N : nullptr, last_pose ? last_pose + q * 3 * N : nullptr);
+  }
+  if (rc != SLAM_OK) static_fail(err, err_len, rc, c->err);
+  slam_destroy(c);
+  return rc;
+}
+
 }  // extern "C"
