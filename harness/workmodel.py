@@ -56,13 +56,17 @@ class WindowStructure:
 
     # elimination offsets: [passive landmarks | chain poses | observed landmarks | newest | anchor]
     def obs(self):
-        m = 0
-        for k in range(self.c):
-            m |= self.rbm[k]
-        return m
+        key = (self.c, tuple(self.rbm))          # (cached: first() asks for it hundreds of times per step)
+        if getattr(self, "_obs_key", None) != key:
+            m = 0
+            for k in range(self.c):
+                m |= self.rbm[k]
+            self._obs_key, self._obs, self._npas = key, m, self.L - _popcount(m)
+        return self._obs
 
     def npas(self):
-        return self.L - _popcount(self.obs())
+        self.obs()
+        return self._npas
 
     def off_slot(self, k):
         return 3 * (self.W - 2) + 2 * self.L if k == self.c - 1 else 2 * self.npas() + 3 * (k - 1)
@@ -155,15 +159,30 @@ class WindowStructure:
 def envelope_flops(first: np.ndarray):
     """(F_chol, F_fwd, F_back, envelope words incl. the rhs row) for a given `first` array."""
     n = first.shape[0]
-    f_chol = 0
-    for i in range(n):
-        j = np.arange(first[i], i + 1)
-        f_chol += int((2 * (j - np.maximum(first[i], first[j])) + 1).sum())
+    idx = np.arange(n)
+    live = (idx[None, :] >= first[:, None]) & (idx[None, :] <= idx[:, None])          # j in [first_i, i]
+    f_chol = int(((2 * (idx[None, :] - np.maximum(first[:, None], first[None, :])) + 1) * live).sum())
     lens = np.arange(n) - first
     f_fwd = int((2 * lens + 1).sum())
     f_back = f_fwd
     words = int((lens + 1).sum()) + n + 1
     return f_chol, f_fwd, f_back, words
+
+
+def step_work_parallel(data: dict, iters: int, envs, steps: int | None = None, procs: int = 8) -> dict:
+    """step_work over `envs` split across `procs` forked processes (pure host logic; the structure replay is
+    Python and takes ~1 ms per env-step)."""
+    import multiprocessing as mp
+    envs = np.asarray(envs)
+    procs = max(1, min(procs, len(envs)))
+    if procs == 1:
+        return step_work(data, iters, envs, steps)
+    chunks = [c for c in np.array_split(envs, procs) if len(c)]
+    keys = ("cfg", "T", "lc_back", "rb_mask")
+    slim = {k: data[k] for k in keys}
+    with mp.get_context("fork").Pool(len(chunks)) as pool:
+        parts = pool.starmap(step_work, [(slim, iters, c, steps) for c in chunks])
+    return {k: sum(p[k] * len(c) for p, c in zip(parts, chunks)) / len(envs) for k in parts[0]}
 
 
 def step_work(data: dict, iters: int, envs, steps: int | None = None) -> dict:

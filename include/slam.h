@@ -36,7 +36,8 @@ typedef struct slam_ctx slam_ctx; /* opaque host object */
 
 enum { SLAM_OK = 0, SLAM_EINVAL = 1, SLAM_ESTATE = 2, SLAM_ENOMEM = 3, SLAM_ECUDA = 4 };
 /* bits of the per-environment status word */
-enum { SLAM_ENV_OK = 0, SLAM_ENV_NOT_PD = 1, SLAM_ENV_NONFINITE = 2 };
+enum { SLAM_ENV_OK = 0, SLAM_ENV_NOT_PD = 1, SLAM_ENV_NONFINITE = 2,
+       SLAM_ENV_INTERNAL = 4 /* an environment did not fit the shared-memory pool: cannot happen for sizes slam_create accepts */ };
 
 #define SLAM_MAX_WINDOW 64    /* compiled maxima: window <= 64, landmarks <= 64 */
 #define SLAM_MAX_LANDMARKS 64
@@ -65,7 +66,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
 void slam_destroy(slam_ctx* ctx); /* frees the host object only */
 
 /* count = 1; anchor pose = init_pose ([3][N], NULL -> origin); prior N(init_pose, diag(prior_sigma^2))
- * on it (reading R9); clears landmarks, factors and status. */
+ * on it (reading R9); clears landmarks, factors, status and a pending slam_set_unary registration. */
 int slam_reset(slam_ctx* ctx, const float* init_pose);
 
 /* NEXT-2: per-environment episode reset (episodes end after 2048 steps or on collision).
@@ -75,7 +76,8 @@ int slam_reset(slam_ctx* ctx, const float* init_pose);
  * a reset environment simply has fewer live poses until its own window is full again: it is not
  * marginalised before that, its read-outs (slam_get_poses) report only its own poses, and loop closures
  * that reach behind its reset are ignored like any loop closure that leaves the window.
- * Call it between steps (after slam_marginalize_oldest / slam_step). */
+ * Call it between steps (after slam_marginalize_oldest / slam_step).  A pending slam_set_unary registration
+ * is kept: it belongs to the pose the next push appends, for reset environments too (mask it with `valid`). */
 int slam_reset_envs(slam_ctx* ctx, const int32_t* mask, const float* init_pose);
 
 /* S0 push (BASELINE.json "initial guess is dead-reckoned"): appends one pose with the
@@ -129,9 +131,12 @@ int slam_step(slam_ctx* ctx, const float* odom, const int32_t* lc_back, const fl
               const uint32_t* rb_mask, const float* rb_meas, int iters, float* cov, float* logdet,
               float* last_pose);
 
-/* The same step with HOST buffers (pinned memory recommended): copies the inputs to device staging
- * inside the workspace, runs slam_step, copies cov/logdet/last_pose back, all asynchronously on the
- * context's stream (the caller synchronises the stream before reading the outputs). */
+/* The same step with HOST buffers: copies the inputs to device staging inside the workspace, runs
+ * slam_step, copies cov/logdet/last_pose back, all on the context's stream.  With PAGE-LOCKED host
+ * buffers (cudaHostAlloc / cudaHostRegister) every copy is asynchronous and the call returns at once;
+ * with pageable memory each copy blocks the host until it is done (same results).  Either way the
+ * caller synchronises the stream before reading the outputs.  Errors: as slam_step; SLAM_ECUDA if a
+ * copy is refused (each copy's return code is checked). */
 int slam_step_host(slam_ctx* ctx, const float* odom_host, const int32_t* lc_back_host, const float* lc_meas_host,
                    const uint32_t* rb_mask_host, const float* rb_meas_host, int iters, float* cov_host,
                    float* logdet_host, float* last_pose_host);
@@ -219,6 +224,24 @@ int slam_set_precision(slam_ctx* ctx, int mode, float ratio_hi, float ratio_lo);
 int slam_run_static(int batch, int window, int landmarks, int steps, int iters, const slam_config* cfg, const float* odom,
                     const int32_t* lc_back, const float* lc_meas, const uint32_t* rb_mask, const float* rb_meas, float* cov,
                     float* logdet, float* last_pose, void* cuda_stream, char* err, size_t err_len);
+
+/* Measurement aid: per-kernel device time of the step launches.  slam_kernel_timing(ctx, max_steps) creates
+ * 4 * max_steps CUDA events (max_steps = 0 frees them and switches the timing off; this is the one call besides
+ * slam_create that creates CUDA objects); from then on every call that launches the step kernel records an event
+ * before it, after it, after the fp64 kernel and after the ordering kernel, for the next max_steps such calls.
+ * slam_kernel_timing_read waits for the last recorded event, stores the summed milliseconds of
+ * [0] slam_step_kernel, [1] slam_ref64_kernel, [2] slam_order_kernel in ms3 (host double[3]) and the number of
+ * calls they cover in *steps (host, may be NULL), and restarts the recording. */
+int slam_kernel_timing(slam_ctx* ctx, int max_steps);
+int slam_kernel_timing_read(slam_ctx* ctx, double* ms3, int* steps);
+
+/* Measurement aid for the roofline's denominator ("P_fp32 ... the bench must measure it
+ * with a register-resident FMA microbenchmark"): enqueues ONE launch of a kernel that fills every SM with
+ * independent FP32 FMA chains held in registers (8 CTAs of 256 threads per SM, 64 FMAs per loop iteration and
+ * thread, `iters` iterations, no memory traffic in the loop) and stores the number of floating-point operations
+ * that launch performs (2 per FMA) in *flops (host, may be NULL).  The caller times the launch with events on
+ * `cuda_stream`.  sink: device float[1], never written for the arguments used.  No context needed. */
+int slam_fma_probe(long long iters, float* sink, void* cuda_stream, double* flops);
 
 int slam_count(const slam_ctx* ctx);                /* host-side window count c in [1, window] */
 long long slam_launch_count(const slam_ctx* ctx);   /* kernels launched by this context so far */

@@ -4,9 +4,8 @@ The product is the C-ABI library declared in ``include/slam.h`` (built from ``cs
 ctypes binding in :mod:`paper_2603_25834_b200.binding`.  Importing this package does NOT load the
 CUDA library; ``binding`` does, and fails loudly if it is missing (there is no CPU fallback).
 
-:mod:`paper_2603_25834_b200.synth` is the seeded synthetic-trajectory generator that serves both the
-product tests/bench and the independent fp64 oracle under ``oracle/``; it contains none of the
-method's arithmetic.
+The seeded synthetic-input generator, the roofline work model and the replica helpers are harness code and
+live in the top-level ``harness/`` package, not here.
 """
 
-__all__ = ["binding", "synth"]
+__all__ = ["binding", "build"]

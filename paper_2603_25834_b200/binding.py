@@ -15,7 +15,7 @@ import torch
 from . import build as _build
 
 SLAM_OK, SLAM_EINVAL, SLAM_ESTATE, SLAM_ENOMEM, SLAM_ECUDA = 0, 1, 2, 3, 4
-SLAM_ENV_NOT_PD, SLAM_ENV_NONFINITE = 1, 2
+SLAM_ENV_NOT_PD, SLAM_ENV_NONFINITE, SLAM_ENV_INTERNAL = 1, 2, 4
 _ERR = {1: "SLAM_EINVAL", 2: "SLAM_ESTATE", 3: "SLAM_ENOMEM", 4: "SLAM_ECUDA"}
 
 # every symbol include/slam.h declares (checked by tests/test_abi.py)
@@ -23,7 +23,7 @@ SYMBOLS = (
     "slam_default_config", "slam_workspace_bytes", "slam_create", "slam_destroy", "slam_reset",
     "slam_reset_envs", "slam_push_step", "slam_set_unary", "slam_observe_first", "slam_solve", "slam_marginal_cov", "slam_dopt",
     "slam_marginalize_oldest", "slam_step", "slam_step_host", "slam_get_poses", "slam_get_landmarks",
-    "slam_get_status", "slam_get_stats", "slam_set_precision", "slam_run_static", "slam_reward", "slam_scan_match", "slam_grid_update", "slam_count", "slam_launch_count", "slam_last_error", "slam_kernel_info",
+    "slam_get_status", "slam_get_stats", "slam_set_precision", "slam_run_static", "slam_fma_probe", "slam_kernel_timing", "slam_kernel_timing_read", "slam_reward", "slam_scan_match", "slam_grid_update", "slam_count", "slam_launch_count", "slam_last_error", "slam_kernel_info",
 )
 
 
@@ -84,6 +84,9 @@ def _load() -> C.CDLL:
     lib.slam_grid_update.argtypes = [C.POINTER(ScanParams), C.c_int, fp, fp, fp, fp, C.c_float, C.c_float, C.c_float, vp]
     lib.slam_set_precision.argtypes = [vp, C.c_int, C.c_float, C.c_float]
     lib.slam_run_static.argtypes = [C.c_int] * 5 + [C.POINTER(SlamConfig), fp, ip, fp, ip, fp, fp, fp, fp, vp, C.c_char_p, C.c_size_t]
+    lib.slam_kernel_timing.argtypes = [vp, C.c_int]
+    lib.slam_kernel_timing_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int)]
+    lib.slam_fma_probe.argtypes = [C.c_longlong, fp, vp, C.POINTER(C.c_double)]
     lib.slam_count.argtypes = [vp]
     lib.slam_launch_count.argtypes = [vp]
     lib.slam_launch_count.restype = C.c_longlong
@@ -135,6 +138,20 @@ def grid_update(par: ScanParams, grid, pose, ranges, weight, l_free: float, l_oc
     if rc != SLAM_OK:
         raise SlamError(rc, "slam_grid_update")
     return grid
+
+
+def fma_probe(iters: int, device="cuda:0") -> float:
+    """slam_fma_probe: enqueues one launch of the register-resident FP32 FMA kernel on `device`'s current stream and
+    returns the floating-point operations that launch performs (the caller times it with CUDA events)."""
+    dev = torch.device(device)
+    sink = torch.zeros(1, device=dev)
+    flops = C.c_double(0.0)
+    with torch.cuda.device(dev):
+        rc = LIB.slam_fma_probe(int(iters), C.c_void_p(sink.data_ptr()), C.c_void_p(torch.cuda.current_stream(dev).cuda_stream),
+                                C.byref(flops))
+    if rc != SLAM_OK:
+        raise SlamError(rc, "slam_fma_probe")
+    return float(flops.value)
 
 
 STATIC_MAX_BYTES = 16 << 20
@@ -308,6 +325,16 @@ class FixedLagSlam:
     def set_precision(self, mode: int, ratio_hi: float = 0.0, ratio_lo: float = 0.0):
         """-1 default rule, 0 fp32 only, 1 fp32 + fp64 fallback on ill-conditioned windows, 2 fp64 everywhere."""
         self._chk(LIB.slam_set_precision(self._h, int(mode), float(ratio_hi), float(ratio_lo)))
+
+    def kernel_timing(self, max_steps: int):
+        """Record per-kernel events for the next `max_steps` step launches (0: off)."""
+        self._chk(LIB.slam_kernel_timing(self._h, int(max_steps)))
+
+    def kernel_timing_read(self) -> dict:
+        """Summed device milliseconds per kernel of the recorded step launches (synchronises)."""
+        ms, n = (C.c_double * 3)(), C.c_int()
+        self._chk(LIB.slam_kernel_timing_read(self._h, ms, C.byref(n)))
+        return dict(step_kernel_ms=ms[0], ref64_kernel_ms=ms[1], order_kernel_ms=ms[2], steps=n.value)
 
     def reward(self, params: RewardParams, u, u_prev, dcells, d_min, collision, out=None):
         out = self._new(self.N) if out is None else out

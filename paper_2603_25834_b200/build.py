@@ -8,7 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libslam_b200.so")
 SOURCES = ["slam_api.cu", "slam_scan.cu"]
-DEPS = ["slam_api.cu", "slam_scan.cu", "slam_kernels.cuh", "slam_layout.h", os.path.join("..", "..", "include", "slam.h")]
+DEPS = ["slam_api.cu", "slam_scan.cu", "slam_kernels.cuh", "slam_ref64.cuh", "slam_layout.h", os.path.join("..", "..", "include", "slam.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-shared",
               "-Xcompiler", "-fPIC", "--use_fast_math=false"]
 

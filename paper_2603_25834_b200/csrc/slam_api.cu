@@ -406,11 +406,30 @@ __global__ void slam_reward_kernel(int N, slam_reward_params p, const float* u, 
   reward[env] = r_explore * alpha - r_abs + (drop > 0.f ? r_delta * alpha : r_delta);     // (16), (17), (7)
 }
 
+// Register-resident FP32 FMA microbenchmark (the roofline's FP32 peak has to be MEASURED):
+// 16 independent accumulator chains per thread, no memory traffic inside the loop; 2 flop per FMA.
+__global__ void __launch_bounds__(256) slam_fma_probe_kernel(long long iters, float a, float b, float* sink) {
+  float acc[16];
+#pragma unroll
+  for (int k = 0; k < 16; ++k) acc[k] = (float)(threadIdx.x + k) * 1e-3f;
+  for (long long i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+#pragma unroll
+      for (int k = 0; k < 16; ++k) acc[k] = fmaf(acc[k], a, b);
+  }
+  float t = 0.f;
+#pragma unroll
+  for (int k = 0; k < 16; ++k) t += acc[k];
+  if (t == 123.456f) sink[0] = t;   // (never true for the arguments used: keeps the chains alive)
+}
+
 // ------------------------------------------------------------------ host object
 struct slam_ctx {
   Layout ly;
   Params pr;
   cudaStream_t stream;
+  int device;                 // the CUDA device the context was created on (every call makes it current)
   float* state;
   float* cov_cache;
   unsigned long long* stats;  // [8] device counters: max / sum / count of envelope words, ...
@@ -434,6 +453,9 @@ struct slam_ctx {
   const int32_t* un_valid;
   long long launches;
   int grid, smem_bytes, ctas_per_sm;
+  // optional per-kernel timing of the step launches (slam_kernel_timing): 4 events per step in a ring
+  cudaEvent_t* tev;
+  int tev_steps, tev_cap;
   char err[256];
 };
 
@@ -448,6 +470,24 @@ static int check_cuda(slam_ctx* c, const char* what) {
   return SLAM_ECUDA;
 }
 static size_t al256(size_t x) { return (x + 255) & ~(size_t)255; }
+// Makes the context's device current for the duration of a call (a context created on cuda:1 must not launch on
+// whatever device the caller's thread happens to have current).
+struct DevGuard {
+  int prev;
+  bool swapped;
+  explicit DevGuard(const slam_ctx* c) : prev(-1), swapped(false) {
+    if (c && cudaGetDevice(&prev) == cudaSuccess && prev != c->device) swapped = cudaSetDevice(c->device) == cudaSuccess;
+  }
+  ~DevGuard() { if (swapped) cudaSetDevice(prev); }
+};
+static int sm_count() {  // SMs of the current device (148 on B200)
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) {
+    cudaGetLastError();
+    sms = 148;
+  }
+  return sms;
+}
 
 static bool sizes_ok(int batch, int window, int landmarks) {
   return batch >= 1 && window >= 2 && window <= SLAM_MAX_WINDOW && landmarks >= 0 && landmarks <= SLAM_MAX_LANDMARKS;
@@ -462,7 +502,7 @@ static int pick_team(int W, int L, int batch) {
   const char* e = getenv("SLAM_TEAM");
   if (e) { const int t = atoi(e); if (t == 32 || t == 64 || t == 128) return t; }
   const int n = 3 * W + 2 * L;
-  if (n >= 48 && batch < 148 * 8) return 64;
+  if (n >= 48 && batch < sm_count() * 8) return 64;
   return 32;
 }
 static int max_teams(int team) {  // threads per CTA: register file (launch bounds), 15 named barriers, 16 table slots
@@ -533,6 +573,20 @@ static int pick_pairs(int W, int L, int team) {
   return L == 0 && team == 32 && 16.0 * (d.team_words + 0.3 * d.dense) > SMEM_BUDGET / 4;
 }
 
+// The ONE place that decides the launch shape of the step kernel for given sizes (slam_workspace_bytes and
+// slam_create both go through it): threads per environment, envelope grouping, teams per CTA, pool words.
+static bool pick_layout(int batch, int window, int landmarks, Layout* out) {
+  const int team = pick_team(window, landmarks, batch);
+  const int pairs = pick_pairs(window, landmarks, team);
+  int pool = 0;
+  const int wpc = pick_launch(window, landmarks, team, pairs, &pool);
+  if (wpc < 1) return false;
+  *out = make_layout(batch, window, landmarks, pool, wpc);
+  out->team = team;
+  out->pairs = pairs;
+  return true;
+}
+
 // fp64 path: dynamic shared memory of one CTA (everything but H, plus H when it fits) and the global scratch
 // for H when it does not (one packed triangle per resident CTA; grid = 2 CTAs per SM then)
 static const int REF_MAX_GRID_GLOBAL = 2 * 160;
@@ -576,10 +630,9 @@ void slam_default_config(slam_config* cfg) {
 
 size_t slam_workspace_bytes(int batch, int window, int landmarks) {
   if (!sizes_ok(batch, window, landmarks)) return 0;
-  int pool = 0;
-  const int wpc = pick_launch(window, landmarks, pick_team(window, landmarks, batch), 0, &pool);
-  if (wpc < 1) return 0;
-  return plan(make_layout(batch, window, landmarks, pool, wpc)).total;
+  Layout ly;
+  if (!pick_layout(batch, window, landmarks, &ly)) return 0;
+  return plan(ly).total;
 }
 
 int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam_config* cfg, void* workspace,
@@ -587,10 +640,9 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   if (!out) return SLAM_EINVAL;
   *out = nullptr;
   if (!sizes_ok(batch, window, landmarks) || !workspace || ((uintptr_t)workspace & 255)) return SLAM_EINVAL;
-  const int team = pick_team(window, landmarks, batch);
-  int pool = 0;
-  const int wpc = pick_launch(window, landmarks, team, pick_pairs(window, landmarks, team), &pool);
-  if (wpc < 1) return SLAM_EINVAL;
+  Layout ly0;
+  if (!pick_layout(batch, window, landmarks, &ly0)) return SLAM_EINVAL;
+  const int team = ly0.team, wpc = ly0.wpc;
   slam_config dc;
   slam_default_config(&dc);
   if (!cfg) cfg = &dc;
@@ -599,9 +651,8 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   if (!(cfg->rb_sigma[0] > 0.f) || !(cfg->rb_sigma[1] > 0.f)) return SLAM_EINVAL;
   slam_ctx* c = new (std::nothrow) slam_ctx();
   if (!c) return SLAM_ENOMEM;
-  c->ly = make_layout(batch, window, landmarks, pool, wpc);
-  c->ly.team = team;
-  c->ly.pairs = pick_pairs(window, landmarks, team);
+  c->ly = ly0;
+  if (cudaGetDevice(&c->device) != cudaSuccess) { cudaGetLastError(); delete c; return SLAM_ECUDA; }
   { const char* e = getenv("SLAM_LOCK"); if (e) c->ly.lock = atoi(e); }
   { const char* e = getenv("SLAM_LCACHE"); if (e) c->ly.lcache = atoi(e); }
   const WsPlan p = plan(c->ly);
@@ -630,6 +681,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   c->st_logdet = (float*)(base + p.ld);
   c->st_pose = (float*)(base + p.pose);
   c->launches = 0;
+  c->tev = nullptr; c->tev_steps = 0; c->tev_cap = 0;
   c->err[0] = 0;
   c->un_pose = nullptr; c->un_info = nullptr; c->un_valid = nullptr;
   c->fb_list = (int*)(base + p.fbl);
@@ -679,22 +731,32 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
 
 void slam_destroy(slam_ctx* ctx) {
   if (!ctx) return;
+  if (ctx->tev) {
+    DevGuard dg(ctx);
+    for (int i = 0; i < 4 * ctx->tev_cap; ++i) cudaEventDestroy(ctx->tev[i]);
+    delete[] ctx->tev;
+  }
   delete ctx;
 }
 
 int slam_reset(slam_ctx* c, const float* init_pose) {
   if (!c) return SLAM_EINVAL;
+  DevGuard dg(c);
   const int threads = 256, blocks = (int)(((size_t)c->ly.N * 32 + threads - 1) / threads);
   cudaMemsetAsync(c->stats, 0, 256, c->stream);
   cudaMemsetAsync(c->fb_cnt, 0, 64, c->stream);
   slam_reset_kernel<<<blocks, threads, 0, c->stream>>>(c->ly, c->pr, c->state, init_pose, c->perm, c->keys);
   c->launches++;
   c->head = 0; c->count = 1; c->cov_valid = false;
+  c->un_pose = nullptr; c->un_info = nullptr; c->un_valid = nullptr;   // a pending slam_set_unary belongs to the old episode
   return check_cuda(c, "slam_reset");
 }
 
 static int launch_step(slam_ctx* c, int flags, int iters, const StepIO& io) {
+  DevGuard dg(c);
   const step_fn fn = kernel_of(c->ly.team, c->ly.pairs, c->ly.L);
+  cudaEvent_t* tv = (c->tev && c->tev_steps < c->tev_cap) ? c->tev + 4 * c->tev_steps : nullptr;
+  if (tv) cudaEventRecord(tv[0], c->stream);
   if (c->precision == 2) {   // device reference: every environment through the fp64 path
     const int threads = 256, blocks = (c->ly.N + threads - 1) / threads;
     slam_fill_list_kernel<<<blocks, threads, 0, c->stream>>>(c->ly.N, c->fb_list, c->fb_cnt);
@@ -707,6 +769,7 @@ static int launch_step(slam_ctx* c, int flags, int iters, const StepIO& io) {
                                                                         c->precision == 1 ? c->fb_list : nullptr, c->fb_cnt);
     c->launches++;
   }
+  if (tv) cudaEventRecord(tv[1], c->stream);
   if (c->precision >= 1) {   // the environments the fp32 kernel queued: fp64 records, and the windows it refused to commit
     slamr::RefArgs ra = {c->state, c->state64, c->head, c->count, flags, iters, c->fb_list, c->fb_cnt, c->stats, c->hglob,
                          (double)c->ratio_lo, c->precision == 2 ? 1 : 0};
@@ -716,6 +779,7 @@ static int launch_step(slam_ctx* c, int flags, int iters, const StepIO& io) {
     slamr::slam_ref64_kernel<<<c->ref_grid, slamr::NT, c->ref_smem, c->stream>>>(c->ly, c->pr, ra, io);
     c->launches++;
   }
+  if (tv) cudaEventRecord(tv[2], c->stream);
   // the solve left fresh cost keys: order the next launches by them (pointless unless every CTA runs
   // several rounds; a small batch is latency bound: one more kernel boundary per step would show; and
   // measured only landmark windows gain -- their cost varies most: config 3 2.40 -> 2.31 ms per step,
@@ -724,6 +788,7 @@ static int launch_step(slam_ctx* c, int flags, int iters, const StepIO& io) {
     slam_order_kernel<<<1, 1024, 0, c->stream>>>(c->ly.N, c->ly.dense, c->keys, c->perm);
     c->launches++;
   }
+  if (tv) { cudaEventRecord(tv[3], c->stream); c->tev_steps++; }
   return check_cuda(c, "slam_step_kernel");
 }
 
@@ -760,6 +825,7 @@ int slam_set_unary(slam_ctx* c, const float* pose, const float* info, const int3
 
 int slam_reset_envs(slam_ctx* c, const int32_t* mask, const float* init_pose) {
   if (!c || !mask) return c ? fail(c, SLAM_EINVAL, "mask is NULL") : SLAM_EINVAL;
+  DevGuard dg(c);
   const int threads = 256, blocks = (int)(((size_t)c->ly.N * 32 + threads - 1) / threads);
   slam_reset_envs_kernel<<<blocks, threads, 0, c->stream>>>(c->ly, c->pr, c->state, c->count, mask, init_pose);
   c->launches++;
@@ -787,6 +853,7 @@ int slam_solve(slam_ctx* c, int iters) {
 }
 
 static int cov_call(slam_ctx* c, float* cov, float* logdet, float* dopt) {
+  DevGuard dg(c);
   if (c->cov_valid) {
     const int threads = 256, blocks = (c->ly.N + threads - 1) / threads;
     slam_copycov_kernel<<<blocks, threads, 0, c->stream>>>(c->ly.N, c->cov_cache, cov, logdet, dopt);
@@ -844,30 +911,36 @@ int slam_step(slam_ctx* c, const float* odom, const int32_t* lc_back, const floa
 int slam_step_host(slam_ctx* c, const float* odom, const int32_t* lc_back, const float* lc_meas, const uint32_t* rb_mask,
                    const float* rb_meas, int iters, float* cov, float* logdet, float* last_pose) {
   if (!c) return SLAM_EINVAL;
+  DevGuard dg(c);
   int rc = check_push_args(c, odom, lc_back, lc_meas, rb_mask, rb_meas);
   if (rc) return rc;
   const size_t N = (size_t)c->ly.N;
-  cudaMemcpyAsync(c->st_odom, odom, N * 3 * 4, cudaMemcpyHostToDevice, c->stream);
-  if (lc_back) {
-    cudaMemcpyAsync(c->st_lc_back, lc_back, N * 4, cudaMemcpyHostToDevice, c->stream);
-    cudaMemcpyAsync(c->st_lc_meas, lc_meas, N * 3 * 4, cudaMemcpyHostToDevice, c->stream);
+  // (page-locked host buffers make these copies asynchronous; with pageable memory each one blocks the host
+  // until it is done -- the results are the same)
+  cudaError_t e = cudaMemcpyAsync(c->st_odom, odom, N * 3 * 4, cudaMemcpyHostToDevice, c->stream);
+  if (e == cudaSuccess && lc_back) {
+    e = cudaMemcpyAsync(c->st_lc_back, lc_back, N * 4, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c->st_lc_meas, lc_meas, N * 3 * 4, cudaMemcpyHostToDevice, c->stream);
   }
-  if (c->ly.L > 0) {
-    cudaMemcpyAsync(c->st_rb_mask, rb_mask, N * c->ly.nw * 4, cudaMemcpyHostToDevice, c->stream);
-    cudaMemcpyAsync(c->st_rb_meas, rb_meas, N * 2 * c->ly.L * 4, cudaMemcpyHostToDevice, c->stream);
+  if (e == cudaSuccess && c->ly.L > 0) {
+    e = cudaMemcpyAsync(c->st_rb_mask, rb_mask, N * c->ly.nw * 4, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c->st_rb_meas, rb_meas, N * 2 * c->ly.L * 4, cudaMemcpyHostToDevice, c->stream);
   }
+  if (e != cudaSuccess) { cudaGetLastError(); snprintf(c->err, sizeof(c->err), "slam_step_host: input copy: %s", cudaGetErrorString(e)); return SLAM_ECUDA; }
   rc = slam_step(c, c->st_odom, lc_back ? c->st_lc_back : nullptr, lc_back ? c->st_lc_meas : nullptr,
                  c->ly.L > 0 ? c->st_rb_mask : nullptr, c->ly.L > 0 ? c->st_rb_meas : nullptr, iters,
                  cov ? c->st_cov : nullptr, logdet ? c->st_logdet : nullptr, last_pose ? c->st_pose : nullptr);
   if (rc) return rc;
-  if (cov) cudaMemcpyAsync(cov, c->st_cov, N * 9 * 4, cudaMemcpyDeviceToHost, c->stream);
-  if (logdet) cudaMemcpyAsync(logdet, c->st_logdet, N * 4, cudaMemcpyDeviceToHost, c->stream);
-  if (last_pose) cudaMemcpyAsync(last_pose, c->st_pose, N * 3 * 4, cudaMemcpyDeviceToHost, c->stream);
-  return check_cuda(c, "slam_step_host copies");
+  if (cov) e = cudaMemcpyAsync(cov, c->st_cov, N * 9 * 4, cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess && logdet) e = cudaMemcpyAsync(logdet, c->st_logdet, N * 4, cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess && last_pose) e = cudaMemcpyAsync(last_pose, c->st_pose, N * 3 * 4, cudaMemcpyDeviceToHost, c->stream);
+  if (e != cudaSuccess) { cudaGetLastError(); snprintf(c->err, sizeof(c->err), "slam_step_host: output copy: %s", cudaGetErrorString(e)); return SLAM_ECUDA; }
+  return SLAM_OK;
 }
 
 int slam_get_poses(slam_ctx* c, float* poses) {
   if (!c || !poses) return SLAM_EINVAL;
+  DevGuard dg(c);
   const int threads = 128, blocks = (c->ly.N + threads - 1) / threads;
   slam_poses_kernel<<<blocks, threads, 0, c->stream>>>(c->ly, c->state, c->state64, c->head, c->count, poses);
   c->launches++;
@@ -878,6 +951,7 @@ int slam_get_landmarks(slam_ctx* c, float* lm, uint32_t* active) {
   if (!c) return SLAM_EINVAL;
   if (c->ly.L == 0) return SLAM_OK;
   if (!lm || !active) return fail(c, SLAM_EINVAL, "lm/active are NULL");
+  DevGuard dg(c);
   const int threads = 128, blocks = (c->ly.N + threads - 1) / threads;
   slam_landmarks_kernel<<<blocks, threads, 0, c->stream>>>(c->ly, c->state, c->state64, lm, active);
   c->launches++;
@@ -886,6 +960,7 @@ int slam_get_landmarks(slam_ctx* c, float* lm, uint32_t* active) {
 
 int slam_get_status(slam_ctx* c, int32_t* status) {
   if (!c || !status) return SLAM_EINVAL;
+  DevGuard dg(c);
   const int threads = 128, blocks = (c->ly.N + threads - 1) / threads;
   slam_status_kernel<<<blocks, threads, 0, c->stream>>>(c->ly, c->state, status);
   c->launches++;
@@ -894,6 +969,7 @@ int slam_get_status(slam_ctx* c, int32_t* status) {
 
 int slam_get_stats(slam_ctx* c, unsigned long long* stats8) {
   if (!c || !stats8) return SLAM_EINVAL;
+  DevGuard dg(c);
 #ifdef SLAM_REF_PROFILE
   cudaMemcpyAsync(stats8, c->stats + 8, 64, cudaMemcpyDeviceToDevice, c->stream);
 #else
@@ -906,6 +982,7 @@ int slam_reward(slam_ctx* c, const slam_reward_params* p, const float* u, const 
                 const float* d_min, const int32_t* collision, float* reward) {
   if (!c || !p || !u || !u_prev || !dcells || !d_min || !collision || !reward) return c ? fail(c, SLAM_EINVAL, "NULL argument") : SLAM_EINVAL;
   if (!(p->u_hi > 0.f) || !(p->kappa > 0.f) || !(p->d_full > p->d_crash)) return fail(c, SLAM_EINVAL, "u_hi, kappa > 0 and d_full > d_crash required");
+  DevGuard dg(c);
   const int threads = 256, blocks = (c->ly.N + threads - 1) / threads;
   slam_reward_kernel<<<blocks, threads, 0, c->stream>>>(c->ly.N, *p, u, u_prev, dcells, d_min, collision, reward);
   c->launches++;
@@ -923,6 +1000,54 @@ int slam_set_precision(slam_ctx* c, int mode, float ratio_hi, float ratio_lo) {
   if (c->ratio_lo > c->ratio_hi) c->ratio_lo = c->ratio_hi;
   c->cov_valid = false;
   return SLAM_OK;
+}
+
+int slam_kernel_timing(slam_ctx* c, int max_steps) {
+  if (!c || max_steps < 0 || max_steps > (1 << 16)) return c ? fail(c, SLAM_EINVAL, "max_steps out of range") : SLAM_EINVAL;
+  DevGuard dg(c);
+  if (c->tev) {
+    for (int i = 0; i < 4 * c->tev_cap; ++i) cudaEventDestroy(c->tev[i]);
+    delete[] c->tev;
+    c->tev = nullptr; c->tev_cap = 0;
+  }
+  c->tev_steps = 0;
+  if (max_steps == 0) return SLAM_OK;
+  c->tev = new (std::nothrow) cudaEvent_t[4 * (size_t)max_steps];
+  if (!c->tev) return fail(c, SLAM_ENOMEM, "slam_kernel_timing: host allocation failed");
+  for (int i = 0; i < 4 * max_steps; ++i)
+    if (cudaEventCreate(&c->tev[i]) != cudaSuccess) {
+      for (int j = 0; j < i; ++j) cudaEventDestroy(c->tev[j]);
+      delete[] c->tev;
+      c->tev = nullptr;
+      check_cuda(c, "cudaEventCreate");
+      return SLAM_ECUDA;
+    }
+  c->tev_cap = max_steps;
+  return SLAM_OK;
+}
+
+int slam_kernel_timing_read(slam_ctx* c, double* ms3, int* steps) {
+  if (!c || !ms3) return c ? fail(c, SLAM_EINVAL, "ms3 is NULL") : SLAM_EINVAL;
+  DevGuard dg(c);
+  ms3[0] = ms3[1] = ms3[2] = 0.0;
+  if (steps) *steps = c->tev_steps;
+  if (c->tev_steps > 0 && cudaEventSynchronize(c->tev[4 * (c->tev_steps - 1) + 3]) != cudaSuccess) return check_cuda(c, "slam_kernel_timing_read");
+  for (int i = 0; i < c->tev_steps; ++i)
+    for (int k = 0; k < 3; ++k) {
+      float ms = 0.f;
+      if (cudaEventElapsedTime(&ms, c->tev[4 * i + k], c->tev[4 * i + k + 1]) != cudaSuccess) return check_cuda(c, "cudaEventElapsedTime");
+      ms3[k] += (double)ms;
+    }
+  c->tev_steps = 0;
+  return SLAM_OK;
+}
+
+int slam_fma_probe(long long iters, float* sink, void* cuda_stream, double* flops) {
+  if (iters < 1 || !sink) return SLAM_EINVAL;
+  const int blocks = sm_count() * 8, threads = 256;
+  slam_fma_probe_kernel<<<blocks, threads, 0, (cudaStream_t)cuda_stream>>>(iters, 0.999f, 1e-3f, sink);
+  if (flops) *flops = (double)blocks * threads * (double)iters * 64.0 * 2.0;
+  return check_cuda(nullptr, "slam_fma_probe_kernel");
 }
 
 int slam_count(const slam_ctx* c) { return c ? c->count : -1; }

@@ -2,7 +2,7 @@
 import numpy as np
 import torch
 
-from paper_2603_25834_b200 import synth  # noqa: F401  (kept for callers)
+from harness import synth  # noqa: F401  (kept for callers)
 
 
 def to_dev(data, device="cuda:0"):

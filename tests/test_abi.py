@@ -65,7 +65,7 @@ def test_create_rejects_bad_arguments(lib):
 
 
 def test_default_config(lib):
-    from paper_2603_25834_b200 import synth
+    from harness import synth
 
     class Cfg(ctypes.Structure):
         _fields_ = [("p", ctypes.c_float * 3), ("o", ctypes.c_float * 3), ("l", ctypes.c_float * 3), ("r", ctypes.c_float * 2)]

@@ -10,7 +10,7 @@ tests/helpers.determined (from the oracle alone) and require that they are at mo
 import numpy as np
 
 import oracle
-from paper_2603_25834_b200 import synth
+from harness import synth
 from tests.gpu_driver import parity_errors
 from tests.helpers import determined, drive
 

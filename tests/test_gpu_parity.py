@@ -8,7 +8,7 @@ import pytest
 import torch
 
 import oracle
-from paper_2603_25834_b200 import synth
+from harness import synth
 from tests.gpu_driver import parity_errors, run_gpu, to_dev
 from tests.helpers import determined, drive
 

@@ -7,7 +7,7 @@ import torch
 import torch.distributed as dist
 import torch.multiprocessing as mp
 
-from paper_2603_25834_b200 import replicas, synth
+from harness import replicas, synth
 
 
 def _free_port():

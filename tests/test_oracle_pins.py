@@ -23,7 +23,7 @@ import pytest
 
 import oracle
 from oracle import Oracle
-from paper_2603_25834_b200 import synth
+from harness import synth
 from tests import fullbatch
 from tests.helpers import drive, rb_inputs, step_inputs
 

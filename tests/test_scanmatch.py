@@ -6,7 +6,7 @@ import numpy as np
 import pytest
 
 from oracle import scanmatch as osm
-from paper_2603_25834_b200 import synth
+from harness import synth
 
 PAR = dict(res=0.1, hx=3, hy=3, ht=4, sxy=0.1, sth=0.01)
 

@@ -4,7 +4,7 @@ permuted into the kernels' elimination order, and its flop formula against brute
 import numpy as np
 
 from oracle import Oracle
-from paper_2603_25834_b200 import synth, workmodel
+from harness import synth, workmodel
 from tests.helpers import rb_inputs, step_inputs
 
 

@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 import torch
 
-from paper_2603_25834_b200 import synth
+from harness import synth
 from tests.gpu_driver import parity_errors, run_gpu, to_dev
 
 pytestmark = pytest.mark.gpu
