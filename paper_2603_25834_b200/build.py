@@ -1,4 +1,5 @@
-"""Builds the C-ABI CUDA library ``libslam_b200.so`` in-tree with nvcc for sm_100a."""
+"""Builds the C-ABI CUDA library ``libslam_b200.so`` in-tree with nvcc for sm_100a: one object per source file
+(rebuilt only when that file or a header changed), then one link."""
 from __future__ import annotations
 
 import os
@@ -6,11 +7,11 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libslam_b200.so")
 SOURCES = ["slam_api.cu", "slam_scan.cu"]
-DEPS = ["slam_api.cu", "slam_scan.cu", "slam_kernels.cuh", "slam_ref64.cuh", "slam_layout.h", os.path.join("..", "..", "include", "slam.h")]
-NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-shared",
-              "-Xcompiler", "-fPIC", "--use_fast_math=false"]
+HEADERS = ["slam_kernels.cuh", "slam_ref64.cuh", "slam_layout.h", os.path.join("..", "..", "include", "slam.h")]
+NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC"]
 
 
 def _nvcc() -> str:
@@ -18,19 +19,36 @@ def _nvcc() -> str:
     return cand if os.path.exists(cand) else "nvcc"
 
 
-def needs_build() -> bool:
-    if not os.path.exists(LIB):
+def _newest_header() -> float:
+    return max(os.path.getmtime(os.path.join(CSRC, h)) for h in HEADERS)
+
+
+def _stale(target: str, src: str) -> bool:
+    if not os.path.exists(target):
         return True
-    t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(os.path.join(CSRC, d)) > t for d in DEPS)
+    t = os.path.getmtime(target)
+    return os.path.getmtime(src) > t or _newest_header() > t
+
+
+def needs_build() -> bool:
+    return any(_stale(LIB, os.path.join(CSRC, s)) for s in SOURCES)
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    if force or needs_build():
-        flags = [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")]
-        cmd = [_nvcc()] + flags + (["-Xptxas", "-v"] if verbose else []) + \
-              [os.path.join(CSRC, s) for s in SOURCES] + ["-o", LIB]
-        subprocess.check_call(cmd)
+    if not (force or needs_build()):
+        return LIB
+    os.makedirs(OBJ, exist_ok=True)
+    objs, procs = [], []
+    for s in SOURCES:
+        src, obj = os.path.join(CSRC, s), os.path.join(OBJ, s.replace(".cu", ".o"))
+        objs.append(obj)
+        if force or _stale(obj, src):
+            cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
+            procs.append((cmd, subprocess.Popen(cmd)))
+    for cmd, pr in procs:
+        if pr.wait() != 0:
+            raise subprocess.CalledProcessError(pr.returncode, cmd)
+    subprocess.check_call([_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a"] + objs + ["-o", LIB])
     return LIB
 
 

@@ -553,14 +553,18 @@ static int pick_launch(int W, int L, int team, int pairs, int* pool_words) {
 }
 typedef void (*step_fn)(Layout, Params, float*, int, int, int, int, StepIO, unsigned long long*, const int*, int*, int*, int*);
 template <bool PAIRS, bool LM>
-static step_fn kernel_pick(int team) {
+[[maybe_unused]] static step_fn kernel_pick(int team) {
   return team == 128 ? slam_step_kernel<128, PAIRS, LM> : (team == 64 ? slam_step_kernel<64, PAIRS, LM> : slam_step_kernel<32, PAIRS, LM>);
 }
 // One instantiation per (team size, envelope rows in pairs, window has landmarks): the pose-only kernels
 // carry no code for cached landmark columns, the fours kernels none for split dot products.
 static step_fn kernel_of(int team, int pairs, int landmarks) {
+#ifdef SLAM_DEV_SINGLE   // developer build (compiles in a fifth of the time): only the kernels of BASELINE configs 3 and 4
+  return landmarks ? slam_step_kernel<32, false, true> : slam_step_kernel<32, true, false>;
+#else
   if (pairs) return landmarks ? kernel_pick<true, true>(team) : kernel_pick<true, false>(team);
   return landmarks ? kernel_pick<false, true>(team) : kernel_pick<false, false>(team);
+#endif
 }
 // Envelope rows in pairs instead of fours: 12-18 % fewer shared-memory words per environment, ~5 % more
 // instructions.  Pays where the pool bounds the environments in flight even at a third of the dense

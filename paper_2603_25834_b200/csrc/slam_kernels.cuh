@@ -147,6 +147,11 @@ __device__ __forceinline__ int tri_row(int t) {
   if (p * (p + 1) / 2 > t) --p;
   return p;
 }
+// (p, q) of packed index t -> of t + step, without the square root: q moves right and wraps over the row ends
+__device__ __forceinline__ void tri_advance(int& p, int& q, int step) {
+  q += step;
+  while (q > p) { q -= p + 1; ++p; }
+}
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULLMASK, v, o);
@@ -726,6 +731,7 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
     const int ntri = s * (s + 1) >> 1;
     // loads first, scatter second: the compiler cannot move a global load above the shared-memory update
     // of the previous entry, so without the explicit batch every iteration pays a full L2 round trip
+    int tp = tri_row(lane), tq = lane - (tp * (tp + 1) >> 1);   // (row, column) of this lane's entry, advanced incrementally
     for (int t0 = lane; t0 < ntri; t0 += 8 * TEAM) {
       float v[8];
 #pragma unroll
@@ -734,10 +740,10 @@ __device__ void assemble(const Layout& ly, const Params& pr, const Ord& od, cons
       for (int u = 0; u < 8; ++u) {
         const int t = t0 + u * TEAM;
         if (t < ntri) {
-          const int p = tri_row(t), q = t - (p * (p + 1) >> 1);
-          const int ip = sup_off(w.sup[p]), iq = sup_off(w.sup[q]);
+          const int ip = sup_off(w.sup[tp]), iq = sup_off(w.sup[tq]);
           const int hi = max(ip, iq), lo = min(ip, iq);
           if (lo >= cb) w.H[rb_of(w, hi) + lo] += v[u];
+          tri_advance(tp, tq, TEAM);
         }
       }
     }
@@ -1484,10 +1490,11 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
   {
     const float* lam = rec + ly.o_lam;
     const int ntri = s_old * (s_old + 1) >> 1;
+    int tp = tri_row(lane), tq = lane - (tp * (tp + 1) >> 1);
 #pragma unroll 4
     for (int t = lane; t < ntri; t += TEAM) {
-      const int p = tri_row(t), q = t - (p * (p + 1) >> 1);
-      Hs[tri(omap[p], omap[q])] = lam[t];
+      Hs[tri(omap[tp], omap[tq])] = lam[t];
+      tri_advance(tp, tq, TEAM);
     }
     for (int p = lane; p < s_old; p += TEAM) {
       float acc = rec[ly.o_g + p];
@@ -1591,11 +1598,8 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
   };
   auto bpos = [&](int b) -> int { return b == 0 ? 0 : (b <= npn ? 3 + 3 * (b - 1) : 3 + 3 * npn + 2 * (b - 1 - npn)); };
   const int npairs = nbk * (nbk + 1) >> 1;
-  for (int t = lane; t < npairs; t += TEAM) {
-    int bi = (int)((sqrtf(8.f * (float)t + 1.f) - 1.f) * 0.5f);
-    while ((bi + 1) * (bi + 2) / 2 <= t) ++bi;
-    while (bi * (bi + 1) / 2 > t) --bi;
-    const int bj = t - bi * (bi + 1) / 2;
+  int bi = tri_row(lane), bj = lane - (bi * (bi + 1) >> 1);
+  for (int t = lane; t < npairs; t += TEAM, tri_advance(bi, bj, TEAM)) {
     const int pi = bpos(bi), pj = bpos(bj), di = bi <= npn ? 3 : 2, dj = bj <= npn ? 3 : 2;
     const Etype Ei = etype(bi), Ej = etype(bj);
     float M[3][3];
@@ -1692,16 +1696,13 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
   // --- J. write (Lambda', g', vbar') on the support without w, packed lower, canonical order
   {
     float* lam = rec + ly.o_lam;
-    for (int r = lane >> 5; r < s; r += TEAM / 32) {  // one packed row per warp at a time
-      if (r >= 3 && r < 6) continue;
-      const int R = r < 3 ? r : r - 3;
-      const float k0 = X[3 * r], k1 = X[3 * r + 1], k2 = X[3 * r + 2];
-      float* lrow = lam + (R * (R + 1) >> 1);
-      for (int q = lane & 31; q <= r; q += 32) {
-        if (q >= 3 && q < 6) continue;
-        const int Qn = q < 3 ? q : q - 3;
-        lrow[Qn] = Hs[tri(r, q)] - (k0 * Q[3 * q] + k1 * Q[3 * q + 1] + k2 * Q[3 * q + 2]);
-      }
+    // flat over the packed triangle of the new prior (support without w): coalesced stores, every lane busy
+    const int sr = s - 3, nout = sr * (sr + 1) >> 1;
+    int tp = tri_row(lane), tq = lane - (tp * (tp + 1) >> 1);
+    for (int t = lane; t < nout; t += TEAM) {
+      const int r = tp < 3 ? tp : tp + 3, q = tq < 3 ? tq : tq + 3;
+      lam[t] = Hs[tri(r, q)] - (X[3 * r] * Q[3 * q] + X[3 * r + 1] * Q[3 * q + 1] + X[3 * r + 2] * Q[3 * q + 2]);
+      tri_advance(tp, tq, TEAM);
     }
     for (int r = lane; r < s; r += TEAM) {
       if (r >= 3 && r < 6) continue;
