@@ -1575,7 +1575,10 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
   for (int p = lane; p < s; p += TEAM) {
     float q0 = 0.f, q1 = 0.f, q2 = 0.f;
     {
-      for (int q = 0; q < s; ++q) {
+      // the landmark rows of X are zero (landmarks are global: untouched by re-anchoring): only the anchor and
+      // pose columns of H_s contribute (the skipped terms are exact zeros)
+      const int sx = 3 + 3 * npn;
+      for (int q = 0; q < sx; ++q) {
         const float h = sym_get(Hs, p, q);
         q0 = fmaf(h, X[3 * q], q0); q1 = fmaf(h, X[3 * q + 1], q1); q2 = fmaf(h, X[3 * q + 2], q2);
       }
@@ -1600,6 +1603,8 @@ __device__ int marginalize(const Layout& ly, const Params& pr, float* rec, const
   const int npairs = nbk * (nbk + 1) >> 1;
   int bi = tri_row(lane), bj = lane - (bi * (bi + 1) >> 1);
   for (int t = lane; t < npairs; t += TEAM, tri_advance(bi, bj, TEAM)) {
+    // E is the identity for w (block 1) and for the landmarks: a pair of such blocks keeps its entries as they are
+    if ((bi == 1 || bi > npn) && (bj == 1 || bj > npn)) continue;
     const int pi = bpos(bi), pj = bpos(bj), di = bi <= npn ? 3 : 2, dj = bj <= npn ? 3 : 2;
     const Etype Ei = etype(bi), Ej = etype(bj);
     float M[3][3];
