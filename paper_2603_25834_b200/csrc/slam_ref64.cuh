@@ -325,12 +325,18 @@ __device__ void ref_assemble(const Layout& ly, const Params& pr, const Ctx& e, c
   // prior: H = Lambda on the support; b = -(Lambda d + g) read back from shared memory (no second pass over HBM)
   {
     const int st = e.s * (e.s + 1) / 2;
-    for (int t = tid; t < st; t += NT) {
-      int p = (int)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
-      while ((p + 1) * (p + 2) / 2 <= t) ++p;
-      while (p * (p + 1) / 2 > t) --p;
-      const int q = t - p * (p + 1) / 2;
-      Hat(H, s.pos[s.sidx[p]], s.pos[s.sidx[q]]) = ldr(e, ly.o_lam + t);
+    if (tid < st) {  // (row, column) of this thread's first entry by one square root, then advanced NT entries at a time
+      int p = (int)((sqrtf(8.0f * (float)tid + 1.0f) - 1.0f) * 0.5f);
+      while ((p + 1) * (p + 2) / 2 <= tid) ++p;
+      while (p * (p + 1) / 2 > tid) --p;
+      int q = tid - p * (p + 1) / 2;
+      for (int t = tid;;) {
+        Hat(H, s.pos[s.sidx[p]], s.pos[s.sidx[q]]) = ldr(e, ly.o_lam + t);
+        t += NT;
+        if (t >= st) break;
+        q += NT;
+        while (q > p) { q -= p + 1; ++p; }
+      }
     }
     __syncthreads();
     for (int p = tid; p < e.s; p += NT) {
@@ -569,7 +575,10 @@ __device__ void ref_assemble(const Layout& ly, const Params& pr, const Ctx& e, c
 __device__ int ref_cholesky(const Layout& ly, const Sm& s, int tid, real* ratio) {
   const int n = ly.n;
   real* H = s.H;
-  real* col4 = s.X;   // [n][4] (X and Q are contiguous: 6n doubles; only the marginalisation uses them as X, Q)
+  // L(i, j..j+3) of the active rows, component-major and compact: cmp[x * NC + position in the list] (X and Q are
+  // contiguous: 6n doubles; only the marginalisation uses them as X, Q)
+  real* cmp = s.X;
+  const int NC = (n + 3) & ~1;
   real* dinv = s.d;   // 1 / L_jj for the back substitution (the prior displacement is dead by now)
   int* act = s.omap;  // compact list of the rows that take part in the current block
   for (int p = tid; p < n; p += NT) {  // envelope: first non-zero of each row (fill stays inside it)
@@ -660,24 +669,41 @@ __device__ int ref_cholesky(const Layout& ly, const Sm& s, int tid, real* ratio)
         if (nb > 1) hp[1] = l1;
         if (nb > 2) hp[2] = l2;
         if (nb > 3) hp[3] = l3;
-        reinterpret_cast<double2*>(col4 + 4 * i)[0] = make_double2(l0, l1);
-        reinterpret_cast<double2*>(col4 + 4 * i)[1] = make_double2(l2, l3);
+        const int at = base + __popc(bal[ch] & ((1u << lane) - 1u));   // position in the compact list (ascending rows)
+        cmp[at] = l0; cmp[NC + at] = l1; cmp[2 * NC + at] = l2; cmp[3 * NC + at] = l3;
         s.b[i] -= l0 * sh_y[0] + l1 * sh_y[1] + l2 * sh_y[2] + l3 * sh_y[3];
-        act[base + __popc(bal[ch] & ((1u << lane) - 1u))] = i;
+        act[at] = i;
       }
     }
     __syncthreads();
     // rank-4 update of the trailing envelope, flat over the pairs (a >= b) of active rows
-    const int npair = m * (m + 1) >> 1;
-    for (int p = tid; p < npair; p += NT) {
-      int a = (int)((sqrtf(8.0f * (float)p + 1.0f) - 1.0f) * 0.5f);
-      if ((a + 1) * (a + 2) / 2 <= p) ++a;
-      if (a * (a + 1) / 2 > p) --a;
-      const int bq = p - (a * (a + 1) >> 1);
-      const int i = act[a], k = act[bq];
-      const double2 a01 = reinterpret_cast<const double2*>(col4 + 4 * i)[0], a23 = reinterpret_cast<const double2*>(col4 + 4 * i)[1];
-      const double2 b01 = reinterpret_cast<const double2*>(col4 + 4 * k)[0], b23 = reinterpret_cast<const double2*>(col4 + 4 * k)[1];
-      H[tri(i, k)] -= a01.x * b01.x + a01.y * b01.y + a23.x * b23.x + a23.y * b23.y;
+    // in 2 x 2 tiles of list positions (rows 2a, 2a+1 x columns 2b, 2b+1, b <= a): the eight loads of a tile are
+    // 128-bit, the row side a broadcast and the column side contiguous over the lanes (conflict-free), a quarter of
+    // the shared-memory traffic of one pair per thread (measured: the flat update was bound by the LSU, 24
+    // wavefronts per pair).  The (a, b) of this thread's first tile by one square root, then advanced NT tiles at a time.
+    const int m2 = (m + 1) >> 1, ntile = m2 * (m2 + 1) >> 1;
+    if (tid < ntile) {
+      int a = (int)((sqrtf(8.0f * (float)tid + 1.0f) - 1.0f) * 0.5f);
+      if ((a + 1) * (a + 2) / 2 <= tid) ++a;
+      if (a * (a + 1) / 2 > tid) --a;
+      int bq = tid - (a * (a + 1) >> 1);
+      for (int p = tid;;) {
+        const int ia = 2 * a, ib = 2 * bq;
+        const double2 A0 = *reinterpret_cast<const double2*>(cmp + ia), A1 = *reinterpret_cast<const double2*>(cmp + NC + ia);
+        const double2 A2 = *reinterpret_cast<const double2*>(cmp + 2 * NC + ia), A3 = *reinterpret_cast<const double2*>(cmp + 3 * NC + ia);
+        const double2 B0 = *reinterpret_cast<const double2*>(cmp + ib), B1 = *reinterpret_cast<const double2*>(cmp + NC + ib);
+        const double2 B2 = *reinterpret_cast<const double2*>(cmp + 2 * NC + ib), B3 = *reinterpret_cast<const double2*>(cmp + 3 * NC + ib);
+        const bool ra1 = ia + 1 < m, cb1 = ib + 1 < m;
+        const int i0 = act[ia], i1 = ra1 ? act[ia + 1] : 0, k0 = act[ib], k1 = cb1 ? act[ib + 1] : 0;
+        H[tri(i0, k0)] -= A0.x * B0.x + A1.x * B1.x + A2.x * B2.x + A3.x * B3.x;
+        if (ra1) H[tri(i1, k0)] -= A0.y * B0.x + A1.y * B1.x + A2.y * B2.x + A3.y * B3.x;
+        if (cb1 && bq < a) H[tri(i0, k1)] -= A0.x * B0.y + A1.x * B1.y + A2.x * B2.y + A3.x * B3.y;   // (above the diagonal when b == a)
+        if (ra1 && cb1) H[tri(i1, k1)] -= A0.y * B0.y + A1.y * B1.y + A2.y * B2.y + A3.y * B3.y;
+        p += NT;
+        if (p >= ntile) break;
+        bq += NT;
+        while (bq > a) { bq -= a + 1; ++a; }
+      }
     }
     __syncthreads();
   }
