@@ -36,7 +36,7 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
                  unsigned long long* stats, const int* __restrict__ perm, int* __restrict__ keys,
                  int* __restrict__ fb_list, int* __restrict__ fb_cnt) {
   extern __shared__ float4 smem4[];
-  __shared__ int s_env[16], s_need[16], s_off[16], s_new[16], s_ctl[2];
+  __shared__ int s_env[16], s_need[16], s_off[16], s_new[16], s_nxt[16], s_ctl[2];
   float* smem = reinterpret_cast<float*>(smem4);
   const int team = threadIdx.x / TEAM, lane = threadIdx.x % TEAM;
   const int LOCK = ly.lock;
@@ -82,9 +82,25 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
         live += s_env[t] >= 0;
       }
       s_ctl[0] = nk; s_ctl[1] = live;
+      // the environments of the NEXT round (if no team has to wait for pool space): their records are pulled
+      // into L2 by the bulk-copy engine while this round computes, see below
+      if (ly.pf_bytes > 0)
+        for (int t = 0; t < ly.wpc; ++t, ++nk) {
+          const long long idx = ((long long)(nk / ly.wpc) * gridDim.x + blockIdx.x) * ly.wpc + nk % ly.wpc;
+          s_nxt[t] = idx < ly.N ? perm[idx] : -1;
+        }
     }
     __syncthreads();
     if (s_ctl[1] == 0) break;
+    // Staging of the next environments' factors (north_star (c)): ONE cp.async.bulk.prefetch.L2 per team brings the
+    // live part of the next record (state, masks, measurements, prior mean / gradient and the head of the packed
+    // Lambda) from HBM into L2 a whole round (~0.3 ms) before load_env / assemble touch it; their first-touch
+    // DRAM round trips become L2 hits.  Not staged into shared memory: every KB of it is pool space, i.e.
+    // environments in flight (DESIGN.md section 12 has the measurement).
+    if (ly.pf_bytes > 0 && lane == 0 && s_nxt[team] >= 0) {
+      const float* nrec = state + (size_t)s_nxt[team] * ly.rec;
+      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(nrec), "r"(ly.pf_bytes) : "memory");
+    }
     if (!waiting) {
       env = s_env[team];
       // an environment whose state and prior live in the fp64 shadow record belongs to the fp64 path
@@ -659,6 +675,16 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   if (cudaGetDevice(&c->device) != cudaSuccess) { cudaGetLastError(); delete c; return SLAM_ECUDA; }
   { const char* e = getenv("SLAM_LOCK"); if (e) c->ly.lock = atoi(e); }
   { const char* e = getenv("SLAM_LCACHE"); if (e) c->ly.lcache = atoi(e); }
+  // bytes of the next round's records the step kernel prefetches into L2 (SLAM_PREFETCH=0 disables): everything up
+  // to the prior mean and gradient, plus the packed Lambda of a typical support (a third of the state)
+  {
+    const int s_typ = c->ly.n / 3 + 6;
+    long long b = 4ll * (c->ly.o_lam + s_typ * (s_typ + 1) / 2);
+    if (b > 4ll * c->ly.rec) b = 4ll * c->ly.rec;
+    c->ly.pf_bytes = (int)(b & ~15ll);
+    const char* e = getenv("SLAM_PREFETCH");
+    if (e) c->ly.pf_bytes = atoi(e) > 0 ? (atoi(e) == 1 ? c->ly.pf_bytes : (atoi(e) & ~15)) : 0;
+  }
   const WsPlan p = plan(c->ly);
   if (workspace_bytes < p.total) { delete c; return SLAM_EINVAL; }
   for (int k = 0; k < 3; ++k) {
