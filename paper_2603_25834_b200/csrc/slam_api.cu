@@ -236,171 +236,6 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
   }
 }
 
-// ------------------------------------------------------------------ free-running variant (one warp per environment)
-// EXPERIMENT (SLAM_FREERUN=1): the same per-environment phases without rounds.  Every warp takes
-// the next environment of the cost-ordered list from ONE queue for the whole grid (most expensive first:
-// longest-processing-time scheduling), learns its need in the symbolic phase, takes that many words from the CTA
-// pool and gives them back when the environment is stored.  No CTA barrier after the start.  Measured slower than
-// the lock-step rounds (3.25-3.38 against 2.52 ms per step on config 3): the fused kernel is ~220 KB of code, and
-// warps in different phases each stream their own copy of it (no_instruction 30-70 % of the warp samples).
-//   Pool allocator (shared memory, per CTA): a_off/a_size[t] = the block team t holds (size 0: none).  Requests
-// are served in ticket order (no starvation: the head of the line gets in at the latest when every other team has
-// finished, the pool holds a dense window); the ticket holder is the only one that allocates, with the whole warp:
-// lane t proposes the end of team t's block (lane wpc: offset 0) as the start, checks it against every block by
-// shuffles, the lowest proposal that fits wins (first fit, no internal fragmentation).  Giving back is one store of
-// a_size[t] = 0.  Which block an environment gets changes no bit of its result.
-__device__ __forceinline__ int pool_alloc(int* a_off, int* a_size, int* tick, int team, int wpc, int need, int pool, int lane,
-                                          unsigned long long* stats) {
-  int my = 0;
-  if (lane == 0) my = atomicAdd(tick, 1);
-  my = __shfl_sync(FULLMASK, my, 0);
-  bool waited = false;
-  for (;;) {
-    if (*reinterpret_cast<volatile int*>(tick + 1) == my) {
-      const int o = lane < wpc ? reinterpret_cast<volatile int*>(a_off)[lane] : 0;
-      const int sz = lane < wpc ? reinterpret_cast<volatile int*>(a_size)[lane] : 0;
-      const int cand = lane < wpc ? (sz > 0 ? o + sz : -1) : (lane == wpc ? 0 : -1);
-      bool ok = cand >= 0 && cand + need <= pool;
-      for (int u = 0; u < wpc; ++u) {
-        const int ou = __shfl_sync(FULLMASK, o, u), su = __shfl_sync(FULLMASK, sz, u);
-        if (su > 0 && cand < ou + su && ou < cand + need) ok = false;
-      }
-      int best = ok ? cand : 0x7fffffff;
-#pragma unroll
-      for (int d = 16; d > 0; d >>= 1) best = min(best, __shfl_xor_sync(FULLMASK, best, d));
-      if (best != 0x7fffffff) {
-        if (lane == 0) {
-          a_off[team] = best;
-          reinterpret_cast<volatile int*>(a_size)[team] = need;
-          __threadfence_block();
-          *reinterpret_cast<volatile int*>(tick + 1) = my + 1;
-          if (waited && stats) atomicAdd(stats + 3, 1ull);
-        }
-        __syncwarp();
-        return best;
-      }
-    }
-    waited = true;
-    __nanosleep(256);
-  }
-}
-__device__ __forceinline__ void pool_free(int* a_size, int team, int lane) {
-  __syncwarp();
-  if (lane == 0) { __threadfence_block(); reinterpret_cast<volatile int*>(a_size)[team] = 0; }
-}
-
-template <bool PAIRS, bool LM>
-__global__ void __launch_bounds__(SLAM_MAXTHREADS)
-slam_step_free_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flags, int iters, StepIO io,
-                      unsigned long long* stats, const int* __restrict__ perm, int* __restrict__ keys,
-                      int* __restrict__ fb_list, int* __restrict__ fb_cnt) {
-  constexpr int TEAM = 32;
-  extern __shared__ float4 smem4[];
-  __shared__ int a_off[16], a_size[16], a_tick[2];
-  float* smem = reinterpret_cast<float*>(smem4);
-  const int team = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  float* base = smem + (size_t)team * ly.team_words;
-  float* pool = smem + (size_t)ly.wpc * ly.team_words;
-  WS w = make_ws(ly, base);
-  Team<TEAM> tm;
-  tm.bar = 0;
-  tm.scr = base + ly.s_scr;
-  int* queue = reinterpret_cast<int*>(stats + 16);  // [0] next entry of the ordered list, [1] CTAs finished
-  const int nlin = iters + ((flags & F_COV) ? 1 : 0);
-  if (threadIdx.x < 16) { a_off[threadIdx.x] = 0; a_size[threadIdx.x] = 0; }
-  if (threadIdx.x < 2) a_tick[threadIdx.x] = 0;
-  __syncthreads();
-  for (;;) {
-    int idx = 0;
-    if (lane == 0) idx = atomicAdd(queue, 1);
-    idx = __shfl_sync(FULLMASK, idx, 0);
-    if (idx >= ly.N) break;
-    const int env = perm[idx];
-    float* rec = state + (size_t)env * ly.rec;
-    if (fb_list && reinterpret_cast<const int*>(rec)[ly.o_mode] != 0) {  // lives in the fp64 shadow record: fp64 path
-      if (lane == 0) fb_list[atomicAdd(fb_cnt, 1)] = env;
-      continue;
-    }
-    const int k0 = reinterpret_cast<const int*>(rec)[ly.o_k0];
-    const int head = (head_g + k0) % ly.W;
-    int cc = c - k0;
-    Masks mk;
-    load_env<TEAM>(ly, rec, w, tm, lane, head, cc, mk);
-    if (flags & F_OBS0) record_rb<TEAM>(ly, rec, w, tm, lane, env, head, 0, 0.f, 0.f, 0.f, io, mk);
-    if (flags & F_PUSH) cc = push_env<TEAM>(ly, rec, w, tm, lane, env, head, cc, io, mk);
-    const Ord od = make_ord(ly, w.rbm, cc);
-    const int s = build_support<TEAM>(ly, od, w, tm, lane, cc, mk.ps, mk.ls);
-    const bool do_marg = (flags & F_MARG) && k0 == 0;
-    int need = do_marg ? marg_need(ly, w, lane, cc, mk) : 0, total = 0;
-    if (nlin > 0) {
-      total = symbolic<TEAM>(ly, od, w, tm, lane, cc, mk, s);
-      need = max(need, total + reinterpret_cast<const int*>(tm.scr)[10]);
-      if (flags & F_COV) need = max(need, 272);
-      if (lane == 0) {
-        keys[env] = total;
-        if (stats) {
-          atomicMax(stats + 0, (unsigned long long)total);
-          atomicAdd(stats + 1, (unsigned long long)total);
-          atomicAdd(stats + 2, 1ull);
-        }
-      }
-    }
-    need = max((need + 3) & ~3, 4);
-    if (need > ly.pool) {  // (cannot happen: the pool holds a dense window)
-      if (lane == 0) reinterpret_cast<int*>(rec)[ly.o_status] |= 4;
-      continue;
-    }
-    const int off = pool_alloc(a_off, a_size, a_tick, team, ly.wpc, need, ly.pool, lane, stats);
-    w.H = pool + off;
-    w.amask = reinterpret_cast<uint32_t*>(w.H + total);
-    int status = 0;
-    if (nlin > 0) {
-      build_lists<TEAM>(ly, w, tm, lane);
-#pragma unroll 1
-      for (int it = 0; it < nlin; ++it) {
-        const int ncb = (LM && it > 0 && ly.lcache) ? od.npas >> 1 : 0;
-        assemble<TEAM>(ly, pr, od, rec, w, tm, lane, head, cc, mk, s, total, 4 * ncb);
-        tm.sync();
-        status |= cholesky<TEAM, PAIRS, LM>(ly, w, tm, lane, ncb);
-        if (it < iters) {
-          back_substitute<TEAM, PAIRS>(ly, w, tm, lane);
-          status |= apply_update<TEAM>(ly, od, w, tm, lane, cc, mk);
-        } else {
-          covariance<TEAM>(ly, w, tm, lane, env, cc, io);
-          tm.sync();
-        }
-      }
-    }
-    bool redo = false;
-    if (fb_list && nlin > 0) {
-      redo = tm.any(status != 0, lane);
-      if (redo && lane == 0) fb_list[atomicAdd(fb_cnt, 1)] = env;
-    }
-    if (!redo) {
-      status &= ~ENV_ILLCOND;
-      if (io.last_pose && lane == 0) {
-        float sn, cn;
-        sincos_pi(w.st[2], &sn, &cn);
-        const float* e = w.st + st_pose(cc - 1);
-        io.last_pose[env] = w.st[0] + cn * e[0] - sn * e[1];
-        io.last_pose[(size_t)ly.N + env] = w.st[1] + sn * e[0] + cn * e[1];
-        io.last_pose[2 * (size_t)ly.N + env] = wrapf(w.st[2] + e[2]);
-      }
-      if (do_marg) status |= marginalize<TEAM>(ly, pr, rec, w, tm, lane, head, cc, mk, s);
-      else if ((flags & F_MARG) && lane == 0) reinterpret_cast<int*>(rec)[ly.o_k0] = k0 - 1;
-      store_state<TEAM>(ly, rec, w, tm, lane, head, cc, mk);
-      if (status && lane == 0) atomicOr(reinterpret_cast<int*>(rec) + ly.o_status, status);
-    }
-    pool_free(a_size, team, lane);
-  }
-  // the last CTA to leave rewinds the queue for the next launch
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    __threadfence();
-    if (atomicAdd(queue + 1, 1) == (int)gridDim.x - 1) { queue[0] = 0; queue[1] = 0; __threadfence(); }
-  }
-}
-
 // Cost order of the environments for the next launches: counting sort of keys[] (envelope words of the
 // last solve, a good predictor of this step's cost: the window slides by one pose) into perm[], most
 // expensive first.  One CTA.  Keys cluster (many environments share an envelope size), so lanes with the
@@ -739,15 +574,10 @@ template <bool PAIRS, bool LM>
 }
 // One instantiation per (team size, envelope rows in pairs, window has landmarks): the pose-only kernels
 // carry no code for cached landmark columns, the fours kernels none for split dot products.
-static step_fn kernel_of(int team, int pairs, int landmarks, int freerun = 0) {
+static step_fn kernel_of(int team, int pairs, int landmarks) {
 #ifdef SLAM_DEV_SINGLE   // developer build (compiles in a fifth of the time): only the kernels of BASELINE configs 3 and 4
-  if (freerun) return landmarks ? slam_step_free_kernel<false, true> : slam_step_free_kernel<true, false>;
   return landmarks ? slam_step_kernel<32, false, true> : slam_step_kernel<32, true, false>;
 #else
-  if (team == 32 && freerun) {
-    if (pairs) return landmarks ? slam_step_free_kernel<true, true> : slam_step_free_kernel<true, false>;
-    return landmarks ? slam_step_free_kernel<false, true> : slam_step_free_kernel<false, false>;
-  }
   if (pairs) return landmarks ? kernel_pick<true, true>(team) : kernel_pick<true, false>(team);
   return landmarks ? kernel_pick<false, true>(team) : kernel_pick<false, false>(team);
 #endif
@@ -774,8 +604,6 @@ static bool pick_layout(int batch, int window, int landmarks, Layout* out) {
   *out = make_layout(batch, window, landmarks, pool, wpc);
   out->team = team;
   out->pairs = pairs;
-  // SLAM_FREERUN=1: the free-running experiment kernel (one warp per environment only)
-  { const char* e = getenv("SLAM_FREERUN"); out->freerun = team == 32 && e && e[0] == '1'; }
   return true;
 }
 
@@ -904,7 +732,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
     return SLAM_ECUDA;
   }
   c->smem_bytes = (c->ly.team_words * wpc + c->ly.pool) * 4;
-  if (cudaFuncSetAttribute(kernel_of(team, c->ly.pairs, c->ly.L, c->ly.freerun), cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET) != cudaSuccess) {
+  if (cudaFuncSetAttribute(kernel_of(team, c->ly.pairs, c->ly.L), cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET) != cudaSuccess) {
     cudaGetLastError();
     delete c;
     return SLAM_ECUDA;
@@ -912,7 +740,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   int dev = 0, sms = 0, occ = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel_of(team, c->ly.pairs, c->ly.L, c->ly.freerun), wpc * team, c->smem_bytes);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel_of(team, c->ly.pairs, c->ly.L), wpc * team, c->smem_bytes);
   if (occ < 1 || sms < 1) { cudaGetLastError(); delete c; return SLAM_ECUDA; }
   c->ctas_per_sm = occ;
   const int need = (batch + wpc - 1) / wpc;
@@ -956,7 +784,7 @@ int slam_reset(slam_ctx* c, const float* init_pose) {
 
 static int launch_step(slam_ctx* c, int flags, int iters, const StepIO& io) {
   DevGuard dg(c);
-  const step_fn fn = kernel_of(c->ly.team, c->ly.pairs, c->ly.L, c->ly.freerun);
+  const step_fn fn = kernel_of(c->ly.team, c->ly.pairs, c->ly.L);
   cudaEvent_t* tv = (c->tev && c->tev_steps < c->tev_cap) ? c->tev + 4 * c->tev_steps : nullptr;
   if (tv) cudaEventRecord(tv[0], c->stream);
   if (c->precision == 2) {   // device reference: every environment through the fp64 path
