@@ -92,11 +92,11 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
     }
     __syncthreads();
     if (s_ctl[1] == 0) break;
-    // Staging of the next environments' factors (north_star (c)): ONE cp.async.bulk.prefetch.L2 per team brings the
-    // live part of the next record (state, masks, measurements, prior mean / gradient and the head of the packed
-    // Lambda) from HBM into L2 a whole round (~0.3 ms) before load_env / assemble touch it; their first-touch
-    // DRAM round trips become L2 hits.  Not staged into shared memory: every KB of it is pool space, i.e.
-    // environments in flight (DESIGN.md section 12 has the measurement).
+    // Staging of the next environments' factors (north_star (c); an experiment switch, off by default): ONE
+    // cp.async.bulk.prefetch.L2 per team brings the live part of the next record (state, masks, measurements, prior
+    // mean / gradient and the head of the packed Lambda) from HBM into L2 a whole round (~0.3 ms) before load_env /
+    // assemble touch it.  Not staged into shared memory: every KB of it is pool space, i.e. environments in flight
+    // (DESIGN.md section 12 has the measurement).
     if (ly.pf_bytes > 0 && lane == 0 && s_nxt[team] >= 0) {
       const float* nrec = state + (size_t)s_nxt[team] * ly.rec;
       asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(nrec), "r"(ly.pf_bytes) : "memory");
@@ -675,15 +675,17 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   if (cudaGetDevice(&c->device) != cudaSuccess) { cudaGetLastError(); delete c; return SLAM_ECUDA; }
   { const char* e = getenv("SLAM_LOCK"); if (e) c->ly.lock = atoi(e); }
   { const char* e = getenv("SLAM_LCACHE"); if (e) c->ly.lcache = atoi(e); }
-  // bytes of the next round's records the step kernel prefetches into L2 (SLAM_PREFETCH=0 disables): everything up
-  // to the prior mean and gradient, plus the packed Lambda of a typical support (a third of the state)
+  // Bytes of the next round's records the step kernel prefetches into L2.  OFF by default: measured -0.4 % on the
+  // step kernel for +45 % DRAM traffic and no drop of the long-scoreboard share.
+  // SLAM_PREFETCH=1: everything up to the prior mean and gradient plus the packed Lambda of a typical support (a
+  // third of the state); SLAM_PREFETCH=<bytes>: that many.
   {
     const int s_typ = c->ly.n / 3 + 6;
     long long b = 4ll * (c->ly.o_lam + s_typ * (s_typ + 1) / 2);
     if (b > 4ll * c->ly.rec) b = 4ll * c->ly.rec;
-    c->ly.pf_bytes = (int)(b & ~15ll);
     const char* e = getenv("SLAM_PREFETCH");
-    if (e) c->ly.pf_bytes = atoi(e) > 0 ? (atoi(e) == 1 ? c->ly.pf_bytes : (atoi(e) & ~15)) : 0;
+    const int v = e ? atoi(e) : 0;
+    c->ly.pf_bytes = v <= 0 ? 0 : (v == 1 ? (int)(b & ~15ll) : (int)((v < 4ll * c->ly.rec ? v : 4ll * c->ly.rec) & ~15ll));
   }
   const WsPlan p = plan(c->ly);
   if (workspace_bytes < p.total) { delete c; return SLAM_EINVAL; }

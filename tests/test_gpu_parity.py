@@ -357,7 +357,7 @@ def test_results_do_not_depend_on_capacity_or_team(monkeypatch):
     assert np.array_equal(a["cov"], b["cov"]) and np.array_equal(a["logdet"], b["logdet"])
     assert (b["status"] == 0).all()
     monkeypatch.delenv("SLAM_POOL_FRAC")
-    monkeypatch.setenv("SLAM_PREFETCH", "0")              # the L2 bulk prefetch of the next round's records is a hint only
+    monkeypatch.setenv("SLAM_PREFETCH", "1")              # the L2 bulk prefetch of the next round's records is a hint only
     p0 = run_gpu(_slam(cfg.N, cfg.W, cfg.L), data, cfg.iters, fused=True, want_poses=False)
     assert np.array_equal(a["cov"], p0["cov"]) and np.array_equal(a["logdet"], p0["logdet"])
     monkeypatch.delenv("SLAM_PREFETCH")
