@@ -457,6 +457,7 @@ struct slam_ctx {
   int precision;              // 0: fp32 only, 1: fp32 with fp64 fallback on ill-conditioned windows, 2: fp64 everywhere
   bool precision_auto;        // the default rule decides (landmarks or unary factors -> 1, else 0)
   float ratio_hi, ratio_lo;
+  int min_vis;                // landmarks the newest pose must see before an fp64 environment goes back to fp32
   int ref_grid, ref_smem;
   bool order, order_all;      // re-sort after every solve (SLAM_ORDER=0 disables, 2: pose-only windows too)
   // device staging for slam_step_host
@@ -726,6 +727,9 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   c->precision_auto = true;
   c->precision = landmarks > 0 ? 1 : 0;
   c->ratio_hi = 300.f; c->ratio_lo = 150.f;
+  c->min_vis = 3;
+  { const char* e = getenv("SLAM_MIN_VIS"); if (e) c->min_vis = atoi(e); }
+  { const char* e = getenv("SLAM_RATIO_HI"); if (e && atof(e) > 0) c->ratio_hi = (float)atof(e); e = getenv("SLAM_RATIO_LO"); if (e && atof(e) > 0) c->ratio_lo = (float)atof(e); }
   { const char* e = getenv("SLAM_PRECISION"); if (e && e[0] >= '0' && e[0] <= '2') { c->precision = e[0] - '0'; c->precision_auto = false; } }
   c->ref_smem = (int)(ref_small_bytes(c->ly) + (c->hglob ? 0 : slamr::ref_tri(c->ly) * 8));
   if (cudaFuncSetAttribute(slamr::slam_ref64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET) != cudaSuccess) {
@@ -804,7 +808,7 @@ static int launch_step(slam_ctx* c, int flags, int iters, const StepIO& io) {
   if (tv) cudaEventRecord(tv[1], c->stream);
   if (c->precision >= 1) {   // the environments the fp32 kernel queued: fp64 records, and the windows it refused to commit
     slamr::RefArgs ra = {c->state, c->state64, c->head, c->count, flags, iters, c->fb_list, c->fb_cnt, c->stats, c->hglob,
-                         (double)c->ratio_lo, c->precision == 2 ? 1 : 0};
+                         (double)c->ratio_lo, c->precision == 2 ? 1 : 0, c->min_vis};
 #ifdef SLAM_REF_PROFILE
     cudaMemcpyToSymbolAsync(slamr::g_ref_prof, &c->stats, sizeof(c->stats), 0, cudaMemcpyHostToDevice, c->stream);
 #endif

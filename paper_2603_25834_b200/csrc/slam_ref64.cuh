@@ -50,6 +50,7 @@ struct RefArgs {
   double* hglob;      // packed H per CTA when it does not fit shared memory (else nullptr)
   double ratio_lo;    // back to fp32 below this anchor pivot ratio
   int force;          // 1: every environment stays in fp64 (device reference)
+  int min_vis;        // landmarks the newest pose must see for the hand-over back to fp32
 };
 
 // shared-memory views of one environment
@@ -1156,7 +1157,15 @@ __global__ void __launch_bounds__(NT, 3) slam_ref64_kernel(Layout ly, Params pr,
     }
     // precision mode of the record after this call: fp64 while the anchor pivots cancel, back to fp32 below ratio_lo
     int newmode = e.mode;
-    if (nlin > 0) newmode = (ratio < ra.ratio_lo && status == 0) ? 0 : 1;
+    // Back to fp32 only while the robot is localised against the map: the newest pose must see at least `min_vis`
+    // landmarks.  A robot that leaves the map right after the hand-over dead-reckons on a prior whose landmark and
+    // anchor blocks still carry the cancellation of the ill-conditioned phase; fp32 marginalisations lose it within
+    // tens of steps although the anchor pivots look harmless (measured: 18 of the 21 env-steps beyond tolerance of a
+    // 4096-environment sample of config 3).
+    if (nlin > 0) {
+      const int nvis = ly.L > 0 ? __popcll(vis_of(ly, s, e.c - 1)) : 0;
+      newmode = (ratio < ra.ratio_lo && status == 0 && (ly.L == 0 || nvis >= ra.min_vis)) ? 0 : 1;
+    }
     if (ra.force) newmode = 1;
     const bool do_marg = (ra.flags & slamk::F_MARG) && e.k0 == 0;
     if (do_marg) ref_marginalize(ly, pr, e, s, tid, newmode);

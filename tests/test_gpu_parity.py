@@ -39,7 +39,7 @@ def _fused_equals_separate(cfg, data, ref=None):
         _check(b, ref, what=("cov", "logdet"))
 
 
-def _check(gpu, ref, what=("poses", "last_pose", "cov", "logdet"), det=None):
+def _check(gpu, ref, what=("poses", "last_pose", "cov", "logdet"), det=None, min_determined=0.999):
     """Every (step, env) must be within the stated tolerances R23 (error <= 1.0 in tolerance units).  `det` (config 3
     only): the env-steps the ORACLE itself determines (tests/helpers.determined: its outputs do not move when one
     input changes by one float32 ulp); at least 99.9 % must be, the others are not compared.
@@ -53,7 +53,7 @@ def _check(gpu, ref, what=("poses", "last_pose", "cov", "logdet"), det=None):
     G = np.max([err[k] for k in keys], axis=0)
     assert np.isfinite(G).all()
     if det is not None:
-        assert det.mean() >= 0.999, f"only {det.mean():.5f} of the env-steps are determined by the oracle"
+        assert det.mean() >= min_determined, f"only {det.mean():.5f} of the env-steps are determined by the oracle"
         G = np.where(det, G, 0.0)
     worst = float(G.max())
     assert worst <= 1.0, f"{worst:.3g} x tolerance at (step, env) {np.unravel_index(G.argmax(), G.shape)}: " + \
@@ -139,14 +139,14 @@ def test_noise_free_recovers_ground_truth():
         assert np.abs(err).max() < 2e-4 * max(1.0, np.abs(gt).max())
 
 
-def _full_config(cfg, n_sample, steps=None, check_determined=False):
+def _full_config(cfg, n_sample, steps=None, check_determined=False, extra_envs=(), min_determined=0.999):
     """The FULL batch in the launch configuration bench.py times (fused slam_step, default precision), compared on
     `n_sample` environments spread over the batch: newest pose (`last_pose`), covariance and ln det at every
     step, the whole window (slam_get_poses) after the last step; and, on EVERY environment, properties that hold at
     any size."""
     data = synth.generate(cfg, steps=steps)
     T = data["T"]
-    envs = np.unique(np.linspace(0, cfg.N - 1, n_sample).astype(np.int32))
+    envs = np.unique(np.concatenate([np.linspace(0, cfg.N - 1, n_sample), np.asarray(extra_envs, dtype=np.float64)]).astype(np.int32))
     ref = oracle.run_batch(data, cfg.iters, envs=envs)
     assert ref["bad"] == 0
     det = determined(oracle, data, cfg.iters, envs, ref) if check_determined else None
@@ -154,7 +154,7 @@ def _full_config(cfg, n_sample, steps=None, check_determined=False):
     gpu = run_gpu(slam, data, cfg.iters, fused=True, want_poses=False)
     assert (gpu["status"] == 0).all()
     assert np.isfinite(gpu["cov"]).all() and np.isfinite(gpu["logdet"]).all() and np.isfinite(gpu["last_pose"]).all()
-    _check(_sub(gpu, envs), ref, what=("last_pose", "cov", "logdet"), det=det)
+    _check(_sub(gpu, envs), ref, what=("last_pose", "cov", "logdet"), det=det, min_determined=min_determined)
     _window_after_step(slam, ref, T, envs, det)
     S = gpu["cov"]
     assert np.array_equal(S, S.transpose(0, 1, 3, 2))
@@ -177,7 +177,7 @@ def test_config3_full_size_sampled_envs():
     cfg = synth.CONFIGS[3]
     slam, data, envs, ref, gpu = _full_config(cfg, 256, check_determined=True)
     st = slam.get_stats()
-    assert 0 < st["fp64_calls"] < 0.10 * cfg.N * cfg.T, st     # a few percent of the env-steps (measured: 4.4 %)
+    assert 0 < st["fp64_calls"] < 0.15 * cfg.N * cfg.T, st     # a few percent of the env-steps (measured: 7.7 %)
     # landmarks: the read-out against the oracle's (single environments driven step by step)
     lm, act = slam.get_landmarks()
     lm, act = lm.cpu().numpy(), act.cpu().numpy().view(np.uint32)
@@ -191,6 +191,18 @@ def test_config3_full_size_sampled_envs():
         assert np.array_equal(gact, oact)
         d = np.abs(lm[:, :, env].T - olm)
         assert d.max() <= 1e-4 * max(1.0, np.abs(olm).max()), (env, d.max())
+
+
+def test_config3_environments_that_come_back_from_fp64():
+    """Environments that re-observe a landmark after dead reckoning (the fp64 kernel takes them), lose sight of the
+    map again and dead-reckon on: found on a 4096-environment sample of config 3 as the env-steps where a hand-over
+    back to fp32 by the pivot ratio alone went beyond tolerance tens of steps later (up to 2.0 x in ln det).  With
+    the rule of slam_ref64_kernel -- back to fp32 only while the newest pose sees at least three landmarks -- they
+    hold the stated tolerances on every env-step the oracle determines, like everybody else.  (The sample is
+    hand-picked for trouble, so fewer of its env-steps are determined than of a uniform sample: measured 98.3 %.)"""
+    cfg = synth.CONFIGS[3]
+    found = (11512, 2132, 16216, 12552, 4140, 10608, 852, 16156, 7592, 11540, 6584, 15300)
+    _full_config(cfg, 32, check_determined=True, extra_envs=found, min_determined=0.97)
 
 
 @pytest.mark.parametrize("N,n_sample,steps", [(256, 64, 70), (16384, 128, None), (65536, 64, 70)])
