@@ -184,7 +184,10 @@ int slam_reward(slam_ctx* ctx, const slam_reward_params* p, const float* u, cons
  * and is left to the caller, see slam_set_unary).  Ties go to the lowest candidate index.
  * slam_grid_update: every valid ray of the scan taken at `pose` [3][N] adds -l_free*weight to the cells it
  * crosses (Amanatides-Woo traversal) and +l_occ*weight to its end cell; then the grid is clamped to
- * [-l_clamp, l_clamp].  weight [N] = the confidence (e.g. the match score). */
+ * [-l_clamp, l_clamp].  weight [N] = the confidence (e.g. the match score).
+ * The sums are accumulated with fp32 atomic adds, one per (ray, cell): the ORDER of the additions to a cell varies
+ * from run to run, so a cell crossed by several rays can differ in the last bit between two runs (the cells a ray
+ * crosses are integer decisions taken in fp64 and do not vary).  Everything else in this header is deterministic. */
 typedef struct {
   int G; float res; int R; float r_min, r_max; int hx, hy, ht; float sxy, sth;
 } slam_scan_params;
