@@ -567,13 +567,67 @@ __device__ void ref_assemble(const Layout& ly, const Params& pr, const Ctx& e, c
 }
 
 // ------------------------------------------------------------------ Cholesky (right-looking, blocks of 4 columns)
-// Per block: the first warp factorises the 4x4 diagonal tile (and the rhs entries of the block) in registers and
-// publishes it; the rows with entries in the block scale their four entries (kept in col4 for the others) and are
-// gathered in a compact list; the rank-4 update of the trailing envelope runs flat over the pairs of that list.
-// Two barriers per block.  On exit H holds L (diagonal = L_jj), b holds y = L^{-1} b, s.d holds 1 / L_jj.
+// Per block: the rows with entries in the block scale their four entries with the block's factorised 4x4 tile and
+// are gathered in a compact list; the rank-4 update of the trailing envelope runs over 2x2 tiles of that list.
+// LOOK-AHEAD: while warps 1.. update the trailing envelope, the first warp applies the update to the NEXT block's
+// diagonal tile (the pairs among the first four list entries), factorises it (and the rhs entries of that block)
+// in registers and publishes it in the other of two buffers -- the four dependent fp64 rsqrt of a tile (~700 cycles)
+// are off the critical path, and a block costs two CTA barriers instead of three.
+// On exit H holds L (diagonal = L_jj), b holds y = L^{-1} b, s.d holds 1 / L_jj.
 // Returns status bits; *ratio = max over the anchor rows of H_ii / L_ii^2 (the cancellation the fp32 kernel
 // cannot afford).
+struct RefTile { real t[4][4], ti[4], y[4]; };
+
+// first warp: factorise the tile of block j (nb columns), identity-padded when nb < 4 (every lane the same arithmetic)
+__device__ __forceinline__ int ref_factor_tile(real* H, real* b, real* dinv, int j, int nb, int lane, RefTile* out) {
+  real t[4][4], y[4], ti[4];
+  int flag = 0;
+#pragma unroll
+  for (int x = 0; x < 4; ++x) {
+#pragma unroll
+    for (int c = 0; c < 4; ++c) t[x][c] = (x < nb && c <= x) ? H[tri(j + x, j + c)] : (x == c ? 1.0 : 0.0);
+    y[x] = x < nb ? b[j + x] : 0.0;
+  }
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    real piv = t[c][c];
+#pragma unroll
+    for (int k = 0; k < c; ++k) piv -= t[c][k] * t[c][k];
+    if (!(piv > 0.0)) { flag |= slamk::ENV_NOT_PD; piv = 1.0; }
+    const real inv = rsqrt(piv);
+    t[c][c] = piv * inv; ti[c] = inv;
+#pragma unroll
+    for (int x = c + 1; x < 4; ++x) {
+      real v = t[x][c];
+#pragma unroll
+      for (int k = 0; k < c; ++k) v -= t[x][k] * t[c][k];
+      t[x][c] = v * inv;
+    }
+    real yy = y[c];
+#pragma unroll
+    for (int k = 0; k < c; ++k) yy -= t[c][k] * y[k];
+    y[c] = yy * inv;
+  }
+  __syncwarp();   // every lane has read the tile before lane 0 overwrites it
+  if (lane == 0) {
+#pragma unroll
+    for (int x = 0; x < 4; ++x) {
+#pragma unroll
+      for (int c = 0; c < 4; ++c) out->t[x][c] = t[x][c];
+      out->ti[x] = ti[x]; out->y[x] = y[x];
+      if (x < nb) {
+#pragma unroll
+        for (int c = 0; c <= x; ++c) H[tri(j + x, j + c)] = t[x][c];
+        b[j + x] = y[x];
+        dinv[j + x] = ti[x];
+      }
+    }
+  }
+  return flag;
+}
+
 __device__ int ref_cholesky(const Layout& ly, const Sm& s, int tid, real* ratio) {
+  static_assert(NT >= 64, "the look-ahead needs a second warp");
   const int n = ly.n;
   real* H = s.H;
   // L(i, j..j+3) of the active rows, component-major and compact: cmp[x * NC + position in the list] (X and Q are
@@ -592,65 +646,30 @@ __device__ int ref_cholesky(const Layout& ly, const Sm& s, int tid, real* ratio)
   for (int x = 0; x < 3; ++x) ha[x] = H[tri(n - 3 + x, n - 3 + x)];
   int flag = 0;
   __shared__ int sh_cnt[3][NT / 32];   // active rows per (chunk of NT rows, warp)
-  __shared__ real sh_t[4][4], sh_ti[4], sh_y[4];
+  __shared__ RefTile sh_tile[2];       // the current block's factorised tile and the next one's (look-ahead)
   __shared__ int sh_flag;
   const int lane = tid & 31, wid = tid >> 5;
   __syncthreads();
-  for (int j = 0; j < n; j += 4) {
-    const int nb = n - j < 4 ? n - j : 4, r0 = j + nb;
-    // rows below the block that have entries in it (first < r0): ballots now, list after the barrier
-    unsigned bal[3];
+  // rows below block [j, r0) that have entries in it (first < r0): ballots for the list of the rows phase
+  unsigned bal[3];
+  auto ballots = [&](int r0) {
 #pragma unroll
     for (int ch = 0; ch < 3; ++ch) {
       const int i = r0 + ch * NT + tid;
       bal[ch] = __ballot_sync(0xffffffffu, i < n && s.first[i] < r0);
       if (lane == 0) sh_cnt[ch][wid] = __popc(bal[ch]);
     }
-    if (wid == 0) {   // diagonal tile, identity-padded when nb < 4 (every lane the same arithmetic)
-      real t[4][4], y[4], ti[4];
-#pragma unroll
-      for (int x = 0; x < 4; ++x) {
-#pragma unroll
-        for (int c = 0; c < 4; ++c) t[x][c] = (x < nb && c <= x) ? H[tri(j + x, j + c)] : (x == c ? 1.0 : 0.0);
-        y[x] = x < nb ? s.b[j + x] : 0.0;
-      }
-#pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        real piv = t[c][c];
-#pragma unroll
-        for (int k = 0; k < c; ++k) piv -= t[c][k] * t[c][k];
-        if (!(piv > 0.0)) { flag |= slamk::ENV_NOT_PD; piv = 1.0; }
-        const real inv = rsqrt(piv);
-        t[c][c] = piv * inv; ti[c] = inv;
-#pragma unroll
-        for (int x = c + 1; x < 4; ++x) {
-          real v = t[x][c];
-#pragma unroll
-          for (int k = 0; k < c; ++k) v -= t[x][k] * t[c][k];
-          t[x][c] = v * inv;
-        }
-        real yy = y[c];
-#pragma unroll
-        for (int k = 0; k < c; ++k) yy -= t[c][k] * y[k];
-        y[c] = yy * inv;
-      }
-      __syncwarp();   // every lane has read the tile before lane 0 overwrites it
-      if (lane == 0) {
-#pragma unroll
-        for (int x = 0; x < 4; ++x) {
-#pragma unroll
-          for (int c = 0; c < 4; ++c) sh_t[x][c] = t[x][c];
-          sh_ti[x] = ti[x]; sh_y[x] = y[x];
-          if (x < nb) {
-#pragma unroll
-            for (int c = 0; c <= x; ++c) H[tri(j + x, j + c)] = t[x][c];
-            s.b[j + x] = y[x];
-            dinv[j + x] = ti[x];
-          }
-        }
-      }
-    }
-    __syncthreads();
+  };
+  {
+    const int nb0 = n < 4 ? n : 4;
+    ballots(nb0);
+    if (wid == 0) flag |= ref_factor_tile(H, s.b, dinv, 0, nb0, lane, &sh_tile[0]);
+  }
+  __syncthreads();
+  int cur = 0;
+  for (int j = 0; j < n; j += 4, cur ^= 1) {
+    const int nb = n - j < 4 ? n - j : 4, r0 = j + nb;
+    const RefTile& T = sh_tile[cur];
     // active rows: L(i, j..j+3) by forward substitution with the tile; the rhs rides along
     int m = 0;
 #pragma unroll
@@ -661,51 +680,71 @@ __device__ int ref_cholesky(const Layout& ly, const Sm& s, int tid, real* ratio)
       if ((bal[ch] >> lane) & 1u) {
         const int i = r0 + ch * NT + tid;
         real* hp = H + tri(i, j);
-        const real l0 = hp[0] * sh_ti[0];
+        const real l0 = hp[0] * T.ti[0];
         real l1 = 0.0, l2 = 0.0, l3 = 0.0;
-        if (nb > 1) l1 = (hp[1] - l0 * sh_t[1][0]) * sh_ti[1];
-        if (nb > 2) l2 = (hp[2] - l0 * sh_t[2][0] - l1 * sh_t[2][1]) * sh_ti[2];
-        if (nb > 3) l3 = (hp[3] - l0 * sh_t[3][0] - l1 * sh_t[3][1] - l2 * sh_t[3][2]) * sh_ti[3];
+        if (nb > 1) l1 = (hp[1] - l0 * T.t[1][0]) * T.ti[1];
+        if (nb > 2) l2 = (hp[2] - l0 * T.t[2][0] - l1 * T.t[2][1]) * T.ti[2];
+        if (nb > 3) l3 = (hp[3] - l0 * T.t[3][0] - l1 * T.t[3][1] - l2 * T.t[3][2]) * T.ti[3];
         hp[0] = l0;
         if (nb > 1) hp[1] = l1;
         if (nb > 2) hp[2] = l2;
         if (nb > 3) hp[3] = l3;
         const int at = base + __popc(bal[ch] & ((1u << lane) - 1u));   // position in the compact list (ascending rows)
         cmp[at] = l0; cmp[NC + at] = l1; cmp[2 * NC + at] = l2; cmp[3 * NC + at] = l3;
-        s.b[i] -= l0 * sh_y[0] + l1 * sh_y[1] + l2 * sh_y[2] + l3 * sh_y[3];
+        s.b[i] -= l0 * T.y[0] + l1 * T.y[1] + l2 * T.y[2] + l3 * T.y[3];
         act[at] = i;
       }
     }
     __syncthreads();
-    // rank-4 update of the trailing envelope, flat over the pairs (a >= b) of active rows
-    // in 2 x 2 tiles of list positions (rows 2a, 2a+1 x columns 2b, 2b+1, b <= a): the eight loads of a tile are
-    // 128-bit, the row side a broadcast and the column side contiguous over the lanes (conflict-free), a quarter of
-    // the shared-memory traffic of one pair per thread (measured: the flat update was bound by the LSU, 24
-    // wavefronts per pair).  The (a, b) of this thread's first tile by one square root, then advanced NT tiles at a time.
+    // rank-4 update of the trailing envelope in 2 x 2 tiles of list positions (rows 2a, 2a+1 x columns 2b, 2b+1,
+    // b <= a): the eight loads of a tile are 128-bit, the row side a broadcast and the column side contiguous over the
+    // lanes (conflict-free), a quarter of the shared-memory traffic of one pair per thread (measured: a flat update
+    // was bound by the LSU, 24 wavefronts per pair).
     const int m2 = (m + 1) >> 1, ntile = m2 * (m2 + 1) >> 1;
-    if (tid < ntile) {
-      int a = (int)((sqrtf(8.0f * (float)tid + 1.0f) - 1.0f) * 0.5f);
-      if ((a + 1) * (a + 2) / 2 <= tid) ++a;
-      if (a * (a + 1) / 2 > tid) --a;
-      int bq = tid - (a * (a + 1) >> 1);
-      for (int p = tid;;) {
-        const int ia = 2 * a, ib = 2 * bq;
-        const double2 A0 = *reinterpret_cast<const double2*>(cmp + ia), A1 = *reinterpret_cast<const double2*>(cmp + NC + ia);
-        const double2 A2 = *reinterpret_cast<const double2*>(cmp + 2 * NC + ia), A3 = *reinterpret_cast<const double2*>(cmp + 3 * NC + ia);
-        const double2 B0 = *reinterpret_cast<const double2*>(cmp + ib), B1 = *reinterpret_cast<const double2*>(cmp + NC + ib);
-        const double2 B2 = *reinterpret_cast<const double2*>(cmp + 2 * NC + ib), B3 = *reinterpret_cast<const double2*>(cmp + 3 * NC + ib);
-        const bool ra1 = ia + 1 < m, cb1 = ib + 1 < m;
-        const int i0 = act[ia], i1 = ra1 ? act[ia + 1] : 0, k0 = act[ib], k1 = cb1 ? act[ib + 1] : 0;
-        H[tri(i0, k0)] -= A0.x * B0.x + A1.x * B1.x + A2.x * B2.x + A3.x * B3.x;
-        if (ra1) H[tri(i1, k0)] -= A0.y * B0.x + A1.y * B1.x + A2.y * B2.x + A3.y * B3.x;
-        if (cb1 && bq < a) H[tri(i0, k1)] -= A0.x * B0.y + A1.x * B1.y + A2.x * B2.y + A3.x * B3.y;   // (above the diagonal when b == a)
-        if (ra1 && cb1) H[tri(i1, k1)] -= A0.y * B0.y + A1.y * B1.y + A2.y * B2.y + A3.y * B3.y;
-        p += NT;
-        if (p >= ntile) break;
-        bq += NT;
-        while (bq > a) { bq -= a + 1; ++a; }
+    if (wid == 0) {
+      // look-ahead: the list is ascending, so the rows of the next block that are in it are among its first four
+      // entries; the pairs among those four (= the 2x2 tiles 0, 1, 2) are updated here, one pair per lane, then the
+      // next tile is factorised
+      if (lane < 10) {
+        const int pp = lane >= 6 ? 3 : (lane >= 3 ? 2 : (lane >= 1 ? 1 : 0)), qq = lane - (pp * (pp + 1) >> 1);
+        if (pp < m) {
+          const int i = act[pp], k = act[qq];
+          H[tri(i, k)] -= cmp[pp] * cmp[qq] + cmp[NC + pp] * cmp[NC + qq] + cmp[2 * NC + pp] * cmp[2 * NC + qq] +
+                          cmp[3 * NC + pp] * cmp[3 * NC + qq];
+        }
+      }
+      __syncwarp();
+      if (r0 < n) flag |= ref_factor_tile(H, s.b, dinv, r0, n - r0 < 4 ? n - r0 : 4, lane, &sh_tile[cur ^ 1]);
+    } else if (ntile > 3) {
+      // the other warps: tiles 3.. ; the (a, b) of this thread's first tile by one square root, then advanced
+      constexpr int NU = NT - 32;
+      const int t0 = 3 + tid - 32;
+      if (t0 < ntile) {
+        int a = (int)((sqrtf(8.0f * (float)t0 + 1.0f) - 1.0f) * 0.5f);
+        if ((a + 1) * (a + 2) / 2 <= t0) ++a;
+        if (a * (a + 1) / 2 > t0) --a;
+        int bq = t0 - (a * (a + 1) >> 1);
+        for (int p = t0;;) {
+          const int ia = 2 * a, ib = 2 * bq;
+          const double2 A0 = *reinterpret_cast<const double2*>(cmp + ia), A1 = *reinterpret_cast<const double2*>(cmp + NC + ia);
+          const double2 A2 = *reinterpret_cast<const double2*>(cmp + 2 * NC + ia), A3 = *reinterpret_cast<const double2*>(cmp + 3 * NC + ia);
+          const double2 B0 = *reinterpret_cast<const double2*>(cmp + ib), B1 = *reinterpret_cast<const double2*>(cmp + NC + ib);
+          const double2 B2 = *reinterpret_cast<const double2*>(cmp + 2 * NC + ib), B3 = *reinterpret_cast<const double2*>(cmp + 3 * NC + ib);
+          const bool ra1 = ia + 1 < m, cb1 = ib + 1 < m;
+          const int i0 = act[ia], i1 = ra1 ? act[ia + 1] : 0, k0 = act[ib], k1 = cb1 ? act[ib + 1] : 0;
+          H[tri(i0, k0)] -= A0.x * B0.x + A1.x * B1.x + A2.x * B2.x + A3.x * B3.x;
+          if (ra1) H[tri(i1, k0)] -= A0.y * B0.x + A1.y * B1.x + A2.y * B2.x + A3.y * B3.x;
+          if (cb1 && bq < a) H[tri(i0, k1)] -= A0.x * B0.y + A1.x * B1.y + A2.x * B2.y + A3.x * B3.y;   // (above the diagonal when b == a)
+          if (ra1 && cb1) H[tri(i1, k1)] -= A0.y * B0.y + A1.y * B1.y + A2.y * B2.y + A3.y * B3.y;
+          p += NU;
+          if (p >= ntile) break;
+          bq += NU;
+          while (bq > a) { bq -= a + 1; ++a; }
+        }
       }
     }
+    // the list of the next block (the readers of sh_cnt of this block are past the barrier above)
+    if (r0 < n) ballots(r0 + (n - r0 < 4 ? n - r0 : 4));
     __syncthreads();
   }
   real r = 0.0;
