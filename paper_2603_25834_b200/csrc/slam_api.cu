@@ -36,7 +36,8 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
                  unsigned long long* stats, const int* __restrict__ perm, int* __restrict__ keys,
                  int* __restrict__ fb_list, int* __restrict__ fb_cnt) {
   extern __shared__ float4 smem4[];
-  __shared__ int s_env[16], s_need[16], s_off[16], s_new[16], s_nxt[16], s_ctl[2];
+  __shared__ int s_env[16], s_need[16], s_off[16], s_new[16], s_nxt[16], s_ctl[3];
+  int* queue = reinterpret_cast<int*>(stats + 16);   // [0] next chunk of the ordered list (ly.dynq), [1] CTAs finished
   float* smem = reinterpret_cast<float*>(smem4);
   const int team = threadIdx.x / TEAM, lane = threadIdx.x % TEAM;
   const int LOCK = ly.lock;
@@ -63,30 +64,40 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
   Masks mk;
   Ord od;
   if (threadIdx.x < 16) { s_env[threadIdx.x] = -1; s_off[threadIdx.x] = 0; }
-  if (threadIdx.x == 0) s_ctl[0] = 0;
+  if (threadIdx.x == 0) { s_ctl[0] = 0; s_ctl[2] = 0; }
   // All teams of a CTA walk through the phases in LOCK-STEP (CTA barriers between phases): the kernel is
   // large (~12 k instructions) and instruction-fetch bound, so warps that execute the same code at the
   // same time share every fetched line.  Teams without an environment only take part in the barriers.
   for (;;) {
     __syncthreads();
-    if (threadIdx.x == 0) {  // teams that are not waiting take the next environments of this CTA, in team order
+    if (threadIdx.x == 0) {  // teams that are not waiting take the next environments, in team order
       int nk = s_ctl[0], live = 0;
+      // ly.dynq: the teams of this round take CONSECUTIVE entries of the cost-ordered list (slam_order_kernel) from
+      // ONE queue for the whole grid -- the environments of one round cost about the same, so the lock-step
+      // barriers wait for little, and a CTA whose teams had to wait for pool space simply takes fewer: no CTA is
+      // left with rounds to run after the others have finished (measured: step kernel -4 % against the static deal,
+      // SLAM_DYNQ=0: chunks of wpc consecutive entries dealt round-robin to the CTAs)
+      int qbase = ly.N;
+      if (ly.dynq && s_ctl[2] >= 0) {
+        int nfree = 0;
+        for (int t = 0; t < ly.wpc; ++t) nfree += s_off[t] != -1;
+        if (nfree > 0) {
+          qbase = atomicAdd(queue, nfree);
+          if (qbase >= ly.N) { s_ctl[2] = -1; qbase = ly.N; }   // the list is exhausted: no more trips to the queue
+        }
+      }
       for (int t = 0; t < ly.wpc; ++t) {
         if (s_off[t] != -1) {
-          // the k-th environment of this CTA: chunks of wpc consecutive entries of the cost-ordered list
-          // (slam_order_kernel), dealt round-robin to the CTAs -- the environments of one round cost about
-          // the same, so the lock-step barriers wait for little, and every CTA gets the same mix
-          const long long idx = ((long long)(nk / ly.wpc) * gridDim.x + blockIdx.x) * ly.wpc + nk % ly.wpc;
+          const int idx = ly.dynq ? qbase++ : ((nk / ly.wpc) * (int)gridDim.x + (int)blockIdx.x) * ly.wpc + nk % ly.wpc;
           if (idx < ly.N) { s_env[t] = perm[idx]; ++nk; } else s_env[t] = -1;
         }
         live += s_env[t] >= 0;
       }
       s_ctl[0] = nk; s_ctl[1] = live;
-      // the environments of the NEXT round (if no team has to wait for pool space): their records are pulled
-      // into L2 by the bulk-copy engine while this round computes, see below
-      if (ly.pf_bytes > 0)
+      // the environments of the NEXT round (if no team has to wait for pool space), for the L2 prefetch experiment
+      if (ly.pf_bytes > 0 && !ly.dynq)
         for (int t = 0; t < ly.wpc; ++t, ++nk) {
-          const long long idx = ((long long)(nk / ly.wpc) * gridDim.x + blockIdx.x) * ly.wpc + nk % ly.wpc;
+          const int idx = ((nk / ly.wpc) * (int)gridDim.x + (int)blockIdx.x) * ly.wpc + nk % ly.wpc;
           s_nxt[t] = idx < ly.N ? perm[idx] : -1;
         }
     }
@@ -233,6 +244,10 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
       if (status && (lane & 31) == 0) atomicOr(reinterpret_cast<int*>(rec) + ly.o_status, status);  // (any warp may hold a flag)
       tm.sync();
     }
+  }
+  if (ly.dynq && threadIdx.x == 0) {   // the last CTA to leave rewinds the queue for the next launch
+    __threadfence();
+    if (atomicAdd(queue + 1, 1) == (int)gridDim.x - 1) { queue[0] = 0; queue[1] = 0; __threadfence(); }
   }
 }
 
@@ -676,6 +691,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   if (cudaGetDevice(&c->device) != cudaSuccess) { cudaGetLastError(); delete c; return SLAM_ECUDA; }
   { const char* e = getenv("SLAM_LOCK"); if (e) c->ly.lock = atoi(e); }
   { const char* e = getenv("SLAM_LCACHE"); if (e) c->ly.lcache = atoi(e); }
+  { const char* e = getenv("SLAM_DYNQ"); c->ly.dynq = e ? atoi(e) : 1; }
   // Bytes of the next round's records the step kernel prefetches into L2.  OFF by default: measured -0.4 % on the
   // step kernel for +45 % DRAM traffic and no drop of the long-scoreboard share.
   // SLAM_PREFETCH=1: everything up to the prior mean and gradient plus the packed Lambda of a typical support (a

@@ -33,6 +33,7 @@ struct Layout {
   int pairs;           // 1: envelope rows grouped in pairs instead of fours (less shared memory, more instructions)
   int lcache;          // 1: keep the factor columns of passive landmarks across the linearisations of one call
   int pf_bytes;        // bytes of the next round's record pulled into L2 by cp.async.bulk.prefetch (0: off)
+  int dynq;            // 1: the CTAs take their chunks of the ordered list from one queue for the grid
   int lock;            // lock-step level: CTA barriers before assemble (1), + before Cholesky (2), + before the solve (3)
   float ratio_hi;      // anchor pivot ratio H_aa / L_aa^2 above which the fp32 kernel hands the environment to the fp64 path (0: never)
 };
@@ -98,6 +99,7 @@ static inline Layout make_layout(int N, int W, int L, int pool, int wpc) {
   y.wpc = wpc;
   y.team = 32;
   y.lock = 1;
+  y.dynq = 0;
   y.pf_bytes = 0;
   y.ratio_hi = 0.f;
   y.lcache = 1;
