@@ -599,14 +599,16 @@ static step_fn kernel_of(int team, int pairs, int landmarks) {
 #endif
 }
 // Envelope rows in pairs instead of fours: 12-18 % fewer shared-memory words per environment, ~5 % more
-// instructions.  Pays where the pool bounds the environments in flight even at a third of the dense
-// size per environment (large pose-only windows; measured, ms per step, fours / pairs: config 4 3.18 /
-// 2.90, config 2 0.399 / 0.417, config 3 2.08 / 2.10).  SLAM_PAIRS=0/1 overrides.
+// instructions.  Pays where the pool bounds the environments in flight: at a third of the dense size per
+// environment for pose-only windows (measured, ms per step, fours / pairs: config 4 3.48 / 3.09, config 2 0.373 /
+// 0.417), at half of it for windows with landmarks, whose envelope is denser (config 3 while the robots are among
+// the landmarks: 2.46 / 2.33, pool waits halved; over the whole 300 steps, whose late windows are nearly empty,
+// 1.72 / 1.76 -- the dear phase decides).  SLAM_PAIRS=0/1 overrides.
 static int pick_pairs(int W, int L, int team) {
   const char* e = getenv("SLAM_PAIRS");
   if (e && (e[0] == '0' || e[0] == '1')) return e[0] == '1';
   const Layout d = make_layout(1, W, L, 0, 1);
-  return L == 0 && team == 32 && 16.0 * (d.team_words + 0.3 * d.dense) > SMEM_BUDGET / 4;
+  return team == 32 && 16.0 * (d.team_words + (L > 0 ? 0.5 : 0.3) * d.dense) > SMEM_BUDGET / 4;
 }
 
 // The ONE place that decides the launch shape of the step kernel for given sizes (slam_workspace_bytes and
