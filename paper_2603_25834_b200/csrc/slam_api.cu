@@ -474,7 +474,7 @@ struct slam_ctx {
   float ratio_hi, ratio_lo;
   int min_vis;                // landmarks the newest pose must see before an fp64 environment goes back to fp32
   int ref_grid, ref_smem;
-  bool order, order_all;      // re-sort after every solve (SLAM_ORDER=0 disables, 2: pose-only windows too)
+  bool order, order_all;      // re-sort after every solve (SLAM_ORDER=0 disables, 1: windows with landmarks only)
   // device staging for slam_step_host
   float *st_odom, *st_lc_meas, *st_rb_meas, *st_cov, *st_logdet, *st_pose;
   int32_t* st_lc_back;
@@ -720,7 +720,7 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   c->stats = (unsigned long long*)(base + p.stats);
   c->perm = (int*)(base + p.perm);
   c->keys = (int*)(base + p.keys);
-  { const char* e = getenv("SLAM_ORDER"); c->order = !(e && e[0] == '0'); c->order_all = e && e[0] == '2'; }
+  { const char* e = getenv("SLAM_ORDER"); c->order = !(e && e[0] == '0'); c->order_all = !(e && e[0] == '1'); }
   c->state = (float*)(base + p.state);
   c->cov_cache = (float*)(base + p.cache);
   c->st_odom = (float*)(base + p.odom);
@@ -835,9 +835,10 @@ static int launch_step(slam_ctx* c, int flags, int iters, const StepIO& io) {
   }
   if (tv) cudaEventRecord(tv[2], c->stream);
   // the solve left fresh cost keys: order the next launches by them (pointless unless every CTA runs
-  // several rounds; a small batch is latency bound: one more kernel boundary per step would show; and
-  // measured only landmark windows gain -- their cost varies most: config 3 2.40 -> 2.31 ms per step,
-  // config 4 3.49 -> 3.53)
+  // several rounds; a small batch is latency bound: one more kernel boundary per step would show).  Landmark
+  // windows gain most -- their cost varies most: config 3 2.40 -> 2.31 ms per step under the static deal of
+  // round 1; pose-only windows gain since the list is handed out from one queue for the grid (most expensive
+  // first = longest-processing-time scheduling): config 4 at N = 16384 3.09 -> 3.04, at 65536 11.7 -> 11.3
   if (c->order && iters > 0 && (c->ly.L > 0 || c->order_all) && (long long)c->ly.N >= 4ll * c->grid * c->ly.wpc) {
     slam_order_kernel<<<1, 1024, 0, c->stream>>>(c->ly.N, c->ly.dense, c->keys, c->perm);
     c->launches++;
