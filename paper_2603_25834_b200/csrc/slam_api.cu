@@ -565,7 +565,7 @@ static int pick_launch(int W, int L, int team, int pairs, int* pool_words) {
   // config 3 2.076 / 2.043; config 4, whose windows need half a pool of 8 teams and more, 2.845 / 3.004:
   // the estimate keeps it on one CTA).  SLAM_SPLIT_CTA=0 disables.
   const char* sp = getenv("SLAM_SPLIT_CTA");
-  const int max_ctas = ((sp && sp[0] == '0') || pairs) ? 1 : 2;   // (rows in pairs = shared memory binds: one pool)
+  const int max_ctas = ((sp && sp[0] == '0') || (pairs && !(sp && sp[0] == '2'))) ? 1 : 2;   // (rows in pairs = shared memory binds: one pool; SLAM_SPLIT_CTA=2 tries two anyway)
   for (int ctas = 1; ctas <= max_ctas; ++ctas) {
     const int budget = ctas == 1 ? SMEM_BUDGET : (228 * 1024 / 2 - 1024 - 512);
     for (int wpc = 1; wpc * ctas <= max_teams(team); ++wpc) {
@@ -592,7 +592,7 @@ template <bool PAIRS, bool LM>
 // carry no code for cached landmark columns, the fours kernels none for split dot products.
 static step_fn kernel_of(int team, int pairs, int landmarks) {
 #ifdef SLAM_DEV_SINGLE   // developer build (compiles in a fifth of the time): only the kernels of BASELINE configs 3 and 4
-  return landmarks ? slam_step_kernel<32, false, true> : slam_step_kernel<32, true, false>;
+  return landmarks ? slam_step_kernel<32, true, true> : slam_step_kernel<32, true, false>;
 #else
   if (pairs) return landmarks ? kernel_pick<true, true>(team) : kernel_pick<true, false>(team);
   return landmarks ? kernel_pick<false, true>(team) : kernel_pick<false, false>(team);
