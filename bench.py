@@ -456,6 +456,10 @@ def main():
                 "work_sample_envs": int(len(sample)),
                 "envelope_words_avg": float(work["env_words"][P:].mean()), "prior_support_avg": float(work["support"][P:].mean()),
                 "fp64_env_calls_frac": stats["fp64_calls"] / max(stats["solved"] + stats["fp64_calls"], 1)}
+        # the dominant kernel ALONE: the algorithmic flops of the environments it solved over its own launch time
+        # (`frac` above charges the whole step, fp64 and ordering launches included, to the same flops)
+        roof["frac_step_kernel_alone"] = (flops_total / K * (1.0 - roof["fp64_env_calls_frac"])) / \
+            max(k_step * 1e-3, 1e-12) / (p_fp32 * 1e12)
         out = {
             "metric": METRIC, "value": value, "unit": "env-steps/s", "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
