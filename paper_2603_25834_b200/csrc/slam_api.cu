@@ -60,6 +60,7 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
   const int nlin = iters + ((flags & F_COV) ? 1 : 0);
   // the environment this team has in hand (kept across rounds while it waits for pool space)
   int env = -1, k0 = 0, head = 0, cc = 0, s = 0, total = 0, need = 0;
+  float rhi = 0.f;   // this environment's threshold of the conditioning watch
   bool waiting = false, do_marg = false;
   Masks mk;
   Ord od;
@@ -131,6 +132,15 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
         if (flags & F_OBS0) record_rb<TEAM>(ly, rec, w, tm, lane, env, head, 0, 0.f, 0.f, 0.f, io, mk);
         if (flags & F_PUSH) cc = push_env<TEAM>(ly, rec, w, tm, lane, env, head, cc, io, mk);
         od = make_ord(ly, w.rbm, cc);
+        // A robot that is WELL localised against the map (its newest pose sees at least box_vis landmarks) gets twice
+        // the thresholds of the conditioning watch: with that many fresh measurements per step the result hardly
+        // leans on the prior, so what fp32 loses in the anchor's pivots does not accumulate.
+        rhi = ly.ratio_hi;
+        if (LM && ly.box_vis > 0) {
+          int nv = __popc(w.rbm[(cc - 1) * ly.nw]);
+          if (ly.nw > 1) nv += __popc(w.rbm[(cc - 1) * ly.nw + 1]);
+          if (nv >= ly.box_vis) rhi *= 2.f;
+        }
         s = build_support<TEAM>(ly, od, w, tm, lane, cc, mk.ps, mk.ls);
         do_marg = (flags & F_MARG) && k0 == 0;   // a reset environment is not full yet
         need = do_marg ? marg_need(ly, w, lane, cc, mk) : 0;
@@ -196,10 +206,10 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
           // does the factorisation with shuffles and __syncwarp only: no named barriers, no
           // shared-memory exchange of the diagonal tile.  The other warps of the team wait.
           if (TEAM > 32 && single_warp) {
-            if ((lane >> 5) == solo) status |= cholesky<32, PAIRS, LM>(ly, w, tm32, lane & 31, ncb);
+            if ((lane >> 5) == solo) status |= cholesky<32, PAIRS, LM>(ly, w, tm32, lane & 31, ncb, rhi);
             tm.sync();
           } else {
-            status |= cholesky<TEAM, PAIRS, LM>(ly, w, tm, lane, ncb);
+            status |= cholesky<TEAM, PAIRS, LM>(ly, w, tm, lane, ncb, rhi);
           }
         }
         if (LOCK >= 3) __syncthreads();
@@ -473,6 +483,7 @@ struct slam_ctx {
   bool precision_auto;        // the default rule decides (landmarks or unary factors -> 1, else 0)
   float ratio_hi, ratio_lo;
   int min_vis;                // landmarks the newest pose must see before an fp64 environment goes back to fp32
+  int box_vis;                // ... and to count as well localised: twice the thresholds (0: never)
   int ref_grid, ref_smem;
   bool order, order_all;      // re-sort after every solve (SLAM_ORDER=0 disables, 1: windows with landmarks only)
   // device staging for slam_step_host
@@ -746,6 +757,8 @@ int slam_create(slam_ctx** out, int batch, int window, int landmarks, const slam
   c->precision = landmarks > 0 ? 1 : 0;
   c->ratio_hi = 300.f; c->ratio_lo = 150.f;
   c->min_vis = 3;
+  c->box_vis = 9;
+  { const char* e = getenv("SLAM_BOX_VIS"); if (e) c->box_vis = atoi(e); }
   { const char* e = getenv("SLAM_MIN_VIS"); if (e) c->min_vis = atoi(e); }
   { const char* e = getenv("SLAM_RATIO_HI"); if (e && atof(e) > 0) c->ratio_hi = (float)atof(e); e = getenv("SLAM_RATIO_LO"); if (e && atof(e) > 0) c->ratio_lo = (float)atof(e); }
   { const char* e = getenv("SLAM_PRECISION"); if (e && e[0] >= '0' && e[0] <= '2') { c->precision = e[0] - '0'; c->precision_auto = false; } }
@@ -818,6 +831,7 @@ static int launch_step(slam_ctx* c, int flags, int iters, const StepIO& io) {
   } else {
     Layout ly = c->ly;
     ly.ratio_hi = c->precision == 1 ? c->ratio_hi : 0.f;
+    ly.box_vis = c->box_vis;
     fn<<<c->grid, c->ly.wpc * c->ly.team, c->smem_bytes, c->stream>>>(ly, c->pr, c->state, c->head, c->count, flags, iters, io,
                                                                         c->stats, c->perm, c->keys,
                                                                         c->precision == 1 ? c->fb_list : nullptr, c->fb_cnt);
@@ -826,7 +840,7 @@ static int launch_step(slam_ctx* c, int flags, int iters, const StepIO& io) {
   if (tv) cudaEventRecord(tv[1], c->stream);
   if (c->precision >= 1) {   // the environments the fp32 kernel queued: fp64 records, and the windows it refused to commit
     slamr::RefArgs ra = {c->state, c->state64, c->head, c->count, flags, iters, c->fb_list, c->fb_cnt, c->stats, c->hglob,
-                         (double)c->ratio_lo, c->precision == 2 ? 1 : 0, c->min_vis};
+                         (double)c->ratio_lo, c->precision == 2 ? 1 : 0, c->min_vis, c->box_vis};
 #ifdef SLAM_REF_PROFILE
     cudaMemcpyToSymbolAsync(slamr::g_ref_prof, &c->stats, sizeof(c->stats), 0, cudaMemcpyHostToDevice, c->stream);
 #endif

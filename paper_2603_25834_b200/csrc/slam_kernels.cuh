@@ -1069,7 +1069,7 @@ __device__ __forceinline__ void st4(float* p, float4 v) { *reinterpret_cast<floa
   ACC = fmaf(-XV.w, BV.w, ACC);
 
 template <int TEAM, bool PAIRS, bool CACHE>
-__device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int lane, int ncb) {
+__device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int lane, int ncb, float rhi) {
   // ncb: number of leading column blocks whose factor is still valid from the previous factorisation of
   // this call (see assemble): there only the rhs pair -- the last entry of the column's list -- is
   // processed, on the lanes and with the K-split it has in a full pass, so y is bit-identical.
@@ -1081,7 +1081,7 @@ __device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int
   // dead-reckoned and re-observes a landmark has information on `a` spanning six decades.  Keep the assembled
   // diagonal of the three anchor rows; after the last column block compare it with the pivots.
   float ha0 = 0.f, ha1 = 0.f, ha2 = 0.f;
-  if (ly.ratio_hi > 0.f) {
+  if (rhi > 0.f) {   // rhi: this environment's threshold (slam_step_kernel), 0 = no watch
     const int oA = np - 3;
     ha0 = w.H[rb_of(w, oA) + oA]; ha1 = w.H[rb_of(w, oA + 1) + oA + 1]; ha2 = w.H[rb_of(w, oA + 2) + oA + 2];
   }
@@ -1199,7 +1199,7 @@ __device__ int cholesky(const Layout& ly, const WS& w, const Team<TEAM>& tm, int
           if (!(t33 > 0.f)) d3 = 1.f;
         }
         // rows np-3 .. np-1 of the last block are the anchor: H_ii / L_ii^2 = H_ii d_i^2
-        if (J == G - 1 && fmaxf(fmaxf(ha0 * d1 * d1, ha1 * d2 * d2), ha2 * d3 * d3) > ly.ratio_hi && ly.ratio_hi > 0.f) flag |= ENV_ILLCOND;
+        if (J == G - 1 && fmaxf(fmaxf(ha0 * d1 * d1, ha1 * d2 * d2), ha2 * d3 * d3) > rhi && rhi > 0.f) flag |= ENV_ILLCOND;
       }
       if (act && t == 0) {
         if (first_pass && q < 2) {

@@ -35,6 +35,7 @@ struct Layout {
   int pf_bytes;        // bytes of the next round's record pulled into L2 by cp.async.bulk.prefetch (0: off)
   int dynq;            // 1: the CTAs take their chunks of the ordered list from one queue for the grid
   int lock;            // lock-step level: CTA barriers before assemble (1), + before Cholesky (2), + before the solve (3)
+  int box_vis;         // landmarks the newest pose must see to count as well localised (doubles the thresholds of the watch; 0: off)
   float ratio_hi;      // anchor pivot ratio H_aa / L_aa^2 above which the fp32 kernel hands the environment to the fp64 path (0: never)
 };
 
@@ -102,6 +103,7 @@ static inline Layout make_layout(int N, int W, int L, int pool, int wpc) {
   y.dynq = 0;
   y.pf_bytes = 0;
   y.ratio_hi = 0.f;
+  y.box_vis = 0;
   y.lcache = 1;
   y.pairs = 0;
   return y;

@@ -51,6 +51,7 @@ struct RefArgs {
   double ratio_lo;    // back to fp32 below this anchor pivot ratio
   int force;          // 1: every environment stays in fp64 (device reference)
   int min_vis;        // landmarks the newest pose must see for the hand-over back to fp32
+  int box_vis;        // ... and to count as well localised (twice the thresholds; 0: never)
 };
 
 // shared-memory views of one environment
@@ -1203,7 +1204,8 @@ __global__ void __launch_bounds__(NT, 3) slam_ref64_kernel(Layout ly, Params pr,
     // 4096-environment sample of config 3).
     if (nlin > 0) {
       const int nvis = ly.L > 0 ? __popcll(vis_of(ly, s, e.c - 1)) : 0;
-      newmode = (ratio < ra.ratio_lo && status == 0 && (ly.L == 0 || nvis >= ra.min_vis)) ? 0 : 1;
+      const bool well = ly.L > 0 && ra.box_vis > 0 && nvis >= ra.box_vis;   // well localised: twice the threshold, as in slam_step_kernel
+      newmode = (ratio < (well ? 2.0 : 1.0) * ra.ratio_lo && status == 0 && (ly.L == 0 || nvis >= ra.min_vis)) ? 0 : 1;
     }
     if (ra.force) newmode = 1;
     const bool do_marg = (ra.flags & slamk::F_MARG) && e.k0 == 0;

@@ -27,7 +27,7 @@ def main():
     from tests.gpu_driver import parity_errors, run_gpu
 
     stride = int(sys.argv[1]) if len(sys.argv) > 1 else 4
-    settings = [tuple(float(x) for x in a.split(":")) for a in sys.argv[2:]] or [(300, 150, 3), (300, 150, 0)]
+    settings = [tuple(float(x) for x in a.split(":")) for a in sys.argv[2:]] or [(300, 150, 3), (300, 150, 0)]   # hi:lo:min_vis[:box_vis]
     cfg = synth.CONFIGS[3]
     data = synth.generate(cfg)
     envs = np.arange(0, cfg.N, stride, dtype=np.int32)
@@ -43,7 +43,7 @@ def main():
         st = slam.get_stats()
         line = [f"{name}: fp64 calls {st['fp64_calls'] / (cfg.N * cfg.T):.4f}"]
         for k, v in err.items():
-            line.append(f"{k} max {v.max():.3f}, {int((v > 1).sum())} of {v.size} beyond tolerance")
+            line.append(f"{k} max {v.max():.3f}, {int((v > 1).sum())} of {v.size} beyond tolerance ({int((v > 0.5).sum())} beyond half of it)")
         print(" | ".join(line), flush=True)
         return err
 
@@ -52,11 +52,14 @@ def main():
     g64 = sub(run_gpu(slam, data, cfg.iters, fused=True, want_poses=False))
     e64 = report("device reference (every environment in fp64)", slam, g64)
     del slam
-    for hi, lo, mv in settings:
+    for st_ in settings:
+        hi, lo, mv = st_[:3]
         os.environ["SLAM_RATIO_HI"], os.environ["SLAM_RATIO_LO"], os.environ["SLAM_MIN_VIS"] = str(hi), str(lo), str(int(mv))
+        if len(st_) > 3:
+            os.environ["SLAM_BOX_VIS"] = str(int(st_[3]))
         slam = FixedLagSlam(cfg.N, cfg.W, cfg.L, device="cuda:0")
         g = sub(run_gpu(slam, data, cfg.iters, fused=True, want_poses=False))
-        err = report(f"ratio_hi {hi:g} ratio_lo {lo:g} min_vis {int(mv)}", slam, g)
+        err = report(f"ratio_hi {hi:g} ratio_lo {lo:g} min_vis {int(mv)}" + (f" box_vis {int(st_[3])}" if len(st_) > 3 else ""), slam, g)
         bad = np.argwhere((err["logdet"] > 1) | (err["cov"] > 1) | (err["last_pose"] > 1))
         for t, i in bad[:60]:
             print(f"    step {int(t) + 1} env {int(envs[i])}: ln det {err['logdet'][t, i]:.2f} cov {err['cov'][t, i]:.2f} "
