@@ -59,7 +59,6 @@ struct Sm {
   real* v;      // [n] state, natural index: a 0..2, e_k 3k.., g_l 3W+2l..
   real* b;      // [n] rhs / y / delta, elimination order
   real* d;      // [n] prior displacement on the support; scratch
-  real* col;    // [n] current column of L
   real* cs;     // [2W] cos, sin of each slot's heading (anchor frame)
   real* part;   // [max(W,L)][9] partial sums of the anchor block
   real* X;      // [3n] marginalisation: X rows
@@ -75,7 +74,8 @@ struct Sm {
 
 __host__ __device__ inline size_t ref_smem_doubles(const Layout& ly) {  // everything but H
   const int n = ly.n, m = ly.W > ly.L ? ly.W : ly.L;
-  return (size_t)4 * n + 2 * ly.W + ((9 * m + 1) & ~1) + 6 * n + 16;
+  (void)m;   // (part and cs alias X, Q: 9 m + 2 W <= 6 n always)
+  return (size_t)2 * n + ((n + 1) & ~1) + 6 * n + 2;
 }
 __host__ __device__ inline size_t ref_smem_ints(const Layout& ly) { return (size_t)4 * ly.n + ly.W + ly.W * (ly.nw ? ly.nw : 1) + 8; }
 __host__ __device__ inline size_t ref_tri(const Layout& ly) { return (size_t)ly.n * (ly.n + 1) / 2; }
@@ -165,8 +165,12 @@ __device__ inline Sm carve(const Layout& ly, double* base, double* hglob) {
   Sm s;
   const int n = ly.n, m = ly.W > ly.L ? ly.W : ly.L;
   double* p = base;
-  s.v = p; p += n; s.b = p; p += n; s.d = p; p += n; s.col = p; p += n;
-  s.cs = p; p += 2 * ly.W; s.part = p; p += (9 * m + 1) & ~1; s.X = p; p += 3 * n; s.Q = p; p += 3 * n; p += 16;
+  s.v = p; p += n; s.b = p; p += n; s.d = p; p += (n + 1) & ~1;   // (X 16-byte aligned: 128-bit loads in ref_cholesky)
+  s.X = p; p += 3 * n; s.Q = p; p += 3 * n; p += 2;
+  // only ref_assemble needs the partial sums and the cos / sin table, and nothing else lives in X, Q while it runs
+  // (ref_cholesky's compact columns and the marginalisation come later): they share that storage, which is what
+  // lets FOUR environments fit an SM at config 3
+  s.part = s.X; s.cs = s.X + ((9 * m + 1) & ~1);
   int* q = reinterpret_cast<int*>(p);
   s.pos = q; q += n; s.first = q; q += n; s.sidx = q; q += n; s.omap = q; q += n; s.lct = q; q += ly.W;
   s.rbm = reinterpret_cast<uint32_t*>(q); q += ly.W * (ly.nw ? ly.nw : 1); q += 8;
@@ -1145,7 +1149,7 @@ __device__ void ref_store(const Layout& ly, const Ctx& e, const Sm& s, int tid, 
 }
 
 // ------------------------------------------------------------------ the kernel: persistent CTAs pull environments from the list
-__global__ void __launch_bounds__(NT, 3) slam_ref64_kernel(Layout ly, Params pr, RefArgs ra, StepIO io) {
+__global__ void __launch_bounds__(NT, 4) slam_ref64_kernel(Layout ly, Params pr, RefArgs ra, StepIO io) {
   extern __shared__ double ref_smem[];
   __shared__ int sh_i;
   const int tid = threadIdx.x;
