@@ -840,7 +840,7 @@ static int launch_step(slam_ctx* c, int flags, int iters, const StepIO& io) {
   if (tv) cudaEventRecord(tv[1], c->stream);
   if (c->precision >= 1) {   // the environments the fp32 kernel queued: fp64 records, and the windows it refused to commit
     slamr::RefArgs ra = {c->state, c->state64, c->head, c->count, flags, iters, c->fb_list, c->fb_cnt, c->stats, c->hglob,
-                         (double)c->ratio_lo, c->precision == 2 ? 1 : 0, c->min_vis, c->box_vis};
+                         (double)c->ratio_lo, c->precision == 2 ? 1 : 0, c->min_vis, c->box_vis, c->keys};
 #ifdef SLAM_REF_PROFILE
     cudaMemcpyToSymbolAsync(slamr::g_ref_prof, &c->stats, sizeof(c->stats), 0, cudaMemcpyHostToDevice, c->stream);
 #endif

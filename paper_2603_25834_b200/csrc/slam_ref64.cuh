@@ -52,6 +52,7 @@ struct RefArgs {
   int force;          // 1: every environment stays in fp64 (device reference)
   int min_vis;        // landmarks the newest pose must see for the hand-over back to fp32
   int box_vis;        // ... and to count as well localised (twice the thresholds; 0: never)
+  int* keys;          // cost keys of the step kernel's order (see the end of the kernel), or nullptr
 };
 
 // shared-memory views of one environment
@@ -1219,6 +1220,11 @@ __global__ void __launch_bounds__(NT, 4) slam_ref64_kernel(Layout ly, Params pr,
     if (tid == 0) {
       if (status) atomicOr(reinterpret_cast<int*>(e.r32) + ly.o_status, status);
       if (ra.stats) atomicAdd(ra.stats + 4, 1ull);
+      // An environment that stays here costs the step kernel nothing: key 0 sorts it to the END of the cost-ordered
+      // list, so the teams that draw it (they only pass it on to this kernel and idle for the round) do so in the
+      // last rounds of a launch instead of leaving holes in every round.  One that goes back gets a middling key
+      // for one step.
+      if (ra.keys) ra.keys[e.env] = newmode ? 0 : ly.dense / 3;
     }
   }
   // the last CTA to leave resets the list for the next launch
