@@ -15,8 +15,8 @@
 using namespace slamk;
 
 // ------------------------------------------------------------------ kernels
-// One TEAM of 32/64/128 threads per environment, `wpc` teams per CTA, persistent loop over the
-// environments of its CTA (chunks of the cost-ordered list, see the assignment below) in ROUNDS.  flags select the phases, so that the
+// One TEAM of 32/64/128 threads per environment, `wpc` teams per CTA, persistent CTAs that take their environments
+// from one queue over the cost-ordered list (see the assignment below) in ROUNDS.  flags select the phases, so that the
 // separate ABI calls and the fused slam_step share the same device code and are bit-for-bit identical.
 //
 // Shared memory = a fixed part per team (state, factor data, row tables) + ONE POOL per CTA.  The
@@ -37,7 +37,7 @@ slam_step_kernel(Layout ly, Params pr, float* state, int head_g, int c, int flag
                  int* __restrict__ fb_list, int* __restrict__ fb_cnt) {
   extern __shared__ float4 smem4[];
   __shared__ int s_env[16], s_need[16], s_off[16], s_new[16], s_nxt[16], s_ctl[3];
-  int* queue = reinterpret_cast<int*>(stats + 16);   // [0] next chunk of the ordered list (ly.dynq), [1] CTAs finished
+  int* queue = reinterpret_cast<int*>(stats + 16);   // [0] next entry of the cost-ordered list (ly.dynq), [1] CTAs finished
   float* smem = reinterpret_cast<float*>(smem4);
   const int team = threadIdx.x / TEAM, lane = threadIdx.x % TEAM;
   const int LOCK = ly.lock;
