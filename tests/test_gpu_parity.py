@@ -373,6 +373,10 @@ def test_results_do_not_depend_on_capacity_or_team(monkeypatch):
     p0 = run_gpu(_slam(cfg.N, cfg.W, cfg.L), data, cfg.iters, fused=True, want_poses=False)
     assert np.array_equal(a["cov"], p0["cov"]) and np.array_equal(a["logdet"], p0["logdet"])
     monkeypatch.delenv("SLAM_PREFETCH")
+    monkeypatch.setenv("SLAM_DYNQ", "0")                  # static deal of the list to the CTAs instead of the one queue
+    q0 = run_gpu(_slam(cfg.N, cfg.W, cfg.L), data, cfg.iters, fused=True, want_poses=False)
+    assert np.array_equal(a["cov"], q0["cov"]) and np.array_equal(a["logdet"], q0["logdet"])
+    monkeypatch.delenv("SLAM_DYNQ")
     ref = oracle.run_batch(data, cfg.iters, envs=np.arange(0, cfg.N, 25, dtype=np.int32))
     for team in ("32", "128"):
         monkeypatch.setenv("SLAM_TEAM", team)
